@@ -1,0 +1,5 @@
+"""CPU oracle for the EmuGEMM hot path -- TEST INFRASTRUCTURE, not the product.
+
+Only tests/, __graft_entry__.smoke() and bench.py's cpu_baseline / --impl reference
+legs may import this package.  See oracle/emugemm_oracle.c for the arithmetic.
+"""
