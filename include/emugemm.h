@@ -1,0 +1,150 @@
+/*
+ * emugemm.h -- C ABI of the B200-native EmuGEMM hot path (arxiv/paper_2606_25453).
+ *
+ * High-precision GEMM  C = alpha*A*B + beta*C  emulated on INT8 tensor cores
+ * (tcgen05.mma kind::i8, sm_100a only):
+ *   Scheme I  (Eq. 1-3; fused kernel PAPER.md:171-209, Alg. 1)
+ *   Scheme II (Eq. 4-8; fused mod-reduction PAPER.md:225-240)
+ *   3M complex on Scheme II (Eq. 16-18)
+ *
+ * Conventions common to every call
+ *   - Layout: row-major, no transposes.  A is m x k with row stride lda >= k,
+ *     B is k x n with ldb >= n, C is m x n with ldc >= n; strides in elements
+ *     (complex entry point: in complex elements, storage is (re, im) pairs).
+ *   - m, n, k >= 0.  m*n == 0 is a no-op; k == 0 scales C by beta.
+ *   - All matrix pointers are DEVICE pointers owned by the caller.  A and B are
+ *     read-only.  C is read only when beta != 0 (BLAS rule: beta == 0 means C is
+ *     not read, NaNs in C do not propagate) and is overwritten.
+ *   - alpha / beta are host scalars passed by value (complex: host pointer to
+ *     two doubles, read during the call).
+ *   - Workspace is caller-owned device memory handed over with
+ *     emugemm_set_workspace(); the library never allocates device memory on the
+ *     hot path.  emugemm_workspace_bytes() says how much a call needs.
+ *   - Calls are asynchronous on the handle's stream (emugemm_set_stream; default
+ *     stream 0).  One handle per host thread.  The handle owns only host state.
+ *   - Alignment: A, B, C base pointers 16-byte aligned, workspace 1024-byte.
+ *   - Non-finite inputs: result unspecified, no fault.
+ *   - Return value: EMUGEMM_OK (0) or a negative emugemm_status; no exceptions,
+ *     no exit(), no stdout.  There is NO CPU fallback: on a device that is not
+ *     sm_100 every compute call returns EMUGEMM_ERR_DEVICE.
+ */
+#ifndef EMUGEMM_H_
+#define EMUGEMM_H_
+
+#include <stddef.h>
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct emugemm_ctx *emugemm_handle_t;
+
+enum emugemm_status {
+  EMUGEMM_OK = 0,
+  EMUGEMM_ERR_ARG = -1,       /* null pointer, negative size, ld too small, p / n_moduli out of range */
+  EMUGEMM_ERR_ALIGNMENT = -2, /* A, B, C not 16-byte aligned or workspace not 1024-byte aligned */
+  EMUGEMM_ERR_WORKSPACE = -3, /* workspace missing or smaller than emugemm_workspace_bytes() */
+  EMUGEMM_ERR_PRECISION = -4, /* Scheme II: k too large for this n_moduli (bit budget T < 2) */
+  EMUGEMM_ERR_DEVICE = -5,    /* no CUDA device or not compute capability 10.x */
+  EMUGEMM_ERR_CUDA = -6       /* a CUDA call failed; see emugemm_last_cuda_error() */
+};
+
+enum emugemm_scheme { EMUGEMM_OZ1 = 1, EMUGEMM_OZ2 = 2, EMUGEMM_OZ2_3M = 3 };
+
+/* ---- handle ------------------------------------------------------------- */
+int emugemm_create(emugemm_handle_t *h);  /* host-only state; checks the device */
+int emugemm_destroy(emugemm_handle_t h);
+int emugemm_set_stream(emugemm_handle_t h, void *cuda_stream /* cudaStream_t */);
+int emugemm_set_workspace(emugemm_handle_t h, void *dev_ptr, size_t bytes);
+/* Bytes of workspace a call with these arguments needs.  elem = bytes per
+ * matrix element: 4 (float), 8 (double), 16 (complex128).  p_or_nmoduli = p for
+ * Scheme I, n_moduli for Scheme II / 3M.  Returns 0 for invalid arguments. */
+size_t emugemm_workspace_bytes(int scheme, int elem, int64_t m, int64_t n, int64_t k, int p_or_nmoduli);
+const char *emugemm_status_string(int status);
+int emugemm_last_cuda_error(emugemm_handle_t h); /* cudaError_t of the last EMUGEMM_ERR_CUDA */
+
+/* ---- Scheme I ------------------------------------------ *
+ * C = alpha*A*B + beta*C with p signed INT8 slices of beta_bits = 7 bits each
+ * under power-of-two row (A) / column (B) exponent scaling; the p(p+1)/2 slice
+ * products with i + j < p are computed by ONE fused kernel into p INT32
+ * accumulators kept in tensor memory, k is split into chunks that cannot
+ * overflow INT32, the epilogue applies Eq. 3 and alpha/beta in FP64.
+ * Range: double 1 <= p <= 8, float 1 <= p <= 4.                               */
+int emugemm_dgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha,
+                      const double *A, int64_t lda, const double *B, int64_t ldb, double beta,
+                      double *C, int64_t ldc, int p);
+int emugemm_sgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, float alpha,
+                      const float *A, int64_t lda, const float *B, int64_t ldb, float beta,
+                      float *C, int64_t ldc, int p);
+
+/* ---- Scheme II ---------------------------------------- *
+ * n_moduli pairwise-coprime moduli <= 256 (256, 255, 253, 251, 247, ... greedy
+ * descending); symmetric INT8 residues; one INT8 GEMM per modulus with the
+ * mod-reduction fused into its epilogue (Eq. 6-7); CRT (Eq. 8) and inverse
+ * scaling in FP64.  Range: 2 <= n_moduli <= 20.                               */
+int emugemm_dgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha,
+                      const double *A, int64_t lda, const double *B, int64_t ldb, double beta,
+                      double *C, int64_t ldc, int n_moduli);
+
+/* ---- Scheme II complex via 3M ------------------------ *
+ * A, B, C hold complex128 as (re, im) pairs; alpha, beta point to HOST {re, im}. */
+int emugemm_zgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2],
+                         const double *A, int64_t lda, const double *B, int64_t ldb,
+                         const double beta[2], double *C, int64_t ldc, int n_moduli);
+
+/* ---- per-stage timing of the last call (bench only) --------------------- *
+ * When enabled, compute calls bracket their stages with CUDA events on the
+ * handle's stream; emugemm_stage_ms() synchronises and returns milliseconds of
+ * stage 0 = pre-pass, 1 = tensor-core GEMM kernel(s), 2 = reconstruction, and the
+ * number of kernel launches of the last call in *launches (may be NULL).      */
+int emugemm_enable_stage_timing(emugemm_handle_t h, int on);
+int emugemm_stage_ms(emugemm_handle_t h, float ms[3], int *launches);
+
+/* ---- test hooks (used only by tests/; canonical layouts, device pointers) -
+ * They expose the integer intermediates the parity tests compare bit-exactly
+ * without exposing the library's private operand layouts.
+ * "Canonical slice view": int8 [planes][rows][k] with k contiguous; for operand
+ * B the rows are the COLUMNS j of B.  elem = 4 / 8 / 16 as above (16: complex,
+ * exponent shared by re and im).                                              */
+
+/* Row (by_cols = 0: X is rows x k, ldx >= k) or column (by_cols = 1: X is
+ * k x rows, ldx >= rows) max-exponent scan -> int32 e_out[rows].             */
+int emugemm_dbg_exponents(emugemm_handle_t h, int elem, int by_cols, int64_t rows, int64_t k,
+                          const void *X, int64_t ldx, int32_t *e_out);
+/* Scheme I slices of one operand -> int8 out[p][rows][k], int32 e_out[rows]. */
+int emugemm_dbg_oz1_slices(emugemm_handle_t h, int elem, int by_cols, int64_t rows, int64_t k,
+                           const void *X, int64_t ldx, int p, int8_t *out, int32_t *e_out);
+/* Fused Scheme I kernel with the INT32 accumulators of every k-chunk dumped:
+ * out[chunk][p][m][n] (int32), *n_chunks_out chunks (host int).  chunk_k = 0
+ * uses the library's overflow-safe chunk length, else that many k per chunk. */
+int emugemm_dbg_oz1_accumulators(emugemm_handle_t h, int elem, int64_t m, int64_t n, int64_t k,
+                                 const void *A, int64_t lda, const void *B, int64_t ldb, int p,
+                                 int64_t chunk_k, int32_t *out, int *n_chunks_out);
+/* Scheme II residues of one operand.  elem 8: out[N][rows][k]; elem 16 (3M):
+ * out[3][N][rows][k] = re, im, Sigma planes.  t_bits = tA or tB.             */
+int emugemm_dbg_oz2_residues(emugemm_handle_t h, int elem, int by_cols, int64_t rows, int64_t k,
+                             const void *X, int64_t ldx, int n_moduli, int t_bits, int8_t *out,
+                             int32_t *e_out);
+/* Per-modulus products with fused reduction from canonical residue planes:
+ * real: RA[N][m][k], RB[N][n][k] -> out[N][m][n];
+ * is3m: RA[3][N][m][k], RB[3][N][n][k] -> out[2][N][m][n] (re, im).           */
+int emugemm_dbg_oz2_modgemm(emugemm_handle_t h, int is3m, int64_t m, int64_t n, int64_t k,
+                            int n_moduli, const int8_t *RA, const int8_t *RB, int8_t *out);
+/* CRT + scaling alone: CR[N][m][n] int8 -> C (double, ldc), alpha/beta as in dgemm_oz2. */
+int emugemm_dbg_oz2_crt(emugemm_handle_t h, int64_t m, int64_t n, int n_moduli, const int8_t *CR,
+                        const int32_t *eA, const int32_t *eB, int tA, int tB, double alpha,
+                        double beta, double *C, int64_t ldc);
+/* Host-side helpers (no GPU): bit budget (returns T or < 0), overflow-safe chunk length. */
+int emugemm_oz2_budget(int n_moduli, int64_t k, int is3m, int *tA, int *tB);
+int64_t emugemm_oz1_chunk_k(int p);
+/* Issue-bound tcgen05.mma kind::i8 probe (no global loads in the loop): runs
+ * `iters` MMAs of 128 x n_mma x 32 per CTA on every SM and returns milliseconds
+ * in *ms; ops = 2*128*n_mma*32*iters*ctas.  Used by bench.py for the third
+ * INT8 denominator.                                             */
+int emugemm_dbg_i8_peak_probe(emugemm_handle_t h, int n_mma, int iters, float *ms, int *ctas);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* EMUGEMM_H_ */

@@ -1,0 +1,240 @@
+"""ctypes binding for libemugemm.so: same names as include/emugemm.h, argument marshalling only.
+
+PyTorch is used for device memory and streams (tensor.data_ptr(), torch.cuda.current_stream());
+every step of the hot path runs in the library's CUDA kernels.  There is no CPU fallback.
+"""
+import ctypes as C
+import os
+import re
+
+LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libemugemm.so")
+_HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "emugemm.h")
+
+OZ1, OZ2, OZ2_3M = 1, 2, 3
+_i64, _int, _dbl, _flt, _vp, _sz = C.c_int64, C.c_int, C.c_double, C.c_float, C.c_void_p, C.c_size_t
+
+
+class EmuGemmError(RuntimeError):
+    def __init__(self, status, msg):
+        super().__init__(f"emugemm status {status}: {msg}")
+        self.status = status
+
+
+_lib = None
+
+
+def load_library():
+    """dlopen the in-tree library; raises (never falls back) if it has not been built."""
+    global _lib
+    if _lib is None:
+        if not os.path.exists(LIB_PATH):
+            raise FileNotFoundError(f"{LIB_PATH} not built: run `python -m paper_2606_25453_b200.build` "
+                                    "(the product path has no CPU fallback)")
+        lib = C.CDLL(LIB_PATH)
+        lib.emugemm_status_string.restype = C.c_char_p
+        lib.emugemm_workspace_bytes.restype = _sz
+        lib.emugemm_workspace_bytes.argtypes = [_int, _int, _i64, _i64, _i64, _int]
+        lib.emugemm_oz1_chunk_k.restype = _i64
+        _lib = lib
+    return _lib
+
+
+def exported_symbols():
+    """Names declared in include/emugemm.h (used by the not-gpu load test)."""
+    text = open(_HEADER).read()
+    return sorted(set(re.findall(r"\b(emugemm_[a-z0-9_]+)\s*\(", text)))
+
+
+def oz2_budget(n_moduli, k, is3m=False):
+    a, b = _int(0), _int(0)
+    T = load_library().emugemm_oz2_budget(_int(n_moduli), _i64(k), _int(1 if is3m else 0), C.byref(a), C.byref(b))
+    return int(T), a.value, b.value
+
+
+def oz1_chunk_k(p):
+    return int(load_library().emugemm_oz1_chunk_k(_int(p)))
+
+
+def _ptr(t):
+    return _vp(t.data_ptr()) if t is not None else _vp(None)
+
+
+class EmuGemm:
+    """One handle (= one host thread, one stream).  Tensors are row-major CUDA tensors; strides are taken
+    from the tensors (last dim contiguous).  Workspace is a torch uint8 tensor owned by this object and
+    grown on demand OUTSIDE the timed hot path via reserve()."""
+
+    def __init__(self):
+        import torch
+        self._torch = torch
+        self._lib = load_library()
+        self._h = _vp(None)
+        self._check(self._lib.emugemm_create(C.byref(self._h)))
+        self._ws = None
+        self.set_stream(torch.cuda.current_stream())
+
+    def close(self):
+        if self._h:
+            self._lib.emugemm_destroy(self._h)
+            self._h = _vp(None)
+
+    def __del__(self):
+        try:
+            self.close()
+        except Exception:
+            pass
+
+    def _check(self, st):
+        if st != 0:
+            raise EmuGemmError(st, self._lib.emugemm_status_string(_int(st)).decode())
+
+    # ---- handle ------------------------------------------------------------
+    def set_stream(self, stream):
+        self._check(self._lib.emugemm_set_stream(self._h, _vp(stream.cuda_stream)))
+
+    def workspace_bytes(self, scheme, elem, m, n, k, pn):
+        return int(self._lib.emugemm_workspace_bytes(scheme, elem, m, n, k, pn))
+
+    def reserve(self, nbytes):
+        torch = self._torch
+        if self._ws is None or self._ws.numel() < nbytes + 1024:
+            self._ws = None
+            raw = torch.empty(int(nbytes) + 2048, dtype=torch.uint8, device="cuda")
+            self._ws = raw
+        off = (-self._ws.data_ptr()) % 1024
+        self._check(self._lib.emugemm_set_workspace(self._h, _vp(self._ws.data_ptr() + off), _sz(self._ws.numel() - off)))
+
+    def _reserve_for(self, scheme, elem, m, n, k, pn):
+        need = self.workspace_bytes(scheme, elem, m, n, k, pn)
+        if self._ws is None or self._ws.numel() - 1024 < need:
+            self.reserve(need)
+
+    def enable_stage_timing(self, on=True):
+        self._check(self._lib.emugemm_enable_stage_timing(self._h, _int(1 if on else 0)))
+
+    def stage_ms(self):
+        ms = (_flt * 3)()
+        n = _int(0)
+        self._check(self._lib.emugemm_stage_ms(self._h, ms, C.byref(n)))
+        return [float(x) for x in ms], n.value
+
+    # ---- compute (names follow include/emugemm.h) --------------------------
+    @staticmethod
+    def _ld(t):
+        assert t.stride(-1) == 1, "row-major tensors with a contiguous last dimension are required"
+        return t.stride(0)
+
+    def dgemm_oz1(self, A, B, C_, p, alpha=1.0, beta=0.0):
+        m, k = A.shape
+        n = B.shape[1]
+        self._reserve_for(OZ1, 8, m, n, k, p)
+        self._check(self._lib.emugemm_dgemm_oz1(self._h, _i64(m), _i64(n), _i64(k), _dbl(alpha), _ptr(A), _i64(self._ld(A)),
+                                                 _ptr(B), _i64(self._ld(B)), _dbl(beta), _ptr(C_), _i64(self._ld(C_)), _int(p)))
+        return C_
+
+    def sgemm_oz1(self, A, B, C_, p, alpha=1.0, beta=0.0):
+        m, k = A.shape
+        n = B.shape[1]
+        self._reserve_for(OZ1, 4, m, n, k, p)
+        self._check(self._lib.emugemm_sgemm_oz1(self._h, _i64(m), _i64(n), _i64(k), _flt(alpha), _ptr(A), _i64(self._ld(A)),
+                                                 _ptr(B), _i64(self._ld(B)), _flt(beta), _ptr(C_), _i64(self._ld(C_)), _int(p)))
+        return C_
+
+    def dgemm_oz2(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0):
+        m, k = A.shape
+        n = B.shape[1]
+        self._reserve_for(OZ2, 8, m, n, k, n_moduli)
+        self._check(self._lib.emugemm_dgemm_oz2(self._h, _i64(m), _i64(n), _i64(k), _dbl(alpha), _ptr(A), _i64(self._ld(A)),
+                                                 _ptr(B), _i64(self._ld(B)), _dbl(beta), _ptr(C_), _i64(self._ld(C_)), _int(n_moduli)))
+        return C_
+
+    def zgemm_oz2_3m(self, A, B, C_, n_moduli, alpha=1.0 + 0j, beta=0j):
+        """A, B, C_: complex128 CUDA tensors."""
+        m, k = A.shape
+        n = B.shape[1]
+        self._reserve_for(OZ2_3M, 16, m, n, k, n_moduli)
+        al = (_dbl * 2)(complex(alpha).real, complex(alpha).imag)
+        be = (_dbl * 2)(complex(beta).real, complex(beta).imag)
+        self._check(self._lib.emugemm_zgemm_oz2_3m(self._h, _i64(m), _i64(n), _i64(k), al, _ptr(A), _i64(self._ld(A)),
+                                                    _ptr(B), _i64(self._ld(B)), be, _ptr(C_), _i64(self._ld(C_)), _int(n_moduli)))
+        return C_
+
+    # ---- test hooks -----------------------------------------------------------
+    def _elem(self, X):
+        torch = self._torch
+        return {torch.float32: 4, torch.float64: 8, torch.complex128: 16}[X.dtype]
+
+    def dbg_exponents(self, X, by_cols):
+        torch = self._torch
+        rows, k = (X.shape[1], X.shape[0]) if by_cols else X.shape
+        self.reserve(max(8 * rows + 4096, 1 << 20))
+        e = torch.empty(rows, dtype=torch.int32, device="cuda")
+        self._check(self._lib.emugemm_dbg_exponents(self._h, _int(self._elem(X)), _int(int(by_cols)), _i64(rows), _i64(k),
+                                                     _ptr(X), _i64(self._ld(X)), _ptr(e)))
+        return e
+
+    def dbg_oz1_slices(self, X, by_cols, p):
+        torch = self._torch
+        rows, k = (X.shape[1], X.shape[0]) if by_cols else X.shape
+        kpad = (k + 127) // 128 * 128
+        self.reserve(8 * rows + p * rows * kpad + (1 << 16))
+        out = torch.empty((p, rows, k), dtype=torch.int8, device="cuda")
+        e = torch.empty(rows, dtype=torch.int32, device="cuda")
+        self._check(self._lib.emugemm_dbg_oz1_slices(self._h, _int(self._elem(X)), _int(int(by_cols)), _i64(rows), _i64(k),
+                                                      _ptr(X), _i64(self._ld(X)), _int(p), _ptr(out), _ptr(e)))
+        return out, e
+
+    def dbg_oz1_accumulators(self, A, B, p, chunk_k=0):
+        torch = self._torch
+        m, k = A.shape
+        n = B.shape[1]
+        self._reserve_for(OZ1, self._elem(A), m, n, k, p)
+        kpad = (k + 127) // 128 * 128
+        ck = chunk_k if chunk_k > 0 else oz1_chunk_k(p)
+        ck = min((ck + 127) // 128 * 128, oz1_chunk_k(p))
+        nch = max(1, -(-kpad // ck))
+        out = torch.empty((nch, p, m, n), dtype=torch.int32, device="cuda")
+        got = _int(0)
+        self._check(self._lib.emugemm_dbg_oz1_accumulators(self._h, _int(self._elem(A)), _i64(m), _i64(n), _i64(k), _ptr(A),
+                                                            _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), _int(p), _i64(chunk_k),
+                                                            _ptr(out), C.byref(got)))
+        assert got.value == nch, (got.value, nch)
+        return out
+
+    def dbg_oz2_residues(self, X, by_cols, n_moduli, t_bits):
+        torch = self._torch
+        rows, k = (X.shape[1], X.shape[0]) if by_cols else X.shape
+        kpad = (k + 127) // 128 * 128
+        parts = 3 if X.dtype == torch.complex128 else 1
+        self.reserve(8 * rows + parts * n_moduli * rows * kpad + (1 << 16))
+        shape = (parts, n_moduli, rows, k) if parts == 3 else (n_moduli, rows, k)
+        out = torch.empty(shape, dtype=torch.int8, device="cuda")
+        e = torch.empty(rows, dtype=torch.int32, device="cuda")
+        self._check(self._lib.emugemm_dbg_oz2_residues(self._h, _int(self._elem(X)), _int(int(by_cols)), _i64(rows), _i64(k),
+                                                        _ptr(X), _i64(self._ld(X)), _int(n_moduli), _int(t_bits), _ptr(out), _ptr(e)))
+        return out, e
+
+    def dbg_oz2_modgemm(self, RA, RB, is3m=False):
+        torch = self._torch
+        N, m, k = RA.shape[-3:]
+        n = RB.shape[-2]
+        kpad = (k + 127) // 128 * 128
+        parts = 3 if is3m else 1
+        self.reserve(parts * N * (m + n) * kpad + (1 << 16))
+        shape = (2, N, m, n) if is3m else (N, m, n)
+        out = torch.empty(shape, dtype=torch.int8, device="cuda")
+        self._check(self._lib.emugemm_dbg_oz2_modgemm(self._h, _int(int(is3m)), _i64(m), _i64(n), _i64(k), _int(N),
+                                                       _ptr(RA.contiguous()), _ptr(RB.contiguous()), _ptr(out)))
+        return out
+
+    def dbg_oz2_crt(self, CR, eA, eB, tA, tB, C_, alpha=1.0, beta=0.0):
+        N, m, n = CR.shape
+        self._check(self._lib.emugemm_dbg_oz2_crt(self._h, _i64(m), _i64(n), _int(N), _ptr(CR), _ptr(eA), _ptr(eB), _int(tA),
+                                                   _int(tB), _dbl(alpha), _dbl(beta), _ptr(C_), _i64(self._ld(C_))))
+        return C_
+
+    def dbg_i8_peak_probe(self, n_mma=256, iters=20000):
+        ms, ctas = _flt(0), _int(0)
+        self._check(self._lib.emugemm_dbg_i8_peak_probe(self._h, _int(n_mma), _int(iters), C.byref(ms), C.byref(ctas)))
+        ops = 2.0 * 128 * n_mma * 32 * iters * ctas.value
+        return ms.value, ops / (ms.value * 1e-3) / 1e12  # ms, Top/s

@@ -1,0 +1,436 @@
+// api.cu -- the C ABI of include/emugemm.h: handle, workspace carving, the
+// per-call stage sequence (pre-pass -> fused tensor-core GEMM -> reconstruction)
+// and the test hooks.  Host code only; every compute step runs in the kernels of
+// prepass.cu / gemm_oz1.cu / gemm_oz2.cu / crt.cu.  There is no CPU fallback.
+#include <cudaTypedefs.h>
+
+#include <new>
+
+#include "common.cuh"
+
+using namespace emu;
+
+namespace emu {
+
+int encode_planes_tmap(emugemm_ctx *ctx, CUtensorMap *tm, const void *base, int64_t kpad, int64_t rows,
+                       int64_t planes, int box_rows, int box_planes) {
+  const cuuint64_t dims[3] = {static_cast<cuuint64_t>(kpad), static_cast<cuuint64_t>(rows),
+                              static_cast<cuuint64_t>(planes)};
+  const cuuint64_t strides[2] = {static_cast<cuuint64_t>(kpad), static_cast<cuuint64_t>(kpad) * static_cast<cuuint64_t>(rows)};
+  const cuuint32_t box[3] = {static_cast<cuuint32_t>(kBlockK), static_cast<cuuint32_t>(box_rows),
+                             static_cast<cuuint32_t>(box_planes)};
+  const cuuint32_t estr[3] = {1, 1, 1};
+  const CUresult r = ctx->encode(tm, CU_TENSOR_MAP_DATA_TYPE_UINT8, 3, const_cast<void *>(base), dims, strides, box, estr,
+                                 CU_TENSOR_MAP_INTERLEAVE_NONE, CU_TENSOR_MAP_SWIZZLE_128B,
+                                 CU_TENSOR_MAP_L2_PROMOTION_L2_256B, CU_TENSOR_MAP_FLOAT_OOB_FILL_NONE);
+  if (r != CUDA_SUCCESS) {
+    ctx->last_cuda = static_cast<int>(r);
+    return EMUGEMM_ERR_CUDA;
+  }
+  return EMUGEMM_OK;
+}
+
+// bump allocator over the caller's workspace (1024-byte granules)
+struct Carver {
+  uint8_t *p;
+  size_t left;
+  bool ok = true;
+  Carver(void *base, size_t bytes) : p(static_cast<uint8_t *>(base)), left(bytes) {}
+  template <typename T>
+  T *take(size_t count) {
+    const size_t bytes = static_cast<size_t>(round_up(static_cast<int64_t>(count * sizeof(T)), 1024));
+    if (bytes > left) { ok = false; return nullptr; }
+    T *r = reinterpret_cast<T *>(p);
+    p += bytes;
+    left -= bytes;
+    return r;
+  }
+};
+static size_t granule(size_t bytes) { return static_cast<size_t>(round_up(static_cast<int64_t>(bytes), 1024)); }
+
+static int oz1_chunks(int p, int64_t kpad, int64_t chunk_override, int64_t *chunk_len) {
+  int64_t c = chunk_override > 0 ? round_up(chunk_override, kBlockK) : oz1_chunk_k_host(p);
+  if (c > oz1_chunk_k_host(p)) c = oz1_chunk_k_host(p);
+  int n = static_cast<int>((kpad + c - 1) / c);
+  if (n < 1) n = 1;
+  // equalise the chunks (same number, balanced length, still <= the safe bound)
+  if (chunk_override <= 0) c = round_up((kpad + n - 1) / n, kBlockK);
+  *chunk_len = c;
+  return n;
+}
+
+static size_t ws_common(int64_t m, int64_t n) {
+  return granule(8 * m) + granule(8 * n) + granule(4 * m) + granule(4 * n);
+}
+
+__global__ void scale_c_kernel(int64_t m, int64_t n, double br, double bi, void *C, int64_t ldc, int elem) {
+  const int64_t idx = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
+  if (idx >= m * n) return;
+  const int64_t i = idx / n, j = idx - i * n;
+  if (elem == 8) {
+    double *o = static_cast<double *>(C) + i * ldc + j;
+    *o = (br == 0.0) ? 0.0 : br * *o;
+  } else if (elem == 4) {
+    float *o = static_cast<float *>(C) + i * ldc + j;
+    *o = (br == 0.0) ? 0.0f : static_cast<float>(br) * *o;
+  } else {
+    double *o = static_cast<double *>(C) + 2 * (i * ldc + j);
+    const double re = o[0], im = o[1];
+    if (br == 0.0 && bi == 0.0) { o[0] = 0.0; o[1] = 0.0; }
+    else { o[0] = br * re - bi * im; o[1] = br * im + bi * re; }
+  }
+}
+
+static int scale_c(emugemm_ctx *h, int64_t m, int64_t n, double br, double bi, void *C, int64_t ldc, int elem) {
+  scale_c_kernel<<<static_cast<unsigned>((m * n + 255) / 256), 256, 0, h->stream>>>(m, n, br, bi, C, ldc, elem);
+  h->launches++;
+  EMU_CUDA(h, cudaGetLastError());
+  return EMUGEMM_OK;
+}
+
+static int mark(emugemm_ctx *h, int i) {
+  if (h->timing) EMU_CUDA(h, cudaEventRecord(h->ev[i], h->stream));
+  return EMUGEMM_OK;
+}
+
+static int check_gemm_args(emugemm_ctx *h, int64_t m, int64_t n, int64_t k, const void *A, int64_t lda, const void *B,
+                           int64_t ldb, const void *C, int64_t ldc) {
+  if (!h) return EMUGEMM_ERR_ARG;
+  if (m < 0 || n < 0 || k < 0) return EMUGEMM_ERR_ARG;
+  if (m == 0 || n == 0) return EMUGEMM_OK;
+  if (!C || ldc < n) return EMUGEMM_ERR_ARG;
+  if (k > 0 && (!A || !B || lda < k || ldb < n)) return EMUGEMM_ERR_ARG;
+  if ((reinterpret_cast<uintptr_t>(A) | reinterpret_cast<uintptr_t>(B) | reinterpret_cast<uintptr_t>(C)) & 15)
+    return EMUGEMM_ERR_ALIGNMENT;
+  if (k >= (1LL << 31) - 256 || m >= (1LL << 31) - 256 || n >= (1LL << 31) - 256) return EMUGEMM_ERR_ARG;
+  return EMUGEMM_OK;
+}
+
+// Scheme I call sequence; out_mode: 0 final, 2 = INT32 dump per chunk into `dump`
+static int run_oz1(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k, double alpha, const void *A, int64_t lda,
+                   const void *B, int64_t ldb, double beta, void *C, int64_t ldc, int p, int32_t *dump,
+                   int64_t chunk_override, int *n_chunks_out) {
+  EMU_TRY(check_gemm_args(h, m, n, k, A, lda, B, ldb, dump ? static_cast<const void *>(dump) : C, dump ? n : ldc));
+  if (p < 1 || p > (elem == kF32 ? 4 : 8)) return EMUGEMM_ERR_ARG;
+  h->launches = 0;
+  if (m == 0 || n == 0) return EMUGEMM_OK;
+  EMU_TRY(mark(h, 0));
+  if (k == 0) {
+    if (!dump) EMU_TRY(scale_c(h, m, n, beta, 0.0, C, ldc, elem));
+    if (n_chunks_out) *n_chunks_out = 0;
+    EMU_TRY(mark(h, 1)); EMU_TRY(mark(h, 2)); EMU_TRY(mark(h, 3));
+    return EMUGEMM_OK;
+  }
+  const int64_t kpad = round_up(k, kBlockK);
+  int64_t clen;
+  const int nch = oz1_chunks(p, kpad, chunk_override, &clen);
+  if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
+  Carver cv(h->ws, h->ws_bytes);
+  auto *mbA = cv.take<unsigned long long>(m);
+  auto *mbB = cv.take<unsigned long long>(n);
+  auto *eA = cv.take<int32_t>(m);
+  auto *eB = cv.take<int32_t>(n);
+  auto *SA = cv.take<int8_t>(static_cast<size_t>(p) * m * kpad);
+  auto *SB = cv.take<int8_t>(static_cast<size_t>(p) * n * kpad);
+  double *part = (nch > 1 && !dump) ? cv.take<double>(static_cast<size_t>(nch) * m * n * 2) : nullptr;
+  if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+
+  EMU_TRY(launch_exponent_scan(h, elem, 0, m, k, A, lda, mbA, eA));
+  EMU_TRY(launch_exponent_scan(h, elem, 1, n, k, B, ldb, mbB, eB));
+  EMU_TRY(launch_oz1_slice(h, elem, 0, m, k, kpad, A, lda, eA, p, SA));
+  EMU_TRY(launch_oz1_slice(h, elem, 1, n, k, kpad, B, ldb, eB, p, SB));
+  EMU_TRY(mark(h, 1));
+
+  Oz1GemmArgs g;
+  g.m = m; g.n = n; g.kpad = kpad; g.p = p; g.SA = SA; g.SB = SB; g.eA = eA; g.eB = eB;
+  g.alpha = alpha; g.beta = beta; g.C = C; g.ldc = ldc;
+  const int final_kind = (elem == kF32) ? 1 : 0;
+  for (int c = 0; c < nch; ++c) {
+    g.k0 = c * clen;
+    g.k1 = (g.k0 + clen < kpad) ? g.k0 + clen : kpad;
+    if (dump) { g.out_kind = 2; g.C = dump + static_cast<int64_t>(c) * p * m * n; }
+    else if (nch == 1) g.out_kind = final_kind;
+    else { g.out_kind = 3; g.C = part + static_cast<int64_t>(c) * m * n * 2; }
+    EMU_TRY(launch_oz1_gemm(h, g));
+  }
+  EMU_TRY(mark(h, 2));
+  if (nch > 1 && !dump) EMU_TRY(launch_oz1_chunk_reduce(h, m, n, nch, part, final_kind, alpha, beta, C, ldc));
+  EMU_TRY(mark(h, 3));
+  if (n_chunks_out) *n_chunks_out = nch;
+  return EMUGEMM_OK;
+}
+
+// Scheme II call sequence (real and 3M)
+static int run_oz2(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_t k, const double alpha[2], const void *A,
+                   int64_t lda, const void *B, int64_t ldb, const double beta[2], double *C, int64_t ldc, int N) {
+  EMU_TRY(check_gemm_args(h, m, n, k, A, lda, B, ldb, C, ldc));
+  if (N < 2 || N > kMaxModuli) return EMUGEMM_ERR_ARG;
+  h->launches = 0;
+  if (m == 0 || n == 0) return EMUGEMM_OK;
+  const int elem = is3m ? kZ128 : kF64;
+  EMU_TRY(mark(h, 0));
+  if (k == 0) {
+    EMU_TRY(scale_c(h, m, n, beta[0], beta[1], C, ldc, elem));
+    EMU_TRY(mark(h, 1)); EMU_TRY(mark(h, 2)); EMU_TRY(mark(h, 3));
+    return EMUGEMM_OK;
+  }
+  int tA, tB;
+  if (oz2_budget_host(N, k, is3m, &tA, &tB) < 2) return EMUGEMM_ERR_PRECISION;
+  if (k > 131071) return EMUGEMM_ERR_PRECISION;  // INT32 accumulation bound k * 128^2 < 2^31 (R7)
+  const int64_t kpad = round_up(k, kBlockK);
+  const int parts_in = is3m ? 3 : 1, parts_out = is3m ? 2 : 1;
+  if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
+  Carver cv(h->ws, h->ws_bytes);
+  auto *mbA = cv.take<unsigned long long>(m);
+  auto *mbB = cv.take<unsigned long long>(n);
+  auto *eA = cv.take<int32_t>(m);
+  auto *eB = cv.take<int32_t>(n);
+  auto *RA = cv.take<int8_t>(static_cast<size_t>(parts_in) * N * m * kpad);
+  auto *RB = cv.take<int8_t>(static_cast<size_t>(parts_in) * N * n * kpad);
+  auto *CR = cv.take<int8_t>(static_cast<size_t>(parts_out) * N * m * n);
+  if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+
+  EMU_TRY(launch_exponent_scan(h, elem, 0, m, k, A, lda, mbA, eA));
+  EMU_TRY(launch_exponent_scan(h, elem, 1, n, k, B, ldb, mbB, eB));
+  EMU_TRY(launch_oz2_residues(h, elem, 0, m, k, kpad, A, lda, eA, N, tA, RA));
+  EMU_TRY(launch_oz2_residues(h, elem, 1, n, k, kpad, B, ldb, eB, N, tB, RB));
+  EMU_TRY(mark(h, 1));
+  Oz2GemmArgs g;
+  g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = N; g.is3m = is3m; g.RA = RA; g.RB = RB; g.CR = CR;
+  EMU_TRY(launch_oz2_gemm(h, g));
+  EMU_TRY(mark(h, 2));
+  Oz2CrtArgs c;
+  c.m = m; c.n = n; c.n_moduli = N; c.CR = CR; c.eA = eA; c.eB = eB; c.tA = tA; c.tB = tB; c.is_complex = is3m;
+  c.alpha[0] = alpha[0]; c.alpha[1] = alpha[1]; c.beta[0] = beta[0]; c.beta[1] = beta[1];
+  c.C = C; c.ldc = ldc;
+  EMU_TRY(launch_oz2_crt(h, c));
+  EMU_TRY(mark(h, 3));
+  return EMUGEMM_OK;
+}
+
+}  // namespace emu
+
+// =============================================================================
+extern "C" {
+#pragma GCC visibility push(default)
+
+int emugemm_create(emugemm_handle_t *out) {
+  if (!out) return EMUGEMM_ERR_ARG;
+  *out = nullptr;
+  int dev = 0;
+  if (cudaGetDevice(&dev) != cudaSuccess) return EMUGEMM_ERR_DEVICE;
+  cudaDeviceProp prop;
+  if (cudaGetDeviceProperties(&prop, dev) != cudaSuccess) return EMUGEMM_ERR_DEVICE;
+  if (prop.major != 10) return EMUGEMM_ERR_DEVICE;  // tcgen05 kind::i8 is sm_100a-only: no fallback
+  emugemm_ctx *h = new (std::nothrow) emugemm_ctx();
+  if (!h) return EMUGEMM_ERR_ARG;
+  h->num_sms = prop.multiProcessorCount;
+  void *fn = nullptr;
+  cudaDriverEntryPointQueryResult qres;
+  if (cudaGetDriverEntryPoint("cuTensorMapEncodeTiled", &fn, cudaEnableDefault, &qres) != cudaSuccess || !fn) {
+    delete h;
+    return EMUGEMM_ERR_DEVICE;
+  }
+  h->encode = reinterpret_cast<PFN_cuTensorMapEncodeTiled_v12000>(fn);
+  for (int i = 0; i < 4; ++i)
+    if (cudaEventCreate(&h->ev[i]) != cudaSuccess) { delete h; return EMUGEMM_ERR_CUDA; }
+  *out = h;
+  return EMUGEMM_OK;
+}
+
+int emugemm_destroy(emugemm_handle_t h) {
+  if (!h) return EMUGEMM_ERR_ARG;
+  for (int i = 0; i < 4; ++i) if (h->ev[i]) cudaEventDestroy(h->ev[i]);
+  delete h;
+  return EMUGEMM_OK;
+}
+
+int emugemm_set_stream(emugemm_handle_t h, void *s) {
+  if (!h) return EMUGEMM_ERR_ARG;
+  h->stream = static_cast<cudaStream_t>(s);
+  return EMUGEMM_OK;
+}
+
+int emugemm_set_workspace(emugemm_handle_t h, void *p, size_t bytes) {
+  if (!h) return EMUGEMM_ERR_ARG;
+  if (reinterpret_cast<uintptr_t>(p) & 1023) return EMUGEMM_ERR_ALIGNMENT;
+  h->ws = p;
+  h->ws_bytes = bytes;
+  return EMUGEMM_OK;
+}
+
+size_t emugemm_workspace_bytes(int scheme, int elem, int64_t m, int64_t n, int64_t k, int pn) {
+  if (m < 0 || n < 0 || k < 0 || pn < 1) return 0;
+  if (m == 0 || n == 0 || k == 0) return 1024;
+  const int64_t kpad = round_up(k, kBlockK);
+  size_t total = ws_common(m, n);
+  if (scheme == EMUGEMM_OZ1) {
+    if (pn > 8 || (elem != 4 && elem != 8)) return 0;
+    total += granule(static_cast<size_t>(pn) * m * kpad) + granule(static_cast<size_t>(pn) * n * kpad);
+    int64_t clen;
+    const int nch = oz1_chunks(pn, kpad, 0, &clen);
+    if (nch > 1) total += granule(static_cast<size_t>(nch) * m * n * 16);
+  } else if (scheme == EMUGEMM_OZ2 || scheme == EMUGEMM_OZ2_3M) {
+    if (pn > kMaxModuli) return 0;
+    const size_t pi = scheme == EMUGEMM_OZ2_3M ? 3 : 1, po = scheme == EMUGEMM_OZ2_3M ? 2 : 1;
+    total += granule(pi * pn * m * kpad) + granule(pi * pn * n * kpad) + granule(po * pn * m * n);
+  } else {
+    return 0;
+  }
+  return total;
+}
+
+const char *emugemm_status_string(int s) {
+  switch (s) {
+    case EMUGEMM_OK: return "ok";
+    case EMUGEMM_ERR_ARG: return "invalid argument";
+    case EMUGEMM_ERR_ALIGNMENT: return "pointer not aligned";
+    case EMUGEMM_ERR_WORKSPACE: return "workspace missing or too small";
+    case EMUGEMM_ERR_PRECISION: return "k too large for this number of moduli";
+    case EMUGEMM_ERR_DEVICE: return "no sm_100 CUDA device";
+    case EMUGEMM_ERR_CUDA: return "CUDA error";
+    default: return "unknown status";
+  }
+}
+
+int emugemm_last_cuda_error(emugemm_handle_t h) { return h ? h->last_cuda : 0; }
+
+int emugemm_dgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,
+                      const double *B, int64_t ldb, double beta, double *C, int64_t ldc, int p) {
+  return run_oz1(h, kF64, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, p, nullptr, 0, nullptr);
+}
+
+int emugemm_sgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda,
+                      const float *B, int64_t ldb, float beta, float *C, int64_t ldc, int p) {
+  return run_oz1(h, kF32, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, p, nullptr, 0, nullptr);
+}
+
+int emugemm_dgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,
+                      const double *B, int64_t ldb, double beta, double *C, int64_t ldc, int n_moduli) {
+  const double al[2] = {alpha, 0.0}, be[2] = {beta, 0.0};
+  return run_oz2(h, 0, m, n, k, al, A, lda, B, ldb, be, C, ldc, n_moduli);
+}
+
+int emugemm_zgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2], const double *A,
+                         int64_t lda, const double *B, int64_t ldb, const double beta[2], double *C, int64_t ldc,
+                         int n_moduli) {
+  if (!alpha || !beta) return EMUGEMM_ERR_ARG;
+  return run_oz2(h, 1, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, n_moduli);
+}
+
+int emugemm_enable_stage_timing(emugemm_handle_t h, int on) {
+  if (!h) return EMUGEMM_ERR_ARG;
+  h->timing = on ? 1 : 0;
+  return EMUGEMM_OK;
+}
+
+int emugemm_stage_ms(emugemm_handle_t h, float ms[3], int *launches) {
+  if (!h || !ms) return EMUGEMM_ERR_ARG;
+  if (!h->timing) return EMUGEMM_ERR_ARG;
+  EMU_CUDA(h, cudaEventSynchronize(h->ev[3]));
+  for (int i = 0; i < 3; ++i) EMU_CUDA(h, cudaEventElapsedTime(&ms[i], h->ev[i], h->ev[i + 1]));
+  if (launches) *launches = h->launches;
+  return EMUGEMM_OK;
+}
+
+// ---- test hooks --------------------------------------------------------------
+static int unpad_planes(emugemm_ctx *h, int8_t *dst, const int8_t *src, int64_t planes_rows, int64_t k, int64_t kpad) {
+  EMU_CUDA(h, cudaMemcpy2DAsync(dst, k, src, kpad, k, planes_rows, cudaMemcpyDeviceToDevice, h->stream));
+  return EMUGEMM_OK;
+}
+
+int emugemm_dbg_exponents(emugemm_handle_t h, int elem, int by_cols, int64_t rows, int64_t k, const void *X, int64_t ldx,
+                          int32_t *e_out) {
+  if (!h || rows < 0 || k < 0 || !e_out) return EMUGEMM_ERR_ARG;
+  if (!h->ws) return EMUGEMM_ERR_WORKSPACE;
+  Carver cv(h->ws, h->ws_bytes);
+  auto *mb = cv.take<unsigned long long>(rows);
+  if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+  return launch_exponent_scan(h, elem, by_cols, rows, k, X, ldx, mb, e_out);
+}
+
+int emugemm_dbg_oz1_slices(emugemm_handle_t h, int elem, int by_cols, int64_t rows, int64_t k, const void *X, int64_t ldx,
+                           int p, int8_t *out, int32_t *e_out) {
+  if (!h || rows <= 0 || k <= 0 || !out || !e_out || p < 1 || p > 8) return EMUGEMM_ERR_ARG;
+  if (!h->ws) return EMUGEMM_ERR_WORKSPACE;
+  const int64_t kpad = round_up(k, kBlockK);
+  Carver cv(h->ws, h->ws_bytes);
+  auto *mb = cv.take<unsigned long long>(rows);
+  auto *S = cv.take<int8_t>(static_cast<size_t>(p) * rows * kpad);
+  if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+  EMU_TRY(launch_exponent_scan(h, elem, by_cols, rows, k, X, ldx, mb, e_out));
+  EMU_TRY(launch_oz1_slice(h, elem, by_cols, rows, k, kpad, X, ldx, e_out, p, S));
+  return unpad_planes(h, out, S, static_cast<int64_t>(p) * rows, k, kpad);
+}
+
+int emugemm_dbg_oz1_accumulators(emugemm_handle_t h, int elem, int64_t m, int64_t n, int64_t k, const void *A, int64_t lda,
+                                 const void *B, int64_t ldb, int p, int64_t chunk_k, int32_t *out, int *n_chunks_out) {
+  if (!out) return EMUGEMM_ERR_ARG;
+  return run_oz1(h, elem, m, n, k, 1.0, A, lda, B, ldb, 0.0, nullptr, n, p, out, chunk_k, n_chunks_out);
+}
+
+int emugemm_dbg_oz2_residues(emugemm_handle_t h, int elem, int by_cols, int64_t rows, int64_t k, const void *X, int64_t ldx,
+                             int n_moduli, int t_bits, int8_t *out, int32_t *e_out) {
+  if (!h || rows <= 0 || k <= 0 || !out || !e_out || n_moduli < 1 || n_moduli > kMaxModuli) return EMUGEMM_ERR_ARG;
+  if (!h->ws) return EMUGEMM_ERR_WORKSPACE;
+  const int64_t kpad = round_up(k, kBlockK);
+  const int parts = (elem == kZ128) ? 3 : 1;
+  Carver cv(h->ws, h->ws_bytes);
+  auto *mb = cv.take<unsigned long long>(rows);
+  auto *R = cv.take<int8_t>(static_cast<size_t>(parts) * n_moduli * rows * kpad);
+  if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+  EMU_TRY(launch_exponent_scan(h, elem, by_cols, rows, k, X, ldx, mb, e_out));
+  EMU_TRY(launch_oz2_residues(h, elem, by_cols, rows, k, kpad, X, ldx, e_out, n_moduli, t_bits, R));
+  return unpad_planes(h, out, R, static_cast<int64_t>(parts) * n_moduli * rows, k, kpad);
+}
+
+int emugemm_dbg_oz2_modgemm(emugemm_handle_t h, int is3m, int64_t m, int64_t n, int64_t k, int n_moduli, const int8_t *RA,
+                            const int8_t *RB, int8_t *out) {
+  if (!h || m <= 0 || n <= 0 || k <= 0 || !RA || !RB || !out || n_moduli < 1 || n_moduli > kMaxModuli) return EMUGEMM_ERR_ARG;
+  if (!h->ws) return EMUGEMM_ERR_WORKSPACE;
+  const int64_t kpad = round_up(k, kBlockK);
+  const int parts = is3m ? 3 : 1;
+  Oz2GemmArgs g;
+  g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = n_moduli; g.is3m = is3m; g.CR = out;
+  if (kpad == k) {
+    g.RA = RA; g.RB = RB;
+  } else {  // canonical planes are unpadded: stage zero-padded copies in the workspace
+    Carver cv(h->ws, h->ws_bytes);
+    auto *PA = cv.take<int8_t>(static_cast<size_t>(parts) * n_moduli * m * kpad);
+    auto *PB = cv.take<int8_t>(static_cast<size_t>(parts) * n_moduli * n * kpad);
+    if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+    EMU_CUDA(h, cudaMemsetAsync(PA, 0, static_cast<size_t>(parts) * n_moduli * m * kpad, h->stream));
+    EMU_CUDA(h, cudaMemsetAsync(PB, 0, static_cast<size_t>(parts) * n_moduli * n * kpad, h->stream));
+    EMU_CUDA(h, cudaMemcpy2DAsync(PA, kpad, RA, k, k, static_cast<size_t>(parts) * n_moduli * m, cudaMemcpyDeviceToDevice, h->stream));
+    EMU_CUDA(h, cudaMemcpy2DAsync(PB, kpad, RB, k, k, static_cast<size_t>(parts) * n_moduli * n, cudaMemcpyDeviceToDevice, h->stream));
+    g.RA = PA; g.RB = PB;
+  }
+  return launch_oz2_gemm(h, g);
+}
+
+int emugemm_dbg_oz2_crt(emugemm_handle_t h, int64_t m, int64_t n, int n_moduli, const int8_t *CR, const int32_t *eA,
+                        const int32_t *eB, int tA, int tB, double alpha, double beta, double *C, int64_t ldc) {
+  if (!h || m <= 0 || n <= 0 || !CR || !eA || !eB || !C || n_moduli < 2 || n_moduli > kMaxModuli) return EMUGEMM_ERR_ARG;
+  Oz2CrtArgs c;
+  c.m = m; c.n = n; c.n_moduli = n_moduli; c.CR = CR; c.eA = eA; c.eB = eB; c.tA = tA; c.tB = tB; c.is_complex = 0;
+  c.alpha[0] = alpha; c.alpha[1] = 0; c.beta[0] = beta; c.beta[1] = 0; c.C = C; c.ldc = ldc;
+  return launch_oz2_crt(h, c);
+}
+
+int emugemm_oz2_budget(int n_moduli, int64_t k, int is3m, int *tA, int *tB) {
+  int a = 0, b = 0;
+  const int T = oz2_budget_host(n_moduli, k, is3m, &a, &b);
+  if (tA) *tA = a;
+  if (tB) *tB = b;
+  return T;
+}
+
+int64_t emugemm_oz1_chunk_k(int p) { return (p >= 1 && p <= 8) ? oz1_chunk_k_host(p) : 0; }
+
+int emugemm_dbg_i8_peak_probe(emugemm_handle_t h, int n_mma, int iters, float *ms, int *ctas) {
+  if (!h || !ms || !ctas) return EMUGEMM_ERR_ARG;
+  return launch_i8_peak_probe(h, n_mma, iters, ms, ctas);
+}
+
+#pragma GCC visibility pop
+}  // extern "C"

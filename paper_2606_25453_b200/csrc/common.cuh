@@ -1,0 +1,120 @@
+// common.cuh -- host-side context, error handling, TMA descriptor encoding and
+// the internal interfaces between the stage drivers (pre-pass, fused GEMMs, CRT).
+#pragma once
+#include <cuda.h>
+#include <cudaTypedefs.h>
+#include <cuda_runtime.h>
+#include <cstddef>
+#include <cstdint>
+
+#include "../../include/emugemm.h"
+
+namespace emu {
+
+constexpr int kBeta = 7;          // bits per signed slice (R1)
+constexpr int kMaxModuli = 20;    // API range of n_moduli
+constexpr int kTileM = 128;       // rows per CTA tile == tcgen05.mma M (PAPER.md:43 t_M = 128 on Blackwell)
+constexpr int kBlockK = 128;      // bytes of k per pipeline block (one 128B swizzle row, 4 MMAs of K = 32)
+
+struct StageTimer;
+
+}  // namespace emu
+
+struct emugemm_ctx {
+  cudaStream_t stream = nullptr;
+  void *ws = nullptr;
+  size_t ws_bytes = 0;
+  int last_cuda = 0;
+  int num_sms = 0;
+  int timing = 0;
+  cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
+  int launches = 0;
+  PFN_cuTensorMapEncodeTiled_v12000 encode = nullptr;
+};
+
+namespace emu {
+
+#define EMU_CUDA(ctx, call)                     \
+  do {                                          \
+    cudaError_t _e = (call);                    \
+    if (_e != cudaSuccess) {                    \
+      (ctx)->last_cuda = static_cast<int>(_e);  \
+      return EMUGEMM_ERR_CUDA;                  \
+    }                                           \
+  } while (0)
+
+#define EMU_TRY(expr)            \
+  do {                           \
+    int _s = (expr);             \
+    if (_s != EMUGEMM_OK) return _s; \
+  } while (0)
+
+inline int64_t round_up(int64_t x, int64_t a) { return (x + a - 1) / a * a; }
+
+// int8 tensor [planes][rows][kpad] (k contiguous), box {kBlockK, box_rows, box_planes},
+// 128-byte swizzle, out-of-bounds rows / planes read as zero.
+int encode_planes_tmap(emugemm_ctx *ctx, CUtensorMap *tm, const void *base, int64_t kpad, int64_t rows,
+                       int64_t planes, int box_rows, int box_planes);
+
+// ---- stage drivers (all asynchronous on ctx->stream) ------------------------
+enum ElemKind { kF32 = 4, kF64 = 8, kZ128 = 16 };
+
+// Max-|x| bit pattern per row (by_cols = 0) or column (by_cols = 1) -> frexp exponent e_out[rows];
+// maxbits is a rows x u64 scratch (zeroed inside).  For kZ128 the exponent covers re and im.
+int launch_exponent_scan(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, const void *X,
+                         int64_t ldx, unsigned long long *maxbits, int32_t *e_out);
+
+// Scheme I slicing: out[p][rows][kpad] int8 (zero padded to kpad), exponents e[rows] (already computed).
+int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
+                     const void *X, int64_t ldx, const int32_t *e, int p, int8_t *out);
+
+// Scheme II residues: elem 8: out[N][rows][kpad]; elem 16: out[3][N][rows][kpad] (re, im, Sigma).
+int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
+                        const void *X, int64_t ldx, const int32_t *e, int n_moduli, int t_bits, int8_t *out);
+
+struct Oz1GemmArgs {
+  int64_t m, n, kpad;          // kpad: padded k of the slice planes (multiple of kBlockK)
+  int64_t k0, k1;              // k-chunk [k0, k1) handled by this launch (multiples of kBlockK)
+  int p;
+  const int8_t *SA, *SB;       // [p][m][kpad], [p][n][kpad]
+  const int32_t *eA, *eB;
+  int out_kind;                // 0: final FP64 C, 1: final FP32 C, 2: INT32 dump [p][m][n], 3: double-double partial [m][n][2]
+  double alpha, beta;
+  void *C;
+  int64_t ldc;
+};
+int launch_oz1_gemm(emugemm_ctx *ctx, const Oz1GemmArgs &a);
+// Sum n_chunks double-double partials part[c][m][n][2] and apply alpha/beta (out_kind 0 / 1 as above).
+int launch_oz1_chunk_reduce(emugemm_ctx *ctx, int64_t m, int64_t n, int n_chunks, const double *part,
+                            int out_kind, double alpha, double beta, void *C, int64_t ldc);
+
+struct Oz2GemmArgs {
+  int64_t m, n, kpad;
+  int n_moduli;
+  int is3m;
+  const int8_t *RA, *RB;       // real: [N][rows][kpad]; 3M: [3][N][rows][kpad]
+  int8_t *CR;                  // real: [N][m][n]; 3M: [2][N][m][n]
+};
+int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &a);
+
+struct Oz2CrtArgs {
+  int64_t m, n;
+  int n_moduli;
+  const int8_t *CR;            // [N][m][n] (3M: second part at CR + N*m*n)
+  const int32_t *eA, *eB;
+  int tA, tB;
+  int is_complex;              // 0: real alpha/beta; 1: complex, C is (re, im) pairs
+  double alpha[2], beta[2];
+  double *C;
+  int64_t ldc;
+};
+int launch_oz2_crt(emugemm_ctx *ctx, const Oz2CrtArgs &a);
+
+int launch_i8_peak_probe(emugemm_ctx *ctx, int n_mma, int iters, float *ms, int *ctas);
+
+// host helpers shared by api.cu and the drivers
+int oz2_moduli_host(int n, int *mod);                  // greedy coprime list, descending from 256
+int oz2_budget_host(int n, int64_t k, int is3m, int *tA, int *tB);
+int64_t oz1_chunk_k_host(int p);
+
+}  // namespace emu

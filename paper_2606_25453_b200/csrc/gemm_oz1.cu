@@ -1,0 +1,411 @@
+// gemm_oz1.cu -- fused Ozaki Scheme I GEMM for sm_100a.
+//
+// What it computes (Eq. 2-3; Alg. 1): for one
+// 128 x NT output tile, the p INT32 accumulators C_s = sum_{t+u=s} A'_t B'_u
+// (s < p, only the p(p+1)/2 pairs with t + u < p), kept in tensor memory for the
+// whole k-chunk, then C = alpha 2^(eA_i+eB_j-7(p+1)) sum_s 2^(7(p-1-s)) C_s + beta C
+// in the epilogue.  INT32 never reaches global memory.
+//
+// B200-first design (differs from the paper's DeepGEMM kernel):
+//  * Operands are slice-major K-major planes [p][rows][kpad]; one 3-D TMA box
+//    brings ALL p slices of a 128-byte k-block of B into shared memory as one
+//    contiguous (p*NT) x 128 B operand, A slices stream through their own ring
+//    (A_t is needed only against B_0..B_{p-1-t}).
+//  * "N-concatenation": the accumulators C_0..C_{p-1} are consecutive NT-column
+//    blocks of TMEM and the B slices are consecutive NT-row blocks of one SMEM
+//    operand, so A_t x [B_0 | ... | B_{p-1-t}] is ONE tcgen05.mma of width
+//    (p-t) NT (split at 256) writing columns [t NT, p NT): exactly the products
+//    A_t B_u -> C_{t+u}.  A_t is read from shared memory once per <= 256 columns
+//    instead of once per product (12 instead of 36 MMAs per k32 at p = 8), which
+//    keeps the SMEM read rate under the 128 B/clk/SM port.
+//  * Warp-specialised persistent CTA: warp 0 = TMA producer, warp 1 = MMA issuer
+//    (one elected thread) + TMEM allocator, warps 2-9 = epilogue.
+#include "common.cuh"
+#include "ptx.cuh"
+#include "gemm_common.cuh"
+
+namespace emu {
+
+
+template <int P>
+struct Oz1Cfg {
+  // NT: tile width; P * NT <= 512 TMEM columns, every MMA width a multiple of 16
+  static constexpr int NT = (P <= 2) ? 256 : (P == 3) ? 160 : (P == 4) ? 128 : (P == 5) ? 96 : (P == 6) ? 80 : 64;
+  static constexpr int kBStageBytes = P * NT * kBlockK;
+  static constexpr int SB = 2;
+  static constexpr int SA = (kSmemLimit - 2048 - SB * kBStageBytes) / kAStageBytes > 8
+                                ? 8
+                                : (kSmemLimit - 2048 - SB * kBStageBytes) / kAStageBytes;
+  static constexpr int kTmemCols = (P * NT <= 256) ? 256 : 512;
+  static constexpr int kSmemBytes = SB * kBStageBytes + SA * kAStageBytes + 1024 /*align*/ + 256 /*barriers*/;
+  static_assert(P * NT <= 512, "TMEM budget");
+  static_assert(kSmemBytes <= kSmemLimit, "SMEM budget");
+  static_assert(SA >= 3, "A ring too shallow");
+};
+
+struct Oz1Dev {
+  int64_t m, n;
+  int kb0, kb1;       // k-blocks [kb0, kb1) of 128
+  int mt, nt_tiles;   // tile grid
+  const int32_t *eA, *eB;
+  int out_kind;
+  double alpha, beta;
+  void *C;
+  int64_t ldc;
+};
+
+__device__ __forceinline__ double pow2d(int e) {  // 2^e for -1022 <= e <= 1023
+  return __hiloint2double((1023 + e) << 20, 0);
+}
+// exact double of x * 2^sh (x int32) without I2F: bit pattern 2^(52+sh) + (x + 2^31) 2^sh, minus that offset
+__device__ __forceinline__ double i32_scaled(uint32_t x, int sh) {
+  const double magic = __hiloint2double((0x433 + sh) << 20, static_cast<int>(x ^ 0x80000000u));
+  const double off = __hiloint2double((0x433 + sh) << 20, 0) + __hiloint2double((0x3FF + 31 + sh) << 20, 0);
+  return magic - off;
+}
+
+template <int P>
+__global__ void __launch_bounds__(kGemmThreads, 1)
+oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const Oz1Dev a) {
+  using Cfg = Oz1Cfg<P>;
+  constexpr int NT = Cfg::NT, SA = Cfg::SA, SB = Cfg::SB;
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  uint8_t *sB = smem;
+  uint8_t *sA = smem + SB * Cfg::kBStageBytes;
+  uint64_t *bars = reinterpret_cast<uint64_t *>(sA + SA * kAStageBytes);
+  uint64_t *bfull = bars, *bempty = bars + SB, *afull = bars + 2 * SB, *aempty = bars + 2 * SB + SA;
+  uint64_t *tfull = bars + 2 * SB + 2 * SA, *tempty = tfull + 1;
+  uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 1);
+
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const int num_tiles = a.mt * a.nt_tiles;
+
+  if (threadIdx.x == 0) {
+    for (int i = 0; i < SB; ++i) { mbar_init(&bfull[i], 1); mbar_init(&bempty[i], 1); }
+    for (int i = 0; i < SA; ++i) { mbar_init(&afull[i], 1); mbar_init(&aempty[i], 1); }
+    mbar_init(tfull, 1);
+    mbar_init(tempty, kEpiWarps);
+    fence_mbar_init();
+    tma_prefetch_desc(&tmA);
+    tma_prefetch_desc(&tmB);
+  }
+  if (warp == 1) {
+    tmem_alloc(tmem_slot, Cfg::kTmemCols);
+    tmem_relinquish();
+  }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tmem_base = *tmem_slot;
+
+  if (warp == 0) {
+    // ===================== TMA producer =====================
+    if (lane == 0) {
+      int sa = 0, sb = 0;
+      uint32_t pa = 0, pb = 0;
+      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+        int mb, nb;
+        tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
+        for (int kb = a.kb0; kb < a.kb1; ++kb) {
+          mbar_wait(&bempty[sb], pb ^ 1);
+          mbar_arrive_expect_tx(&bfull[sb], Cfg::kBStageBytes);
+          tma_load_3d(sB + sb * Cfg::kBStageBytes, &tmB, &bfull[sb], kb * kBlockK, nb * NT, 0);
+          if (++sb == SB) { sb = 0; pb ^= 1; }
+#pragma unroll 1
+          for (int t = 0; t < P; ++t) {
+            mbar_wait(&aempty[sa], pa ^ 1);
+            mbar_arrive_expect_tx(&afull[sa], kAStageBytes);
+            tma_load_3d(sA + sa * kAStageBytes, &tmA, &afull[sa], kb * kBlockK, mb * kTileM, t);
+            if (++sa == SA) { sa = 0; pa ^= 1; }
+          }
+        }
+      }
+    }
+    __syncwarp();
+  } else if (warp == 1) {
+    // ===================== MMA issuer =====================
+    if (lane == 0) {
+      int sa = 0, sb = 0;
+      uint32_t pa = 0, pb = 0, pt = 0;
+      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+        mbar_wait(tempty, pt ^ 1);  // epilogue has drained the accumulators of the previous tile
+        tc_fence_after();
+        for (int kb = a.kb0; kb < a.kb1; ++kb) {
+          mbar_wait(&bfull[sb], pb);
+          const uint32_t b_base = smem_u32(sB + sb * Cfg::kBStageBytes);
+#pragma unroll
+          for (int t = 0; t < P; ++t) {
+            mbar_wait(&afull[sa], pa);
+            tc_fence_after();
+            const uint32_t a_base = smem_u32(sA + sa * kAStageBytes);
+            constexpr int kColsMax = P * NT;
+#pragma unroll
+            for (int ks = 0; ks < kBlockK / 32; ++ks) {
+              const uint64_t adesc = make_sdesc_sw128(a_base + ks * 32);
+#pragma unroll
+              for (int c0 = 0; c0 < kColsMax; c0 += 256) {
+                const int cols = (P - t) * NT;  // A_t x [B_0 | ... | B_{P-1-t}]
+                if (c0 < cols) {
+                  const int nn = (cols - c0 < 256) ? (cols - c0) : 256;
+                  const uint32_t accumulate = (kb != a.kb0 || ks != 0 || t != 0) ? 1u : 0u;
+                  umma_i8(tmem_base + t * NT + c0, adesc, make_sdesc_sw128(b_base + c0 * kBlockK + ks * 32),
+                          make_idesc_i8(kTileM, nn), accumulate);
+                }
+              }
+            }
+            umma_commit(&aempty[sa]);  // slot reusable once these MMAs have read it
+            if (++sa == SA) { sa = 0; pa ^= 1; }
+          }
+          umma_commit(&bempty[sb]);
+          if (++sb == SB) { sb = 0; pb ^= 1; }
+        }
+        umma_commit(tfull);  // accumulators complete
+        pt ^= 1;
+      }
+    }
+    __syncwarp();
+  } else {
+    // ===================== epilogue =====================
+    const int ew = warp - 2;
+    const int quad = warp & 3;     // TMEM lane quadrant this warp may read
+    const int half = ew >> 2;      // column half
+    const int row = quad * 32 + lane;
+    const uint32_t trow = tmem_base + (static_cast<uint32_t>(quad * 32) << 16);
+    uint32_t pt = 0;
+    const bool vec_ok64 = (a.ldc % 4 == 0) && ((reinterpret_cast<uintptr_t>(a.C) & 31) == 0);
+    for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      int mb, nb;
+      tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
+      const int64_t grow = static_cast<int64_t>(mb) * kTileM + row;
+      const bool row_ok = grow < a.m;
+      const int eArow = row_ok ? __ldg(a.eA + grow) - kBeta * (P + 1) : 0;
+      mbar_wait(tfull, pt);
+      tc_fence_after();
+#pragma unroll 1
+      for (int c0 = half * (NT / 2); c0 < (half + 1) * (NT / 2); c0 += 8) {
+        uint32_t v[P][8];
+#pragma unroll
+        for (int s = 0; s < P; ++s) tmem_ld8(trow + s * NT + c0, v[s]);
+        tmem_ld_wait();
+        const int64_t gcol = static_cast<int64_t>(nb) * NT + c0;
+        if (a.out_kind == 2) {  // INT32 accumulator dump [P][m][n] (test hook)
+          if (row_ok) {
+            int32_t *o = static_cast<int32_t *>(a.C);
+#pragma unroll
+            for (int s = 0; s < P; ++s)
+#pragma unroll
+              for (int c = 0; c < 8; ++c)
+                if (gcol + c < a.n) o[(static_cast<int64_t>(s) * a.m + grow) * a.n + gcol + c] = static_cast<int32_t>(v[s][c]);
+          }
+          continue;
+        }
+        double r[8], rlo[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+          // shift-reduce (Eq. 3), least significant accumulator first; every term is exact,
+          // each addition rounds at most 1/2 ulp of a partial sum bounded by (|A'||B'|)_ij
+          double acc = i32_scaled(v[P - 1][c], 0), lo = 0.0;
+          if (a.out_kind != 3) {
+#pragma unroll
+            for (int s = P - 2; s >= 0; --s) acc += i32_scaled(v[s][c], kBeta * (P - 1 - s));
+          } else {  // exact double-double (TwoSum): hi + lo == S exactly (S < 2^82)
+#pragma unroll
+            for (int s = P - 2; s >= 0; --s) {
+              const double t = i32_scaled(v[s][c], kBeta * (P - 1 - s));
+              const double sum = acc + t;
+              const double bb = sum - acc;
+              lo += (acc - (sum - bb)) + (t - bb);
+              acc = sum;
+            }
+          }
+          const int eb = (gcol + c < a.n) ? __ldg(a.eB + gcol + c) : 0;
+          const int E = eArow + eb;  // power-of-two scaling, split so both factors are normal doubles
+          const double d1 = pow2d(E >> 1), d2 = pow2d(E - (E >> 1));
+          r[c] = acc * d1 * d2;
+          rlo[c] = lo * d1 * d2;
+        }
+        if (!row_ok) continue;
+        if (a.out_kind == 3) {  // k-chunk partial as double-double [m][n][2]
+          double *o = static_cast<double *>(a.C) + (grow * a.n + gcol) * 2;
+#pragma unroll
+          for (int c = 0; c < 8; ++c)
+            if (gcol + c < a.n) { o[2 * c] = r[c]; o[2 * c + 1] = rlo[c]; }
+        } else if (a.out_kind == 0) {
+          double *o = static_cast<double *>(a.C) + grow * a.ldc + gcol;
+          const bool full = gcol + 8 <= a.n;
+          if (a.beta != 0.0) {
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+              if (gcol + c < a.n) r[c] = fma(a.alpha, r[c], a.beta * o[c]);
+          } else if (a.alpha != 1.0) {
+#pragma unroll
+            for (int c = 0; c < 8; ++c) r[c] *= a.alpha;
+          }
+          if (full && vec_ok64) {
+            asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(o), "d"(r[0]), "d"(r[1]), "d"(r[2]), "d"(r[3]) : "memory");
+            asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(o + 4), "d"(r[4]), "d"(r[5]), "d"(r[6]), "d"(r[7]) : "memory");
+          } else {
+#pragma unroll
+            for (int c = 0; c < 8; ++c)
+              if (gcol + c < a.n) o[c] = r[c];
+          }
+        } else {  // out_kind 1: FP32 C, one rounding to float
+          float *o = static_cast<float *>(a.C) + grow * a.ldc + gcol;
+#pragma unroll
+          for (int c = 0; c < 8; ++c)
+            if (gcol + c < a.n) {
+              double x = a.alpha * r[c];
+              if (a.beta != 0.0) x = fma(a.beta, static_cast<double>(o[c]), x);
+              o[c] = static_cast<float>(x);
+            }
+        }
+      }
+      // all TMEM reads of this tile are complete (tcgen05.wait::ld above): release the accumulators
+      tc_fence_before();
+      __syncwarp();
+      if (lane == 0) mbar_arrive(tempty);
+      pt ^= 1;
+    }
+  }
+
+  tc_fence_before();
+  __syncthreads();
+  if (warp == 1) tmem_dealloc(tmem_base, Cfg::kTmemCols);
+}
+
+template <int P>
+static int launch_p(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
+  using Cfg = Oz1Cfg<P>;
+  CUtensorMap tmA, tmB;
+  EMU_TRY(encode_planes_tmap(ctx, &tmA, g.SA, g.kpad, g.m, P, kTileM, 1));
+  EMU_TRY(encode_planes_tmap(ctx, &tmB, g.SB, g.kpad, g.n, P, Cfg::NT, P));
+  Oz1Dev d;
+  d.m = g.m; d.n = g.n;
+  d.kb0 = static_cast<int>(g.k0 / kBlockK);
+  d.kb1 = static_cast<int>(g.k1 / kBlockK);
+  d.mt = static_cast<int>((g.m + kTileM - 1) / kTileM);
+  d.nt_tiles = static_cast<int>((g.n + Cfg::NT - 1) / Cfg::NT);
+  d.eA = g.eA; d.eB = g.eB;
+  d.out_kind = g.out_kind; d.alpha = g.alpha; d.beta = g.beta; d.C = g.C; d.ldc = g.ldc;
+  const int tiles = d.mt * d.nt_tiles;
+  const int grid = tiles < ctx->num_sms ? tiles : ctx->num_sms;
+  auto kern = oz1_gemm_kernel<P>;
+  EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
+  kern<<<grid, kGemmThreads, Cfg::kSmemBytes, ctx->stream>>>(tmA, tmB, d);
+  ctx->launches++;
+  EMU_CUDA(ctx, cudaGetLastError());
+  return EMUGEMM_OK;
+}
+
+int launch_oz1_gemm(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
+  if (g.m == 0 || g.n == 0 || g.k1 <= g.k0) return EMUGEMM_OK;
+  switch (g.p) {
+    case 1: return launch_p<1>(ctx, g);
+    case 2: return launch_p<2>(ctx, g);
+    case 3: return launch_p<3>(ctx, g);
+    case 4: return launch_p<4>(ctx, g);
+    case 5: return launch_p<5>(ctx, g);
+    case 6: return launch_p<6>(ctx, g);
+    case 7: return launch_p<7>(ctx, g);
+    case 8: return launch_p<8>(ctx, g);
+    default: return EMUGEMM_ERR_ARG;
+  }
+}
+
+// Overflow-safe k-chunk (R7): the fullest accumulator C_{p-1} sums p products of k_c
+// terms each bounded by 127^2, so p k_c 127^2 <= 2^31 - 1; rounded down to a multiple of 128.
+int64_t oz1_chunk_k_host(int p) {
+  const int64_t bound = 2147483647LL / (static_cast<int64_t>(p) * 127 * 127);
+  return bound / kBlockK * kBlockK;
+}
+
+// ---- k-chunk reduction: C = alpha * sum_c (hi_c + lo_c) + beta C, double-double sum ----
+__global__ void __launch_bounds__(256) oz1_chunk_reduce_kernel(int64_t m, int64_t n, int n_chunks,
+                                                               const double *__restrict__ part, int out_kind,
+                                                               double alpha, double beta, void *C, int64_t ldc) {
+  const int64_t idx = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
+  if (idx >= m * n) return;
+  const int64_t i = idx / n, j = idx - i * n;
+  double hi = 0.0, lo = 0.0;
+  for (int c = 0; c < n_chunks; ++c) {
+    const double2 v = *reinterpret_cast<const double2 *>(part + (static_cast<int64_t>(c) * m * n + idx) * 2);
+    const double sum = hi + v.x;
+    const double bb = sum - hi;
+    lo += (hi - (sum - bb)) + (v.x - bb) + v.y;
+    hi = sum;
+  }
+  const double s = hi + lo;
+  if (out_kind == 0) {
+    double *o = static_cast<double *>(C) + i * ldc + j;
+    *o = (beta != 0.0) ? fma(alpha, s, beta * *o) : alpha * s;
+  } else {
+    float *o = static_cast<float *>(C) + i * ldc + j;
+    double x = alpha * s;
+    if (beta != 0.0) x = fma(beta, static_cast<double>(*o), x);
+    *o = static_cast<float>(x);
+  }
+}
+
+int launch_oz1_chunk_reduce(emugemm_ctx *ctx, int64_t m, int64_t n, int n_chunks, const double *part,
+                            int out_kind, double alpha, double beta, void *C, int64_t ldc) {
+  if (m * n == 0) return EMUGEMM_OK;
+  const unsigned grid = static_cast<unsigned>((m * n + 255) / 256);
+  oz1_chunk_reduce_kernel<<<grid, 256, 0, ctx->stream>>>(m, n, n_chunks, part, out_kind, alpha, beta, C, ldc);
+  ctx->launches++;
+  EMU_CUDA(ctx, cudaGetLastError());
+  return EMUGEMM_OK;
+}
+
+// ---- issue-bound INT8 tensor-core probe (third denominator) ----
+// One CTA per SM; operands are whatever bytes sit in shared memory (zero-filled); no loads in the loop.
+__global__ void __launch_bounds__(128, 1) i8_probe_kernel(int n_mma, int iters) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  __shared__ uint64_t bar;
+  __shared__ uint32_t slot;
+  for (int i = threadIdx.x; i < (16384 + 32768) / 4; i += 128) reinterpret_cast<uint32_t *>(smem)[i] = 0x01010101u;
+  if (threadIdx.x == 0) { mbar_init(&bar, 1); fence_mbar_init(); }
+  fence_proxy_async_smem();
+  if (threadIdx.x < 32) { tmem_alloc(&slot, 512); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tb = slot;
+  if (threadIdx.x == 0) {
+    const uint32_t abase = smem_u32(smem), bbase = smem_u32(smem + 16384);
+    const uint32_t idesc = make_idesc_i8(128, n_mma);
+    for (int it = 0; it < iters; ++it) {
+      // rotate over the two 256-column halves and the four k32 sub-blocks like the real kernel
+      umma_i8(tb + (it & 1) * 256, make_sdesc_sw128(abase + (it & 3) * 32), make_sdesc_sw128(bbase + (it & 3) * 32),
+              idesc, it > 1);
+    }
+    umma_commit(&bar);
+    mbar_wait(&bar, 0);
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (threadIdx.x < 32) tmem_dealloc(tb, 512);
+}
+
+int launch_i8_peak_probe(emugemm_ctx *ctx, int n_mma, int iters, float *ms, int *ctas) {
+  if (n_mma < 16 || n_mma > 256 || n_mma % 16 || iters < 1) return EMUGEMM_ERR_ARG;
+  const int smem = 16384 + 32768 + 1024;
+  EMU_CUDA(ctx, cudaFuncSetAttribute(i8_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  cudaEvent_t e0, e1;
+  EMU_CUDA(ctx, cudaEventCreate(&e0));
+  EMU_CUDA(ctx, cudaEventCreate(&e1));
+  i8_probe_kernel<<<ctx->num_sms, 128, smem, ctx->stream>>>(n_mma, iters / 8 + 1);  // warm-up
+  EMU_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
+  i8_probe_kernel<<<ctx->num_sms, 128, smem, ctx->stream>>>(n_mma, iters);
+  EMU_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
+  EMU_CUDA(ctx, cudaEventSynchronize(e1));
+  EMU_CUDA(ctx, cudaEventElapsedTime(ms, e0, e1));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  *ctas = ctx->num_sms;
+  ctx->launches += 2;
+  return EMUGEMM_OK;
+}
+
+}  // namespace emu

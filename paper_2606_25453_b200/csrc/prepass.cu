@@ -1,0 +1,439 @@
+// prepass.cu -- bandwidth-bound decomposition kernels.
+//
+//  * exponent scan: max |x| bit pattern per row of A / per column of B -> frexp
+//    exponent ("each row of A is scaled by a power-of-two factor";
+//    DESIGN.md R2).
+//  * Scheme I slicing (Eq. 1): p signed 7-bit digits per element,
+//    integer work on the FP bit pattern only (shift / mask / sign).
+//  * Scheme II residues (Eq. 5): a' = trunc(a 2^(t-e)) as a
+//    <= 70-bit integer held in three 32-bit words, a' mod m_l by byte dot products
+//    against (256^j mod m_l) + one multiply-high reduction, symmetric INT8 range.
+//
+// Output layout (library-private): int8 planes
+// [plane][row][kpad], k contiguous, zero padded to kpad (multiple of 128) so the
+// fused GEMMs fetch K-major 128-byte rows with TMA for BOTH operands; operand B
+// (k x n row-major) is therefore transposed on the fly through shared memory.
+#include "common.cuh"
+
+namespace emu {
+
+// ----------------------------------------------------------------------------
+// element decode: |x| = M * 2^ex2 with integer M
+// ----------------------------------------------------------------------------
+__device__ __forceinline__ void decode_bits(double v, unsigned long long &M, int &ex2, bool &neg) {
+  const unsigned long long b = static_cast<unsigned long long>(__double_as_longlong(v));
+  neg = (b >> 63) != 0;
+  const int E = static_cast<int>((b >> 52) & 0x7FF);
+  const unsigned long long frac = b & 0xFFFFFFFFFFFFFull;
+  M = E ? (frac | (1ull << 52)) : frac;
+  ex2 = (E ? E : 1) - 1075;
+}
+__device__ __forceinline__ void decode_bits(float v, unsigned long long &M, int &ex2, bool &neg) {
+  const unsigned int b = __float_as_uint(v);
+  neg = (b >> 31) != 0;
+  const int E = static_cast<int>((b >> 23) & 0xFF);
+  const unsigned int frac = b & 0x7FFFFFu;
+  M = E ? (frac | (1u << 23)) : frac;
+  ex2 = (E ? E : 1) - 150;
+}
+__device__ __forceinline__ unsigned long long abs_bits(double v) {
+  return static_cast<unsigned long long>(__double_as_longlong(v)) & 0x7FFFFFFFFFFFFFFFull;
+}
+__device__ __forceinline__ unsigned long long abs_bits(float v) { return __float_as_uint(v) & 0x7FFFFFFFu; }
+
+// ----------------------------------------------------------------------------
+// exponent scan
+// ----------------------------------------------------------------------------
+template <typename T, int W /* scalars per element: 1 real, 2 complex */>
+__global__ void __launch_bounds__(256) rowmax_kernel(const T *__restrict__ X, int64_t ldx, int64_t k,
+                                                     unsigned long long *__restrict__ maxbits) {
+  const int64_t row = blockIdx.x;
+  const T *src = X + row * ldx * W;
+  unsigned long long mx = 0;
+  for (int64_t h = threadIdx.x; h < k * W; h += 256) {
+    const unsigned long long b = abs_bits(src[h]);
+    mx = b > mx ? b : mx;
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    const unsigned long long y = __shfl_xor_sync(0xffffffffu, mx, o);
+    mx = y > mx ? y : mx;
+  }
+  __shared__ unsigned long long red[8];
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    for (int w = 1; w < 8; ++w) mx = red[w] > mx ? red[w] : mx;
+    maxbits[row] = mx;
+  }
+}
+
+// X is k x rows (ldx), one thread per column, grid.y splits k; atomicMax merges.
+template <typename T, int W>
+__global__ void __launch_bounds__(256) colmax_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows, int64_t k,
+                                                     int64_t kseg, unsigned long long *__restrict__ maxbits) {
+  const int64_t j = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
+  if (j >= rows) return;
+  const int64_t h0 = static_cast<int64_t>(blockIdx.y) * kseg;
+  const int64_t h1 = (h0 + kseg < k) ? h0 + kseg : k;
+  unsigned long long mx = 0;
+#pragma unroll 4
+  for (int64_t h = h0; h < h1; ++h) {
+#pragma unroll
+    for (int c = 0; c < W; ++c) {
+      const unsigned long long b = abs_bits(X[(h * ldx + j) * W + c]);
+      mx = b > mx ? b : mx;
+    }
+  }
+  if (mx) atomicMax(&maxbits[j], mx);
+}
+
+template <typename T>
+__global__ void bits_to_exponent_kernel(const unsigned long long *__restrict__ maxbits, int64_t rows,
+                                        int32_t *__restrict__ e_out) {
+  const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (i >= rows) return;
+  const unsigned long long b = maxbits[i];
+  unsigned long long M;
+  int ex2;
+  bool neg;
+  if (sizeof(T) == 8) decode_bits(__longlong_as_double(static_cast<long long>(b)), M, ex2, neg);
+  else decode_bits(__uint_as_float(static_cast<unsigned int>(b)), M, ex2, neg);
+  e_out[i] = M ? ex2 + (64 - __clzll(static_cast<long long>(M))) : 0;  // frexp exponent; zero row -> 0 (R2)
+}
+
+int launch_exponent_scan(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, const void *X,
+                         int64_t ldx, unsigned long long *maxbits, int32_t *e_out) {
+  if (rows == 0) return EMUGEMM_OK;
+  cudaStream_t st = ctx->stream;
+  EMU_CUDA(ctx, cudaMemsetAsync(maxbits, 0, sizeof(unsigned long long) * rows, st));
+  if (k > 0) {
+    if (!by_cols) {
+      const unsigned grid = static_cast<unsigned>(rows);
+      if (elem == kF64) rowmax_kernel<double, 1><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, k, maxbits);
+      else if (elem == kF32) rowmax_kernel<float, 1><<<grid, 256, 0, st>>>(static_cast<const float *>(X), ldx, k, maxbits);
+      else rowmax_kernel<double, 2><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, k, maxbits);
+    } else {
+      // enough k-segments to fill the machine: ~8 CTAs per SM
+      const int64_t gx = (rows + 255) / 256;
+      int64_t segs = (static_cast<int64_t>(ctx->num_sms) * 8 + gx - 1) / gx;
+      if (segs > (k + 63) / 64) segs = (k + 63) / 64;
+      if (segs < 1) segs = 1;
+      const int64_t kseg = (k + segs - 1) / segs;
+      const dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>((k + kseg - 1) / kseg));
+      if (elem == kF64) colmax_kernel<double, 1><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits);
+      else if (elem == kF32) colmax_kernel<float, 1><<<grid, 256, 0, st>>>(static_cast<const float *>(X), ldx, rows, k, kseg, maxbits);
+      else colmax_kernel<double, 2><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits);
+    }
+    ctx->launches++;
+  }
+  const unsigned g2 = static_cast<unsigned>((rows + 255) / 256);
+  if (elem == kF32) bits_to_exponent_kernel<float><<<g2, 256, 0, st>>>(maxbits, rows, e_out);
+  else bits_to_exponent_kernel<double><<<g2, 256, 0, st>>>(maxbits, rows, e_out);
+  ctx->launches++;
+  EMU_CUDA(ctx, cudaGetLastError());
+  return EMUGEMM_OK;
+}
+
+// ----------------------------------------------------------------------------
+// digitizers.  MODE 0: Scheme I digits, MODE 1: Scheme II residues.
+// ----------------------------------------------------------------------------
+struct Prep {            // one scalar prepared for plane extraction
+  unsigned int w0, w1, w2;  // magnitude: OZ1 X (<= 56 bits) in w0,w1; OZ2 |a'| (<= 70 bits) in w0..w2
+  bool neg;
+};
+
+template <typename T>
+__device__ __forceinline__ Prep prepare(T v, int e_row, int scale_bits /* 7p or t */) {
+  unsigned long long M;
+  int ex2;
+  bool neg;
+  decode_bits(v, M, ex2, neg);
+  const int sh = ex2 + scale_bits - e_row;  // |value| = M * 2^sh, truncated toward zero (R3)
+  unsigned long long lo, hi = 0;
+  if (sh >= 64) {       // only tiny subnormal mantissas reach this: M 2^sh < 2^scale_bits <= 2^96
+    lo = 0ull;
+    hi = M << (sh - 64);
+  } else if (sh >= 0) {
+    lo = M << sh;
+    hi = sh ? (M >> (64 - sh)) : 0ull;
+  } else {
+    lo = (sh > -64) ? (M >> (-sh)) : 0ull;
+  }
+  Prep r;
+  r.w0 = static_cast<unsigned int>(lo);
+  r.w1 = static_cast<unsigned int>(lo >> 32);
+  r.w2 = static_cast<unsigned int>(hi);
+  r.neg = neg;
+  return r;
+}
+
+__device__ __forceinline__ int oz1_digit(const Prep &q, int t, int p) {
+  const unsigned long long X = (static_cast<unsigned long long>(q.w1) << 32) | q.w0;
+  const int d = static_cast<int>((X >> (kBeta * (p - 1 - t))) & 127ull);
+  return q.neg ? -d : d;
+}
+
+// moduli: greedy pairwise-coprime list descending from 256 (R10)
+__device__ __constant__ int c_moduli[24] = {256, 255, 253, 251, 247, 241, 239, 233, 229, 227, 223, 217,
+                                            211, 199, 197, 193, 191, 181, 179, 173, 167, 163, 157, 151};
+constexpr int h_moduli[24] = {256, 255, 253, 251, 247, 241, 239, 233, 229, 227, 223, 217,
+                              211, 199, 197, 193, 191, 181, 179, 173, 167, 163, 157, 151};
+
+__host__ __device__ constexpr unsigned int pow256_mod(int j, int m) {
+  unsigned int r = 1u % static_cast<unsigned int>(m);
+  for (int i = 0; i < j; ++i) r = (r * 256u) % static_cast<unsigned int>(m);
+  return r;
+}
+__host__ __device__ constexpr unsigned int pack_w(int word, int m) {  // bytes 256^(4 word + b) mod m
+  return pow256_mod(4 * word, m) | (pow256_mod(4 * word + 1, m) << 8) | (pow256_mod(4 * word + 2, m) << 16) |
+         (pow256_mod(4 * word + 3, m) << 24);
+}
+__host__ __device__ constexpr unsigned int magic32(int m) {  // ceil(2^32 / m)
+  return static_cast<unsigned int>(((1ull << 32) + static_cast<unsigned long long>(m) - 1ull) /
+                                   static_cast<unsigned long long>(m));
+}
+
+// symmetric residue of sign * (w2:w1:w0) modulo the L-th modulus (L compile-time)
+template <int L>
+__device__ __forceinline__ int oz2_residue(const Prep &q) {
+  constexpr int m = h_moduli[L];
+  constexpr unsigned int c0 = pack_w(0, m), c1 = pack_w(1, m), c2 = pack_w(2, m), mg = magic32(m);
+  unsigned int s = __dp4a(q.w0, c0, 0u);
+  s = __dp4a(q.w1, c1, s);
+  s = __dp4a(q.w2, c2, s);                       // < 12 * 255 * 255 < 2^20, congruent to |a'| mod m
+  const unsigned int qq = __umulhi(s, mg);       // floor(s / m): error s / 2^32 < 2^-12 < 1/m
+  int r = static_cast<int>(s - qq * static_cast<unsigned int>(m));  // [0, m)
+  if (q.neg && r) r = m - r;                     // floored mod of the signed value (R13)
+  if (r >= (m + 1) / 2) r -= m;                  // symmetric range (R11)
+  return r;
+}
+template <int L>
+__device__ __forceinline__ int sym_small(int t) {  // t in (-m, m): re-reduce to the symmetric range (R15)
+  constexpr int m = h_moduli[L];
+  if (t >= (m + 1) / 2) t -= m;
+  else if (t < (m + 1) / 2 - m) t += m;
+  return t;
+}
+
+// ----------------------------------------------------------------------------
+// plane emission.  Each thread owns 4 consecutive k of one row/column ("quad")
+// and emits one packed 32-bit word per plane through `sink(plane, word)`.
+// ----------------------------------------------------------------------------
+__device__ __forceinline__ unsigned int pack4(int a, int b, int c, int d) {
+  return (static_cast<unsigned int>(a) & 0xFFu) | ((static_cast<unsigned int>(b) & 0xFFu) << 8) |
+         ((static_cast<unsigned int>(c) & 0xFFu) << 16) | ((static_cast<unsigned int>(d) & 0xFFu) << 24);
+}
+
+template <typename Sink>
+__device__ __forceinline__ void emit_oz1(const Prep (&q)[4], int p, Sink sink) {
+#pragma unroll
+  for (int t = 0; t < 8; ++t)
+    if (t < p) sink(t, pack4(oz1_digit(q[0], t, p), oz1_digit(q[1], t, p), oz1_digit(q[2], t, p), oz1_digit(q[3], t, p)));
+}
+
+template <int L, typename Sink>
+__device__ __forceinline__ void emit_oz2_real_from(const Prep (&q)[4], int N, Sink sink) {
+  if constexpr (L < kMaxModuli) {
+    if (L < N) {
+      sink(L, pack4(oz2_residue<L>(q[0]), oz2_residue<L>(q[1]), oz2_residue<L>(q[2]), oz2_residue<L>(q[3])));
+      emit_oz2_real_from<L + 1>(q, N, sink);
+    }
+  }
+}
+template <int L, typename Sink>
+__device__ __forceinline__ void emit_oz2_cplx_from(const Prep (&re)[4], const Prep (&im)[4], int N, Sink sink) {
+  if constexpr (L < kMaxModuli) {
+    if (L < N) {
+      int a[4], b[4], s[4];
+#pragma unroll
+      for (int i = 0; i < 4; ++i) {
+        a[i] = oz2_residue<L>(re[i]);
+        b[i] = oz2_residue<L>(im[i]);
+        s[i] = sym_small<L>(a[i] + b[i]);
+      }
+      sink(L, pack4(a[0], a[1], a[2], a[3]));
+      sink(N + L, pack4(b[0], b[1], b[2], b[3]));
+      sink(2 * N + L, pack4(s[0], s[1], s[2], s[3]));
+      emit_oz2_cplx_from<L + 1>(re, im, N, sink);
+    }
+  }
+}
+
+// MODE 0: OZ1 (param = p, scale_bits = 7p); MODE 1: OZ2 (param = N, scale_bits = t)
+template <typename T, int W, int MODE, typename Sink>
+__device__ __forceinline__ void emit_quad(const T (&v)[4][W], int e_row, int param, int scale_bits, Sink sink) {
+  Prep a[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) a[i] = prepare(v[i][0], e_row, scale_bits);
+  if constexpr (MODE == 0) {
+    emit_oz1(a, param, sink);
+  } else if constexpr (W == 1) {
+    emit_oz2_real_from<0>(a, param, sink);
+  } else {
+    Prep b[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) b[i] = prepare(v[i][W - 1], e_row, scale_bits);
+    emit_oz2_cplx_from<0>(a, b, param, sink);
+  }
+}
+
+// ---- rows: X is rows x k (ldx); out[plane][row][kpad]; thread = one quad -----
+template <typename T, int W, int MODE>
+__global__ void __launch_bounds__(256) planes_rows_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows,
+                                                          int64_t k, int64_t kpad, const int32_t *__restrict__ e,
+                                                          int param, int scale_bits, int8_t *__restrict__ out) {
+  const int64_t row = blockIdx.y;
+  const int64_t h0 = (static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x) * 4;
+  if (h0 >= kpad) return;
+  const T *src = X + row * ldx * W;
+  T v[4][W];
+#pragma unroll
+  for (int i = 0; i < 4; ++i)
+#pragma unroll
+    for (int c = 0; c < W; ++c) v[i][c] = (h0 + i < k) ? src[(h0 + i) * W + c] : T(0);
+  const int e_row = e[row];
+  const int64_t plane_stride = rows * kpad;
+  int8_t *dst = out + row * kpad + h0;
+  emit_quad<T, W, MODE>(v, e_row, param, scale_bits, [&](int plane, unsigned int word) {
+    *reinterpret_cast<unsigned int *>(dst + plane * plane_stride) = word;
+  });
+}
+
+// ---- columns: X is k x rows (ldx); transposed through shared memory ----------
+// tile = 32 columns x TH k; thread (lane = column, warp = k-quad index).
+template <typename T, int W, int MODE, int TH>
+__global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows,
+                                                          int64_t k, int64_t kpad, const int32_t *__restrict__ e,
+                                                          int param, int scale_bits, int nplanes,
+                                                          int8_t *__restrict__ out) {
+  extern __shared__ unsigned int tile[];  // [plane][32][TH/4 + 1]
+  constexpr int PW = TH / 4 + 1;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t j = static_cast<int64_t>(blockIdx.x) * 32 + lane;
+  const int64_t hb = static_cast<int64_t>(blockIdx.y) * TH;
+  const int e_row = (j < rows) ? e[j] : 0;
+  for (int hw = warp; hw < TH / 4; hw += 8) {
+    const int64_t h0 = hb + hw * 4;
+    T v[4][W];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int c = 0; c < W; ++c) v[i][c] = (j < rows && h0 + i < k) ? X[((h0 + i) * ldx + j) * W + c] : T(0);
+    emit_quad<T, W, MODE>(v, e_row, param, scale_bits, [&](int plane, unsigned int word) {
+      tile[(plane * 32 + lane) * PW + hw] = word;
+    });
+  }
+  __syncthreads();
+  // write-out: rows of TH bytes, (TH/4) lanes per row
+  constexpr int LPR = TH / 4;          // lanes per row
+  constexpr int RPW = 32 / LPR;        // rows per warp pass
+  const int nrows = nplanes * 32;
+  for (int r = warp * RPW + lane / LPR; r < nrows; r += 8 * RPW) {
+    const int plane = r >> 5, jj = r & 31;
+    const int64_t jg = static_cast<int64_t>(blockIdx.x) * 32 + jj;
+    if (jg < rows) {
+      const int wd = lane % LPR;
+      *reinterpret_cast<unsigned int *>(out + (static_cast<int64_t>(plane) * rows + jg) * kpad + hb + wd * 4) =
+          tile[(plane * 32 + jj) * PW + wd];
+    }
+  }
+}
+
+template <typename T, int W, int MODE>
+static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X,
+                         int64_t ldx, const int32_t *e, int param, int scale_bits, int nplanes, int8_t *out) {
+  if (rows == 0 || kpad == 0) return EMUGEMM_OK;
+  cudaStream_t st = ctx->stream;
+  const T *x = static_cast<const T *>(X);
+  if (!by_cols) {
+    const dim3 grid(static_cast<unsigned>((kpad / 4 + 255) / 256), static_cast<unsigned>(rows));
+    // grid.y is limited to 65535: loop over row blocks
+    for (int64_t r0 = 0; r0 < rows; r0 += 65535) {
+      const int64_t nr = (rows - r0 < 65535) ? rows - r0 : 65535;
+      const dim3 g(grid.x, static_cast<unsigned>(nr));
+      // planes of the sub-block still use the full [rows][kpad] plane stride: pass full `rows`, offset pointers
+      planes_rows_kernel<T, W, MODE><<<g, 256, 0, st>>>(x + r0 * ldx * W, ldx, rows, k, kpad, e + r0, param, scale_bits,
+                                                         out + r0 * kpad);
+      ctx->launches++;
+    }
+  } else {
+    if (nplanes <= 20) {
+      constexpr int TH = 128;
+      const size_t smem = static_cast<size_t>(nplanes) * 32 * (TH / 4 + 1) * 4;
+      auto kern = planes_cols_kernel<T, W, MODE, TH>;
+      EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 20 * 32 * (TH / 4 + 1) * 4));
+      const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH));
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, nplanes, out);
+    } else {
+      constexpr int TH = 32;
+      const size_t smem = static_cast<size_t>(nplanes) * 32 * (TH / 4 + 1) * 4;
+      auto kern = planes_cols_kernel<T, W, MODE, TH>;
+      EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 60 * 32 * (TH / 4 + 1) * 4));
+      const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH));
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, nplanes, out);
+    }
+    ctx->launches++;
+  }
+  EMU_CUDA(ctx, cudaGetLastError());
+  return EMUGEMM_OK;
+}
+
+int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
+                     const void *X, int64_t ldx, const int32_t *e, int p, int8_t *out) {
+  if (elem == kF64) return launch_planes<double, 1, 0>(ctx, by_cols, rows, k, kpad, X, ldx, e, p, kBeta * p, p, out);
+  if (elem == kF32) return launch_planes<float, 1, 0>(ctx, by_cols, rows, k, kpad, X, ldx, e, p, kBeta * p, p, out);
+  return EMUGEMM_ERR_ARG;
+}
+
+int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
+                        const void *X, int64_t ldx, const int32_t *e, int n_moduli, int t_bits, int8_t *out) {
+  if (elem == kF64)
+    return launch_planes<double, 1, 1>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, n_moduli, out);
+  if (elem == kZ128)
+    return launch_planes<double, 2, 1>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, 3 * n_moduli, out);
+  return EMUGEMM_ERR_ARG;
+}
+
+// ---- host helpers -----------------------------------------------------------
+int oz2_moduli_host(int n, int *mod) {
+  if (n < 1 || n > 24) return -1;
+  for (int i = 0; i < n; ++i) mod[i] = h_moduli[i];
+  return 0;
+}
+
+// T = max{T : k 2^(T+guard) <= P}, guard = 2 (real) / 3 (3M) (R12), with P as a
+// 192-bit integer (three 64-bit limbs are enough: P < 2^156 for 20 moduli).
+int oz2_budget_host(int n, int64_t k, int is3m, int *tA, int *tB) {
+  if (n < 2 || n > kMaxModuli || k < 1) return -1;
+  unsigned long long P[3] = {1, 0, 0};
+  for (int l = 0; l < n; ++l) {
+    unsigned __int128 c = 0;
+    for (int i = 0; i < 3; ++i) {
+      c += static_cast<unsigned __int128>(P[i]) * static_cast<unsigned>(h_moduli[l]);
+      P[i] = static_cast<unsigned long long>(c);
+      c >>= 64;
+    }
+  }
+  const int guard = is3m ? 3 : 2;
+  int T = -1;
+  for (int t = 0; t + guard < 190; ++t) {
+    // lhs = k << (t + guard) as 192 bits
+    unsigned long long L[3] = {0, 0, 0};
+    const int sh = t + guard, ws = sh / 64, bs = sh % 64;
+    const unsigned long long kk = static_cast<unsigned long long>(k);
+    if (ws < 3) L[ws] = kk << bs;
+    if (bs && ws + 1 < 3) L[ws + 1] = kk >> (64 - bs);
+    if (bs && ws + 1 >= 3 && (kk >> (64 - bs))) break;  // overflowed 192 bits
+    int cmp = 0;
+    for (int i = 2; i >= 0; --i) {
+      if (L[i] != P[i]) { cmp = L[i] < P[i] ? -1 : 1; break; }
+    }
+    if (cmp <= 0) T = t; else break;
+  }
+  if (T < 0) return -1;
+  *tB = T / 2;
+  *tA = T - T / 2;
+  return T;
+}
+
+}  // namespace emu

@@ -1,0 +1,50 @@
+"""-m "not gpu": the C-ABI library loads and exports every symbol include/emugemm.h declares; host-only
+helpers agree with the oracle; compute calls fail loudly (never fall back) without a GPU."""
+import ctypes
+
+import pytest
+
+import paper_2606_25453_b200 as E
+from oracle import oracle as O
+
+
+def test_library_exports_every_declared_symbol():
+    lib = E.load_library()
+    syms = E.exported_symbols()
+    assert len(syms) >= 20
+    for s in syms:
+        assert hasattr(lib, s), s
+    for must in ("emugemm_dgemm_oz1", "emugemm_sgemm_oz1", "emugemm_dgemm_oz2", "emugemm_zgemm_oz2_3m"):
+        assert must in syms
+
+
+def test_host_helpers_match_oracle():
+    for N in (2, 12, 14, 16, 18, 20):
+        for k in (1, 4096, 8192, 65536):
+            assert E.oz2_budget(N, k) == O.oz2_budget(N, k)
+            assert E.oz2_budget(N, k, True) == O.oz2_budget(N, k, True)
+    # overflow-safe chunk (R7): p k_c 127^2 <= 2^31 - 1, multiple of 128
+    for p in range(1, 9):
+        ck = E.oz1_chunk_k(p)
+        assert ck % 128 == 0 and p * ck * 127 * 127 <= 2 ** 31 - 1 < p * (ck + 128) * 127 * 127
+
+
+def test_no_cpu_fallback_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    lib = E.load_library()
+    h = ctypes.c_void_p()
+    st = lib.emugemm_create(ctypes.byref(h))
+    assert st == -5  # EMUGEMM_ERR_DEVICE: no silent fallback
+    assert lib.emugemm_status_string(st) == b"no sm_100 CUDA device"
+
+
+def test_workspace_bytes_monotone():
+    lib = E.load_library()
+    a = lib.emugemm_workspace_bytes(1, 8, 1024, 1024, 1024, 4)
+    b = lib.emugemm_workspace_bytes(1, 8, 1024, 1024, 1024, 8)
+    c = lib.emugemm_workspace_bytes(2, 8, 1024, 1024, 1024, 16)
+    d = lib.emugemm_workspace_bytes(3, 16, 1024, 1024, 1024, 16)
+    assert 0 < a < b and c > 0 and d > c
+    assert lib.emugemm_workspace_bytes(1, 8, 1024, 1024, 1024, 9) == 0
