@@ -1,0 +1,351 @@
+#!/usr/bin/env python
+"""bench.py -- one JSON line for the EmuGEMM hot path on N B200s (contract: see DESIGN.md "Measurement").
+
+A step = one pass of the whole hot path (pre-pass + fused tensor-core GEMM + reconstruction) =
+one C-ABI call on one batch of synthetic input of the paper's distribution (Eq. 19).
+Default workload: BASELINE.json configs[1] point m=n=k=8192, phi=0.5, seed 1, p=8 (Scheme I DGEMM).
+`value` = emulated FP64 TFLOP/s = 2mnk/t with inputs resident in HBM; `e2e` = the same metric through
+the C-ABI call with HOST (pinned) buffers, H2D/D2H copies inside the timed region.
+N > 1: independent problems per rank (weak scaling), no data-path collective.
+--impl reference times the CPU oracle (deliberately slow) on a bounded sample of the same workload.
+"""
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import tempfile
+import time
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+NOMINAL_INT8_TOPS = 4500.0  # PAPER.md:276, the denominator of the 75 % target
+METRIC = "emulated FP64 TFLOP/s (2mnk/t) & INT8 Top/s as % of B200 dense INT8 peak"
+
+
+def parse():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--warmup", type=int, default=5)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--scheme", default="oz1", choices=["oz1", "oz1s", "oz2", "oz2z"])
+    ap.add_argument("--size", type=int, default=8192, help="m = n = k")
+    ap.add_argument("--m", type=int, default=0)
+    ap.add_argument("--n", type=int, default=0)
+    ap.add_argument("--k", type=int, default=0)
+    ap.add_argument("--p", type=int, default=0, help="slices (oz1) or moduli (oz2); default 8 / 16")
+    ap.add_argument("--phi", type=float, default=-1.0)
+    ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--no-cpu", action="store_true")
+    ap.add_argument("--no-probe", action="store_true")
+    ap.add_argument("--cpu-sample", type=int, default=0, help="rows = cols of the oracle sample")
+    return ap.parse_args()
+
+
+def workload(a):
+    m = a.m or a.size
+    n = a.n or a.size
+    k = a.k or a.size
+    if a.scheme in ("oz1", "oz1s"):
+        p = a.p or (8 if a.scheme == "oz1" else 4)
+        seed, phi = (1, 0.5) if a.scheme == "oz1" else (4, 1.0)
+        ops = p * (p + 1) * m * n * k  # INT8 ops (p(p+1)/2 products of 2mnk)
+        flops = 2.0 * m * n * k
+        name = f"{'OZ1 DGEMM' if a.scheme == 'oz1' else 'OZ1 SGEMM'} m={m} n={n} k={k} p={p}"
+    else:
+        p = a.p or (16 if a.scheme == "oz2" else 14)
+        seed, phi = (2, 1.0) if a.scheme == "oz2" else (3, 1.0)
+        ops = (1 if a.scheme == "oz2" else 3) * p * 2 * m * n * k
+        flops = (2.0 if a.scheme == "oz2" else 8.0) * m * n * k
+        name = f"{'OZ2 DGEMM' if a.scheme == 'oz2' else 'OZ2 ZGEMM-3M'} m={m} n={n} k={k} N={p}"
+    if a.phi >= 0:
+        phi = a.phi
+    return dict(m=m, n=n, k=k, p=p, seed=seed, phi=phi, ops=float(ops), flops=float(flops), name=name)
+
+
+def make_inputs(a, w, seed_offset=0):
+    import numpy as np
+    import emugemm_inputs as G
+    if a.scheme == "oz2z":
+        A, B = G.complex_pair(w["m"], w["n"], w["k"], w["phi"], w["seed"] + seed_offset)
+    else:
+        A, B = G.real_pair(w["m"], w["n"], w["k"], w["phi"], w["seed"] + seed_offset,
+                           dtype=np.float32 if a.scheme == "oz1s" else np.float64)
+    return A, B
+
+
+class ClockSampler:
+    """nvidia-smi clocks line of B200_PROFILING.md, sampled every 200 ms during the timed region."""
+    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+         "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, gpu_index):
+        self.f = tempfile.NamedTemporaryFile("w+", suffix=".csv", delete=False)
+        self.p = None
+        self.idx = gpu_index
+
+    def start(self):
+        try:
+            self.p = subprocess.Popen(["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
+                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+        except OSError:
+            self.p = None
+
+    def stop(self):
+        if self.p is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.05)
+        self.p.terminate()
+        self.p.wait()
+        self.f.flush()
+        rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
+        os.unlink(self.f.name)
+        sm, mx, pw, reasons = [], [], [], set()
+        for r in rows:
+            if len(r) < 9:
+                continue
+            try:
+                sm.append(float(r[1])); mx.append(float(r[2])); pw.append(float(r[3]))
+            except ValueError:
+                continue
+            for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
+                if v.strip().lower() == "active":
+                    reasons.add(name)
+        if not sm:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
+        busy = [s for s in sm if s > 0.5 * max(sm)] or sm
+        return {"sm_mhz": statistics.median(busy), "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
+                "reasons": sorted(reasons)}
+
+
+def cpu_oracle_leg(a, w, sample):
+    """The oracle as it stands, on this box's host cores, on a bounded sample of the same workload:
+    `sample` rows x `sample` columns of the output, full k (every sampled element costs O(k p^2))."""
+    import numpy as np
+    import emugemm_inputs as G
+    from oracle import oracle as O
+    A, B = make_inputs(a, w)
+    rows = G.sample_indices(w["m"], sample, 1)[:sample]
+    cols = G.sample_indices(w["n"], sample, 2)[:sample]
+    t0 = time.perf_counter()
+    if a.scheme == "oz1":
+        O.oz1_sampled(A, B, w["p"], rows, cols)
+    elif a.scheme == "oz1s":
+        O.oz1_sampled(A.astype(np.float64), B.astype(np.float64), w["p"], rows, cols, is_f32=True)
+    elif a.scheme == "oz2":
+        O.oz2_sampled(A, B, w["p"], rows, cols)
+    else:
+        O.oz2_sampled(A, B, w["p"], rows, cols, is3m=True)
+    dt = time.perf_counter() - t0
+    per_out = w["flops"] / (w["m"] * w["n"])
+    val = per_out * len(rows) * len(cols) / dt / 1e12
+    return {"value": val, "unit": "TFLOP/s", "cores": O.threads(), "kind": "oracle", "seconds": dt,
+            "sample": f"{len(rows)} rows x {len(cols)} cols of the {w['name']} output, full k"}
+
+
+def reference_leg(a, w):
+    """--impl reference: the oracle on host cores; each step = a bounded sample of the workload."""
+    sample = a.cpu_sample or 128
+    vals, cb = [], None
+    for _ in range(max(1, min(a.warmup, 1))):
+        cpu_oracle_leg(a, w, min(sample, 32))
+    t_all = time.perf_counter()
+    for _ in range(max(1, a.steps)):
+        cb = cpu_oracle_leg(a, w, sample)
+        vals.append(cb["value"])
+        if time.perf_counter() - t_all > 150:
+            break
+    v = statistics.median(vals)
+    cb["value"] = v
+    line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "TFLOP/s", "n_gpus": a.gpus, "steps": len(vals),
+            "warmup": a.warmup, "ms_per_step": 1e3 * cb["seconds"], "higher_is_better": True, "scaling": "weak",
+            "vs_baseline": None, "dtype": "int8", "data": "synthetic",
+            "config": {"workload": w["name"], "phi": w["phi"], "seed": w["seed"], "note": "CPU oracle, sampled outputs"},
+            "cpu_baseline": cb, "e2e": {"value": v, "unit": "TFLOP/s", "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0},
+            "gpu_launches": 0}
+    print(json.dumps(line))
+
+
+def main():
+    a = parse()
+    w = workload(a)
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local = int(os.environ.get("LOCAL_RANK", "0"))
+
+    if a.impl == "reference":
+        if rank == 0:
+            reference_leg(a, w)
+        return
+
+    import numpy as np
+    import torch
+    import paper_2606_25453_b200 as E
+
+    assert torch.cuda.is_available(), "bench.py needs a GPU: the product path has no CPU fallback"
+    torch.cuda.set_device(local)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local))
+
+    def barrier():
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    # independent problem per rank (weak scaling): same recipe, seed offset by rank
+    A, B = make_inputs(a, w, seed_offset=1000 * rank)
+    cdtype = {"oz1": torch.float64, "oz1s": torch.float32, "oz2": torch.float64, "oz2z": torch.complex128}[a.scheme]
+    hA, hB = torch.from_numpy(A).pin_memory(), torch.from_numpy(B).pin_memory()
+    hC = torch.empty((w["m"], w["n"]), dtype=cdtype).pin_memory()
+    dA, dB = hA.cuda(), hB.cuda()
+    dC = torch.empty((w["m"], w["n"]), dtype=cdtype, device="cuda")
+    h = E.EmuGemm()
+    stream = torch.cuda.current_stream()
+    h.set_stream(stream)
+    call = {"oz1": h.dgemm_oz1, "oz1s": h.sgemm_oz1, "oz2": h.dgemm_oz2, "oz2z": h.zgemm_oz2_3m}[a.scheme]
+
+    def step():
+        call(dA, dB, dC, w["p"])
+
+    def step_e2e():
+        dA.copy_(hA, non_blocking=True)
+        dB.copy_(hB, non_blocking=True)
+        call(dA, dB, dC, w["p"])
+        hC.copy_(dC, non_blocking=True)
+
+    step()  # sizes the workspace outside every timed region
+    torch.cuda.synchronize()
+
+    # ---- device-resident timing: W warm-ups, then exactly K steps between barriers ----
+    for _ in range(max(a.warmup, 3)):
+        step()
+    h.enable_stage_timing(True)
+    sampler = ClockSampler(local)
+    barrier()
+    sampler.start()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    stage = [[], [], []]
+    launches = 0
+    e0.record(stream)
+    for _ in range(a.steps):
+        step()
+        # stage events sit on the same stream; reading them synchronises after the step, before the next launch
+        ms, nl = h.stage_ms()
+        for i in range(3):
+            stage[i].append(ms[i])
+        launches += nl
+    e1.record(stream)
+    barrier()
+    clocks = sampler.stop()
+    total_ms = e0.elapsed_time(e1)
+    h.enable_stage_timing(False)
+
+    # a second pass without the per-step synchronisation gives the back-to-back step time
+    barrier()
+    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    f0.record(stream)
+    for _ in range(a.steps):
+        step()
+    f1.record(stream)
+    barrier()
+    ms_step = f0.elapsed_time(f1) / a.steps
+    t = torch.tensor([ms_step], dtype=torch.float64, device="cuda")
+    if dist is not None:
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    ms_step = float(t.item())
+    value = world * w["flops"] / (ms_step * 1e-3) / 1e12
+
+    # ---- end to end: host (pinned) buffers, H2D + call + D2H inside the timed region ----
+    e2e = None
+    if not a.no_e2e:
+        for _ in range(2):
+            step_e2e()
+        barrier()
+        g0, g1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        n_e2e = max(3, min(a.steps, 10))
+        g0.record(stream)
+        for _ in range(n_e2e):
+            step_e2e()
+        g1.record(stream)
+        barrier()
+        t2 = torch.tensor([g0.elapsed_time(g1) / n_e2e], dtype=torch.float64, device="cuda")
+        if dist is not None:
+            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
+        e2e = {"value": world * w["flops"] / (float(t2.item()) * 1e-3) / 1e12, "unit": "TFLOP/s",
+               "ms_per_step": float(t2.item()),
+               "h2d_bytes_per_step": int(hA.numel() * hA.element_size() + hB.numel() * hB.element_size()),
+               "d2h_bytes_per_step": int(hC.numel() * hC.element_size())}
+
+    if rank != 0:
+        if dist is not None:
+            dist.destroy_process_group()
+        return
+
+    # ---- roofline of the dominant kernel (the fused tensor-core GEMM), measured live ----
+    peaks = {}
+    try:
+        peaks = json.load(open(os.path.join(ROOT, "MEASURED_PEAKS.json")))
+    except (OSError, ValueError):
+        pass
+    bf16_burst = peaks.get("bf16_tflops", 1590.0)
+    peak_src = "measured bf16 burst x2 (guide's nominal int8:bf16 ratio 4.5:2.25)" if peaks else \
+        "fallback 1.59 PF bf16 x2 (guide's nominal int8:bf16 ratio)"
+    gemm_ms = statistics.median(stage[1])
+    achieved = w["ops"] / (gemm_ms * 1e-3) / 1e12
+    peak = 2.0 * bf16_burst
+    traffic = None
+    try:
+        tr = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
+        traffic = tr.get(w["name"])
+    except (OSError, ValueError):
+        pass
+    roof = {"bound": "tensor", "kernel": "oz1_gemm_kernel" if a.scheme.startswith("oz1") else "oz2_gemm_kernel",
+            "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
+            "peak_source": peak_src, "kernel_ms": gemm_ms, "int8_ops_per_launch": w["ops"],
+            "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS}
+    if peaks.get("bf16_tflops_sustained"):
+        roof["frac_of_sustained"] = achieved / (2.0 * peaks["bf16_tflops_sustained"])
+    if clocks.get("sm_mhz"):
+        roof["frac_of_clock_scaled"] = achieved / (148 * 16384 * clocks["sm_mhz"] * 1e6 / 1e12)
+
+    detail = {"stage_ms_median": {"prepass": statistics.median(stage[0]), "gemm": gemm_ms, "recon": statistics.median(stage[2])},
+              "synced_ms_per_step": total_ms / a.steps,
+              "int8_tops_end_to_end": world * w["ops"] / (ms_step * 1e-3) / 1e12}
+    elem = {"oz1": 8, "oz1s": 4, "oz2": 8, "oz2z": 16}[a.scheme]
+    planes = w["p"] * (3 if a.scheme == "oz2z" else 1)
+    kpad = (w["k"] + 127) // 128 * 128
+    pre_bytes = elem * (w["m"] * w["k"] + w["k"] * w["n"]) + planes * kpad * (w["m"] + w["n"])
+    detail["prepass_algorithmic_GBps"] = pre_bytes / (detail["stage_ms_median"]["prepass"] * 1e-3) / 1e9
+    detail["prepass_frac_of_hbm"] = detail["prepass_algorithmic_GBps"] / peaks.get("hbm_gbs", 6650.0)
+    if not a.no_probe:
+        try:
+            _, tops = h.dbg_i8_peak_probe(256, 40000)
+            detail["i8_issue_probe_tops"] = tops
+            roof["frac_of_probe"] = achieved / tops
+        except Exception as ex:  # the probe is context, never the product
+            detail["i8_issue_probe_error"] = str(ex)
+    detail["paper_context"] = "paper: 3654 Top/s (81% of 4500) EmuGEMM-I end-to-end on B200, other machine (PAPER.md:293)"
+
+    line = {"metric": METRIC, "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
+            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "int8", "data": "synthetic",
+            "config": {"workload": w["name"], "phi": w["phi"], "seed": w["seed"], "alpha": 1, "beta": 0,
+                       "l2": "inputs (A, B, slices > 1 GB) exceed the 126 MB L2, no flush needed",
+                       "parallelism": f"{world} independent problems" if world > 1 else "1 GPU"},
+            "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "detail": detail}
+    if not a.no_cpu:
+        line["cpu_baseline"] = cpu_oracle_leg(a, w, a.cpu_sample or 192)
+    print(json.dumps(line))
+    h.close()
+    if dist is not None:
+        dist.destroy_process_group()
+
+
+if __name__ == "__main__":
+    main()
