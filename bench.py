@@ -325,7 +325,8 @@ def main():
     detail["prepass_frac_of_hbm"] = detail["prepass_algorithmic_GBps"] / peaks.get("hbm_gbs", 6650.0)
     if not a.no_probe:
         try:
-            _, tops = h.dbg_i8_peak_probe(256, 40000)
+            _, tops, opc = h.dbg_i8_peak_probe(256, 40000)
+            detail["i8_issue_probe_op_per_clk_sm"] = opc
             detail["i8_issue_probe_tops"] = tops
             roof["frac_of_probe"] = achieved / tops
         except Exception as ex:  # the probe is context, never the product

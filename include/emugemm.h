@@ -99,6 +99,12 @@ int emugemm_zgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, co
  * stage 0 = pre-pass, 1 = tensor-core GEMM kernel(s), 2 = reconstruction, and the
  * number of kernel launches of the last call in *launches (may be NULL).      */
 int emugemm_enable_stage_timing(emugemm_handle_t h, int on);
+/* SM cycles (SM clock domain, so independent of the clock frequency) that CTA 0 of
+ * the fused tensor-core GEMM kernel(s) of the last compute call spent between its
+ * set-up and its exit, summed over the call's GEMM launches; synchronises the
+ * stream.  INT8 ops / (cycles * SM count) is the per-clock tensor efficiency
+ * bench.py reports against 16384 op/clk/SM.  *cycles is a host pointer.        */
+int emugemm_last_gemm_cycles(emugemm_handle_t h, unsigned long long *cycles);
 int emugemm_stage_ms(emugemm_handle_t h, float ms[3], int *launches);
 
 /* ---- test hooks (used only by tests/; canonical layouts, device pointers) -
@@ -138,11 +144,32 @@ int emugemm_dbg_oz2_crt(emugemm_handle_t h, int64_t m, int64_t n, int n_moduli, 
 /* Host-side helpers (no GPU): bit budget (returns T or < 0), overflow-safe chunk length. */
 int emugemm_oz2_budget(int n_moduli, int64_t k, int is3m, int *tA, int *tB);
 int64_t emugemm_oz1_chunk_k(int p);
-/* Issue-bound tcgen05.mma kind::i8 probe (no global loads in the loop): runs
- * `iters` MMAs of 128 x n_mma x 32 per CTA on every SM and returns milliseconds
- * in *ms; ops = 2*128*n_mma*32*iters*ctas.  Used by bench.py for the third
- * INT8 denominator.                                             */
-int emugemm_dbg_i8_peak_probe(emugemm_handle_t h, int n_mma, int iters, float *ms, int *ctas);
+/* Issue-bound tcgen05.mma kind::i8 probe (operands resident in shared memory, no
+ * loads in the loop), one CTA per SM.  ops = HOST array of n_ops (<= 64) MMAs, five
+ * ints each: {TMEM column of D, width N (multiple of 16, <= 256), A slot 0..7
+ * (128 x 128 B tiles), first row of B (rows of 128 B), A collector hint 0 discard /
+ * 1 fill / 2 use / 3 lastuse}; one iteration issues the
+ * whole schedule, `iters` iterations run back to back.  INT8 ops per CTA =
+ * iters * sum_o 2*128*N_o*32.  Returns milliseconds in *ms, the CTA count in *ctas
+ * and (if not NULL) the SM cycles block 0 spent in *cycles (host pointers).  Needs a
+ * workspace of >= 8 bytes.  bench.py uses it for the third INT8 denominator
+ * (SURVEY 8(d)); DESIGN.md quotes its schedule measurements.                  */
+int emugemm_dbg_i8_probe(emugemm_handle_t h, int n_ops, const int *ops, int iters, float *ms, int *ctas,
+                         long long *cycles);
+
+/* The MMA issue code of the fused Scheme I kernel for p slices, run `iters` times
+ * (one iteration = one 128-byte k-block = 4 k32 steps) on operands resident in
+ * shared memory (pseudo-random bytes), one CTA per SM: the tensor-pipe ceiling of
+ * that schedule without TMA traffic.  INT8 ops per CTA = iters * 4 * p(p+1) * 128 *
+ * NT(p) * 32.  use_collector selects the A-operand collector hints.            */
+int emugemm_dbg_oz1_issue_probe(emugemm_handle_t h, int p, int use_collector, int iters, float *ms, int *ctas,
+                                long long *cycles);
+
+/* Timing experiments on the fused kernels (results become WRONG, never set in
+ * production): bit 0 = the TMA producer stops loading once its ring has been filled
+ * once (barrier traffic unchanged), bit 1 = the epilogue skips its TMEM reads, math
+ * and stores.  Used to attribute tensor-pipe idle time.            */
+int emugemm_dbg_set_flags(emugemm_handle_t h, int flags);
 
 #ifdef __cplusplus
 }

@@ -118,6 +118,11 @@ class EmuGemm:
         self._check(self._lib.emugemm_stage_ms(self._h, ms, C.byref(n)))
         return [float(x) for x in ms], n.value
 
+    def last_gemm_cycles(self):
+        c = C.c_ulonglong(0)
+        self._check(self._lib.emugemm_last_gemm_cycles(self._h, C.byref(c)))
+        return int(c.value)
+
     # ---- compute (names follow include/emugemm.h) --------------------------
     @staticmethod
     def _ld(t):
@@ -233,8 +238,29 @@ class EmuGemm:
                                                    _int(tB), _dbl(alpha), _dbl(beta), _ptr(C_), _i64(self._ld(C_))))
         return C_
 
+    def dbg_i8_probe(self, ops, iters=4000):
+        """ops: list of (tmem_col, N, a_slot, b_row[, collector]).  -> (ms, Top/s, INT8 op / clk / SM from the SM cycle counter)."""
+        ops = [tuple(op) + (0,) * (5 - len(op)) for op in ops]
+        if self._ws is None:
+            self.reserve(1 << 20)
+        flat = (C.c_int * (5 * len(ops)))(*[int(x) for op in ops for x in op])
+        ms, ctas, cyc = _flt(0), _int(0), C.c_longlong(0)
+        self._check(self._lib.emugemm_dbg_i8_probe(self._h, _int(len(ops)), flat, _int(iters), C.byref(ms), C.byref(ctas),
+                                                   C.byref(cyc)))
+        per_cta = iters * sum(2.0 * 128 * op[1] * 32 for op in ops)
+        return ms.value, per_cta * ctas.value / (ms.value * 1e-3) / 1e12, per_cta / max(cyc.value, 1)
+
+    def dbg_oz1_issue_probe(self, p, use_collector=True, iters=2000):
+        """-> (ms, Top/s, fraction of 16384 op/clk/SM) of the fused kernel's issue schedule on resident operands."""
+        if self._ws is None:
+            self.reserve(1 << 20)
+        nt = {1: 256, 2: 256, 3: 160, 4: 128, 5: 96, 6: 80, 7: 64, 8: 64}[p]
+        ms, ctas, cyc = _flt(0), _int(0), C.c_longlong(0)
+        self._check(self._lib.emugemm_dbg_oz1_issue_probe(self._h, _int(p), _int(int(use_collector)), _int(iters), C.byref(ms),
+                                                          C.byref(ctas), C.byref(cyc)))
+        per_cta = iters * 4.0 * p * (p + 1) * 128 * nt * 32
+        return ms.value, per_cta * ctas.value / (ms.value * 1e-3) / 1e12, per_cta / max(cyc.value, 1) / 16384.0
+
     def dbg_i8_peak_probe(self, n_mma=256, iters=20000):
-        ms, ctas = _flt(0), _int(0)
-        self._check(self._lib.emugemm_dbg_i8_peak_probe(self._h, _int(n_mma), _int(iters), C.byref(ms), C.byref(ctas)))
-        ops = 2.0 * 128 * n_mma * 32 * iters * ctas.value
-        return ms.value, ops / (ms.value * 1e-3) / 1e12  # ms, Top/s
+        """uniform 128 x n_mma x 32 MMAs alternating between the two 256-column halves of TMEM."""
+        return self.dbg_i8_probe([(0, n_mma, 0, 0), (256, n_mma, 0, 0)], iters // 2)

@@ -60,7 +60,7 @@ static int oz1_chunks(int p, int64_t kpad, int64_t chunk_override, int64_t *chun
 }
 
 static size_t ws_common(int64_t m, int64_t n) {
-  return granule(8 * m) + granule(8 * n) + granule(4 * m) + granule(4 * n);
+  return 1024 /*diagnostics*/ + granule(8 * m) + granule(8 * n) + granule(4 * m) + granule(4 * n);
 }
 
 __global__ void scale_c_kernel(int64_t m, int64_t n, double br, double bi, void *C, int64_t ldc, int elem) {
@@ -126,6 +126,7 @@ static int run_oz1(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k, do
   const int nch = oz1_chunks(p, kpad, chunk_override, &clen);
   if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
   Carver cv(h->ws, h->ws_bytes);
+  auto *diag = cv.take<unsigned long long>(1);
   auto *mbA = cv.take<unsigned long long>(m);
   auto *mbB = cv.take<unsigned long long>(n);
   auto *eA = cv.take<int32_t>(m);
@@ -134,6 +135,8 @@ static int run_oz1(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k, do
   auto *SB = cv.take<int8_t>(static_cast<size_t>(p) * n * kpad);
   double *part = (nch > 1 && !dump) ? cv.take<double>(static_cast<size_t>(nch) * m * n * 2) : nullptr;
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+  h->diag = diag;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
 
   EMU_TRY(launch_exponent_scan(h, elem, 0, m, k, A, lda, mbA, eA));
   EMU_TRY(launch_exponent_scan(h, elem, 1, n, k, B, ldb, mbB, eB));
@@ -143,7 +146,7 @@ static int run_oz1(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k, do
 
   Oz1GemmArgs g;
   g.m = m; g.n = n; g.kpad = kpad; g.p = p; g.SA = SA; g.SB = SB; g.eA = eA; g.eB = eB;
-  g.alpha = alpha; g.beta = beta; g.C = C; g.ldc = ldc;
+  g.alpha = alpha; g.beta = beta; g.C = C; g.ldc = ldc; g.cycles = diag;
   const int final_kind = (elem == kF32) ? 1 : 0;
   for (int c = 0; c < nch; ++c) {
     g.k0 = c * clen;
@@ -181,6 +184,7 @@ static int run_oz2(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_t k, co
   const int parts_in = is3m ? 3 : 1, parts_out = is3m ? 2 : 1;
   if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
   Carver cv(h->ws, h->ws_bytes);
+  auto *diag = cv.take<unsigned long long>(1);
   auto *mbA = cv.take<unsigned long long>(m);
   auto *mbB = cv.take<unsigned long long>(n);
   auto *eA = cv.take<int32_t>(m);
@@ -189,6 +193,8 @@ static int run_oz2(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_t k, co
   auto *RB = cv.take<int8_t>(static_cast<size_t>(parts_in) * N * n * kpad);
   auto *CR = cv.take<int8_t>(static_cast<size_t>(parts_out) * N * m * n);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+  h->diag = diag;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
 
   EMU_TRY(launch_exponent_scan(h, elem, 0, m, k, A, lda, mbA, eA));
   EMU_TRY(launch_exponent_scan(h, elem, 1, n, k, B, ldb, mbB, eB));
@@ -196,7 +202,7 @@ static int run_oz2(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_t k, co
   EMU_TRY(launch_oz2_residues(h, elem, 1, n, k, kpad, B, ldb, eB, N, tB, RB));
   EMU_TRY(mark(h, 1));
   Oz2GemmArgs g;
-  g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = N; g.is3m = is3m; g.RA = RA; g.RB = RB; g.CR = CR;
+  g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = N; g.is3m = is3m; g.RA = RA; g.RB = RB; g.CR = CR; g.cycles = diag;
   EMU_TRY(launch_oz2_gemm(h, g));
   EMU_TRY(mark(h, 2));
   Oz2CrtArgs c;
@@ -318,6 +324,14 @@ int emugemm_zgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, co
   return run_oz2(h, 1, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, n_moduli);
 }
 
+int emugemm_last_gemm_cycles(emugemm_handle_t h, unsigned long long *cycles) {
+  if (!h || !cycles) return EMUGEMM_ERR_ARG;
+  if (!h->diag) return EMUGEMM_ERR_WORKSPACE;
+  EMU_CUDA(h, cudaStreamSynchronize(h->stream));
+  EMU_CUDA(h, cudaMemcpy(cycles, h->diag, sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+  return EMUGEMM_OK;
+}
+
 int emugemm_enable_stage_timing(emugemm_handle_t h, int on) {
   if (!h) return EMUGEMM_ERR_ARG;
   h->timing = on ? 1 : 0;
@@ -391,7 +405,7 @@ int emugemm_dbg_oz2_modgemm(emugemm_handle_t h, int is3m, int64_t m, int64_t n, 
   const int64_t kpad = round_up(k, kBlockK);
   const int parts = is3m ? 3 : 1;
   Oz2GemmArgs g;
-  g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = n_moduli; g.is3m = is3m; g.CR = out;
+  g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = n_moduli; g.is3m = is3m; g.CR = out; g.cycles = nullptr;
   if (kpad == k) {
     g.RA = RA; g.RB = RB;
   } else {  // canonical planes are unpadded: stage zero-padded copies in the workspace
@@ -427,9 +441,22 @@ int emugemm_oz2_budget(int n_moduli, int64_t k, int is3m, int *tA, int *tB) {
 
 int64_t emugemm_oz1_chunk_k(int p) { return (p >= 1 && p <= 8) ? oz1_chunk_k_host(p) : 0; }
 
-int emugemm_dbg_i8_peak_probe(emugemm_handle_t h, int n_mma, int iters, float *ms, int *ctas) {
+int emugemm_dbg_i8_probe(emugemm_handle_t h, int n_ops, const int *ops, int iters, float *ms, int *ctas,
+                         long long *cycles) {
   if (!h || !ms || !ctas) return EMUGEMM_ERR_ARG;
-  return launch_i8_peak_probe(h, n_mma, iters, ms, ctas);
+  return launch_i8_probe(h, n_ops, ops, iters, ms, ctas, cycles);
+}
+
+int emugemm_dbg_oz1_issue_probe(emugemm_handle_t h, int p, int use_collector, int iters, float *ms, int *ctas,
+                                 long long *cycles) {
+  if (!h || !ms || !ctas) return EMUGEMM_ERR_ARG;
+  return launch_oz1_issue_probe(h, p, use_collector, iters, ms, ctas, cycles);
+}
+
+int emugemm_dbg_set_flags(emugemm_handle_t h, int flags) {
+  if (!h) return EMUGEMM_ERR_ARG;
+  h->dbg_flags = flags;
+  return EMUGEMM_OK;
 }
 
 #pragma GCC visibility pop

@@ -29,6 +29,8 @@ struct emugemm_ctx {
   int timing = 0;
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   int launches = 0;
+  int dbg_flags = 0;
+  unsigned long long *diag = nullptr;  // device: [0] = GEMM-kernel SM cycles of the last call (inside the workspace)
   PFN_cuTensorMapEncodeTiled_v12000 encode = nullptr;
 };
 
@@ -82,6 +84,7 @@ struct Oz1GemmArgs {
   double alpha, beta;
   void *C;
   int64_t ldc;
+  unsigned long long *cycles;  // device counter: += SM cycles CTA 0 spent in the kernel (diagnostic), may be null
 };
 int launch_oz1_gemm(emugemm_ctx *ctx, const Oz1GemmArgs &a);
 // Sum n_chunks double-double partials part[c][m][n][2] and apply alpha/beta (out_kind 0 / 1 as above).
@@ -94,6 +97,7 @@ struct Oz2GemmArgs {
   int is3m;
   const int8_t *RA, *RB;       // real: [N][rows][kpad]; 3M: [3][N][rows][kpad]
   int8_t *CR;                  // real: [N][m][n]; 3M: [2][N][m][n]
+  unsigned long long *cycles;  // as in Oz1GemmArgs
 };
 int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &a);
 
@@ -110,7 +114,8 @@ struct Oz2CrtArgs {
 };
 int launch_oz2_crt(emugemm_ctx *ctx, const Oz2CrtArgs &a);
 
-int launch_i8_peak_probe(emugemm_ctx *ctx, int n_mma, int iters, float *ms, int *ctas);
+int launch_oz1_issue_probe(emugemm_ctx *ctx, int p, int coll, int iters, float *ms, int *ctas, long long *cycles);
+int launch_i8_probe(emugemm_ctx *ctx, int n_ops, const int *ops, int iters, float *ms, int *ctas, long long *cycles);
 
 // host helpers shared by api.cu and the drivers
 int oz2_moduli_host(int n, int *mod);                  // greedy coprime list, descending from 256

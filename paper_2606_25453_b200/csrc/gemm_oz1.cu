@@ -27,21 +27,58 @@
 namespace emu {
 
 
+constexpr bool kUseCollector = true;  // A-operand collector reuse across the MMAs of one (t, ks)
+
 template <int P>
 struct Oz1Cfg {
   // NT: tile width; P * NT <= 512 TMEM columns, every MMA width a multiple of 16
   static constexpr int NT = (P <= 2) ? 256 : (P == 3) ? 160 : (P == 4) ? 128 : (P == 5) ? 96 : (P == 6) ? 80 : 64;
   static constexpr int kBStageBytes = P * NT * kBlockK;
   static constexpr int SB = 2;
-  static constexpr int SA = (kSmemLimit - 2048 - SB * kBStageBytes) / kAStageBytes > 8
-                                ? 8
-                                : (kSmemLimit - 2048 - SB * kBStageBytes) / kAStageBytes;
+  // A ring: one stage = the slice PAIR (j, P-1-j) of a k-block (2 x 16 KB).  Pairing the widest with the
+  // narrowest slice gives every stage the same MMA time ((P+1) NT/2 clk per k32), so the single issuing thread
+  // pays one barrier wait + one commit per ~constant amount of tensor work and the MMA queue never drains
+  // on the narrow slices (measured: +11 % tensor-pipe activity over one barrier per slice).
+  static constexpr int NPAIR = (P + 1) / 2;
+  static constexpr int kAPairBytes = 2 * kAStageBytes;
+  static constexpr int SA = (kSmemLimit - 2048 - SB * kBStageBytes) / kAPairBytes > 4
+                                ? 4
+                                : (kSmemLimit - 2048 - SB * kBStageBytes) / kAPairBytes;
   static constexpr int kTmemCols = (P * NT <= 256) ? 256 : 512;
-  static constexpr int kSmemBytes = SB * kBStageBytes + SA * kAStageBytes + 1024 /*align*/ + 256 /*barriers*/;
+  static constexpr int kSmemBytes = SB * kBStageBytes + SA * kAPairBytes + 1024 /*align*/ + 256 /*barriers*/;
   static_assert(P * NT <= 512, "TMEM budget");
   static_assert(kSmemBytes <= kSmemLimit, "SMEM budget");
-  static_assert(SA >= 3, "A ring too shallow");
+  static_assert(SA >= 2, "A ring too shallow");
 };
+
+// MMAs of slice t for one 128-byte k-block: A_t x [B_0 | ... | B_{P-1-t}] -> TMEM columns [t NT, P NT), split at 256
+// columns, four k32 sub-blocks.  `accumulate` = false only for the very first MMAs of a tile (t = 0, ks = 0).
+template <int P, bool COLL>
+__device__ __forceinline__ void oz1_issue_slice(int t, uint32_t tmem_base, uint32_t a_base, uint32_t b_base, bool accumulate) {
+  constexpr int NT = Oz1Cfg<P>::NT;
+  constexpr int kColsMax = P * NT;
+#pragma unroll
+  for (int ks = 0; ks < kBlockK / 32; ++ks) {
+    const uint64_t adesc = make_sdesc_sw128(a_base + ks * 32);
+#pragma unroll
+    for (int c0 = 0; c0 < kColsMax; c0 += 256) {
+      const int cols = (P - t) * NT;
+      if (c0 < cols) {
+        const int nn = (cols - c0 < 256) ? (cols - c0) : 256;
+        const uint32_t acc = (accumulate || ks != 0) ? 1u : 0u;
+        const uint32_t d = tmem_base + t * NT + c0;
+        const uint64_t bdesc = make_sdesc_sw128(b_base + c0 * kBlockK + ks * 32);
+        const uint32_t idesc = make_idesc_i8(kTileM, nn);
+        // the <= 2 MMAs of one (t, ks) share A_t: the first keeps it in the collector, the last drops it
+        const bool first = (c0 == 0), last = (c0 + 256 >= cols);
+        if (COLL && first && !last) umma_i8<1>(d, adesc, bdesc, idesc, acc);
+        else if (COLL && !first && last) umma_i8<3>(d, adesc, bdesc, idesc, acc);
+        else if (COLL && !first && !last) umma_i8<2>(d, adesc, bdesc, idesc, acc);
+        else umma_i8<0>(d, adesc, bdesc, idesc, acc);
+      }
+    }
+  }
+}
 
 struct Oz1Dev {
   int64_t m, n;
@@ -52,6 +89,8 @@ struct Oz1Dev {
   double alpha, beta;
   void *C;
   int64_t ldc;
+  unsigned long long *cycles;
+  int dbg;  // experiment flags (emugemm_dbg_set_flags): 1 = no TMA after the ring is first filled, 2 = no epilogue math
 };
 
 __device__ __forceinline__ double pow2d(int e) {  // 2^e for -1022 <= e <= 1023
@@ -73,7 +112,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint8_t *sB = smem;
   uint8_t *sA = smem + SB * Cfg::kBStageBytes;
-  uint64_t *bars = reinterpret_cast<uint64_t *>(sA + SA * kAStageBytes);
+  uint64_t *bars = reinterpret_cast<uint64_t *>(sA + SA * Cfg::kAPairBytes);
   uint64_t *bfull = bars, *bempty = bars + SB, *afull = bars + 2 * SB, *aempty = bars + 2 * SB + SA;
   uint64_t *tfull = bars + 2 * SB + 2 * SA, *tempty = tfull + 1;
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 1);
@@ -98,25 +137,37 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  const long long t_start = clock64();
 
   if (warp == 0) {
     // ===================== TMA producer =====================
     if (lane == 0) {
-      int sa = 0, sb = 0;
+      int sa = 0, sb = 0, nloada = 0, nloadb = 0;
       uint32_t pa = 0, pb = 0;
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
         int mb, nb;
         tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
         for (int kb = a.kb0; kb < a.kb1; ++kb) {
           mbar_wait(&bempty[sb], pb ^ 1);
+          if ((a.dbg & 1) && nloadb >= SB) mbar_arrive(&bfull[sb]);
+          else {
           mbar_arrive_expect_tx(&bfull[sb], Cfg::kBStageBytes);
           tma_load_3d(sB + sb * Cfg::kBStageBytes, &tmB, &bfull[sb], kb * kBlockK, nb * NT, 0);
+          }
+          ++nloadb;
           if (++sb == SB) { sb = 0; pb ^= 1; }
 #pragma unroll 1
-          for (int t = 0; t < P; ++t) {
+          for (int j = 0; j < Cfg::NPAIR; ++j) {
+            const int lo = j, hi = P - 1 - j;
             mbar_wait(&aempty[sa], pa ^ 1);
-            mbar_arrive_expect_tx(&afull[sa], kAStageBytes);
-            tma_load_3d(sA + sa * kAStageBytes, &tmA, &afull[sa], kb * kBlockK, mb * kTileM, t);
+            if ((a.dbg & 1) && nloada >= SA) mbar_arrive(&afull[sa]);
+            else {
+              uint8_t *dst = sA + sa * Cfg::kAPairBytes;
+              mbar_arrive_expect_tx(&afull[sa], lo == hi ? kAStageBytes : Cfg::kAPairBytes);
+              tma_load_3d(dst, &tmA, &afull[sa], kb * kBlockK, mb * kTileM, lo);
+              if (hi != lo) tma_load_3d(dst + kAStageBytes, &tmA, &afull[sa], kb * kBlockK, mb * kTileM, hi);
+            }
+            ++nloada;
             if (++sa == SA) { sa = 0; pa ^= 1; }
           }
         }
@@ -128,37 +179,33 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (lane == 0) {
       int sa = 0, sb = 0;
       uint32_t pa = 0, pb = 0, pt = 0;
+      // look-ahead: the barrier of the NEXT stage is probed (non-blocking) before the MMAs of the current stage are
+      // issued, so the ~90-cycle try_wait latency overlaps tensor work instead of draining the MMA queue
+      bool a_ready = false, b_ready = false;
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
         mbar_wait(tempty, pt ^ 1);  // epilogue has drained the accumulators of the previous tile
         tc_fence_after();
         for (int kb = a.kb0; kb < a.kb1; ++kb) {
-          mbar_wait(&bfull[sb], pb);
+          if (!b_ready) mbar_wait(&bfull[sb], pb);
           const uint32_t b_base = smem_u32(sB + sb * Cfg::kBStageBytes);
+          const int sb_next = (sb + 1 == SB) ? 0 : sb + 1;
+          const uint32_t pb_next = (sb + 1 == SB) ? pb ^ 1 : pb;
 #pragma unroll
-          for (int t = 0; t < P; ++t) {
-            mbar_wait(&afull[sa], pa);
+          for (int j = 0; j < Cfg::NPAIR; ++j) {
+            const int lo = j, hi = P - 1 - j;
+            if (!a_ready) mbar_wait(&afull[sa], pa);
             tc_fence_after();
-            const uint32_t a_base = smem_u32(sA + sa * kAStageBytes);
-            constexpr int kColsMax = P * NT;
-#pragma unroll
-            for (int ks = 0; ks < kBlockK / 32; ++ks) {
-              const uint64_t adesc = make_sdesc_sw128(a_base + ks * 32);
-#pragma unroll
-              for (int c0 = 0; c0 < kColsMax; c0 += 256) {
-                const int cols = (P - t) * NT;  // A_t x [B_0 | ... | B_{P-1-t}]
-                if (c0 < cols) {
-                  const int nn = (cols - c0 < 256) ? (cols - c0) : 256;
-                  const uint32_t accumulate = (kb != a.kb0 || ks != 0 || t != 0) ? 1u : 0u;
-                  umma_i8(tmem_base + t * NT + c0, adesc, make_sdesc_sw128(b_base + c0 * kBlockK + ks * 32),
-                          make_idesc_i8(kTileM, nn), accumulate);
-                }
-              }
-            }
-            umma_commit(&aempty[sa]);  // slot reusable once these MMAs have read it
+            const uint32_t a_base = smem_u32(sA + sa * Cfg::kAPairBytes);
+            const int sa_cur = sa;
             if (++sa == SA) { sa = 0; pa ^= 1; }
+            a_ready = mbar_try_wait(&afull[sa], pa);
+            if (j == Cfg::NPAIR - 1) b_ready = mbar_try_wait(&bfull[sb_next], pb_next);
+            oz1_issue_slice<P, kUseCollector>(lo, tmem_base, a_base, b_base, kb != a.kb0 || lo != 0);
+            if (hi != lo) oz1_issue_slice<P, kUseCollector>(hi, tmem_base, a_base + kAStageBytes, b_base, true);
+            umma_commit(&aempty[sa_cur]);  // stage reusable once these MMAs have read it
           }
           umma_commit(&bempty[sb]);
-          if (++sb == SB) { sb = 0; pb ^= 1; }
+          sb = sb_next; pb = pb_next;
         }
         umma_commit(tfull);  // accumulators complete
         pt ^= 1;
@@ -183,7 +230,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       mbar_wait(tfull, pt);
       tc_fence_after();
 #pragma unroll 1
-      for (int c0 = half * (NT / 2); c0 < (half + 1) * (NT / 2); c0 += 8) {
+      for (int c0 = (a.dbg & 2) ? NT : half * (NT / 2); c0 < (half + 1) * (NT / 2); c0 += 8) {
         uint32_t v[P][8];
 #pragma unroll
         for (int s = 0; s < P; ++s) tmem_ld8(trow + s * NT + c0, v[s]);
@@ -272,6 +319,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   tc_fence_before();
   __syncthreads();
   if (warp == 1) tmem_dealloc(tmem_base, Cfg::kTmemCols);
+  if (blockIdx.x == 0 && threadIdx.x == 0 && a.cycles) atomicAdd(a.cycles, static_cast<unsigned long long>(clock64() - t_start));
 }
 
 template <int P>
@@ -288,6 +336,8 @@ static int launch_p(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   d.nt_tiles = static_cast<int>((g.n + Cfg::NT - 1) / Cfg::NT);
   d.eA = g.eA; d.eB = g.eB;
   d.out_kind = g.out_kind; d.alpha = g.alpha; d.beta = g.beta; d.C = g.C; d.ldc = g.ldc;
+  d.cycles = g.cycles;
+  d.dbg = ctx->dbg_flags;
   const int tiles = d.mt * d.nt_tiles;
   const int grid = tiles < ctx->num_sms ? tiles : ctx->num_sms;
   auto kern = oz1_gemm_kernel<P>;
@@ -358,13 +408,25 @@ int launch_oz1_chunk_reduce(emugemm_ctx *ctx, int64_t m, int64_t n, int n_chunks
 }
 
 // ---- issue-bound INT8 tensor-core probe (third denominator) ----
-// One CTA per SM; operands are whatever bytes sit in shared memory (zero-filled); no loads in the loop.
-__global__ void __launch_bounds__(128, 1) i8_probe_kernel(int n_mma, int iters) {
+// One CTA per SM; operands are whatever bytes sit in shared memory; no loads in the loop.  The host passes a
+// schedule of up to 64 MMAs (TMEM column, width N, A slot, B row offset); one "iteration" issues the whole
+// schedule once, the k32 sub-block rotating with the iteration like the real kernels.
+// cycles_out[0] = SM cycles block 0 spent between the first issue and the completion of the last MMA.
+struct ProbeSched {
+  int n_ops;
+  uint16_t col[64], n[64], aslot[64], brow[64], coll[64];
+};
+__global__ void __launch_bounds__(128, 1) i8_probe_kernel(const ProbeSched sc, int iters, long long *cycles_out) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   __shared__ uint64_t bar;
   __shared__ uint32_t slot;
-  for (int i = threadIdx.x; i < (16384 + 32768) / 4; i += 128) reinterpret_cast<uint32_t *>(smem)[i] = 0x01010101u;
+  // pseudo-random operand bytes: the multiplier arrays toggle like on real slices (power-realistic)
+  for (int i = threadIdx.x; i < (8 * 16384 + 65536) / 4; i += 128) {
+    uint32_t x = static_cast<uint32_t>(i) * 2654435761u + blockIdx.x * 40503u;
+    x ^= x >> 15; x *= 2246822519u; x ^= x >> 13;
+    reinterpret_cast<uint32_t *>(smem)[i] = x;
+  }
   if (threadIdx.x == 0) { mbar_init(&bar, 1); fence_mbar_init(); }
   fence_proxy_async_smem();
   if (threadIdx.x < 32) { tmem_alloc(&slot, 512); tmem_relinquish(); }
@@ -373,39 +435,132 @@ __global__ void __launch_bounds__(128, 1) i8_probe_kernel(int n_mma, int iters) 
   tc_fence_after();
   const uint32_t tb = slot;
   if (threadIdx.x == 0) {
-    const uint32_t abase = smem_u32(smem), bbase = smem_u32(smem + 16384);
-    const uint32_t idesc = make_idesc_i8(128, n_mma);
+    const uint32_t abase = smem_u32(smem), bbase = smem_u32(smem + 8 * 16384);
+    const long long t0 = clock64();
     for (int it = 0; it < iters; ++it) {
-      // rotate over the two 256-column halves and the four k32 sub-blocks like the real kernel
-      umma_i8(tb + (it & 1) * 256, make_sdesc_sw128(abase + (it & 3) * 32), make_sdesc_sw128(bbase + (it & 3) * 32),
-              idesc, it > 1);
+      const int ks = it & 3;
+      for (int o = 0; o < sc.n_ops; ++o) {
+        const uint32_t d = tb + sc.col[o], idesc = make_idesc_i8(128, sc.n[o]);
+        const uint64_t ad = make_sdesc_sw128(abase + sc.aslot[o] * 16384 + ks * 32);
+        const uint64_t bd = make_sdesc_sw128(bbase + sc.brow[o] * kBlockK + ks * 32);
+        switch (sc.coll[o]) {
+          case 1: umma_i8<1>(d, ad, bd, idesc, it > 0); break;
+          case 2: umma_i8<2>(d, ad, bd, idesc, it > 0); break;
+          case 3: umma_i8<3>(d, ad, bd, idesc, it > 0); break;
+          default: umma_i8<0>(d, ad, bd, idesc, it > 0); break;
+        }
+      }
     }
     umma_commit(&bar);
     mbar_wait(&bar, 0);
+    if (blockIdx.x == 0 && cycles_out) *cycles_out = clock64() - t0;
   }
   tc_fence_before();
   __syncthreads();
   if (threadIdx.x < 32) tmem_dealloc(tb, 512);
 }
 
-int launch_i8_peak_probe(emugemm_ctx *ctx, int n_mma, int iters, float *ms, int *ctas) {
-  if (n_mma < 16 || n_mma > 256 || n_mma % 16 || iters < 1) return EMUGEMM_ERR_ARG;
-  const int smem = 16384 + 32768 + 1024;
+int launch_i8_probe(emugemm_ctx *ctx, int n_ops, const int *ops, int iters, float *ms, int *ctas, long long *cycles) {
+  if (iters < 1 || n_ops < 1 || n_ops > 64 || !ops) return EMUGEMM_ERR_ARG;
+  ProbeSched sc;
+  sc.n_ops = n_ops;
+  for (int o = 0; o < n_ops; ++o) {
+    const int col = ops[5 * o], n = ops[5 * o + 1], as = ops[5 * o + 2], br = ops[5 * o + 3], cl = ops[5 * o + 4];
+    if (n < 16 || n > 256 || n % 16 || col < 0 || col + n > 512 || as < 0 || as > 7 || br < 0 || br + n > 512 || cl < 0 || cl > 3) return EMUGEMM_ERR_ARG;
+    sc.col[o] = col; sc.n[o] = n; sc.aslot[o] = as; sc.brow[o] = br; sc.coll[o] = cl;
+  }
+  if (!ctx->ws || ctx->ws_bytes < 8) return EMUGEMM_ERR_WORKSPACE;
+  const int smem = 8 * 16384 + 65536 + 1024;
   EMU_CUDA(ctx, cudaFuncSetAttribute(i8_probe_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   cudaEvent_t e0, e1;
   EMU_CUDA(ctx, cudaEventCreate(&e0));
   EMU_CUDA(ctx, cudaEventCreate(&e1));
-  i8_probe_kernel<<<ctx->num_sms, 128, smem, ctx->stream>>>(n_mma, iters / 8 + 1);  // warm-up
+  long long *dcyc = static_cast<long long *>(ctx->ws);
+  i8_probe_kernel<<<ctx->num_sms, 128, smem, ctx->stream>>>(sc, iters / 8 + 1, nullptr);  // warm-up
   EMU_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
-  i8_probe_kernel<<<ctx->num_sms, 128, smem, ctx->stream>>>(n_mma, iters);
+  i8_probe_kernel<<<ctx->num_sms, 128, smem, ctx->stream>>>(sc, iters, dcyc);
   EMU_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
   EMU_CUDA(ctx, cudaEventSynchronize(e1));
   EMU_CUDA(ctx, cudaEventElapsedTime(ms, e0, e1));
+  if (cycles) EMU_CUDA(ctx, cudaMemcpy(cycles, dcyc, sizeof(long long), cudaMemcpyDeviceToHost));
   cudaEventDestroy(e0);
   cudaEventDestroy(e1);
   *ctas = ctx->num_sms;
   ctx->launches += 2;
   return EMUGEMM_OK;
+}
+
+// ---- compiled-schedule probe: the exact MMA issue code of the fused kernel on SMEM-resident operands ----
+template <int P, bool COLL>
+__global__ void __launch_bounds__(128, 1) oz1_issue_probe_kernel(int iters, long long *cycles_out) {
+  extern __shared__ uint8_t smem_raw[];
+  uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
+  __shared__ uint64_t bar;
+  __shared__ uint32_t slot;
+  for (int i = threadIdx.x; i < (8 * 16384 + 65536) / 4; i += 128) {
+    uint32_t x = static_cast<uint32_t>(i) * 2654435761u + blockIdx.x * 40503u;
+    x ^= x >> 15; x *= 2246822519u; x ^= x >> 13;
+    reinterpret_cast<uint32_t *>(smem)[i] = x;
+  }
+  if (threadIdx.x == 0) { mbar_init(&bar, 1); fence_mbar_init(); }
+  fence_proxy_async_smem();
+  if (threadIdx.x < 32) { tmem_alloc(&slot, 512); tmem_relinquish(); }
+  tc_fence_before();
+  __syncthreads();
+  tc_fence_after();
+  const uint32_t tb = slot;
+  if (threadIdx.x == 0) {
+    const uint32_t abase = smem_u32(smem), bbase = smem_u32(smem + 8 * 16384);
+    const long long t0 = clock64();
+    for (int it = 0; it < iters; ++it) {
+#pragma unroll
+      for (int t = 0; t < P; ++t) oz1_issue_slice<P, COLL>(t, tb, abase + t * 16384, bbase, it > 0 || t > 0);
+    }
+    umma_commit(&bar);
+    mbar_wait(&bar, 0);
+    if (blockIdx.x == 0 && cycles_out) *cycles_out = clock64() - t0;
+  }
+  tc_fence_before();
+  __syncthreads();
+  if (threadIdx.x < 32) tmem_dealloc(tb, 512);
+}
+
+template <int P>
+static int issue_probe_p(emugemm_ctx *ctx, int coll, int iters, float *ms, long long *cycles) {
+  const int smem = 8 * 16384 + 65536 + 1024;
+  auto kern = coll ? oz1_issue_probe_kernel<P, true> : oz1_issue_probe_kernel<P, false>;
+  EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
+  cudaEvent_t e0, e1;
+  EMU_CUDA(ctx, cudaEventCreate(&e0));
+  EMU_CUDA(ctx, cudaEventCreate(&e1));
+  long long *dcyc = static_cast<long long *>(ctx->ws);
+  kern<<<ctx->num_sms, 128, smem, ctx->stream>>>(iters / 8 + 1, nullptr);
+  EMU_CUDA(ctx, cudaEventRecord(e0, ctx->stream));
+  kern<<<ctx->num_sms, 128, smem, ctx->stream>>>(iters, dcyc);
+  EMU_CUDA(ctx, cudaEventRecord(e1, ctx->stream));
+  EMU_CUDA(ctx, cudaEventSynchronize(e1));
+  EMU_CUDA(ctx, cudaEventElapsedTime(ms, e0, e1));
+  if (cycles) EMU_CUDA(ctx, cudaMemcpy(cycles, dcyc, sizeof(long long), cudaMemcpyDeviceToHost));
+  cudaEventDestroy(e0);
+  cudaEventDestroy(e1);
+  ctx->launches += 2;
+  return EMUGEMM_OK;
+}
+
+int launch_oz1_issue_probe(emugemm_ctx *ctx, int p, int coll, int iters, float *ms, int *ctas, long long *cycles) {
+  if (iters < 1 || p < 1 || p > 8) return EMUGEMM_ERR_ARG;
+  if (!ctx->ws || ctx->ws_bytes < 8) return EMUGEMM_ERR_WORKSPACE;
+  *ctas = ctx->num_sms;
+  switch (p) {
+    case 1: return issue_probe_p<1>(ctx, coll, iters, ms, cycles);
+    case 2: return issue_probe_p<2>(ctx, coll, iters, ms, cycles);
+    case 3: return issue_probe_p<3>(ctx, coll, iters, ms, cycles);
+    case 4: return issue_probe_p<4>(ctx, coll, iters, ms, cycles);
+    case 5: return issue_probe_p<5>(ctx, coll, iters, ms, cycles);
+    case 6: return issue_probe_p<6>(ctx, coll, iters, ms, cycles);
+    case 7: return issue_probe_p<7>(ctx, coll, iters, ms, cycles);
+    default: return issue_probe_p<8>(ctx, coll, iters, ms, cycles);
+  }
 }
 
 }  // namespace emu

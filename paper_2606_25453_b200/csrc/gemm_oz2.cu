@@ -31,6 +31,7 @@ struct Oz2Dev {
   int mt, nt_tiles, n_moduli;
   int nprod;              // 1 real, 3 for 3M
   int8_t *CR;
+  unsigned long long *cycles;
   int mod[kMaxModuli];
   unsigned magic[kMaxModuli];  // ceil(2^39 / m)
 };
@@ -99,6 +100,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
+  const long long t_start = clock64();
 
   if (warp == 0) {
     if (lane == 0) {
@@ -221,6 +223,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   tc_fence_before();
   __syncthreads();
   if (warp == 1) tmem_dealloc(tmem_base, 512);
+  if (blockIdx.x == 0 && threadIdx.x == 0 && a.cycles) atomicAdd(a.cycles, static_cast<unsigned long long>(clock64() - t_start));
 }
 
 int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
@@ -237,6 +240,7 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
   d.n_moduli = g.n_moduli;
   d.nprod = parts;
   d.CR = g.CR;
+  d.cycles = g.cycles;
   int mod[24];
   oz2_moduli_host(g.n_moduli, mod);
   for (int l = 0; l < kMaxModuli; ++l) {
