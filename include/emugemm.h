@@ -161,7 +161,8 @@ int emugemm_dbg_i8_probe(emugemm_handle_t h, int n_ops, const int *ops, int iter
  * (one iteration = one 128-byte k-block = 4 k32 steps) on operands resident in
  * shared memory (pseudo-random bytes), one CTA per SM: the tensor-pipe ceiling of
  * that schedule without TMA traffic.  INT8 ops per CTA = iters * 4 * p(p+1) * 128 *
- * NT(p) * 32.  use_collector selects the A-operand collector hints.            */
+ * NT(p) * 32.  use_collector bit 0 selects the A-operand collector hints, bit 1 the
+ * one-MMA-per-product schedule (width NT) instead of the N-concatenated one.   */
 int emugemm_dbg_oz1_issue_probe(emugemm_handle_t h, int p, int use_collector, int iters, float *ms, int *ctas,
                                 long long *cycles);
 

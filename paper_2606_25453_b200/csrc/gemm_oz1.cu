@@ -80,6 +80,34 @@ __device__ __forceinline__ void oz1_issue_slice(int t, uint32_t tmem_base, uint3
   }
 }
 
+// Same products, ONE MMA per product (width NT): A_t stays in the collector across its P - t consecutive MMAs.
+// This is the schedule a cta_group::2 pair needs (an N-concatenated MMA would split its columns between the
+// two CTAs' B halves); probed with cta_group::1: MMAs narrower than ~112 columns hit a ~55-cycle
+// per-instruction floor (p = 8, NT = 64: 0.56 of peak), so it only pays for NT >= 128.
+template <int P, bool COLL>
+__device__ __forceinline__ void oz1_issue_slice_per_product(int t, uint32_t tmem_base, uint32_t a_base, uint32_t b_base,
+                                                            bool accumulate) {
+  constexpr int NT = Oz1Cfg<P>::NT;
+  constexpr uint32_t idesc = make_idesc_i8(kTileM, NT);
+#pragma unroll
+  for (int ks = 0; ks < kBlockK / 32; ++ks) {
+    const uint64_t adesc = make_sdesc_sw128(a_base + ks * 32);
+#pragma unroll
+    for (int u = 0; u < P; ++u) {
+      if (u < P - t) {
+        const uint32_t acc = (accumulate || ks != 0) ? 1u : 0u;
+        const uint32_t d = tmem_base + (t + u) * NT;
+        const uint64_t bdesc = make_sdesc_sw128(b_base + u * NT * kBlockK + ks * 32);
+        const bool first = (u == 0), last = (u == P - t - 1);
+        if (COLL && first && !last) umma_i8<1>(d, adesc, bdesc, idesc, acc);
+        else if (COLL && !first && last) umma_i8<3>(d, adesc, bdesc, idesc, acc);
+        else if (COLL && !first && !last) umma_i8<2>(d, adesc, bdesc, idesc, acc);
+        else umma_i8<0>(d, adesc, bdesc, idesc, acc);
+      }
+    }
+  }
+}
+
 struct Oz1Dev {
   int64_t m, n;
   int kb0, kb1;       // k-blocks [kb0, kb1) of 128
@@ -103,7 +131,135 @@ __device__ __forceinline__ double i32_scaled(uint32_t x, int sh) {
   return magic - off;
 }
 
-template <int P>
+// exact double of G * 2^sh for an int64 |G| < 2^51 that already carries the bias magic_bias(sh): the bits are the
+// double (2^52 + 2^51 + G) 2^sh; subtracting 1.5 * 2^(52+sh) is exact.
+__device__ __forceinline__ constexpr long long magic_bias(int sh) { return (static_cast<long long>(0x433 + sh) << 52) + (1LL << 51); }
+__device__ __forceinline__ double unbias(long long biased, int sh) {
+  return __longlong_as_double(biased) - __longlong_as_double((static_cast<long long>(0x433 + sh) << 52) + (1LL << 51));
+}
+
+// Epilogue arithmetic (Eq. 3 + scaling) for one row x 8 columns x P accumulators.
+// The accumulators are folded three at a time into exact 64-bit integers G_g = C_s 2^14 + C_{s+1} 2^7 + C_{s+2}
+// (|G| < 2^46, integer multiply-adds), each converted exactly with the exponent-bias trick, so only
+// ceil(P/3) - 1 FP64 additions round.
+// OUT: 0 final FP64 C, 1 final FP32 C, 2 INT32 accumulator dump (test hook), 3 exact double-double k-chunk partial.
+template <int P, int OUT>
+struct Oz1Epi {
+  static constexpr int NG = (P + 2) / 3;  // groups, most significant first; the last may hold 1 or 2 accumulators
+  bool vec_c, vec_e;
+  __device__ __forceinline__ void init(const Oz1Dev &a) {
+    vec_c = (a.ldc % 4 == 0) && ((reinterpret_cast<uintptr_t>(a.C) & 31) == 0);
+    vec_e = (reinterpret_cast<uintptr_t>(a.eB) & 15) == 0;
+  }
+  // group g covers accumulators s = 3g .. min(3g+2, P-1); its weight is 2^(7 (P-1-last))
+  __device__ __forceinline__ static double group(const uint32_t (&v)[P][8], int c, int g) {
+    const int s0 = 3 * g, s1 = (3 * g + 2 < P - 1) ? 3 * g + 2 : P - 1;
+    const int sh = kBeta * (P - 1 - s1);
+    long long G = magic_bias(sh);
+#pragma unroll
+    for (int s = s0; s <= s1; ++s)  // IMAD.WIDE: sign-extending 32 x 32 -> 64 multiply-add
+      G += static_cast<long long>(static_cast<int32_t>(v[s][c])) * static_cast<long long>(1 << (kBeta * (s1 - s)));
+    return unbias(G, sh);
+  }
+  // column exponents of one 8-column chunk (issued one chunk ahead of their use: the load latency is hidden)
+  __device__ __forceinline__ void load_eb(const Oz1Dev &a, int64_t gcol, int (&eb)[8]) const {
+    if constexpr (OUT != 2) {
+      if (gcol + 8 <= a.n && vec_e) {
+        const int4 e0 = __ldg(reinterpret_cast<const int4 *>(a.eB + gcol)), e1 = __ldg(reinterpret_cast<const int4 *>(a.eB + gcol) + 1);
+        eb[0] = e0.x; eb[1] = e0.y; eb[2] = e0.z; eb[3] = e0.w; eb[4] = e1.x; eb[5] = e1.y; eb[6] = e1.z; eb[7] = e1.w;
+      } else {
+#pragma unroll
+        for (int c = 0; c < 8; ++c) eb[c] = (gcol + c < a.n) ? __ldg(a.eB + gcol + c) : 0;
+      }
+    }
+  }
+  __device__ __forceinline__ void chunk(const Oz1Dev &a, const uint32_t (&v)[P][8], const int (&eb)[8], int64_t grow, bool row_ok,
+                                        int eArow, int64_t gcol) const {
+    if constexpr (OUT == 2) {
+      if (row_ok) {
+        int32_t *o = static_cast<int32_t *>(a.C);
+#pragma unroll
+        for (int s = 0; s < P; ++s)
+#pragma unroll
+          for (int c = 0; c < 8; ++c)
+            if (gcol + c < a.n) o[(static_cast<int64_t>(s) * a.m + grow) * a.n + gcol + c] = static_cast<int32_t>(v[s][c]);
+      }
+      return;
+    } else {
+      const bool full = gcol + 8 <= a.n;
+      double r[8], rlo[8];
+#pragma unroll
+      for (int c = 0; c < 8; ++c) {
+        // least significant group first; every group value is exact, each addition rounds at most 1/2 ulp of a
+        // partial sum bounded by (|A'||B'|)_ij
+        double acc = group(v, c, NG - 1), lo = 0.0;
+        if constexpr (OUT != 3) {
+#pragma unroll
+          for (int g = NG - 2; g >= 0; --g) acc += group(v, c, g);
+        } else {  // exact double-double (TwoSum): hi + lo == S exactly (S < 2^82, the error terms are small integers)
+#pragma unroll
+          for (int g = NG - 2; g >= 0; --g) {
+            const double t = group(v, c, g);
+            const double sum = acc + t;
+            const double bb = sum - acc;
+            lo += (acc - (sum - bb)) + (t - bb);
+            acc = sum;
+          }
+        }
+        // power-of-two scaling 2^E, E = eA_i + eB_j - 7 (p+1), split so that both factors are normal doubles
+        // for every |E| <= 2044 (branch-free; covers subnormal inputs and results)
+        const int E = eArow + eb[c];
+        const double d1 = pow2d(E >> 1), d2 = pow2d(E - (E >> 1));
+        r[c] = acc * d1 * d2;
+        if constexpr (OUT == 3) rlo[c] = lo * d1 * d2;
+      }
+      if (!row_ok || (a.dbg & 4)) return;
+      if constexpr (OUT == 3) {  // k-chunk partial as double-double [m][n][2]
+        double *o = static_cast<double *>(a.C) + (grow * a.n + gcol) * 2;
+#pragma unroll
+        for (int c = 0; c < 8; ++c)
+          if (gcol + c < a.n) { o[2 * c] = r[c]; o[2 * c + 1] = rlo[c]; }
+      } else if constexpr (OUT == 0) {
+        double *o = static_cast<double *>(a.C) + grow * a.ldc + gcol;
+        if (a.beta != 0.0) {
+#pragma unroll
+          for (int c = 0; c < 8; ++c)
+            if (gcol + c < a.n) r[c] = fma(a.alpha, r[c], a.beta * o[c]);
+        } else if (a.alpha != 1.0) {
+#pragma unroll
+          for (int c = 0; c < 8; ++c) r[c] *= a.alpha;
+        }
+        if (full && vec_c) {
+          asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(o), "d"(r[0]), "d"(r[1]), "d"(r[2]), "d"(r[3]) : "memory");
+          asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(o + 4), "d"(r[4]), "d"(r[5]), "d"(r[6]), "d"(r[7]) : "memory");
+        } else {
+#pragma unroll
+          for (int c = 0; c < 8; ++c)
+            if (gcol + c < a.n) o[c] = r[c];
+        }
+      } else {  // OUT == 1: FP32 C, one rounding to float
+        float *o = static_cast<float *>(a.C) + grow * a.ldc + gcol;
+        float f[8];
+#pragma unroll
+        for (int c = 0; c < 8; ++c) {
+          double x = a.alpha * r[c];
+          if (a.beta != 0.0 && gcol + c < a.n) x = fma(a.beta, static_cast<double>(o[c]), x);
+          f[c] = static_cast<float>(x);
+        }
+        if (full && vec_c) {
+          *reinterpret_cast<float4 *>(o) = make_float4(f[0], f[1], f[2], f[3]);
+          *reinterpret_cast<float4 *>(o + 4) = make_float4(f[4], f[5], f[6], f[7]);
+        } else {
+#pragma unroll
+          for (int c = 0; c < 8; ++c)
+            if (gcol + c < a.n) o[c] = f[c];
+        }
+      }
+    }
+  }
+};
+
+template <int P, int OUT>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const Oz1Dev a) {
   using Cfg = Oz1Cfg<P>;
@@ -220,92 +376,66 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     const int row = quad * 32 + lane;
     const uint32_t trow = tmem_base + (static_cast<uint32_t>(quad * 32) << 16);
     uint32_t pt = 0;
-    const bool vec_ok64 = (a.ldc % 4 == 0) && ((reinterpret_cast<uintptr_t>(a.C) & 31) == 0);
+    Oz1Epi<P, OUT> epi;
+    epi.init(a);
+    constexpr int kChunks = NT / 2 / 8;  // 8-column chunks per thread
+    constexpr bool kDoubleBuffer = (P <= 6);  // two register sets of P x 8 accumulator values fit without spilling
     for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
       int mb, nb;
       tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
       const int64_t grow = static_cast<int64_t>(mb) * kTileM + row;
       const bool row_ok = grow < a.m;
       const int eArow = row_ok ? __ldg(a.eA + grow) - kBeta * (P + 1) : 0;
+      const int64_t gcol0 = static_cast<int64_t>(nb) * NT + half * (NT / 2);
+      int ea[8], eb[8];
+      epi.load_eb(a, gcol0, ea);  // first chunk's column exponents: in flight while the tile's MMAs finish
       mbar_wait(tfull, pt);
       tc_fence_after();
+      if (!(a.dbg & 2)) {
+        const uint32_t tcol = trow + half * (NT / 2);
+        if constexpr (kDoubleBuffer) {
+          // software pipeline: the TMEM loads and column exponents of chunk i+1 are in flight while chunk i is
+          // converted and stored
+          uint32_t va[P][8], vb[P][8];
+#pragma unroll
+          for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT, va[s]);
 #pragma unroll 1
-      for (int c0 = (a.dbg & 2) ? NT : half * (NT / 2); c0 < (half + 1) * (NT / 2); c0 += 8) {
-        uint32_t v[P][8];
+          for (int i = 0; i < kChunks; i += 2) {
+            tmem_ld_wait();
+            if (i + 1 < kChunks) {
 #pragma unroll
-        for (int s = 0; s < P; ++s) tmem_ld8(trow + s * NT + c0, v[s]);
-        tmem_ld_wait();
-        const int64_t gcol = static_cast<int64_t>(nb) * NT + c0;
-        if (a.out_kind == 2) {  // INT32 accumulator dump [P][m][n] (test hook)
-          if (row_ok) {
-            int32_t *o = static_cast<int32_t *>(a.C);
+              for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + (i + 1) * 8, vb[s]);
+              epi.load_eb(a, gcol0 + (i + 1) * 8, eb);
+            }
+            epi.chunk(a, va, ea, grow, row_ok, eArow, gcol0 + i * 8);
+            if (i + 1 < kChunks) {
+              tmem_ld_wait();
+              if (i + 2 < kChunks) {
 #pragma unroll
-            for (int s = 0; s < P; ++s)
-#pragma unroll
-              for (int c = 0; c < 8; ++c)
-                if (gcol + c < a.n) o[(static_cast<int64_t>(s) * a.m + grow) * a.n + gcol + c] = static_cast<int32_t>(v[s][c]);
-          }
-          continue;
-        }
-        double r[8], rlo[8];
-#pragma unroll
-        for (int c = 0; c < 8; ++c) {
-          // shift-reduce (Eq. 3), least significant accumulator first; every term is exact,
-          // each addition rounds at most 1/2 ulp of a partial sum bounded by (|A'||B'|)_ij
-          double acc = i32_scaled(v[P - 1][c], 0), lo = 0.0;
-          if (a.out_kind != 3) {
-#pragma unroll
-            for (int s = P - 2; s >= 0; --s) acc += i32_scaled(v[s][c], kBeta * (P - 1 - s));
-          } else {  // exact double-double (TwoSum): hi + lo == S exactly (S < 2^82)
-#pragma unroll
-            for (int s = P - 2; s >= 0; --s) {
-              const double t = i32_scaled(v[s][c], kBeta * (P - 1 - s));
-              const double sum = acc + t;
-              const double bb = sum - acc;
-              lo += (acc - (sum - bb)) + (t - bb);
-              acc = sum;
+                for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + (i + 2) * 8, va[s]);
+                epi.load_eb(a, gcol0 + (i + 2) * 8, ea);
+              }
+              epi.chunk(a, vb, eb, grow, row_ok, eArow, gcol0 + (i + 1) * 8);
             }
           }
-          const int eb = (gcol + c < a.n) ? __ldg(a.eB + gcol + c) : 0;
-          const int E = eArow + eb;  // power-of-two scaling, split so both factors are normal doubles
-          const double d1 = pow2d(E >> 1), d2 = pow2d(E - (E >> 1));
-          r[c] = acc * d1 * d2;
-          rlo[c] = lo * d1 * d2;
-        }
-        if (!row_ok) continue;
-        if (a.out_kind == 3) {  // k-chunk partial as double-double [m][n][2]
-          double *o = static_cast<double *>(a.C) + (grow * a.n + gcol) * 2;
+        } else {
+          // P >= 7: one register set; only the column exponents are prefetched a chunk ahead
+          uint32_t v[P][8];
+#pragma unroll 1
+          for (int i = 0; i < kChunks; i += 2) {
 #pragma unroll
-          for (int c = 0; c < 8; ++c)
-            if (gcol + c < a.n) { o[2 * c] = r[c]; o[2 * c + 1] = rlo[c]; }
-        } else if (a.out_kind == 0) {
-          double *o = static_cast<double *>(a.C) + grow * a.ldc + gcol;
-          const bool full = gcol + 8 <= a.n;
-          if (a.beta != 0.0) {
+            for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + i * 8, v[s]);
+            if (i + 1 < kChunks) epi.load_eb(a, gcol0 + (i + 1) * 8, eb);
+            tmem_ld_wait();
+            epi.chunk(a, v, ea, grow, row_ok, eArow, gcol0 + i * 8);
+            if (i + 1 < kChunks) {
 #pragma unroll
-            for (int c = 0; c < 8; ++c)
-              if (gcol + c < a.n) r[c] = fma(a.alpha, r[c], a.beta * o[c]);
-          } else if (a.alpha != 1.0) {
-#pragma unroll
-            for (int c = 0; c < 8; ++c) r[c] *= a.alpha;
-          }
-          if (full && vec_ok64) {
-            asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(o), "d"(r[0]), "d"(r[1]), "d"(r[2]), "d"(r[3]) : "memory");
-            asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(o + 4), "d"(r[4]), "d"(r[5]), "d"(r[6]), "d"(r[7]) : "memory");
-          } else {
-#pragma unroll
-            for (int c = 0; c < 8; ++c)
-              if (gcol + c < a.n) o[c] = r[c];
-          }
-        } else {  // out_kind 1: FP32 C, one rounding to float
-          float *o = static_cast<float *>(a.C) + grow * a.ldc + gcol;
-#pragma unroll
-          for (int c = 0; c < 8; ++c)
-            if (gcol + c < a.n) {
-              double x = a.alpha * r[c];
-              if (a.beta != 0.0) x = fma(a.beta, static_cast<double>(o[c]), x);
-              o[c] = static_cast<float>(x);
+              for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + (i + 1) * 8, v[s]);
+              if (i + 2 < kChunks) epi.load_eb(a, gcol0 + (i + 2) * 8, ea);
+              tmem_ld_wait();
+              epi.chunk(a, v, eb, grow, row_ok, eArow, gcol0 + (i + 1) * 8);
             }
+          }
         }
       }
       // all TMEM reads of this tile are complete (tcgen05.wait::ld above): release the accumulators
@@ -340,7 +470,14 @@ static int launch_p(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   d.dbg = ctx->dbg_flags;
   const int tiles = d.mt * d.nt_tiles;
   const int grid = tiles < ctx->num_sms ? tiles : ctx->num_sms;
-  auto kern = oz1_gemm_kernel<P>;
+  void (*kern)(CUtensorMap, CUtensorMap, Oz1Dev) = nullptr;
+  switch (g.out_kind) {
+    case 0: kern = oz1_gemm_kernel<P, 0>; break;
+    case 1: kern = oz1_gemm_kernel<(P <= 4 ? P : 4), 1>; break;  // FP32 entry point: p <= 4 (checked by the API)
+    case 2: kern = oz1_gemm_kernel<P, 2>; break;
+    default: kern = oz1_gemm_kernel<P, 3>; break;
+  }
+  if (g.out_kind == 1 && P > 4) return EMUGEMM_ERR_ARG;
   EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
   kern<<<grid, kGemmThreads, Cfg::kSmemBytes, ctx->stream>>>(tmA, tmB, d);
   ctx->launches++;
@@ -491,7 +628,7 @@ int launch_i8_probe(emugemm_ctx *ctx, int n_ops, const int *ops, int iters, floa
 }
 
 // ---- compiled-schedule probe: the exact MMA issue code of the fused kernel on SMEM-resident operands ----
-template <int P, bool COLL>
+template <int P, bool COLL, bool PERPROD>
 __global__ void __launch_bounds__(128, 1) oz1_issue_probe_kernel(int iters, long long *cycles_out) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -514,7 +651,10 @@ __global__ void __launch_bounds__(128, 1) oz1_issue_probe_kernel(int iters, long
     const long long t0 = clock64();
     for (int it = 0; it < iters; ++it) {
 #pragma unroll
-      for (int t = 0; t < P; ++t) oz1_issue_slice<P, COLL>(t, tb, abase + t * 16384, bbase, it > 0 || t > 0);
+      for (int t = 0; t < P; ++t) {
+        if (PERPROD) oz1_issue_slice_per_product<P, COLL>(t, tb, abase + t * 16384, bbase, it > 0 || t > 0);
+        else oz1_issue_slice<P, COLL>(t, tb, abase + t * 16384, bbase, it > 0 || t > 0);
+      }
     }
     umma_commit(&bar);
     mbar_wait(&bar, 0);
@@ -528,7 +668,8 @@ __global__ void __launch_bounds__(128, 1) oz1_issue_probe_kernel(int iters, long
 template <int P>
 static int issue_probe_p(emugemm_ctx *ctx, int coll, int iters, float *ms, long long *cycles) {
   const int smem = 8 * 16384 + 65536 + 1024;
-  auto kern = coll ? oz1_issue_probe_kernel<P, true> : oz1_issue_probe_kernel<P, false>;
+  auto kern = (coll & 2) ? ((coll & 1) ? oz1_issue_probe_kernel<P, true, true> : oz1_issue_probe_kernel<P, false, true>)
+                         : ((coll & 1) ? oz1_issue_probe_kernel<P, true, false> : oz1_issue_probe_kernel<P, false, false>);
   EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, smem));
   cudaEvent_t e0, e1;
   EMU_CUDA(ctx, cudaEventCreate(&e0));
