@@ -81,74 +81,117 @@ static void crt_constants(int N, CrtConst &c) {
 }
 
 // ---- device ------------------------------------------------------------------
+// Integer -> double conversions (I2F.F64) and rint (F2F) run on the XU pipe, which ncu showed saturated
+// (108 %) by the first version of this kernel at 1 conversion / clk / SM; both are replaced by exponent-bias
+// additions on the FP64 pipe (profiles/).
 __device__ __forceinline__ double pow2_dev(int e) { return __hiloint2double((1023 + e) << 20, 0); }
-
-__device__ __forceinline__ double crt_value(const CrtConst &k, const int (&c)[kMaxModuli]) {
-  double shi = 0.0, slo = 0.0;
-#pragma unroll
-  for (int l = 0; l < kMaxModuli; ++l)
-    if (l < k.N) {
-      const double cl = static_cast<double>(c[l]);
-      shi = fma(k.whi[l], cl, shi);
-      slo = fma(k.wlo[l], cl, slo);
-    }
-  const double Q = rint((shi + slo) * k.invP);
-  return fma(-Q, k.Phi, shi) + fma(-Q, k.Plo, slo);
+// exact double of a residue byte b (two's complement int8 in the low 8 bits of w >> sh)
+__device__ __forceinline__ double residue_to_double(unsigned w, int sh) {
+  const unsigned biased = ((w >> sh) & 0xFFu) ^ 0x80u;  // c + 128 in [0, 255]
+  return __hiloint2double(0x43300000, static_cast<int>(biased)) - 4503599627370624.0;  // (2^52 + c + 128) - (2^52 + 128)
+}
+__device__ __forceinline__ double round_nearest(double x) {  // |x| < 2^51: round to nearest even without F2F
+  const double big = 6755399441055744.0;  // 1.5 * 2^52
+  return (x + big) - big;
 }
 
-// one thread per 4 consecutive columns; VEC = 4: aligned 32-bit plane loads, VEC = 1: byte loads
-template <int VEC>
-__global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const int8_t *__restrict__ CR,
-                                                  const int32_t *__restrict__ eA, const int32_t *__restrict__ eB,
-                                                  int tsum, int is_complex, double ar, double ai, double br, double bi,
-                                                  double *__restrict__ C, int64_t ldc, const CrtConst k) {
-  const int64_t ncol4 = (n + 3) / 4;
-  const int64_t idx = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
-  if (idx >= m * ncol4) return;
-  const int64_t i = idx / ncol4, j0 = (idx - i * ncol4) * 4;
-  const int64_t plane = m * n;
-  const int eAi = eA[i] - tsum;
-  const int nparts = is_complex ? 2 : 1;
-  double val[2][4];
-  for (int part = 0; part < nparts; ++part) {
-    const int8_t *src = CR + static_cast<int64_t>(part) * k.N * plane + i * n + j0;
-    int c[4][kMaxModuli];
+constexpr int kCrtVec = 8;  // columns per thread on the vector path (one 8-byte load per residue plane)
+
+template <bool VEC>
+__device__ __forceinline__ void crt_accumulate(const CrtConst &k, const int8_t *__restrict__ src, int64_t plane, int64_t j0,
+                                               int64_t n, double (&shi)[kCrtVec], double (&slo)[kCrtVec]) {
 #pragma unroll
-    for (int l = 0; l < kMaxModuli; ++l)
-      if (l < k.N) {
-        if (VEC == 4) {
-          const unsigned w = *reinterpret_cast<const unsigned *>(src + l * plane);
+  for (int e = 0; e < kCrtVec; ++e) { shi[e] = 0.0; slo[e] = 0.0; }
 #pragma unroll
-          for (int e = 0; e < 4; ++e) c[e][l] = static_cast<int>(static_cast<int8_t>((w >> (8 * e)) & 0xFFu));
-        } else {
+  for (int l = 0; l < kMaxModuli; ++l) {
+    if (l < k.N) {
+      unsigned w0, w1;
+      if (VEC) {
+        const uint2 w = __ldg(reinterpret_cast<const uint2 *>(src + l * plane));
+        w0 = w.x; w1 = w.y;
+      } else {
+        w0 = w1 = 0;
 #pragma unroll
-          for (int e = 0; e < 4; ++e) c[e][l] = (j0 + e < n) ? static_cast<int>(src[l * plane + e]) : 0;
+        for (int e = 0; e < 4; ++e) {
+          if (j0 + e < n) w0 |= static_cast<unsigned>(static_cast<uint8_t>(src[l * plane + e])) << (8 * e);
+          if (j0 + 4 + e < n) w1 |= static_cast<unsigned>(static_cast<uint8_t>(src[l * plane + 4 + e])) << (8 * e);
         }
       }
 #pragma unroll
-    for (int e = 0; e < 4; ++e) {
-      const double x = crt_value(k, c[e]);
-      const int E2 = eAi + ((j0 + e < n) ? eB[j0 + e] : 0);
-      val[part][e] = x * pow2_dev(E2 >> 1) * pow2_dev(E2 - (E2 >> 1));
+      for (int e = 0; e < kCrtVec; ++e) {
+        const double cl = residue_to_double(e < 4 ? w0 : w1, 8 * (e & 3));
+        shi[e] = fma(k.whi[l], cl, shi[e]);
+        slo[e] = fma(k.wlo[l], cl, slo[e]);
+      }
     }
   }
+}
+
+__device__ __forceinline__ double crt_finish(const CrtConst &k, double shi, double slo) {
+  const double Q = round_nearest((shi + slo) * k.invP);
+  return fma(-Q, k.Phi, shi) + fma(-Q, k.Plo, slo);
+}
+
+// one thread per 8 consecutive columns of one row
+template <bool VEC, bool CPLX>
+__global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const int8_t *__restrict__ CR,
+                                                  const int32_t *__restrict__ eA, const int32_t *__restrict__ eB,
+                                                  int tsum, double ar, double ai, double br, double bi,
+                                                  double *__restrict__ C, int64_t ldc, const CrtConst k) {
+  const int64_t ncolv = (n + kCrtVec - 1) / kCrtVec;
+  const int64_t idx = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
+  if (idx >= m * ncolv) return;
+  const int64_t i = idx / ncolv, j0 = (idx - i * ncolv) * kCrtVec;
+  const int64_t plane = m * n;
+  const int eAi = eA[i] - tsum;
+  double sc1[kCrtVec], sc2[kCrtVec];
 #pragma unroll
-  for (int e = 0; e < 4; ++e) {
-    if (j0 + e >= n) break;
-    if (!is_complex) {
-      double *o = C + i * ldc + j0 + e;
-      *o = (br != 0.0) ? fma(ar, val[0][e], br * *o) : ar * val[0][e];
+  for (int e = 0; e < kCrtVec; ++e) {
+    const int E2 = eAi + ((j0 + e < n) ? __ldg(eB + j0 + e) : 0);
+    sc1[e] = pow2_dev(E2 >> 1);
+    sc2[e] = pow2_dev(E2 - (E2 >> 1));
+  }
+  double shi[kCrtVec], slo[kCrtVec], vr[kCrtVec];
+  crt_accumulate<VEC>(k, CR + i * n + j0, plane, j0, n, shi, slo);
+#pragma unroll
+  for (int e = 0; e < kCrtVec; ++e) vr[e] = crt_finish(k, shi[e], slo[e]) * sc1[e] * sc2[e];
+  if (!CPLX) {
+    double *o = C + i * ldc + j0;
+    if (br != 0.0) {
+#pragma unroll
+      for (int e = 0; e < kCrtVec; ++e)
+        if (j0 + e < n) vr[e] = fma(ar, vr[e], br * o[e]);
     } else {
-      double *o = C + 2 * (i * ldc + j0 + e);
-      double re = ar * val[0][e] - ai * val[1][e];
-      double im = ar * val[1][e] + ai * val[0][e];
-      if (br != 0.0 || bi != 0.0) {
-        const double cr = o[0], ci = o[1];
+#pragma unroll
+      for (int e = 0; e < kCrtVec; ++e) vr[e] *= ar;
+    }
+    if (VEC && (ldc % 2 == 0) && ((reinterpret_cast<uintptr_t>(C) & 15) == 0)) {
+#pragma unroll
+      for (int e = 0; e < kCrtVec; e += 2) *reinterpret_cast<double2 *>(o + e) = make_double2(vr[e], vr[e + 1]);
+    } else {
+#pragma unroll
+      for (int e = 0; e < kCrtVec; ++e)
+        if (j0 + e < n) o[e] = vr[e];
+    }
+  } else {
+    double vi[kCrtVec];
+    crt_accumulate<VEC>(k, CR + static_cast<int64_t>(k.N) * plane + i * n + j0, plane, j0, n, shi, slo);
+#pragma unroll
+    for (int e = 0; e < kCrtVec; ++e) vi[e] = crt_finish(k, shi[e], slo[e]) * sc1[e] * sc2[e];
+    double *o = C + 2 * (i * ldc + j0);
+    const bool has_beta = (br != 0.0 || bi != 0.0);
+#pragma unroll
+    for (int e = 0; e < kCrtVec; ++e) {
+      if (j0 + e >= n) break;
+      double re = ar * vr[e] - ai * vi[e];
+      double im = ar * vi[e] + ai * vr[e];
+      if (has_beta) {
+        const double cr = o[2 * e], ci = o[2 * e + 1];
         re += br * cr - bi * ci;
         im += br * ci + bi * cr;
       }
-      o[0] = re;
-      o[1] = im;
+      if ((reinterpret_cast<uintptr_t>(C) & 15) == 0) *reinterpret_cast<double2 *>(o + 2 * e) = make_double2(re, im);
+      else { o[2 * e] = re; o[2 * e + 1] = im; }
     }
   }
 }
@@ -157,15 +200,18 @@ int launch_oz2_crt(emugemm_ctx *ctx, const Oz2CrtArgs &a) {
   if (a.m == 0 || a.n == 0) return EMUGEMM_OK;
   CrtConst k;
   crt_constants(a.n_moduli, k);
-  const int64_t work = a.m * ((a.n + 3) / 4);
+  const int64_t work = a.m * ((a.n + kCrtVec - 1) / kCrtVec);
   const unsigned grid = static_cast<unsigned>((work + 255) / 256);
-  const bool vec = (a.n % 4 == 0) && ((reinterpret_cast<uintptr_t>(a.CR) & 3) == 0);
-  if (vec)
-    crt_kernel<4><<<grid, 256, 0, ctx->stream>>>(a.m, a.n, a.CR, a.eA, a.eB, a.tA + a.tB, a.is_complex, a.alpha[0], a.alpha[1],
-                                                 a.beta[0], a.beta[1], a.C, a.ldc, k);
-  else
-    crt_kernel<1><<<grid, 256, 0, ctx->stream>>>(a.m, a.n, a.CR, a.eA, a.eB, a.tA + a.tB, a.is_complex, a.alpha[0], a.alpha[1],
-                                                 a.beta[0], a.beta[1], a.C, a.ldc, k);
+  const bool vec = (a.n % kCrtVec == 0) && ((reinterpret_cast<uintptr_t>(a.CR) & 7) == 0);
+  const int tsum = a.tA + a.tB;
+#define EMU_CRT_LAUNCH(V, Z)                                                                                              \
+  crt_kernel<V, Z><<<grid, 256, 0, ctx->stream>>>(a.m, a.n, a.CR, a.eA, a.eB, tsum, a.alpha[0], a.alpha[1], a.beta[0], \
+                                                   a.beta[1], a.C, a.ldc, k)
+  if (vec && a.is_complex) EMU_CRT_LAUNCH(true, true);
+  else if (vec) EMU_CRT_LAUNCH(true, false);
+  else if (a.is_complex) EMU_CRT_LAUNCH(false, true);
+  else EMU_CRT_LAUNCH(false, false);
+#undef EMU_CRT_LAUNCH
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
   return EMUGEMM_OK;

@@ -29,50 +29,51 @@ struct Oz2Dev {
   int64_t m, n;
   int kblocks;
   int mt, nt_tiles, n_moduli;
-  int nprod;              // 1 real, 3 for 3M
   int8_t *CR;
   unsigned long long *cycles;
+  int dbg;
   int mod[kMaxModuli];
-  unsigned magic[kMaxModuli];  // ceil(2^39 / m)
+  unsigned cvec[kMaxModuli];    // bytes (256^j mod m), j = 0..3 (byte 0 = 256^0)
+  unsigned c0[kMaxModuli];      // (m - 2^31 mod m) mod m
+  unsigned magic[kMaxModuli];   // ceil(2^32 / m)
 };
 
-// symmetric residue of a signed INT32 accumulator (|x| < 2^31) modulo m (odd m, 151 <= m <= 255) or 256.
-// u = |x| < 2^31; q = floor(u magic / 2^39) with magic = ceil(2^39/m) < 2^32 is exact because the error
-// term u (magic - 2^39/m) / 2^39 < 2^31 / 2^39 = 2^-8 <= 1/m.
-__device__ __forceinline__ int sym_mod_i32(int x, int m, unsigned magic) {
-  if (m == 256) return static_cast<int>(static_cast<int8_t>(x & 0xFF));  // two's complement low byte
-  const unsigned u = static_cast<unsigned>(x < 0 ? -x : x);
-  const unsigned q = __umulhi(u, magic) >> 7;
-  int r = static_cast<int>(u - q * static_cast<unsigned>(m));  // [0, m)
-  if (r >= (m + 1) / 2) r -= m;                                // symmetric, odd m: sym(-u) = -sym(u)
-  return x < 0 ? -r : r;
+// Symmetric residue of a signed INT32 accumulator modulo m <= 256 in 6 integer instructions, no branch:
+//   u = x + 2^31 (flip the sign bit), s = sum_j byte_j(u) (256^j mod m) + c0  ==  x (mod m), 0 <= s < 2^18
+//   q = floor(s M / 2^32), M = ceil(2^32 / m): exact because s (M m - 2^32) / (m 2^32) < 2^18 / 2^32 < 1/m
+//   r = s - q m in [0, m), then r -= m if r >= ceil(m/2)  (R11, R13).  m = 256 reduces to the low byte.
+struct ModK {
+  unsigned cvec, c0, magic, m, half;
+};
+__device__ __forceinline__ unsigned dot_mod(uint32_t x, const ModK &k) {  // == x (mod m), in [0, 2^18)
+  return __dp4a(x ^ 0x80000000u, k.cvec, k.c0);
 }
-__device__ __forceinline__ int sym_small_rt(int t, int m) {  // t in (-2m, 2m) -> symmetric range (R15)
-  const int hi = (m + 1) / 2;
-  if (t >= hi) t -= m;
-  if (t >= hi) t -= m;
-  if (t < hi - m) t += m;
-  if (t < hi - m) t += m;
-  return t;
+__device__ __forceinline__ unsigned reduce_mod(unsigned s, const ModK &k) {  // s < 2^24 -> [0, m)
+  return s - __umulhi(s, k.magic) * k.m;
 }
-__device__ __forceinline__ unsigned pack4i(int a, int b, int c, int d) {
-  return (static_cast<unsigned>(a) & 0xFFu) | ((static_cast<unsigned>(b) & 0xFFu) << 8) |
-         ((static_cast<unsigned>(c) & 0xFFu) << 16) | ((static_cast<unsigned>(d) & 0xFFu) << 24);
+__device__ __forceinline__ int to_sym(unsigned r, const ModK &k) {  // [0, m) -> [ceil(m/2) - m, ceil(m/2) - 1]
+  return static_cast<int>(r) - (r >= k.half ? static_cast<int>(k.m) : 0);
 }
-__device__ __forceinline__ int unpack_i8(unsigned w, int i) {
-  return static_cast<int>(static_cast<int8_t>((w >> (8 * i)) & 0xFFu));
+__device__ __forceinline__ int sym_mod_i32(uint32_t x, const ModK &k) { return to_sym(reduce_mod(dot_mod(x, k), k), k); }
+// low bytes of a, b, c, d -> one word (3 PRMT)
+__device__ __forceinline__ unsigned pack4i(unsigned a, unsigned b, unsigned c, unsigned d) {
+  return __byte_perm(__byte_perm(a, b, 0x0040), __byte_perm(c, d, 0x0040), 0x5410);
 }
+__device__ __forceinline__ unsigned byte_u(unsigned w, int i) { return __byte_perm(w, 0u, 0x4440u | static_cast<unsigned>(i)); }
 
-__device__ __forceinline__ void store16(int8_t *dst, const unsigned (&w)[4], int64_t gcol, int64_t n, bool vec_ok) {
-  if (vec_ok && gcol + 16 <= n) {
-    *reinterpret_cast<uint4 *>(dst) = make_uint4(w[0], w[1], w[2], w[3]);
+// 32 packed residues (8 words) of one row -> global, two 16-byte stores = one full 32-byte sector
+__device__ __forceinline__ void store32(int8_t *dst, const unsigned (&w)[8], int64_t gcol, int64_t n, bool vec_ok) {
+  if (vec_ok && gcol + 32 <= n) {
+    reinterpret_cast<uint4 *>(dst)[0] = make_uint4(w[0], w[1], w[2], w[3]);
+    reinterpret_cast<uint4 *>(dst)[1] = make_uint4(w[4], w[5], w[6], w[7]);
   } else {
 #pragma unroll
-    for (int c = 0; c < 16; ++c)
+    for (int c = 0; c < 32; ++c)
       if (gcol + c < n) dst[c] = static_cast<int8_t>((w[c >> 2] >> (8 * (c & 3))) & 0xFFu);
   }
 }
 
+template <int NPROD>  // 1: real (Eq. 6-7); 3: 3M (Eq. 16-18)
 __global__ void __launch_bounds__(kGemmThreads, 1)
 oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const Oz2Dev a) {
   extern __shared__ uint8_t smem_raw[];
@@ -110,7 +111,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         const int l = tile / tiles_per_mod;
         int mb, nb;
         tile_coords(tile - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb);
-        for (int q = 0; q < a.nprod; ++q) {
+        for (int q = 0; q < NPROD; ++q) {
           const int plane = q * a.n_moduli + l;
           for (int kb = 0; kb < a.kblocks; ++kb) {
             mbar_wait(&empty[st], ph ^ 1);
@@ -131,7 +132,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       uint32_t item = 0;
       constexpr uint32_t idesc = make_idesc_i8(kTileM, kOz2NT);
       for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
-        for (int q = 0; q < a.nprod; ++q, ++item) {
+        for (int q = 0; q < NPROD; ++q, ++item) {
           const uint32_t slot = item & 1, tph = (item >> 1) & 1;
           mbar_wait(&tempty[slot], tph ^ 1);
           tc_fence_after();
@@ -158,58 +159,73 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     const bool vec_ok = (a.n % 16 == 0) && ((reinterpret_cast<uintptr_t>(a.CR) & 15) == 0);
     const int64_t plane_sz = a.m * a.n;
     uint32_t item = 0;
-    unsigned t1[32], t2[32];  // T1, T2 of this thread's 128 columns as packed INT8 (3M only)
+    unsigned t1[NPROD == 3 ? 32 : 1], t2[NPROD == 3 ? 32 : 1];  // T1, T2 of this thread's 128 columns as packed INT8 (3M)
     for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
       const int l = tile / tiles_per_mod;
       int mb, nb;
       tile_coords(tile - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb);
-      const int mod = a.mod[l];
-      const unsigned magic = a.magic[l];
+      ModK mk;
+      mk.cvec = a.cvec[l]; mk.c0 = a.c0[l]; mk.magic = a.magic[l]; mk.m = static_cast<unsigned>(a.mod[l]); mk.half = (mk.m + 1) / 2;
       const int64_t grow = static_cast<int64_t>(mb) * kTileM + row;
       const bool row_ok = grow < a.m;
-      for (int q = 0; q < a.nprod; ++q, ++item) {
+#pragma unroll
+      for (int q = 0; q < NPROD; ++q, ++item) {
         const uint32_t slot = item & 1, tph = (item >> 1) & 1;
         mbar_wait(&tfull[slot], tph);
         tc_fence_after();
+        if (!(a.dbg & 2)) {
+          // 4 chunks of 32 columns, TMEM loads of chunk i+1 in flight while chunk i is reduced
+          uint32_t va[32], vb[32];
+          const uint32_t tcol = trow + slot * kOz2NT + half * 128;
+          tmem_ld32(tcol, va);
 #pragma unroll
-        for (int ch = 0; ch < 8; ++ch) {
-          const int c0 = half * 128 + ch * 16;
-          uint32_t v[16];
-          tmem_ld16(trow + slot * kOz2NT + c0, v);
-          tmem_ld_wait();
-          unsigned w[4];
+          for (int ch = 0; ch < 4; ++ch) {
+            uint32_t(&v)[32] = (ch & 1) ? vb : va;
+            uint32_t(&vn)[32] = (ch & 1) ? va : vb;
+            tmem_ld_wait();
+            if (ch + 1 < 4) tmem_ld32(tcol + (ch + 1) * 32, vn);
+            const int64_t gcol = static_cast<int64_t>(nb) * kOz2NT + half * 128 + ch * 32;
+            if constexpr (NPROD == 1) {
+              unsigned w[8];
 #pragma unroll
-          for (int g = 0; g < 4; ++g)
-            w[g] = pack4i(sym_mod_i32(static_cast<int>(v[4 * g]), mod, magic), sym_mod_i32(static_cast<int>(v[4 * g + 1]), mod, magic),
-                          sym_mod_i32(static_cast<int>(v[4 * g + 2]), mod, magic), sym_mod_i32(static_cast<int>(v[4 * g + 3]), mod, magic));
-          const int64_t gcol = static_cast<int64_t>(nb) * kOz2NT + c0;
-          if (a.nprod == 1) {
-            if (row_ok && gcol < a.n)
-              store16(a.CR + (static_cast<int64_t>(l) * a.m + grow) * a.n + gcol, w, gcol, a.n, vec_ok);
-          } else if (q == 0) {
+              for (int g = 0; g < 8; ++g)
+                w[g] = pack4i(sym_mod_i32(v[4 * g], mk), sym_mod_i32(v[4 * g + 1], mk), sym_mod_i32(v[4 * g + 2], mk),
+                              sym_mod_i32(v[4 * g + 3], mk));
+              if (row_ok && gcol < a.n && !(a.dbg & 4))
+                store32(a.CR + (static_cast<int64_t>(l) * a.m + grow) * a.n + gcol, w, gcol, a.n, vec_ok);
+            } else if (q < 2) {
+              // T1 / T2 stay on chip as unsigned residues in [0, m), four per register
 #pragma unroll
-            for (int g = 0; g < 4; ++g) t1[ch * 4 + g] = w[g];
-          } else if (q == 1) {
-#pragma unroll
-            for (int g = 0; g < 4; ++g) t2[ch * 4 + g] = w[g];
-          } else {
-            unsigned wr[4], wi[4];
-#pragma unroll
-            for (int g = 0; g < 4; ++g) {
-              int re[4], im[4];
-#pragma unroll
-              for (int b = 0; b < 4; ++b) {
-                const int x1 = unpack_i8(t1[ch * 4 + g], b), x2 = unpack_i8(t2[ch * 4 + g], b), x3 = unpack_i8(w[g], b);
-                re[b] = sym_small_rt(x1 - x2, mod);
-                im[b] = sym_small_rt(x3 - x1 - x2, mod);
+              for (int g = 0; g < 8; ++g) {
+                const unsigned w = pack4i(reduce_mod(dot_mod(v[4 * g], mk), mk), reduce_mod(dot_mod(v[4 * g + 1], mk), mk),
+                                          reduce_mod(dot_mod(v[4 * g + 2], mk), mk), reduce_mod(dot_mod(v[4 * g + 3], mk), mk));
+                if (q == 0) t1[ch * 8 + g] = w; else t2[ch * 8 + g] = w;
               }
-              wr[g] = pack4i(re[0], re[1], re[2], re[3]);
-              wi[g] = pack4i(im[0], im[1], im[2], im[3]);
-            }
-            if (row_ok && gcol < a.n) {
-              int8_t *o = a.CR + (static_cast<int64_t>(l) * a.m + grow) * a.n + gcol;
-              store16(o, wr, gcol, a.n, vec_ok);
-              store16(o + a.n_moduli * plane_sz, wi, gcol, a.n, vec_ok);
+            } else {
+              // c_re = sym(T1 - T2), c_im = sym(T3 - T1 - T2) (Eq. 16): all in residues, one reduction for the
+              // imaginary part (T3's byte dot product + 2m - r1 - r2 < 2^19), two compares for the real part
+              unsigned wr[8], wi[8];
+#pragma unroll
+              for (int g = 0; g < 8; ++g) {
+                unsigned re[4], im[4];
+#pragma unroll
+                for (int b = 0; b < 4; ++b) {
+                  const unsigned r1 = byte_u(t1[ch * 8 + g], b), r2 = byte_u(t2[ch * 8 + g], b);
+                  int d = static_cast<int>(r1) - static_cast<int>(r2);            // (-m, m)
+                  d -= (d >= static_cast<int>(mk.half)) ? static_cast<int>(mk.m) : 0;
+                  d += (d < static_cast<int>(mk.half) - static_cast<int>(mk.m)) ? static_cast<int>(mk.m) : 0;
+                  re[b] = static_cast<unsigned>(d);
+                  const unsigned vi = dot_mod(v[4 * g + b], mk) + 2u * mk.m - r1 - r2;  // >= 0, == T3 - T1 - T2 (mod m)
+                  im[b] = static_cast<unsigned>(to_sym(reduce_mod(vi, mk), mk));
+                }
+                wr[g] = pack4i(re[0], re[1], re[2], re[3]);
+                wi[g] = pack4i(im[0], im[1], im[2], im[3]);
+              }
+              if (row_ok && gcol < a.n && !(a.dbg & 4)) {
+                int8_t *o = a.CR + (static_cast<int64_t>(l) * a.m + grow) * a.n + gcol;
+                store32(o, wr, gcol, a.n, vec_ok);
+                store32(o + a.n_moduli * plane_sz, wi, gcol, a.n, vec_ok);
+              }
             }
           }
         }
@@ -238,20 +254,26 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
   d.mt = static_cast<int>((g.m + kTileM - 1) / kTileM);
   d.nt_tiles = static_cast<int>((g.n + kOz2NT - 1) / kOz2NT);
   d.n_moduli = g.n_moduli;
-  d.nprod = parts;
   d.CR = g.CR;
   d.cycles = g.cycles;
+  d.dbg = ctx->dbg_flags;
   int mod[24];
   oz2_moduli_host(g.n_moduli, mod);
   for (int l = 0; l < kMaxModuli; ++l) {
-    d.mod[l] = l < g.n_moduli ? mod[l] : 256;
-    d.magic[l] = static_cast<unsigned>(((1ull << 39) + static_cast<unsigned long long>(d.mod[l]) - 1ull) /
-                                       static_cast<unsigned long long>(d.mod[l]));
+    const unsigned m = static_cast<unsigned>(l < g.n_moduli ? mod[l] : 256);
+    d.mod[l] = static_cast<int>(m);
+    unsigned pw[4], r = 1u % m;
+    for (int j = 0; j < 4; ++j) { pw[j] = r; r = (r * 256u) % m; }
+    d.cvec[l] = pw[0] | (pw[1] << 8) | (pw[2] << 16) | (pw[3] << 24);
+    const unsigned two31 = static_cast<unsigned>((1ull << 31) % m);
+    d.c0[l] = (m - two31) % m;
+    d.magic[l] = static_cast<unsigned>(((1ull << 32) + m - 1ull) / m);
   }
   const int64_t tiles = static_cast<int64_t>(d.mt) * d.nt_tiles * d.n_moduli;
   const int grid = tiles < ctx->num_sms ? static_cast<int>(tiles) : ctx->num_sms;
-  EMU_CUDA(ctx, cudaFuncSetAttribute(oz2_gemm_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, kOz2Smem));
-  oz2_gemm_kernel<<<grid, kGemmThreads, kOz2Smem, ctx->stream>>>(tmA, tmB, d);
+  auto kern = g.is3m ? oz2_gemm_kernel<3> : oz2_gemm_kernel<1>;
+  EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kOz2Smem));
+  kern<<<grid, kGemmThreads, kOz2Smem, ctx->stream>>>(tmA, tmB, d);
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
   return EMUGEMM_OK;
