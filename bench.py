@@ -79,8 +79,9 @@ def make_inputs(a, w, seed_offset=0):
 
 
 class ClockSampler:
-    """nvidia-smi clocks line of B200_PROFILING.md, sampled every 200 ms during the timed region."""
-    Q = ("index,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
+    """nvidia-smi clocks line of B200_PROFILING.md, sampled every 50 ms; only samples whose timestamp falls inside
+    the timed window [t0, t1] (host clock, taken right after / before a device synchronize) are used."""
+    Q = ("timestamp,clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.active,clocks_event_reasons.hw_slowdown,"
          "clocks_event_reasons.hw_thermal_slowdown,clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
 
     def __init__(self, gpu_index):
@@ -91,35 +92,40 @@ class ClockSampler:
     def start(self):
         try:
             self.p = subprocess.Popen(["nvidia-smi", f"--id={self.idx}", f"--query-gpu={self.Q}", "--format=csv,noheader,nounits",
-                                       "-lms", "100"], stdout=self.f, stderr=subprocess.DEVNULL)
+                                       "-lms", "50"], stdout=self.f, stderr=subprocess.DEVNULL)
         except OSError:
             self.p = None
 
-    def stop(self):
+    def stop(self, t0, t1):
+        import datetime
         if self.p is None:
             return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
-        time.sleep(0.05)
+        time.sleep(0.06)
         self.p.terminate()
         self.p.wait()
         self.f.flush()
         rows = [r.strip().split(", ") for r in open(self.f.name) if r.strip()]
         os.unlink(self.f.name)
-        sm, mx, pw, reasons = [], [], [], set()
+        sm, mx, pw, reasons, n_all = [], [], [], set(), 0
         for r in rows:
             if len(r) < 9:
                 continue
             try:
-                sm.append(float(r[1])); mx.append(float(r[2])); pw.append(float(r[3]))
+                ts = datetime.datetime.strptime(r[0], "%Y/%m/%d %H:%M:%S.%f").timestamp()
+                c, m, w = float(r[1]), float(r[2]), float(r[3])
             except ValueError:
                 continue
+            n_all += 1
+            if not (t0 <= ts <= t1):
+                continue
+            sm.append(c); mx.append(m); pw.append(w)
             for name, v in zip(("hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"), r[5:9]):
                 if v.strip().lower() == "active":
                     reasons.add(name)
         if not sm:
-            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples"]}
-        busy = [s for s in sm if s > 0.5 * max(sm)] or sm
-        return {"sm_mhz": statistics.median(busy), "sm_max_mhz": max(mx), "power_w_max": max(pw), "samples": len(sm),
-                "reasons": sorted(reasons)}
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["no samples in the timed window"], "samples_total": n_all}
+        return {"sm_mhz": statistics.median(sm), "sm_min_mhz": min(sm), "sm_max_mhz": max(mx), "power_w_max": max(pw),
+                "samples": len(sm), "reasons": sorted(reasons)}
 
 
 def cpu_oracle_leg(a, w, sample):
@@ -185,6 +191,7 @@ def main():
     import numpy as np
     import torch
     import paper_2606_25453_b200 as E
+    from paper_2606_25453_b200 import shard
 
     assert torch.cuda.is_available(), "bench.py needs a GPU: the product path has no CPU fallback"
     torch.cuda.set_device(local)
@@ -199,7 +206,7 @@ def main():
         torch.cuda.synchronize()
 
     # independent problem per rank (weak scaling): same recipe, seed offset by rank
-    A, B = make_inputs(a, w, seed_offset=1000 * rank)
+    A, B = make_inputs(a, w, seed_offset=shard.rank_seed(0, rank))
     cdtype = {"oz1": torch.float64, "oz1s": torch.float32, "oz2": torch.float64, "oz2z": torch.complex128}[a.scheme]
     hA, hB = torch.from_numpy(A).pin_memory(), torch.from_numpy(B).pin_memory()
     hC = torch.empty((w["m"], w["n"]), dtype=cdtype).pin_memory()
@@ -223,14 +230,16 @@ def main():
     torch.cuda.synchronize()
 
     # ---- device-resident timing: W warm-ups, then exactly K steps between barriers ----
+    sampler = ClockSampler(local)
+    sampler.start()
     for _ in range(max(a.warmup, 3)):
         step()
     h.enable_stage_timing(True)
-    sampler = ClockSampler(local)
     barrier()
-    sampler.start()
+    t_win0 = time.time()
     e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
     stage = [[], [], []]
+    cycles = []
     launches = 0
     e0.record(stream)
     for _ in range(a.steps):
@@ -240,9 +249,9 @@ def main():
         for i in range(3):
             stage[i].append(ms[i])
         launches += nl
+        cycles.append(h.last_gemm_cycles())
     e1.record(stream)
     barrier()
-    clocks = sampler.stop()
     total_ms = e0.elapsed_time(e1)
     h.enable_stage_timing(False)
 
@@ -254,12 +263,9 @@ def main():
         step()
     f1.record(stream)
     barrier()
-    ms_step = f0.elapsed_time(f1) / a.steps
-    t = torch.tensor([ms_step], dtype=torch.float64, device="cuda")
-    if dist is not None:
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-    ms_step = float(t.item())
-    value = world * w["flops"] / (ms_step * 1e-3) / 1e12
+    clocks = sampler.stop(t_win0, time.time())
+    ms_step = shard.max_over_ranks(f0.elapsed_time(f1) / a.steps, dist, "cuda")
+    value = shard.aggregate_throughput(w["flops"], world, ms_step) / 1e12
 
     # ---- end to end: host (pinned) buffers, H2D + call + D2H inside the timed region ----
     e2e = None
@@ -274,11 +280,9 @@ def main():
             step_e2e()
         g1.record(stream)
         barrier()
-        t2 = torch.tensor([g0.elapsed_time(g1) / n_e2e], dtype=torch.float64, device="cuda")
-        if dist is not None:
-            dist.all_reduce(t2, op=dist.ReduceOp.MAX)
-        e2e = {"value": world * w["flops"] / (float(t2.item()) * 1e-3) / 1e12, "unit": "TFLOP/s",
-               "ms_per_step": float(t2.item()),
+        ms_e2e = shard.max_over_ranks(g0.elapsed_time(g1) / n_e2e, dist, "cuda")
+        e2e = {"value": shard.aggregate_throughput(w["flops"], world, ms_e2e) / 1e12, "unit": "TFLOP/s",
+               "ms_per_step": ms_e2e,
                "h2d_bytes_per_step": int(hA.numel() * hA.element_size() + hB.numel() * hB.element_size()),
                "d2h_bytes_per_step": int(hC.numel() * hC.element_size())}
 
@@ -313,6 +317,11 @@ def main():
         roof["frac_of_sustained"] = achieved / (2.0 * peaks["bf16_tflops_sustained"])
     if clocks.get("sm_mhz"):
         roof["frac_of_clock_scaled"] = achieved / (148 * 16384 * clocks["sm_mhz"] * 1e6 / 1e12)
+    if cycles and min(cycles) > 0:
+        # SM cycle counter of the GEMM kernel (CTA 0): INT8 ops per clock per SM against 16384, clock-independent
+        cyc = statistics.median(cycles)
+        roof["per_clock_efficiency"] = w["ops"] / (cyc * 148) / 16384.0
+        roof["sm_ghz_during_kernel"] = cyc / (gemm_ms * 1e-3) / 1e9
 
     detail = {"stage_ms_median": {"prepass": statistics.median(stage[0]), "gemm": gemm_ms, "recon": statistics.median(stage[2])},
               "synced_ms_per_step": total_ms / a.steps,

@@ -1,0 +1,111 @@
+"""-m gpu: parity at BASELINE.json's full sizes, in the launch configuration bench.py times (same C-ABI
+calls, same workspace path), on SAMPLED outputs the oracle computes one by one (SURVEY 8(c) "Parity at large
+sizes"): ~40 x 40 sampled elements incl. first/last rows/columns and both sides of tile boundaries.
+Tolerance: 2 ulp of (|A||B|)_ij at the sampled elements (FP32 path: 2 ulp in FP32)."""
+import numpy as np
+import pytest
+
+import emugemm_inputs as G
+from gpu_util import assert_within_ulps
+
+pytestmark = pytest.mark.gpu
+
+
+@pytest.fixture(scope="module")
+def env():
+    import torch
+    from oracle import oracle as O
+    import paper_2606_25453_b200 as E
+    h = E.EmuGemm()
+    yield torch, O, h
+    h.close()
+
+
+def _abs_ab(A, B, rows, cols):
+    return np.abs(A[rows, :]).astype(np.float64) @ np.abs(B[:, cols]).astype(np.float64)
+
+
+def _samples(m, n, seed, count=36):
+    return G.sample_indices(m, count, seed)[:48], G.sample_indices(n, count, seed + 1)[:48]
+
+
+@pytest.mark.parametrize("size,p,phi", [(8192, 8, 2.0), (8192, 3, 0.5), (4096, 5, 2.0), (2048, 6, 0.5)])
+def test_config1_oz1_sweep_points(env, size, p, phi):
+    """BASELINE configs[1]: Scheme I DGEMM square sweep, seed 1."""
+    torch, O, h = env
+    A, B = G.real_pair(size, size, size, phi, 1)
+    C = torch.full((size, size), float("nan"), dtype=torch.float64, device="cuda")
+    h.dgemm_oz1(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, p)
+    rows, cols = _samples(size, size, 7)
+    got = C[torch.from_numpy(rows).cuda()][:, torch.from_numpy(cols).cuda()].cpu().numpy()
+    want = O.oz1_sampled(A, B, p, rows, cols)
+    assert_within_ulps(got, want, _abs_ab(A, B, rows, cols), 2, what=f"oz1 {size} p={p}")
+    assert torch.isfinite(C).all()
+
+
+@pytest.mark.parametrize("N", [12, 20])
+def test_config2_oz2_8192(env, N):
+    """BASELINE configs[2]: Scheme II DGEMM 8192^3, phi 1, seed 2."""
+    torch, O, h = env
+    size = 8192
+    A, B = G.real_pair(size, size, size, 1.0, 2)
+    C = torch.full((size, size), float("nan"), dtype=torch.float64, device="cuda")
+    h.dgemm_oz2(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, N)
+    rows, cols = _samples(size, size, 9)
+    got = C[torch.from_numpy(rows).cuda()][:, torch.from_numpy(cols).cuda()].cpu().numpy()
+    want = O.oz2_sampled(A, B, N, rows, cols)
+    assert_within_ulps(got, want, _abs_ab(A, B, rows, cols), 2, what=f"oz2 N={N}")
+    assert torch.isfinite(C).all()
+
+
+@pytest.mark.parametrize("size,N", [(4096, 14), (4096, 18)])
+def test_config3_zgemm_3m(env, size, N):
+    """BASELINE configs[3]: ZGEMM via 3M, phi 1 on re and im, seed 3."""
+    torch, O, h = env
+    A, B = G.complex_pair(size, size, size, 1.0, 3)
+    C = torch.zeros((size, size), dtype=torch.complex128, device="cuda")
+    h.zgemm_oz2_3m(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, N)
+    rows, cols = _samples(size, size, 11, count=24)
+    got = C[torch.from_numpy(rows).cuda()][:, torch.from_numpy(cols).cuda()].cpu().numpy()
+    want = O.oz2_sampled(A, B, N, rows, cols, is3m=True)
+    scale = (np.abs(A.real[rows]) + np.abs(A.imag[rows])) @ (np.abs(B.real[:, cols]) + np.abs(B.imag[:, cols]))
+    assert_within_ulps(got.real, want.real, scale, 2, what="3M re")
+    assert_within_ulps(got.imag, want.imag, scale, 2, what="3M im")
+
+
+def test_config4_tall_skinny_k_chunked(env):
+    """BASELINE configs[4]: p = 7, m = n = 1024, k = 65536 -> 4 overflow-safe k-chunks + exact reduction."""
+    torch, O, h = env
+    m, n, k, p = 1024, 1024, 65536, 7
+    A, B = G.real_pair(m, n, k, 1.0, 4)
+    C = torch.zeros((m, n), dtype=torch.float64, device="cuda")
+    h.dgemm_oz1(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, p)
+    rows, cols = _samples(m, n, 13)
+    got = C[torch.from_numpy(rows).cuda()][:, torch.from_numpy(cols).cuda()].cpu().numpy()
+    assert_within_ulps(got, O.oz1_sampled(A, B, p, rows, cols), _abs_ab(A, B, rows, cols), 2, what="k=65536")
+
+
+def test_config4_wide_m_narrow_n(env):
+    """BASELINE configs[4]: p = 7, m = 16384, n = 256, k = 4096."""
+    torch, O, h = env
+    m, n, k, p = 16384, 256, 4096, 7
+    A, B = G.real_pair(m, n, k, 1.0, 4)
+    C = torch.zeros((m, n), dtype=torch.float64, device="cuda")
+    h.dgemm_oz1(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, p)
+    rows, cols = _samples(m, n, 15)
+    got = C[torch.from_numpy(rows).cuda()][:, torch.from_numpy(cols).cuda()].cpu().numpy()
+    assert_within_ulps(got, O.oz1_sampled(A, B, p, rows, cols), _abs_ab(A, B, rows, cols), 2, what="16384x256")
+
+
+@pytest.mark.parametrize("p", [3, 4])
+def test_config4_sgemm_16384(env, p):
+    """BASELINE configs[4]: FP32-input emulation at m = n = k = 16384."""
+    torch, O, h = env
+    size = 16384
+    A, B = G.real_pair(size, size, size, 1.0, 4, dtype=np.float32)
+    C = torch.zeros((size, size), dtype=torch.float32, device="cuda")
+    h.sgemm_oz1(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, p)
+    rows, cols = _samples(size, size, 17, count=24)
+    got = C[torch.from_numpy(rows).cuda()][:, torch.from_numpy(cols).cuda()].cpu().numpy()
+    want = O.oz1_sampled(A, B, p, rows, cols, is_f32=True)
+    assert_within_ulps(got, want, _abs_ab(A, B, rows, cols), 2, bits=23, what=f"sgemm 16384 p={p}")
