@@ -9,19 +9,24 @@
 // c_re = sym(T1 - T2), c_im = sym(T3 - T1 - T2) are the only two tiles written.
 //
 // B200-first design: ONE persistent launch covers all moduli (work item =
-// (modulus, tile, product)); 128 x 256 tiles, 4-stage TMA ring of 128-byte
-// k-blocks, TMEM holds two 256-column INT32 accumulators so the mod-epilogue of
-// one item overlaps the MMAs of the next (the paper reuses one accumulator and
-// overlaps only with TMA prefetch).
+// (modulus, pair tile, product)).  A CTA PAIR (cluster of 2, tcgen05 cta_group::2)
+// owns a 256 x 256 output tile: each CTA loads its own 128 rows of A and its own
+// 128 of the 256 B rows per 128-byte k-block (32 KB per stage and CTA instead of
+// 48 KB), the leader CTA issues one 256 x 256 x 32 MMA per k32 for both SMs, and
+// each CTA's tensor core reads only half of B from its shared memory.  6-stage
+// TMA ring; TMEM holds two 256-column INT32 accumulators per CTA so the
+// mod-epilogue of one item overlaps the MMAs of the next (the paper reuses one
+// accumulator and overlaps only with TMA prefetch).
 #include "common.cuh"
 #include "ptx.cuh"
 #include "gemm_common.cuh"
 
 namespace emu {
 
-constexpr int kOz2NT = 256;
-constexpr int kOz2Stages = 4;
-constexpr int kOz2BStage = kOz2NT * kBlockK;  // 32 KB
+constexpr int kOz2NT = 256;                   // tile columns
+constexpr int kOz2PairM = 2 * kTileM;         // tile rows of a CTA pair
+constexpr int kOz2Stages = 6;
+constexpr int kOz2BStage = (kOz2NT / 2) * kBlockK;  // 16 KB: this CTA's half of the B rows
 constexpr int kOz2StageBytes = kAStageBytes + kOz2BStage;
 constexpr int kOz2Smem = kOz2Stages * kOz2StageBytes + 1024 + 256;
 
@@ -74,7 +79,7 @@ __device__ __forceinline__ void store32(int8_t *dst, const unsigned (&w)[8], int
 }
 
 template <int NPROD>  // 1: real (Eq. 6-7); 3: 3M (Eq. 16-18)
-__global__ void __launch_bounds__(kGemmThreads, 1)
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1)
 oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const Oz2Dev a) {
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -83,42 +88,50 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   uint32_t *tmem_slot = reinterpret_cast<uint32_t *>(tempty + 2);
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-  const int tiles_per_mod = a.mt * a.nt_tiles;
+  const uint32_t cta = cluster_ctarank();  // 0 = leader (issues the MMAs), 1 = peer
+  const int cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
+  const int tiles_per_mod = a.mt * a.nt_tiles;  // a.mt counts PAIR tiles of 256 rows
   const int num_tiles = tiles_per_mod * a.n_moduli;
 
   if (threadIdx.x == 0) {
+    // full[s] (leader's is the one used): 1 arrival (leader's expect_tx) + the bytes of BOTH CTAs' loads;
+    // empty[s], tfull[b]: 1 arrival from the leader's multicast commit; tempty[b] (leader's): all epilogue warps of the pair
     for (int i = 0; i < kOz2Stages; ++i) { mbar_init(&full[i], 1); mbar_init(&empty[i], 1); }
-    for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], kEpiWarps); }
+    for (int i = 0; i < 2; ++i) { mbar_init(&tfull[i], 1); mbar_init(&tempty[i], 2 * kEpiWarps); }
     fence_mbar_init();
     tma_prefetch_desc(&tmA);
     tma_prefetch_desc(&tmB);
   }
   if (warp == 1) {
-    tmem_alloc(tmem_slot, 512);
-    tmem_relinquish();
+    tmem_alloc_cg2(tmem_slot, 512);
+    tmem_relinquish_cg2();
   }
   tc_fence_before();
-  __syncthreads();
+  cluster_sync_all();  // the peer's barriers must be initialised before remote arrivals / remote complete_tx
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   const long long t_start = clock64();
 
   if (warp == 0) {
+    // ===================== TMA producer (one per CTA: own A rows, own half of the B rows) =====================
     if (lane == 0) {
       int st = 0;
       uint32_t ph = 0;
-      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      for (int tile = cluster_id; tile < num_tiles; tile += num_clusters) {
         const int l = tile / tiles_per_mod;
         int mb, nb;
         tile_coords(tile - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb);
+        const int arow = mb * kOz2PairM + static_cast<int>(cta) * kTileM;
+        const int brow = nb * kOz2NT + static_cast<int>(cta) * (kOz2NT / 2);
         for (int q = 0; q < NPROD; ++q) {
           const int plane = q * a.n_moduli + l;
           for (int kb = 0; kb < a.kblocks; ++kb) {
             mbar_wait(&empty[st], ph ^ 1);
-            mbar_arrive_expect_tx(&full[st], kOz2StageBytes);
+            const uint32_t full_leader = mapa_u32(&full[st], 0);
+            if (cta == 0) mbar_arrive_expect_tx(&full[st], 2 * kOz2StageBytes);
             uint8_t *dst = smem + st * kOz2StageBytes;
-            tma_load_3d(dst, &tmA, &full[st], kb * kBlockK, mb * kTileM, plane);
-            tma_load_3d(dst + kAStageBytes, &tmB, &full[st], kb * kBlockK, nb * kOz2NT, plane);
+            tma_load_3d_cg2(dst, &tmA, full_leader, kb * kBlockK, arow, plane);
+            tma_load_3d_cg2(dst + kAStageBytes, &tmB, full_leader, kb * kBlockK, brow, plane);
             if (++st == kOz2Stages) { st = 0; ph ^= 1; }
           }
         }
@@ -126,28 +139,32 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     }
     __syncwarp();
   } else if (warp == 1) {
-    if (lane == 0) {
+    // ===================== MMA issuer (leader CTA only) =====================
+    if (lane == 0 && cta == 0) {
       int st = 0;
       uint32_t ph = 0;
       uint32_t item = 0;
-      constexpr uint32_t idesc = make_idesc_i8(kTileM, kOz2NT);
-      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      constexpr uint32_t idesc = make_idesc_i8(kOz2PairM, kOz2NT);
+      bool ready = false;  // look-ahead probe of the next stage's barrier (see gemm_oz1.cu)
+      for (int tile = cluster_id; tile < num_tiles; tile += num_clusters) {
         for (int q = 0; q < NPROD; ++q, ++item) {
           const uint32_t slot = item & 1, tph = (item >> 1) & 1;
           mbar_wait(&tempty[slot], tph ^ 1);
           tc_fence_after();
           for (int kb = 0; kb < a.kblocks; ++kb) {
-            mbar_wait(&full[st], ph);
+            if (!ready) mbar_wait(&full[st], ph);
             tc_fence_after();
             const uint32_t a_base = smem_u32(smem + st * kOz2StageBytes), b_base = a_base + kAStageBytes;
+            const int st_cur = st;
+            if (++st == kOz2Stages) { st = 0; ph ^= 1; }
+            ready = mbar_try_wait(&full[st], ph);
 #pragma unroll
             for (int ks = 0; ks < kBlockK / 32; ++ks)
-              umma_i8(tmem_base + slot * kOz2NT, make_sdesc_sw128(a_base + ks * 32), make_sdesc_sw128(b_base + ks * 32),
-                      idesc, (kb | ks) ? 1u : 0u);
-            umma_commit(&empty[st]);
-            if (++st == kOz2Stages) { st = 0; ph ^= 1; }
+              umma_i8_cg2(tmem_base + slot * kOz2NT, make_sdesc_sw128(a_base + ks * 32), make_sdesc_sw128(b_base + ks * 32),
+                          idesc, (kb | ks) ? 1u : 0u);
+            umma_commit_cg2(&empty[st_cur], 3);  // both CTAs' producers may refill the stage
           }
-          umma_commit(&tfull[slot]);
+          umma_commit_cg2(&tfull[slot], 3);      // both CTAs' epilogues may drain their 128 rows
         }
       }
     }
@@ -160,13 +177,14 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     const int64_t plane_sz = a.m * a.n;
     uint32_t item = 0;
     unsigned t1[NPROD == 3 ? 32 : 1], t2[NPROD == 3 ? 32 : 1];  // T1, T2 of this thread's 128 columns as packed INT8 (3M)
-    for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+    const uint32_t tempty_leader[2] = {mapa_u32(&tempty[0], 0), mapa_u32(&tempty[1], 0)};
+    for (int tile = cluster_id; tile < num_tiles; tile += num_clusters) {
       const int l = tile / tiles_per_mod;
       int mb, nb;
       tile_coords(tile - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb);
       ModK mk;
       mk.cvec = a.cvec[l]; mk.c0 = a.c0[l]; mk.magic = a.magic[l]; mk.m = static_cast<unsigned>(a.mod[l]); mk.half = (mk.m + 1) / 2;
-      const int64_t grow = static_cast<int64_t>(mb) * kTileM + row;
+      const int64_t grow = static_cast<int64_t>(mb) * kOz2PairM + cta * kTileM + row;
       const bool row_ok = grow < a.m;
 #pragma unroll
       for (int q = 0; q < NPROD; ++q, ++item) {
@@ -231,14 +249,14 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         }
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(&tempty[slot]);
+        if (lane == 0) mbar_arrive_remote(tempty_leader[slot]);  // the leader's MMA thread waits for both CTAs
       }
     }
   }
 
   tc_fence_before();
-  __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem_base, 512);
+  cluster_sync_all();  // neither CTA may free TMEM / exit while the pair's MMAs or remote arrivals are in flight
+  if (warp == 1) tmem_dealloc_cg2(tmem_base, 512);
   if (blockIdx.x == 0 && threadIdx.x == 0 && a.cycles) atomicAdd(a.cycles, static_cast<unsigned long long>(clock64() - t_start));
 }
 
@@ -247,11 +265,11 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
   const int parts = g.is3m ? 3 : 1;
   CUtensorMap tmA, tmB;
   EMU_TRY(encode_planes_tmap(ctx, &tmA, g.RA, g.kpad, g.m, static_cast<int64_t>(parts) * g.n_moduli, kTileM, 1));
-  EMU_TRY(encode_planes_tmap(ctx, &tmB, g.RB, g.kpad, g.n, static_cast<int64_t>(parts) * g.n_moduli, kOz2NT, 1));
+  EMU_TRY(encode_planes_tmap(ctx, &tmB, g.RB, g.kpad, g.n, static_cast<int64_t>(parts) * g.n_moduli, kOz2NT / 2, 1));
   Oz2Dev d;
   d.m = g.m; d.n = g.n;
   d.kblocks = static_cast<int>(g.kpad / kBlockK);
-  d.mt = static_cast<int>((g.m + kTileM - 1) / kTileM);
+  d.mt = static_cast<int>((g.m + kOz2PairM - 1) / kOz2PairM);  // pair tiles
   d.nt_tiles = static_cast<int>((g.n + kOz2NT - 1) / kOz2NT);
   d.n_moduli = g.n_moduli;
   d.CR = g.CR;
@@ -270,7 +288,8 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
     d.magic[l] = static_cast<unsigned>(((1ull << 32) + m - 1ull) / m);
   }
   const int64_t tiles = static_cast<int64_t>(d.mt) * d.nt_tiles * d.n_moduli;
-  const int grid = tiles < ctx->num_sms ? static_cast<int>(tiles) : ctx->num_sms;
+  const int pairs = ctx->num_sms / 2;
+  const int grid = 2 * (tiles < pairs ? static_cast<int>(tiles) : pairs);
   auto kern = g.is3m ? oz2_gemm_kernel<3> : oz2_gemm_kernel<1>;
   EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kOz2Smem));
   kern<<<grid, kGemmThreads, kOz2Smem, ctx->stream>>>(tmA, tmB, d);
