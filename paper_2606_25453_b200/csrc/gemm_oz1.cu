@@ -29,11 +29,13 @@ namespace emu {
 
 constexpr bool kUseCollector = true;  // A-operand collector reuse across the MMAs of one (t, ks)
 
-template <int P>
+template <int P, bool PAIR = false>
 struct Oz1Cfg {
   // NT: tile width; P * NT <= 512 TMEM columns, every MMA width a multiple of 16
   static constexpr int NT = (P <= 2) ? 256 : (P == 3) ? 160 : (P == 4) ? 128 : (P == 5) ? 96 : (P == 6) ? 80 : 64;
-  static constexpr int kBStageBytes = P * NT * kBlockK;
+  // PAIR (cta_group::2, P <= 4): a CTA pair owns a 256 x NT tile; each CTA stages only NT/2 rows of every B slice
+  static constexpr int kBRows = PAIR ? NT / 2 : NT;
+  static constexpr int kBStageBytes = P * kBRows * kBlockK;
   static constexpr int SB = 2;
   // A ring: one stage = the slice PAIR (j, P-1-j) of a k-block (2 x 16 KB).  Pairing the widest with the
   // narrowest slice gives every stage the same MMA time ((P+1) NT/2 clk per k32), so the single issuing thread
@@ -41,8 +43,9 @@ struct Oz1Cfg {
   // on the narrow slices (measured: +11 % tensor-pipe activity over one barrier per slice).
   static constexpr int NPAIR = (P + 1) / 2;
   static constexpr int kAPairBytes = 2 * kAStageBytes;
-  static constexpr int SA = (kSmemLimit - 2048 - SB * kBStageBytes) / kAPairBytes > 4
-                                ? 4
+  static constexpr int kSAMax = PAIR ? 5 : 4;
+  static constexpr int SA = (kSmemLimit - 2048 - SB * kBStageBytes) / kAPairBytes > kSAMax
+                                ? kSAMax
                                 : (kSmemLimit - 2048 - SB * kBStageBytes) / kAPairBytes;
   static constexpr int kTmemCols = (P * NT <= 256) ? 256 : 512;
   static constexpr int kSmemBytes = SB * kBStageBytes + SA * kAPairBytes + 1024 /*align*/ + 256 /*barriers*/;
@@ -103,6 +106,32 @@ __device__ __forceinline__ void oz1_issue_slice_per_product(int t, uint32_t tmem
         else if (COLL && !first && last) umma_i8<3>(d, adesc, bdesc, idesc, acc);
         else if (COLL && !first && !last) umma_i8<2>(d, adesc, bdesc, idesc, acc);
         else umma_i8<0>(d, adesc, bdesc, idesc, acc);
+      }
+    }
+  }
+}
+
+// CTA-pair schedule (cta_group::2, P <= 4 where NT >= 128): one 256 x NT x 32 MMA per product, issued by the leader
+// CTA for both SMs; CTA r supplies rows 128 r .. of A_t and rows NT/2 r .. of B_u from its own shared memory, so the
+// columns of D come out in natural order and land on C_{t+u}.  A_t stays in the collector across its P - t MMAs.
+template <int P>
+__device__ __forceinline__ void oz1_issue_slice_pair(int t, uint32_t tmem_base, uint32_t a_base, uint32_t b_base, bool accumulate) {
+  constexpr int NT = Oz1Cfg<P, true>::NT;
+  constexpr uint32_t idesc = make_idesc_i8(2 * kTileM, NT);
+#pragma unroll
+  for (int ks = 0; ks < kBlockK / 32; ++ks) {
+    const uint64_t adesc = make_sdesc_sw128(a_base + ks * 32);
+#pragma unroll
+    for (int u = 0; u < P; ++u) {
+      if (u < P - t) {
+        const uint32_t acc = (accumulate || ks != 0) ? 1u : 0u;
+        const uint32_t d = tmem_base + (t + u) * NT;
+        const uint64_t bdesc = make_sdesc_sw128(b_base + u * (NT / 2) * kBlockK + ks * 32);
+        const bool first = (u == 0), last = (u == P - t - 1);
+        if (first && !last) umma_i8_cg2<1>(d, adesc, bdesc, idesc, acc);
+        else if (!first && last) umma_i8_cg2<3>(d, adesc, bdesc, idesc, acc);
+        else if (!first && !last) umma_i8_cg2<2>(d, adesc, bdesc, idesc, acc);
+        else umma_i8_cg2<0>(d, adesc, bdesc, idesc, acc);
       }
     }
   }
@@ -259,10 +288,10 @@ struct Oz1Epi {
   }
 };
 
-template <int P, int OUT>
+template <int P, int OUT, bool PAIR>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const Oz1Dev a) {
-  using Cfg = Oz1Cfg<P>;
+  using Cfg = Oz1Cfg<P, PAIR>;
   constexpr int NT = Cfg::NT, SA = Cfg::SA, SB = Cfg::SB;
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
@@ -275,22 +304,28 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int num_tiles = a.mt * a.nt_tiles;
+  // PAIR: the two CTAs of a cluster work on one 256-row tile; rank 0 (leader) issues the MMAs for both
+  const uint32_t cta = PAIR ? cluster_ctarank() : 0u;
+  const int work_id = PAIR ? static_cast<int>(blockIdx.x >> 1) : static_cast<int>(blockIdx.x);
+  const int num_workers = PAIR ? static_cast<int>(gridDim.x >> 1) : static_cast<int>(gridDim.x);
+  constexpr int kTileRows = PAIR ? 2 * kTileM : kTileM;
+  constexpr uint32_t kTxMul = PAIR ? 2u : 1u;  // the leader's "full" barriers collect the bytes of both CTAs
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < SB; ++i) { mbar_init(&bfull[i], 1); mbar_init(&bempty[i], 1); }
     for (int i = 0; i < SA; ++i) { mbar_init(&afull[i], 1); mbar_init(&aempty[i], 1); }
     mbar_init(tfull, 1);
-    mbar_init(tempty, kEpiWarps);
+    mbar_init(tempty, PAIR ? 2 * kEpiWarps : kEpiWarps);
     fence_mbar_init();
     tma_prefetch_desc(&tmA);
     tma_prefetch_desc(&tmB);
   }
   if (warp == 1) {
-    tmem_alloc(tmem_slot, Cfg::kTmemCols);
-    tmem_relinquish();
+    if constexpr (PAIR) { tmem_alloc_cg2(tmem_slot, Cfg::kTmemCols); tmem_relinquish_cg2(); }
+    else { tmem_alloc(tmem_slot, Cfg::kTmemCols); tmem_relinquish(); }
   }
   tc_fence_before();
-  __syncthreads();
+  if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   const long long t_start = clock64();
@@ -300,15 +335,20 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (lane == 0) {
       int sa = 0, sb = 0, nloada = 0, nloadb = 0;
       uint32_t pa = 0, pb = 0;
-      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      for (int tile = work_id; tile < num_tiles; tile += num_workers) {
         int mb, nb;
         tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
         for (int kb = a.kb0; kb < a.kb1; ++kb) {
           mbar_wait(&bempty[sb], pb ^ 1);
-          if ((a.dbg & 1) && nloadb >= SB) mbar_arrive(&bfull[sb]);
-          else {
-          mbar_arrive_expect_tx(&bfull[sb], Cfg::kBStageBytes);
-          tma_load_3d(sB + sb * Cfg::kBStageBytes, &tmB, &bfull[sb], kb * kBlockK, nb * NT, 0);
+          if constexpr (PAIR) {
+            if (cta == 0) mbar_arrive_expect_tx(&bfull[sb], kTxMul * Cfg::kBStageBytes);
+            tma_load_3d_cg2(sB + sb * Cfg::kBStageBytes, &tmB, mapa_u32(&bfull[sb], 0), kb * kBlockK,
+                            nb * NT + static_cast<int>(cta) * Cfg::kBRows, 0);
+          } else if ((a.dbg & 1) && nloadb >= SB) {
+            mbar_arrive(&bfull[sb]);
+          } else {
+            mbar_arrive_expect_tx(&bfull[sb], Cfg::kBStageBytes);
+            tma_load_3d(sB + sb * Cfg::kBStageBytes, &tmB, &bfull[sb], kb * kBlockK, nb * NT, 0);
           }
           ++nloadb;
           if (++sb == SB) { sb = 0; pb ^= 1; }
@@ -316,9 +356,16 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
           for (int j = 0; j < Cfg::NPAIR; ++j) {
             const int lo = j, hi = P - 1 - j;
             mbar_wait(&aempty[sa], pa ^ 1);
-            if ((a.dbg & 1) && nloada >= SA) mbar_arrive(&afull[sa]);
-            else {
-              uint8_t *dst = sA + sa * Cfg::kAPairBytes;
+            uint8_t *dst = sA + sa * Cfg::kAPairBytes;
+            if constexpr (PAIR) {
+              const uint32_t bar = mapa_u32(&afull[sa], 0);
+              const int arow = mb * kTileRows + static_cast<int>(cta) * kTileM;
+              if (cta == 0) mbar_arrive_expect_tx(&afull[sa], kTxMul * (lo == hi ? kAStageBytes : Cfg::kAPairBytes));
+              tma_load_3d_cg2(dst, &tmA, bar, kb * kBlockK, arow, lo);
+              if (hi != lo) tma_load_3d_cg2(dst + kAStageBytes, &tmA, bar, kb * kBlockK, arow, hi);
+            } else if ((a.dbg & 1) && nloada >= SA) {
+              mbar_arrive(&afull[sa]);
+            } else {
               mbar_arrive_expect_tx(&afull[sa], lo == hi ? kAStageBytes : Cfg::kAPairBytes);
               tma_load_3d(dst, &tmA, &afull[sa], kb * kBlockK, mb * kTileM, lo);
               if (hi != lo) tma_load_3d(dst + kAStageBytes, &tmA, &afull[sa], kb * kBlockK, mb * kTileM, hi);
@@ -331,14 +378,14 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     }
     __syncwarp();
   } else if (warp == 1) {
-    // ===================== MMA issuer =====================
-    if (lane == 0) {
+    // ===================== MMA issuer (PAIR: leader CTA only) =====================
+    if (lane == 0 && cta == 0) {
       int sa = 0, sb = 0;
       uint32_t pa = 0, pb = 0, pt = 0;
       // look-ahead: the barrier of the NEXT stage is probed (non-blocking) before the MMAs of the current stage are
       // issued, so the ~90-cycle try_wait latency overlaps tensor work instead of draining the MMA queue
       bool a_ready = false, b_ready = false;
-      for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+      for (int tile = work_id; tile < num_tiles; tile += num_workers) {
         mbar_wait(tempty, pt ^ 1);  // epilogue has drained the accumulators of the previous tile
         tc_fence_after();
         for (int kb = a.kb0; kb < a.kb1; ++kb) {
@@ -356,14 +403,20 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             if (++sa == SA) { sa = 0; pa ^= 1; }
             a_ready = mbar_try_wait(&afull[sa], pa);
             if (j == Cfg::NPAIR - 1) b_ready = mbar_try_wait(&bfull[sb_next], pb_next);
-            oz1_issue_slice<P, kUseCollector>(lo, tmem_base, a_base, b_base, kb != a.kb0 || lo != 0);
-            if (hi != lo) oz1_issue_slice<P, kUseCollector>(hi, tmem_base, a_base + kAStageBytes, b_base, true);
-            umma_commit(&aempty[sa_cur]);  // stage reusable once these MMAs have read it
+            if constexpr (PAIR) {
+              oz1_issue_slice_pair<P>(lo, tmem_base, a_base, b_base, kb != a.kb0 || lo != 0);
+              if (hi != lo) oz1_issue_slice_pair<P>(hi, tmem_base, a_base + kAStageBytes, b_base, true);
+              umma_commit_cg2(&aempty[sa_cur], 3);  // both CTAs' stages reusable once these MMAs have read them
+            } else {
+              oz1_issue_slice<P, kUseCollector>(lo, tmem_base, a_base, b_base, kb != a.kb0 || lo != 0);
+              if (hi != lo) oz1_issue_slice<P, kUseCollector>(hi, tmem_base, a_base + kAStageBytes, b_base, true);
+              umma_commit(&aempty[sa_cur]);  // stage reusable once these MMAs have read it
+            }
           }
-          umma_commit(&bempty[sb]);
+          if constexpr (PAIR) umma_commit_cg2(&bempty[sb], 3); else umma_commit(&bempty[sb]);
           sb = sb_next; pb = pb_next;
         }
-        umma_commit(tfull);  // accumulators complete
+        if constexpr (PAIR) umma_commit_cg2(tfull, 3); else umma_commit(tfull);  // accumulators complete
         pt ^= 1;
       }
     }
@@ -380,10 +433,10 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     epi.init(a);
     constexpr int kChunks = NT / 2 / 8;  // 8-column chunks per thread
     constexpr bool kDoubleBuffer = (P <= 6);  // two register sets of P x 8 accumulator values fit without spilling
-    for (int tile = blockIdx.x; tile < num_tiles; tile += gridDim.x) {
+    for (int tile = work_id; tile < num_tiles; tile += num_workers) {
       int mb, nb;
       tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
-      const int64_t grow = static_cast<int64_t>(mb) * kTileM + row;
+      const int64_t grow = static_cast<int64_t>(mb) * kTileRows + cta * kTileM + row;
       const bool row_ok = grow < a.m;
       const int eArow = row_ok ? __ldg(a.eA + grow) - kBeta * (P + 1) : 0;
       const int64_t gcol0 = static_cast<int64_t>(nb) * NT + half * (NT / 2);
@@ -441,48 +494,76 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       // all TMEM reads of this tile are complete (tcgen05.wait::ld above): release the accumulators
       tc_fence_before();
       __syncwarp();
-      if (lane == 0) mbar_arrive(tempty);
+      if (lane == 0) {
+        if constexpr (PAIR) mbar_arrive_remote(mapa_u32(tempty, 0)); else mbar_arrive(tempty);
+      }
       pt ^= 1;
     }
   }
 
   tc_fence_before();
-  __syncthreads();
-  if (warp == 1) tmem_dealloc(tmem_base, Cfg::kTmemCols);
+  if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
+  if (warp == 1) {
+    if constexpr (PAIR) tmem_dealloc_cg2(tmem_base, Cfg::kTmemCols); else tmem_dealloc(tmem_base, Cfg::kTmemCols);
+  }
   if (blockIdx.x == 0 && threadIdx.x == 0 && a.cycles) atomicAdd(a.cycles, static_cast<unsigned long long>(clock64() - t_start));
 }
 
-template <int P>
-static int launch_p(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
-  using Cfg = Oz1Cfg<P>;
+// P <= 4 (NT >= 128) runs as CTA pairs (cta_group::2); P >= 5 needs N-concatenated MMAs, whose columns a pair
+// would split between the two CTAs' B halves, and stays one CTA per tile.
+template <int P, bool PAIR>
+static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
+  using Cfg = Oz1Cfg<P, PAIR>;
+  constexpr int kTileRows = PAIR ? 2 * kTileM : kTileM;
   CUtensorMap tmA, tmB;
   EMU_TRY(encode_planes_tmap(ctx, &tmA, g.SA, g.kpad, g.m, P, kTileM, 1));
-  EMU_TRY(encode_planes_tmap(ctx, &tmB, g.SB, g.kpad, g.n, P, Cfg::NT, P));
+  EMU_TRY(encode_planes_tmap(ctx, &tmB, g.SB, g.kpad, g.n, P, Cfg::kBRows, P));
   Oz1Dev d;
   d.m = g.m; d.n = g.n;
   d.kb0 = static_cast<int>(g.k0 / kBlockK);
   d.kb1 = static_cast<int>(g.k1 / kBlockK);
-  d.mt = static_cast<int>((g.m + kTileM - 1) / kTileM);
+  d.mt = static_cast<int>((g.m + kTileRows - 1) / kTileRows);
   d.nt_tiles = static_cast<int>((g.n + Cfg::NT - 1) / Cfg::NT);
   d.eA = g.eA; d.eB = g.eB;
   d.out_kind = g.out_kind; d.alpha = g.alpha; d.beta = g.beta; d.C = g.C; d.ldc = g.ldc;
   d.cycles = g.cycles;
   d.dbg = ctx->dbg_flags;
   const int tiles = d.mt * d.nt_tiles;
-  const int grid = tiles < ctx->num_sms ? tiles : ctx->num_sms;
+  const int workers = PAIR ? ctx->num_sms / 2 : ctx->num_sms;
+  const int grid = (PAIR ? 2 : 1) * (tiles < workers ? tiles : workers);
   void (*kern)(CUtensorMap, CUtensorMap, Oz1Dev) = nullptr;
   switch (g.out_kind) {
-    case 0: kern = oz1_gemm_kernel<P, 0>; break;
-    case 1: kern = oz1_gemm_kernel<(P <= 4 ? P : 4), 1>; break;  // FP32 entry point: p <= 4 (checked by the API)
-    case 2: kern = oz1_gemm_kernel<P, 2>; break;
-    default: kern = oz1_gemm_kernel<P, 3>; break;
+    case 0: kern = oz1_gemm_kernel<P, 0, PAIR>; break;
+    case 1: kern = oz1_gemm_kernel<(P <= 4 ? P : 4), 1, PAIR>; break;  // FP32 entry point: p <= 4 (checked by the API)
+    case 2: kern = oz1_gemm_kernel<P, 2, PAIR>; break;
+    default: kern = oz1_gemm_kernel<P, 3, PAIR>; break;
   }
   if (g.out_kind == 1 && P > 4) return EMUGEMM_ERR_ARG;
   EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
-  kern<<<grid, kGemmThreads, Cfg::kSmemBytes, ctx->stream>>>(tmA, tmB, d);
+  cudaLaunchConfig_t cfg = {};
+  cfg.gridDim = dim3(static_cast<unsigned>(grid));
+  cfg.blockDim = dim3(kGemmThreads);
+  cfg.dynamicSmemBytes = Cfg::kSmemBytes;
+  cfg.stream = ctx->stream;
+  cudaLaunchAttribute attr[1];
+  attr[0].id = cudaLaunchAttributeClusterDimension;
+  attr[0].val.clusterDim.x = PAIR ? 2 : 1;
+  attr[0].val.clusterDim.y = 1;
+  attr[0].val.clusterDim.z = 1;
+  cfg.attrs = attr;
+  cfg.numAttrs = 1;
+  EMU_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d));
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
   return EMUGEMM_OK;
+}
+
+template <int P>
+static int launch_p(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
+  if constexpr (P <= 4) {
+    if (!(ctx->dbg_flags & 8)) return launch_pp<P, true>(ctx, g);  // dbg bit 3: force the one-CTA N-concatenated kernel (A/B timing)
+  }
+  return launch_pp<P, false>(ctx, g);
 }
 
 int launch_oz1_gemm(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
