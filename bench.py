@@ -303,10 +303,12 @@ def main():
     gemm_ms = statistics.median(stage[1])
     achieved = w["ops"] / (gemm_ms * 1e-3) / 1e12
     peak = 2.0 * bf16_burst
-    traffic = None
+    traffic = None  # dram__bytes_read.sum + dram__bytes_write.sum of the GEMM kernel, per launch, from the committed ncu capture
     try:
-        tr = json.load(open(os.path.join(ROOT, "profiles", "traffic.json")))
-        traffic = tr.get(w["name"])
+        for row in open(os.path.join(ROOT, "profiles", "traffic.csv")):
+            f = [x.strip() for x in row.split(",")]
+            if len(f) >= 3 and f[0] == w["name"]:
+                traffic = float(f[2])
     except (OSError, ValueError):
         pass
     roof = {"bound": "tensor", "kernel": "oz1_gemm_kernel" if a.scheme.startswith("oz1") else "oz2_gemm_kernel",
@@ -334,9 +336,12 @@ def main():
     detail["prepass_frac_of_hbm"] = detail["prepass_algorithmic_GBps"] / peaks.get("hbm_gbs", 6650.0)
     if not a.no_probe:
         try:
-            _, tops, opc = h.dbg_i8_peak_probe(256, 40000)
-            detail["i8_issue_probe_op_per_clk_sm"] = opc
-            detail["i8_issue_probe_tops"] = tops
+            # the kernel's own MMA issue schedule on operands resident in shared memory (no TMA, no epilogue):
+            # what the tensor pipe sustains for this p; Scheme II uses the plain N = 256 schedule (p = 1)
+            pp = w["p"] if a.scheme in ("oz1", "oz1s") else 1
+            _, tops, eff = h.dbg_oz1_issue_probe(pp, True, 4000)
+            detail["issue_probe_per_clock_efficiency"] = eff
+            detail["issue_probe_tops"] = tops
             roof["frac_of_probe"] = achieved / tops
         except Exception as ex:  # the probe is context, never the product
             detail["i8_issue_probe_error"] = str(ex)
@@ -350,7 +355,13 @@ def main():
                        "parallelism": f"{world} independent problems" if world > 1 else "1 GPU"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "detail": detail}
     if not a.no_cpu:
-        line["cpu_baseline"] = cpu_oracle_leg(a, w, a.cpu_sample or 192)
+        if a.cpu_sample:
+            line["cpu_baseline"] = cpu_oracle_leg(a, w, a.cpu_sample)
+        else:  # calibrate on 96 x 96 sampled outputs, then size the sample for ~15 s of CPU work
+            cal = cpu_oracle_leg(a, w, 96)
+            per_elem = cal["seconds"] / (96 * 96)
+            side = int(min(w["m"], w["n"], max(96, (15.0 / max(per_elem, 1e-9)) ** 0.5)))
+            line["cpu_baseline"] = cpu_oracle_leg(a, w, side)
     print(json.dumps(line))
     h.close()
     if dist is not None:

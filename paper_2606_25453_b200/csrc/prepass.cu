@@ -135,41 +135,61 @@ int launch_exponent_scan(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, 
 }
 
 // ----------------------------------------------------------------------------
-// digitizers.  MODE 0: Scheme I digits, MODE 1: Scheme II residues.
+// digitizers.  MODE 0: Scheme I digits (PARAM = p, compile-time so that every digit is one funnel shift + mask),
+// MODE 1: Scheme II residues (PARAM = words of |a'|: 2 when t <= 64, else 3).
 // ----------------------------------------------------------------------------
+// |v| = (M / 2^63) 2^ex with the leading mantissa bit of a normal number at bit 63 (subnormals: no hidden bit)
+__device__ __forceinline__ void decode_top(double v, unsigned long long &M, int &ex, bool &neg) {
+  const unsigned long long b = static_cast<unsigned long long>(__double_as_longlong(v));
+  neg = (b >> 63) != 0;
+  const int E = static_cast<int>((b >> 52) & 0x7FF);
+  M = ((b & 0xFFFFFFFFFFFFFull) | (E ? (1ull << 52) : 0ull)) << 11;
+  ex = (E ? E : 1) - 1023;
+}
+__device__ __forceinline__ void decode_top(float v, unsigned long long &M, int &ex, bool &neg) {
+  const unsigned int b = __float_as_uint(v);
+  neg = (b >> 31) != 0;
+  const int E = static_cast<int>((b >> 23) & 0xFF);
+  M = static_cast<unsigned long long>((b & 0x7FFFFFu) | (E ? (1u << 23) : 0u)) << 40;
+  ex = (E ? E : 1) - 127;
+}
+
 struct Prep {            // one scalar prepared for plane extraction
   unsigned int w0, w1, w2;  // magnitude: OZ1 X (<= 56 bits) in w0,w1; OZ2 |a'| (<= 70 bits) in w0..w2
   bool neg;
 };
 
-template <typename T>
-__device__ __forceinline__ Prep prepare(T v, int e_row, int scale_bits /* 7p or t */) {
+// trunc(|v| 2^(scale_bits - e_row)) (R3: toward zero).  |v| < 2^e_row, so the right shift rs >= 64 - scale_bits.
+template <typename T, int NW>
+__device__ __forceinline__ Prep prepare(T v, int e_row, int scale_bits) {
   unsigned long long M;
-  int ex2;
-  bool neg;
-  decode_bits(v, M, ex2, neg);
-  const int sh = ex2 + scale_bits - e_row;  // |value| = M * 2^sh, truncated toward zero (R3)
-  unsigned long long lo, hi = 0;
-  if (sh >= 64) {       // only tiny subnormal mantissas reach this: M 2^sh < 2^scale_bits <= 2^96
-    lo = 0ull;
-    hi = M << (sh - 64);
-  } else if (sh >= 0) {
-    lo = M << sh;
-    hi = sh ? (M >> (64 - sh)) : 0ull;
-  } else {
-    lo = (sh > -64) ? (M >> (-sh)) : 0ull;
-  }
+  int ex;
   Prep r;
-  r.w0 = static_cast<unsigned int>(lo);
-  r.w1 = static_cast<unsigned int>(lo >> 32);
-  r.w2 = static_cast<unsigned int>(hi);
-  r.neg = neg;
+  decode_top(v, M, ex, r.neg);
+  const int rs = 63 - ex - scale_bits + e_row;
+  if (NW == 2) {  // scale_bits <= 64: rs >= 0, result < 2^64
+    const unsigned long long X = (rs >= 64) ? 0ull : (M >> rs);
+    r.w0 = static_cast<unsigned int>(X);
+    r.w1 = static_cast<unsigned int>(X >> 32);
+    r.w2 = 0u;
+  } else {        // scale_bits <= 95: 96-bit value (M : 0) >> (rs + 32), rs + 32 >= 96 - scale_bits > 0
+    const int W = rs + 32;
+    const unsigned int mh = static_cast<unsigned int>(M >> 32), ml = static_cast<unsigned int>(M);
+    const int q = W >> 5, b = W & 31;
+    const unsigned int hi = (q == 0) ? mh : 0u;
+    const unsigned int mid = (q == 0) ? ml : (q == 1) ? mh : 0u;
+    const unsigned int lo = (q == 0) ? 0u : (q == 1) ? ml : (q == 2) ? mh : 0u;
+    r.w0 = __funnelshift_r(lo, mid, b);
+    r.w1 = __funnelshift_r(mid, hi, b);
+    r.w2 = hi >> b;
+  }
   return r;
 }
 
-__device__ __forceinline__ int oz1_digit(const Prep &q, int t, int p) {
+template <int P>
+__device__ __forceinline__ int oz1_digit(const Prep &q, int t) {
   const unsigned long long X = (static_cast<unsigned long long>(q.w1) << 32) | q.w0;
-  const int d = static_cast<int>((X >> (kBeta * (p - 1 - t))) & 127ull);
+  const int d = static_cast<int>(static_cast<unsigned int>(X >> (kBeta * (P - 1 - t))) & 127u);
   return q.neg ? -d : d;
 }
 
@@ -195,7 +215,7 @@ __host__ __device__ constexpr unsigned int magic32(int m) {  // ceil(2^32 / m)
 
 // symmetric residue of sign * (w2:w1:w0) modulo the L-th modulus (L compile-time)
 template <int L>
-__device__ __forceinline__ int oz2_residue(const Prep &q) {
+__device__ __forceinline__ int oz2_residue(const Prep &q) {  // q.w2 == 0 is a compile-time constant on the two-word path
   constexpr int m = h_moduli[L];
   constexpr unsigned int c0 = pack_w(0, m), c1 = pack_w(1, m), c2 = pack_w(2, m), mg = magic32(m);
   unsigned int s = __dp4a(q.w0, c0, 0u);
@@ -224,11 +244,11 @@ __device__ __forceinline__ unsigned int pack4(int a, int b, int c, int d) {
          ((static_cast<unsigned int>(c) & 0xFFu) << 16) | ((static_cast<unsigned int>(d) & 0xFFu) << 24);
 }
 
-template <typename Sink>
-__device__ __forceinline__ void emit_oz1(const Prep (&q)[4], int p, Sink sink) {
+template <int P, typename Sink>
+__device__ __forceinline__ void emit_oz1(const Prep (&q)[4], Sink sink) {
 #pragma unroll
-  for (int t = 0; t < 8; ++t)
-    if (t < p) sink(t, pack4(oz1_digit(q[0], t, p), oz1_digit(q[1], t, p), oz1_digit(q[2], t, p), oz1_digit(q[3], t, p)));
+  for (int t = 0; t < P; ++t)
+    sink(t, pack4(oz1_digit<P>(q[0], t), oz1_digit<P>(q[1], t), oz1_digit<P>(q[2], t), oz1_digit<P>(q[3], t)));
 }
 
 template <int L, typename Sink>
@@ -259,26 +279,27 @@ __device__ __forceinline__ void emit_oz2_cplx_from(const Prep (&re)[4], const Pr
   }
 }
 
-// MODE 0: OZ1 (param = p, scale_bits = 7p); MODE 1: OZ2 (param = N, scale_bits = t)
-template <typename T, int W, int MODE, typename Sink>
+// MODE 0: OZ1 (PARAM = p, scale_bits = 7p); MODE 1: OZ2 (PARAM = words, param = N, scale_bits = t)
+template <typename T, int W, int MODE, int PARAM, typename Sink>
 __device__ __forceinline__ void emit_quad(const T (&v)[4][W], int e_row, int param, int scale_bits, Sink sink) {
+  constexpr int NW = (MODE == 0) ? 2 : PARAM;
   Prep a[4];
 #pragma unroll
-  for (int i = 0; i < 4; ++i) a[i] = prepare(v[i][0], e_row, scale_bits);
+  for (int i = 0; i < 4; ++i) a[i] = prepare<T, NW>(v[i][0], e_row, scale_bits);
   if constexpr (MODE == 0) {
-    emit_oz1(a, param, sink);
+    emit_oz1<PARAM>(a, sink);
   } else if constexpr (W == 1) {
     emit_oz2_real_from<0>(a, param, sink);
   } else {
     Prep b[4];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) b[i] = prepare(v[i][W - 1], e_row, scale_bits);
+    for (int i = 0; i < 4; ++i) b[i] = prepare<T, NW>(v[i][W - 1], e_row, scale_bits);
     emit_oz2_cplx_from<0>(a, b, param, sink);
   }
 }
 
 // ---- rows: X is rows x k (ldx); out[plane][row][kpad]; thread = one quad -----
-template <typename T, int W, int MODE>
+template <typename T, int W, int MODE, int PARAM>
 __global__ void __launch_bounds__(256) planes_rows_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows,
                                                           int64_t k, int64_t kpad, const int32_t *__restrict__ e,
                                                           int param, int scale_bits, int8_t *__restrict__ out) {
@@ -294,14 +315,14 @@ __global__ void __launch_bounds__(256) planes_rows_kernel(const T *__restrict__ 
   const int e_row = e[row];
   const int64_t plane_stride = rows * kpad;
   int8_t *dst = out + row * kpad + h0;
-  emit_quad<T, W, MODE>(v, e_row, param, scale_bits, [&](int plane, unsigned int word) {
+  emit_quad<T, W, MODE, PARAM>(v, e_row, param, scale_bits, [&](int plane, unsigned int word) {
     *reinterpret_cast<unsigned int *>(dst + plane * plane_stride) = word;
   });
 }
 
 // ---- columns: X is k x rows (ldx); transposed through shared memory ----------
 // tile = 32 columns x TH k; thread (lane = column, warp = k-quad index).
-template <typename T, int W, int MODE, int TH>
+template <typename T, int W, int MODE, int PARAM, int TH>
 __global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows,
                                                           int64_t k, int64_t kpad, const int32_t *__restrict__ e,
                                                           int param, int scale_bits, int nplanes,
@@ -319,7 +340,7 @@ __global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ 
     for (int i = 0; i < 4; ++i)
 #pragma unroll
       for (int c = 0; c < W; ++c) v[i][c] = (j < rows && h0 + i < k) ? X[((h0 + i) * ldx + j) * W + c] : T(0);
-    emit_quad<T, W, MODE>(v, e_row, param, scale_bits, [&](int plane, unsigned int word) {
+    emit_quad<T, W, MODE, PARAM>(v, e_row, param, scale_bits, [&](int plane, unsigned int word) {
       tile[(plane * 32 + lane) * PW + hw] = word;
     });
   }
@@ -339,7 +360,7 @@ __global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ 
   }
 }
 
-template <typename T, int W, int MODE>
+template <typename T, int W, int MODE, int PARAM>
 static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X,
                          int64_t ldx, const int32_t *e, int param, int scale_bits, int nplanes, int8_t *out) {
   if (rows == 0 || kpad == 0) return EMUGEMM_OK;
@@ -352,7 +373,7 @@ static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k,
       const int64_t nr = (rows - r0 < 65535) ? rows - r0 : 65535;
       const dim3 g(grid.x, static_cast<unsigned>(nr));
       // planes of the sub-block still use the full [rows][kpad] plane stride: pass full `rows`, offset pointers
-      planes_rows_kernel<T, W, MODE><<<g, 256, 0, st>>>(x + r0 * ldx * W, ldx, rows, k, kpad, e + r0, param, scale_bits,
+      planes_rows_kernel<T, W, MODE, PARAM><<<g, 256, 0, st>>>(x + r0 * ldx * W, ldx, rows, k, kpad, e + r0, param, scale_bits,
                                                          out + r0 * kpad);
       ctx->launches++;
     }
@@ -360,14 +381,14 @@ static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k,
     if (nplanes <= 20) {
       constexpr int TH = 128;
       const size_t smem = static_cast<size_t>(nplanes) * 32 * (TH / 4 + 1) * 4;
-      auto kern = planes_cols_kernel<T, W, MODE, TH>;
+      auto kern = planes_cols_kernel<T, W, MODE, PARAM, TH>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 20 * 32 * (TH / 4 + 1) * 4));
       const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH));
       kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, nplanes, out);
     } else {
       constexpr int TH = 32;
       const size_t smem = static_cast<size_t>(nplanes) * 32 * (TH / 4 + 1) * 4;
-      auto kern = planes_cols_kernel<T, W, MODE, TH>;
+      auto kern = planes_cols_kernel<T, W, MODE, PARAM, TH>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 60 * 32 * (TH / 4 + 1) * 4));
       const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH));
       kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, nplanes, out);
@@ -378,19 +399,43 @@ static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k,
   return EMUGEMM_OK;
 }
 
+template <typename T, int P>
+static int slice_p(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
+                   const int32_t *e, int8_t *out) {
+  return launch_planes<T, 1, 0, P>(ctx, by_cols, rows, k, kpad, X, ldx, e, P, kBeta * P, P, out);
+}
+
 int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
                      const void *X, int64_t ldx, const int32_t *e, int p, int8_t *out) {
-  if (elem == kF64) return launch_planes<double, 1, 0>(ctx, by_cols, rows, k, kpad, X, ldx, e, p, kBeta * p, p, out);
-  if (elem == kF32) return launch_planes<float, 1, 0>(ctx, by_cols, rows, k, kpad, X, ldx, e, p, kBeta * p, p, out);
+#define EMU_SLICE_CASE(T, PP) case PP: return slice_p<T, PP>(ctx, by_cols, rows, k, kpad, X, ldx, e, out)
+  if (elem == kF64) {
+    switch (p) {
+      EMU_SLICE_CASE(double, 1); EMU_SLICE_CASE(double, 2); EMU_SLICE_CASE(double, 3); EMU_SLICE_CASE(double, 4);
+      EMU_SLICE_CASE(double, 5); EMU_SLICE_CASE(double, 6); EMU_SLICE_CASE(double, 7); EMU_SLICE_CASE(double, 8);
+      default: return EMUGEMM_ERR_ARG;
+    }
+  }
+  if (elem == kF32) {  // 24-bit inputs: more than 4 slices add nothing (API range), the test hook allows up to 8
+    switch (p) {
+      EMU_SLICE_CASE(float, 1); EMU_SLICE_CASE(float, 2); EMU_SLICE_CASE(float, 3); EMU_SLICE_CASE(float, 4);
+      EMU_SLICE_CASE(float, 5); EMU_SLICE_CASE(float, 6); EMU_SLICE_CASE(float, 7); EMU_SLICE_CASE(float, 8);
+      default: return EMUGEMM_ERR_ARG;
+    }
+  }
+#undef EMU_SLICE_CASE
   return EMUGEMM_ERR_ARG;
 }
 
 int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
                         const void *X, int64_t ldx, const int32_t *e, int n_moduli, int t_bits, int8_t *out) {
+  if (t_bits < 1 || t_bits > 95) return EMUGEMM_ERR_ARG;  // three 32-bit words hold |a'| < 2^t (t = 77 at most: N = 20, k = 1)
+  const bool two = t_bits <= 64;  // |a'| < 2^t fits two 32-bit words: one byte dot product less per residue
   if (elem == kF64)
-    return launch_planes<double, 1, 1>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, n_moduli, out);
+    return two ? launch_planes<double, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, n_moduli, out)
+               : launch_planes<double, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, n_moduli, out);
   if (elem == kZ128)
-    return launch_planes<double, 2, 1>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, 3 * n_moduli, out);
+    return two ? launch_planes<double, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, 3 * n_moduli, out)
+               : launch_planes<double, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, 3 * n_moduli, out);
   return EMUGEMM_ERR_ARG;
 }
 
