@@ -288,7 +288,10 @@ struct Oz1Epi {
   }
 };
 
-template <int P, int OUT, bool PAIR>
+// MC (one-CTA tiles, P >= 5): a cluster of 2 CTAs works on two N-adjacent tiles of the same 128-row block; each CTA
+// fetches half of the rows of every A slice and TMA-multicasts them to both, so A crosses L2 -> SM once per
+// cluster (-33 % operand traffic at NT = 64; operand movement costs clock through the power cap).
+template <int P, int OUT, bool PAIR, bool MC>
 __global__ void __launch_bounds__(kGemmThreads, 1)
 oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const Oz1Dev a) {
   using Cfg = Oz1Cfg<P, PAIR>;
@@ -305,15 +308,18 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int num_tiles = a.mt * a.nt_tiles;
   // PAIR: the two CTAs of a cluster work on one 256-row tile; rank 0 (leader) issues the MMAs for both
-  const uint32_t cta = PAIR ? cluster_ctarank() : 0u;
-  const int work_id = PAIR ? static_cast<int>(blockIdx.x >> 1) : static_cast<int>(blockIdx.x);
-  const int num_workers = PAIR ? static_cast<int>(gridDim.x >> 1) : static_cast<int>(gridDim.x);
+  static_assert(!(PAIR && MC), "pairs already share operands");
+  constexpr bool CL2 = PAIR || MC;  // launched as clusters of 2
+  const uint32_t cta = CL2 ? cluster_ctarank() : 0u;
+  const int work_id = CL2 ? static_cast<int>(blockIdx.x >> 1) : static_cast<int>(blockIdx.x);
+  const int num_workers = CL2 ? static_cast<int>(gridDim.x >> 1) : static_cast<int>(gridDim.x);
   constexpr int kTileRows = PAIR ? 2 * kTileM : kTileM;
   constexpr uint32_t kTxMul = PAIR ? 2u : 1u;  // the leader's "full" barriers collect the bytes of both CTAs
 
   if (threadIdx.x == 0) {
     for (int i = 0; i < SB; ++i) { mbar_init(&bfull[i], 1); mbar_init(&bempty[i], 1); }
-    for (int i = 0; i < SA; ++i) { mbar_init(&afull[i], 1); mbar_init(&aempty[i], 1); }
+    // MC: a stage is refilled (in BOTH CTAs, by multicast) only after both CTAs' MMAs have read it
+    for (int i = 0; i < SA; ++i) { mbar_init(&afull[i], 1); mbar_init(&aempty[i], MC ? 2 : 1); }
     mbar_init(tfull, 1);
     mbar_init(tempty, PAIR ? 2 * kEpiWarps : kEpiWarps);
     fence_mbar_init();
@@ -325,7 +331,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     else { tmem_alloc(tmem_slot, Cfg::kTmemCols); tmem_relinquish(); }
   }
   tc_fence_before();
-  if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
+  if constexpr (CL2) cluster_sync_all(); else __syncthreads();
   tc_fence_after();
   const uint32_t tmem_base = *tmem_slot;
   const long long t_start = clock64();
@@ -338,6 +344,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       for (int tile = work_id; tile < num_tiles; tile += num_workers) {
         int mb, nb;
         tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
+        if constexpr (MC) nb = 2 * nb + static_cast<int>(cta);  // a.nt_tiles counts PAIRS of N-tiles
         for (int kb = a.kb0; kb < a.kb1; ++kb) {
           mbar_wait(&bempty[sb], pb ^ 1);
           if constexpr (PAIR) {
@@ -363,6 +370,13 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
               if (cta == 0) mbar_arrive_expect_tx(&afull[sa], kTxMul * (lo == hi ? kAStageBytes : Cfg::kAPairBytes));
               tma_load_3d_cg2(dst, &tmA, bar, kb * kBlockK, arow, lo);
               if (hi != lo) tma_load_3d_cg2(dst + kAStageBytes, &tmA, bar, kb * kBlockK, arow, hi);
+            } else if constexpr (MC) {
+              // this CTA fetches rows [64 cta, 64 cta + 64) of both slices and multicasts them to the pair
+              constexpr int kHalf = kAStageBytes / 2;
+              const int arow = mb * kTileM + static_cast<int>(cta) * (kTileM / 2);
+              mbar_arrive_expect_tx(&afull[sa], lo == hi ? kAStageBytes : Cfg::kAPairBytes);
+              tma_load_3d_mc(dst + cta * kHalf, &tmA, &afull[sa], kb * kBlockK, arow, lo, 3);
+              if (hi != lo) tma_load_3d_mc(dst + kAStageBytes + cta * kHalf, &tmA, &afull[sa], kb * kBlockK, arow, hi, 3);
             } else if ((a.dbg & 1) && nloada >= SA) {
               mbar_arrive(&afull[sa]);
             } else {
@@ -379,7 +393,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     __syncwarp();
   } else if (warp == 1) {
     // ===================== MMA issuer (PAIR: leader CTA only) =====================
-    if (lane == 0 && cta == 0) {
+    if (lane == 0 && (!PAIR || cta == 0)) {
       int sa = 0, sb = 0;
       uint32_t pa = 0, pb = 0, pt = 0;
       // look-ahead: the barrier of the NEXT stage is probed (non-blocking) before the MMAs of the current stage are
@@ -410,7 +424,8 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             } else {
               oz1_issue_slice<P, kUseCollector>(lo, tmem_base, a_base, b_base, kb != a.kb0 || lo != 0);
               if (hi != lo) oz1_issue_slice<P, kUseCollector>(hi, tmem_base, a_base + kAStageBytes, b_base, true);
-              umma_commit(&aempty[sa_cur]);  // stage reusable once these MMAs have read it
+              if constexpr (MC) umma_commit_mc(&aempty[sa_cur], 3);  // both CTAs must be done before either refills
+              else umma_commit(&aempty[sa_cur]);                     // stage reusable once these MMAs have read it
             }
           }
           if constexpr (PAIR) umma_commit_cg2(&bempty[sb], 3); else umma_commit(&bempty[sb]);
@@ -436,7 +451,8 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     for (int tile = work_id; tile < num_tiles; tile += num_workers) {
       int mb, nb;
       tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
-      const int64_t grow = static_cast<int64_t>(mb) * kTileRows + cta * kTileM + row;
+      if constexpr (MC) nb = 2 * nb + static_cast<int>(cta);
+      const int64_t grow = static_cast<int64_t>(mb) * kTileRows + (PAIR ? cta * kTileM : 0u) + row;
       const bool row_ok = grow < a.m;
       const int eArow = row_ok ? __ldg(a.eA + grow) - kBeta * (P + 1) : 0;
       const int64_t gcol0 = static_cast<int64_t>(nb) * NT + half * (NT / 2);
@@ -502,7 +518,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   }
 
   tc_fence_before();
-  if constexpr (PAIR) cluster_sync_all(); else __syncthreads();
+  if constexpr (CL2) cluster_sync_all(); else __syncthreads();
   if (warp == 1) {
     if constexpr (PAIR) tmem_dealloc_cg2(tmem_base, Cfg::kTmemCols); else tmem_dealloc(tmem_base, Cfg::kTmemCols);
   }
@@ -511,12 +527,12 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 
 // P <= 4 (NT >= 128) runs as CTA pairs (cta_group::2); P >= 5 needs N-concatenated MMAs, whose columns a pair
 // would split between the two CTAs' B halves, and stays one CTA per tile.
-template <int P, bool PAIR>
+template <int P, bool PAIR, bool MC>
 static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   using Cfg = Oz1Cfg<P, PAIR>;
   constexpr int kTileRows = PAIR ? 2 * kTileM : kTileM;
   CUtensorMap tmA, tmB;
-  EMU_TRY(encode_planes_tmap(ctx, &tmA, g.SA, g.kpad, g.m, P, kTileM, 1));
+  EMU_TRY(encode_planes_tmap(ctx, &tmA, g.SA, g.kpad, g.m, P, MC ? kTileM / 2 : kTileM, 1));
   EMU_TRY(encode_planes_tmap(ctx, &tmB, g.SB, g.kpad, g.n, P, Cfg::kBRows, P));
   Oz1Dev d;
   d.m = g.m; d.n = g.n;
@@ -524,19 +540,21 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   d.kb1 = static_cast<int>(g.k1 / kBlockK);
   d.mt = static_cast<int>((g.m + kTileRows - 1) / kTileRows);
   d.nt_tiles = static_cast<int>((g.n + Cfg::NT - 1) / Cfg::NT);
+  if (MC) d.nt_tiles = (d.nt_tiles + 1) / 2;  // pairs of N-adjacent tiles, one per CTA of the cluster
   d.eA = g.eA; d.eB = g.eB;
   d.out_kind = g.out_kind; d.alpha = g.alpha; d.beta = g.beta; d.C = g.C; d.ldc = g.ldc;
   d.cycles = g.cycles;
   d.dbg = ctx->dbg_flags;
+  constexpr bool CL2 = PAIR || MC;
   const int tiles = d.mt * d.nt_tiles;
-  const int workers = PAIR ? ctx->num_sms / 2 : ctx->num_sms;
-  const int grid = (PAIR ? 2 : 1) * (tiles < workers ? tiles : workers);
+  const int workers = CL2 ? ctx->num_sms / 2 : ctx->num_sms;
+  const int grid = (CL2 ? 2 : 1) * (tiles < workers ? tiles : workers);
   void (*kern)(CUtensorMap, CUtensorMap, Oz1Dev) = nullptr;
   switch (g.out_kind) {
-    case 0: kern = oz1_gemm_kernel<P, 0, PAIR>; break;
-    case 1: kern = oz1_gemm_kernel<(P <= 4 ? P : 4), 1, PAIR>; break;  // FP32 entry point: p <= 4 (checked by the API)
-    case 2: kern = oz1_gemm_kernel<P, 2, PAIR>; break;
-    default: kern = oz1_gemm_kernel<P, 3, PAIR>; break;
+    case 0: kern = oz1_gemm_kernel<P, 0, PAIR, MC>; break;
+    case 1: kern = oz1_gemm_kernel<(P <= 4 ? P : 4), 1, PAIR, MC>; break;  // FP32 entry point: p <= 4 (checked by the API)
+    case 2: kern = oz1_gemm_kernel<P, 2, PAIR, MC>; break;
+    default: kern = oz1_gemm_kernel<P, 3, PAIR, MC>; break;
   }
   if (g.out_kind == 1 && P > 4) return EMUGEMM_ERR_ARG;
   EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
@@ -547,7 +565,7 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   cfg.stream = ctx->stream;
   cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
-  attr[0].val.clusterDim.x = PAIR ? 2 : 1;
+  attr[0].val.clusterDim.x = CL2 ? 2 : 1;
   attr[0].val.clusterDim.y = 1;
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
@@ -561,9 +579,11 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
 template <int P>
 static int launch_p(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   if constexpr (P <= 4) {
-    if (!(ctx->dbg_flags & 8)) return launch_pp<P, true>(ctx, g);  // dbg bit 3: force the one-CTA N-concatenated kernel (A/B timing)
+    if (!(ctx->dbg_flags & 8)) return launch_pp<P, true, false>(ctx, g);  // dbg bit 3: force the one-CTA N-concatenated kernel (A/B timing)
   }
-  return launch_pp<P, false>(ctx, g);
+  // A multicast pays where A dominates the operand traffic (NT = 64: +2-4 % at p = 8; within noise at p = 5, 6)
+  if (P >= 7 && !(ctx->dbg_flags & 16)) return launch_pp<P, false, true>(ctx, g);  // dbg bit 4: no multicast clusters (A/B timing)
+  return launch_pp<P, false, false>(ctx, g);
 }
 
 int launch_oz1_gemm(emugemm_ctx *ctx, const Oz1GemmArgs &g) {

@@ -47,11 +47,13 @@ __device__ __forceinline__ bool mbar_try_wait(uint64_t *bar, uint32_t parity) {
   return ok != 0;
 }
 // Bounded wait: a pipeline bug must trap, never hang the GPU (a hung box is a strike).
+// Epilogue warps (threadIdx.x >= 64) get twice the budget so that a stuck producer / issuer reports first.
 __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   if (mbar_try_wait(bar, parity)) return;
   const long long t0 = clock64();
+  const long long limit = threadIdx.x >= 64 ? 8000000000LL : 4000000000LL;
   while (!mbar_try_wait(bar, parity)) {
-    if (clock64() - t0 > 4000000000LL) {
+    if (clock64() - t0 > limit) {
       printf("emugemm: mbarrier timeout block %d thread %d bar %u parity %u\n", blockIdx.x, threadIdx.x,
              smem_u32(bar), parity);
       __trap();
@@ -135,6 +137,10 @@ __device__ __forceinline__ void umma_i8(uint32_t d_tmem, uint64_t adesc, uint64_
 __device__ __forceinline__ void umma_commit(uint64_t *bar) {
   asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(smem_u32(bar))
                : "memory");
+}
+// same, barrier given as a shared::cluster address (may be the peer CTA's barrier: mapa_u32)
+__device__ __forceinline__ void umma_commit_addr(uint32_t cluster_addr) {
+  asm volatile("tcgen05.commit.cta_group::1.mbarrier::arrive::one.shared::cluster.b64 [%0];" ::"r"(cluster_addr) : "memory");
 }
 __device__ __forceinline__ void umma_commit_mc(uint64_t *bar, uint16_t mask) {
   asm volatile(
