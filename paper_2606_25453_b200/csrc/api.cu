@@ -138,10 +138,9 @@ static int run_oz1(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k, do
   h->diag = diag;
   EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
 
-  EMU_TRY(launch_exponent_scan(h, elem, 0, m, k, A, lda, mbA, eA));
-  EMU_TRY(launch_exponent_scan(h, elem, 1, n, k, B, ldb, mbB, eB));
-  EMU_TRY(launch_oz1_slice(h, elem, 0, m, k, kpad, A, lda, eA, p, SA));
-  EMU_TRY(launch_oz1_slice(h, elem, 1, n, k, kpad, B, ldb, eB, p, SB));
+  EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB));
+  EMU_TRY(launch_oz1_slice(h, elem, 0, m, k, kpad, A, lda, nullptr, eA, p, SA));
+  EMU_TRY(launch_oz1_slice(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, p, SB));
   EMU_TRY(mark(h, 1));
 
   Oz1GemmArgs g;
@@ -196,10 +195,9 @@ static int run_oz2(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_t k, co
   h->diag = diag;
   EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
 
-  EMU_TRY(launch_exponent_scan(h, elem, 0, m, k, A, lda, mbA, eA));
-  EMU_TRY(launch_exponent_scan(h, elem, 1, n, k, B, ldb, mbB, eB));
-  EMU_TRY(launch_oz2_residues(h, elem, 0, m, k, kpad, A, lda, eA, N, tA, RA));
-  EMU_TRY(launch_oz2_residues(h, elem, 1, n, k, kpad, B, ldb, eB, N, tB, RB));
+  EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB));
+  EMU_TRY(launch_oz2_residues(h, elem, 0, m, k, kpad, A, lda, nullptr, eA, N, tA, RA));
+  EMU_TRY(launch_oz2_residues(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, N, tB, RB));
   EMU_TRY(mark(h, 1));
   Oz2GemmArgs g;
   g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = N; g.is3m = is3m; g.RA = RA; g.RB = RB; g.CR = CR; g.cycles = diag;
@@ -372,8 +370,8 @@ int emugemm_dbg_oz1_slices(emugemm_handle_t h, int elem, int by_cols, int64_t ro
   auto *mb = cv.take<unsigned long long>(rows);
   auto *S = cv.take<int8_t>(static_cast<size_t>(p) * rows * kpad);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
-  EMU_TRY(launch_exponent_scan(h, elem, by_cols, rows, k, X, ldx, mb, e_out));
-  EMU_TRY(launch_oz1_slice(h, elem, by_cols, rows, k, kpad, X, ldx, e_out, p, S));
+  if (by_cols) EMU_TRY(launch_colmax(h, elem, rows, k, X, ldx, mb));
+  EMU_TRY(launch_oz1_slice(h, elem, by_cols, rows, k, kpad, X, ldx, mb, e_out, p, S));
   return unpad_planes(h, out, S, static_cast<int64_t>(p) * rows, k, kpad);
 }
 
@@ -393,8 +391,8 @@ int emugemm_dbg_oz2_residues(emugemm_handle_t h, int elem, int by_cols, int64_t 
   auto *mb = cv.take<unsigned long long>(rows);
   auto *R = cv.take<int8_t>(static_cast<size_t>(parts) * n_moduli * rows * kpad);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
-  EMU_TRY(launch_exponent_scan(h, elem, by_cols, rows, k, X, ldx, mb, e_out));
-  EMU_TRY(launch_oz2_residues(h, elem, by_cols, rows, k, kpad, X, ldx, e_out, n_moduli, t_bits, R));
+  if (by_cols) EMU_TRY(launch_colmax(h, elem, rows, k, X, ldx, mb));
+  EMU_TRY(launch_oz2_residues(h, elem, by_cols, rows, k, kpad, X, ldx, mb, e_out, n_moduli, t_bits, R));
   return unpad_planes(h, out, R, static_cast<int64_t>(parts) * n_moduli * rows, k, kpad);
 }
 

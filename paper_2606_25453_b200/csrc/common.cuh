@@ -66,13 +66,20 @@ enum ElemKind { kF32 = 4, kF64 = 8, kZ128 = 16 };
 int launch_exponent_scan(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, const void *X,
                          int64_t ldx, unsigned long long *maxbits, int32_t *e_out);
 
-// Scheme I slicing: out[p][rows][kpad] int8 (zero padded to kpad), exponents e[rows] (already computed).
-int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
-                     const void *X, int64_t ldx, const int32_t *e, int p, int8_t *out);
+// Column maxima (|x| bit patterns) of X (k x rows): the input of the by_cols = 1 plane kernels.
+int launch_colmax(emugemm_ctx *ctx, int elem, int64_t rows, int64_t k, const void *X, int64_t ldx,
+                  unsigned long long *maxbits);
 
-// Scheme II residues: elem 8: out[N][rows][kpad]; elem 16: out[3][N][rows][kpad] (re, im, Sigma).
+// Scheme I slicing: out[p][rows][kpad] int8 (zero padded to kpad) AND the exponents e[rows] (output).
+// by_cols = 0: one fused kernel scans each row and slices it (maxbits unused); by_cols = 1: maxbits[rows] from
+// launch_colmax, the kernel derives and publishes the exponents.
+int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
+                     const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int p, int8_t *out);
+
+// Scheme II residues: elem 8: out[N][rows][kpad]; elem 16: out[3][N][rows][kpad] (re, im, Sigma); e as above.
 int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
-                        const void *X, int64_t ldx, const int32_t *e, int n_moduli, int t_bits, int8_t *out);
+                        const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int n_moduli,
+                        int t_bits, int8_t *out);
 
 struct Oz1GemmArgs {
   int64_t m, n, kpad;          // kpad: padded k of the slice planes (multiple of kBlockK)

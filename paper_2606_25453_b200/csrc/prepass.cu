@@ -87,44 +87,63 @@ __global__ void __launch_bounds__(256) colmax_kernel(const T *__restrict__ X, in
   if (mx) atomicMax(&maxbits[j], mx);
 }
 
+// frexp exponent of the magnitude whose bit pattern is b (the row / column maximum); zero row -> 0 (R2)
 template <typename T>
-__global__ void bits_to_exponent_kernel(const unsigned long long *__restrict__ maxbits, int64_t rows,
-                                        int32_t *__restrict__ e_out) {
-  const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
-  if (i >= rows) return;
-  const unsigned long long b = maxbits[i];
+__device__ __forceinline__ int exponent_of_maxbits(unsigned long long b) {
   unsigned long long M;
   int ex2;
   bool neg;
   if (sizeof(T) == 8) decode_bits(__longlong_as_double(static_cast<long long>(b)), M, ex2, neg);
   else decode_bits(__uint_as_float(static_cast<unsigned int>(b)), M, ex2, neg);
-  e_out[i] = M ? ex2 + (64 - __clzll(static_cast<long long>(M))) : 0;  // frexp exponent; zero row -> 0 (R2)
+  return M ? ex2 + (64 - __clzll(static_cast<long long>(M))) : 0;
 }
 
+template <typename T>
+__global__ void bits_to_exponent_kernel(const unsigned long long *__restrict__ maxbits, int64_t rows,
+                                        int32_t *__restrict__ e_out) {
+  const int64_t i = static_cast<int64_t>(blockIdx.x) * blockDim.x + threadIdx.x;
+  if (i < rows) e_out[i] = exponent_of_maxbits<T>(maxbits[i]);
+}
+
+// Column maxima of X (k x rows, ldx) as |x| bit patterns -> maxbits[rows] (zeroed here); the column kernels turn them
+// into exponents.
+int launch_colmax(emugemm_ctx *ctx, int elem, int64_t rows, int64_t k, const void *X, int64_t ldx,
+                  unsigned long long *maxbits) {
+  if (rows == 0) return EMUGEMM_OK;
+  cudaStream_t st = ctx->stream;
+  EMU_CUDA(ctx, cudaMemsetAsync(maxbits, 0, sizeof(unsigned long long) * rows, st));
+  if (k == 0) return EMUGEMM_OK;
+  // enough k-segments to fill the machine: ~8 CTAs per SM
+  const int64_t gx = (rows + 255) / 256;
+  int64_t segs = (static_cast<int64_t>(ctx->num_sms) * 8 + gx - 1) / gx;
+  if (segs > (k + 63) / 64) segs = (k + 63) / 64;
+  if (segs < 1) segs = 1;
+  const int64_t kseg = (k + segs - 1) / segs;
+  const dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>((k + kseg - 1) / kseg));
+  if (elem == kF64) colmax_kernel<double, 1><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits);
+  else if (elem == kF32) colmax_kernel<float, 1><<<grid, 256, 0, st>>>(static_cast<const float *>(X), ldx, rows, k, kseg, maxbits);
+  else colmax_kernel<double, 2><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits);
+  ctx->launches++;
+  EMU_CUDA(ctx, cudaGetLastError());
+  return EMUGEMM_OK;
+}
+
+// Exponents alone (test hook emugemm_dbg_exponents): row scan or column scan + bit pattern -> exponent.
 int launch_exponent_scan(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, const void *X,
                          int64_t ldx, unsigned long long *maxbits, int32_t *e_out) {
   if (rows == 0) return EMUGEMM_OK;
   cudaStream_t st = ctx->stream;
-  EMU_CUDA(ctx, cudaMemsetAsync(maxbits, 0, sizeof(unsigned long long) * rows, st));
-  if (k > 0) {
-    if (!by_cols) {
+  if (by_cols) {
+    EMU_TRY(launch_colmax(ctx, elem, rows, k, X, ldx, maxbits));
+  } else {
+    EMU_CUDA(ctx, cudaMemsetAsync(maxbits, 0, sizeof(unsigned long long) * rows, st));
+    if (k > 0) {
       const unsigned grid = static_cast<unsigned>(rows);
       if (elem == kF64) rowmax_kernel<double, 1><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, k, maxbits);
       else if (elem == kF32) rowmax_kernel<float, 1><<<grid, 256, 0, st>>>(static_cast<const float *>(X), ldx, k, maxbits);
       else rowmax_kernel<double, 2><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, k, maxbits);
-    } else {
-      // enough k-segments to fill the machine: ~8 CTAs per SM
-      const int64_t gx = (rows + 255) / 256;
-      int64_t segs = (static_cast<int64_t>(ctx->num_sms) * 8 + gx - 1) / gx;
-      if (segs > (k + 63) / 64) segs = (k + 63) / 64;
-      if (segs < 1) segs = 1;
-      const int64_t kseg = (k + segs - 1) / segs;
-      const dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>((k + kseg - 1) / kseg));
-      if (elem == kF64) colmax_kernel<double, 1><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits);
-      else if (elem == kF32) colmax_kernel<float, 1><<<grid, 256, 0, st>>>(static_cast<const float *>(X), ldx, rows, k, kseg, maxbits);
-      else colmax_kernel<double, 2><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits);
+      ctx->launches++;
     }
-    ctx->launches++;
   }
   const unsigned g2 = static_cast<unsigned>((rows + 255) / 256);
   if (elem == kF32) bits_to_exponent_kernel<float><<<g2, 256, 0, st>>>(maxbits, rows, e_out);
@@ -298,41 +317,69 @@ __device__ __forceinline__ void emit_quad(const T (&v)[4][W], int e_row, int par
   }
 }
 
-// ---- rows: X is rows x k (ldx); out[plane][row][kpad]; thread = one quad -----
+// ---- rows: X is rows x k (ldx); out[plane][row][kpad] --------------------------
+// One CTA per row, two phases: (1) max |x| bit pattern of the row -> exponent (written to e_out), (2) the row is
+// read again -- it was just fetched by this CTA, so it comes from L1 / L2 -- and every thread digitises quads of 4
+// consecutive k.  One DRAM read of A, no separate scan / exponent launches.
 template <typename T, int W, int MODE, int PARAM>
 __global__ void __launch_bounds__(256) planes_rows_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows,
-                                                          int64_t k, int64_t kpad, const int32_t *__restrict__ e,
+                                                          int64_t k, int64_t kpad, int32_t *__restrict__ e_out,
                                                           int param, int scale_bits, int8_t *__restrict__ out) {
-  const int64_t row = blockIdx.y;
-  const int64_t h0 = (static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x) * 4;
-  if (h0 >= kpad) return;
+  const int64_t row = blockIdx.x;
   const T *src = X + row * ldx * W;
-  T v[4][W];
+  unsigned long long mx = 0;
+  for (int64_t h = static_cast<int64_t>(threadIdx.x) * 4; h < k; h += 1024) {
 #pragma unroll
-  for (int i = 0; i < 4; ++i)
+    for (int i = 0; i < 4; ++i)
 #pragma unroll
-    for (int c = 0; c < W; ++c) v[i][c] = (h0 + i < k) ? src[(h0 + i) * W + c] : T(0);
-  const int e_row = e[row];
+      for (int c = 0; c < W; ++c)
+        if (h + i < k) {
+          const unsigned long long b = abs_bits(src[(h + i) * W + c]);
+          mx = b > mx ? b : mx;
+        }
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    const unsigned long long y = __shfl_xor_sync(0xffffffffu, mx, o);
+    mx = y > mx ? y : mx;
+  }
+  __shared__ unsigned long long red[8];
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
+  __syncthreads();
+#pragma unroll
+  for (int w = 0; w < 8; ++w) mx = red[w] > mx ? red[w] : mx;
+  const int e_row = exponent_of_maxbits<T>(mx);
+  if (threadIdx.x == 0) e_out[row] = e_row;
+
   const int64_t plane_stride = rows * kpad;
-  int8_t *dst = out + row * kpad + h0;
-  emit_quad<T, W, MODE, PARAM>(v, e_row, param, scale_bits, [&](int plane, unsigned int word) {
-    *reinterpret_cast<unsigned int *>(dst + plane * plane_stride) = word;
-  });
+  for (int64_t h0 = static_cast<int64_t>(threadIdx.x) * 4; h0 < kpad; h0 += 1024) {
+    T v[4][W];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int c = 0; c < W; ++c) v[i][c] = (h0 + i < k) ? src[(h0 + i) * W + c] : T(0);
+    int8_t *dst = out + row * kpad + h0;
+    emit_quad<T, W, MODE, PARAM>(v, e_row, param, scale_bits, [&](int plane, unsigned int word) {
+      *reinterpret_cast<unsigned int *>(dst + plane * plane_stride) = word;
+    });
+  }
 }
 
 // ---- columns: X is k x rows (ldx); transposed through shared memory ----------
 // tile = 32 columns x TH k; thread (lane = column, warp = k-quad index).
 template <typename T, int W, int MODE, int PARAM, int TH>
 __global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows,
-                                                          int64_t k, int64_t kpad, const int32_t *__restrict__ e,
-                                                          int param, int scale_bits, int nplanes,
+                                                          int64_t k, int64_t kpad,
+                                                          const unsigned long long *__restrict__ maxbits,
+                                                          int32_t *__restrict__ e_out, int param, int scale_bits, int nplanes,
                                                           int8_t *__restrict__ out) {
   extern __shared__ unsigned int tile[];  // [plane][32][TH/4 + 1]
   constexpr int PW = TH / 4 + 1;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t j = static_cast<int64_t>(blockIdx.x) * 32 + lane;
   const int64_t hb = static_cast<int64_t>(blockIdx.y) * TH;
-  const int e_row = (j < rows) ? e[j] : 0;
+  // column exponent from the column-max bit pattern (colmax_kernel ran before); the first k-block publishes it
+  const int e_row = (j < rows) ? exponent_of_maxbits<T>(maxbits[j]) : 0;
+  if (blockIdx.y == 0 && warp == 0 && j < rows) e_out[j] = e_row;
   for (int hw = warp; hw < TH / 4; hw += 8) {
     const int64_t h0 = hb + hw * 4;
     T v[4][W];
@@ -360,23 +407,19 @@ __global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ 
   }
 }
 
+// by_cols = 0: fused scan + planes of the rows of X, exponents written to e.
+// by_cols = 1: planes of the columns of X; maxbits[j] must hold the column maxima (launch_colmax), exponents written to e.
 template <typename T, int W, int MODE, int PARAM>
 static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X,
-                         int64_t ldx, const int32_t *e, int param, int scale_bits, int nplanes, int8_t *out) {
+                         int64_t ldx, const unsigned long long *maxbits, int32_t *e, int param, int scale_bits, int nplanes,
+                         int8_t *out) {
   if (rows == 0 || kpad == 0) return EMUGEMM_OK;
   cudaStream_t st = ctx->stream;
   const T *x = static_cast<const T *>(X);
   if (!by_cols) {
-    const dim3 grid(static_cast<unsigned>((kpad / 4 + 255) / 256), static_cast<unsigned>(rows));
-    // grid.y is limited to 65535: loop over row blocks
-    for (int64_t r0 = 0; r0 < rows; r0 += 65535) {
-      const int64_t nr = (rows - r0 < 65535) ? rows - r0 : 65535;
-      const dim3 g(grid.x, static_cast<unsigned>(nr));
-      // planes of the sub-block still use the full [rows][kpad] plane stride: pass full `rows`, offset pointers
-      planes_rows_kernel<T, W, MODE, PARAM><<<g, 256, 0, st>>>(x + r0 * ldx * W, ldx, rows, k, kpad, e + r0, param, scale_bits,
-                                                         out + r0 * kpad);
-      ctx->launches++;
-    }
+    planes_rows_kernel<T, W, MODE, PARAM><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, param,
+                                                                                        scale_bits, out);
+    ctx->launches++;
   } else {
     if (nplanes <= 20) {
       constexpr int TH = 128;
@@ -384,14 +427,14 @@ static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k,
       auto kern = planes_cols_kernel<T, W, MODE, PARAM, TH>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 20 * 32 * (TH / 4 + 1) * 4));
       const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH));
-      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, nplanes, out);
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, param, scale_bits, nplanes, out);
     } else {
       constexpr int TH = 32;
       const size_t smem = static_cast<size_t>(nplanes) * 32 * (TH / 4 + 1) * 4;
       auto kern = planes_cols_kernel<T, W, MODE, PARAM, TH>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 60 * 32 * (TH / 4 + 1) * 4));
       const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH));
-      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, nplanes, out);
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, param, scale_bits, nplanes, out);
     }
     ctx->launches++;
   }
@@ -401,13 +444,13 @@ static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k,
 
 template <typename T, int P>
 static int slice_p(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
-                   const int32_t *e, int8_t *out) {
-  return launch_planes<T, 1, 0, P>(ctx, by_cols, rows, k, kpad, X, ldx, e, P, kBeta * P, P, out);
+                   const unsigned long long *maxbits, int32_t *e, int8_t *out) {
+  return launch_planes<T, 1, 0, P>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, kBeta * P, P, out);
 }
 
 int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
-                     const void *X, int64_t ldx, const int32_t *e, int p, int8_t *out) {
-#define EMU_SLICE_CASE(T, PP) case PP: return slice_p<T, PP>(ctx, by_cols, rows, k, kpad, X, ldx, e, out)
+                     const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int p, int8_t *out) {
+#define EMU_SLICE_CASE(T, PP) case PP: return slice_p<T, PP>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, out)
   if (elem == kF64) {
     switch (p) {
       EMU_SLICE_CASE(double, 1); EMU_SLICE_CASE(double, 2); EMU_SLICE_CASE(double, 3); EMU_SLICE_CASE(double, 4);
@@ -427,15 +470,16 @@ int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int6
 }
 
 int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
-                        const void *X, int64_t ldx, const int32_t *e, int n_moduli, int t_bits, int8_t *out) {
+                        const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int n_moduli, int t_bits,
+                        int8_t *out) {
   if (t_bits < 1 || t_bits > 95) return EMUGEMM_ERR_ARG;  // three 32-bit words hold |a'| < 2^t (t = 77 at most: N = 20, k = 1)
   const bool two = t_bits <= 64;  // |a'| < 2^t fits two 32-bit words: one byte dot product less per residue
   if (elem == kF64)
-    return two ? launch_planes<double, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, n_moduli, out)
-               : launch_planes<double, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, n_moduli, out);
+    return two ? launch_planes<double, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out)
+               : launch_planes<double, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out);
   if (elem == kZ128)
-    return two ? launch_planes<double, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, 3 * n_moduli, out)
-               : launch_planes<double, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, e, n_moduli, t_bits, 3 * n_moduli, out);
+    return two ? launch_planes<double, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out)
+               : launch_planes<double, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out);
   return EMUGEMM_ERR_ARG;
 }
 
