@@ -59,25 +59,29 @@ struct Oz1Cfg {
 template <int P, bool COLL>
 __device__ __forceinline__ void oz1_issue_slice(int t, uint32_t tmem_base, uint32_t a_base, uint32_t b_base, bool accumulate) {
   constexpr int NT = Oz1Cfg<P>::NT;
-  constexpr int kColsMax = P * NT;
+  // (P - t) NT columns: one MMA if <= 256, else two of near-equal width (multiples of 16).  An even split keeps
+  // both above the ~112-column width below which an MMA is bound by its fixed cost (256 + 32 at p = 5, t = 2 would
+  // run the 32-wide one at a third of the rate; 256 + 64 at p = 6, 7, 8 at two thirds).
+  const int cols = (P - t) * NT;
+  const int n0 = (cols <= 256) ? cols : ((cols / 2 + 15) / 16) * 16;
+  const int n1 = cols - n0;
 #pragma unroll
   for (int ks = 0; ks < kBlockK / 32; ++ks) {
     const uint64_t adesc = make_sdesc_sw128(a_base + ks * 32);
-#pragma unroll
-    for (int c0 = 0; c0 < kColsMax; c0 += 256) {
-      const int cols = (P - t) * NT;
-      if (c0 < cols) {
-        const int nn = (cols - c0 < 256) ? (cols - c0) : 256;
-        const uint32_t acc = (accumulate || ks != 0) ? 1u : 0u;
-        const uint32_t d = tmem_base + t * NT + c0;
-        const uint64_t bdesc = make_sdesc_sw128(b_base + c0 * kBlockK + ks * 32);
-        const uint32_t idesc = make_idesc_i8(kTileM, nn);
-        // the <= 2 MMAs of one (t, ks) share A_t: the first keeps it in the collector, the last drops it
-        const bool first = (c0 == 0), last = (c0 + 256 >= cols);
-        if (COLL && first && !last) umma_i8<1>(d, adesc, bdesc, idesc, acc);
-        else if (COLL && !first && last) umma_i8<3>(d, adesc, bdesc, idesc, acc);
-        else if (COLL && !first && !last) umma_i8<2>(d, adesc, bdesc, idesc, acc);
-        else umma_i8<0>(d, adesc, bdesc, idesc, acc);
+    const uint32_t acc = (accumulate || ks != 0) ? 1u : 0u;
+    const uint32_t d = tmem_base + t * NT;
+    const uint64_t bdesc0 = make_sdesc_sw128(b_base + ks * 32);
+    if (n1 == 0) {
+      umma_i8<0>(d, adesc, bdesc0, make_idesc_i8(kTileM, n0), acc);
+    } else {
+      // the two MMAs share A_t: the first keeps it in the collector, the second drops it
+      const uint64_t bdesc1 = make_sdesc_sw128(b_base + n0 * kBlockK + ks * 32);
+      if (COLL) {
+        umma_i8<1>(d, adesc, bdesc0, make_idesc_i8(kTileM, n0), acc);
+        umma_i8<3>(d + n0, adesc, bdesc1, make_idesc_i8(kTileM, n1), acc);
+      } else {
+        umma_i8<0>(d, adesc, bdesc0, make_idesc_i8(kTileM, n0), acc);
+        umma_i8<0>(d + n0, adesc, bdesc1, make_idesc_i8(kTileM, n1), acc);
       }
     }
   }
