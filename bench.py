@@ -357,10 +357,10 @@ def main():
     if not a.no_cpu:
         if a.cpu_sample:
             line["cpu_baseline"] = cpu_oracle_leg(a, w, a.cpu_sample)
-        else:  # calibrate on 96 x 96 sampled outputs, then size the sample for ~15 s of CPU work
+        else:  # calibrate on 96 x 96 sampled outputs, then size the sample for 10-20 s of CPU work
             cal = cpu_oracle_leg(a, w, 96)
             per_elem = cal["seconds"] / (96 * 96)
-            side = int(min(w["m"], w["n"], max(96, (15.0 / max(per_elem, 1e-9)) ** 0.5)))
+            side = int(min(w["m"], w["n"], max(96, (40.0 / max(per_elem, 1e-9)) ** 0.5)))  # fixed costs make 96 x 96 pessimistic: lands at 10-20 s
             line["cpu_baseline"] = cpu_oracle_leg(a, w, side)
     print(json.dumps(line))
     h.close()
