@@ -43,6 +43,15 @@
 #endif
 
 #define ORACLE_BETA 7 /* R1: beta = 7, all slices signed ("signed-slice method supports beta <= 7") */
+
+/* Slice-digit mode (R23).  7 (default, R1): sign-magnitude 7-bit digits.
+ * 8: balanced signed base-256 digits, d_t in [-128, 127], all-signed INT8 like R1 but 8 bits per slice
+ * ("slices of beta <= 8 bits", PAPER.md:345 the paper's code reaches beta = 8 with a signed leading and
+ * unsigned remaining slices; the balanced form keeps one signedness).  Two guard bits: x = a 2^-(e+2) in
+ * (-1/4, 1/4) so that X + sum_j 128 256^j stays inside [0, 256^p). */
+static int g_slice_bits = 7;
+void oracle_set_slice_bits(int bits) { g_slice_bits = (bits == 8) ? 8 : 7; }
+int oracle_get_slice_bits(void) { return g_slice_bits; }
 #define ORACLE_MAX_MODULI 24
 
 typedef __int128 i128;
@@ -132,7 +141,19 @@ void oracle_col_exponents_z(int64_t k, int64_t n, const double *Z, int64_t ldz, 
 /* (t = 0 most significant) d_t = (X >> beta (p-1-t)) & (2^beta - 1);         */
 /* slice value = sign(a) * d_t in [-127, 127].                                */
 /* ------------------------------------------------------------------------- */
+static void slice_one_balanced(double a, int e, int p, int8_t *digits /* [p] */) {
+  /* X = trunc(a 2^(8p - e - 2)) toward zero (R3), |X| < 2^(8p-2); Y = X + C, C = sum_{j<p} 128 256^j: every byte of
+   * Y minus 128 is a balanced digit, sum_t d_t 256^(p-1-t) == X exactly. */
+  __float128 sc = scalbnq((__float128)a, 8 * p - e - 2);
+  int64_t X = (int64_t)truncq(sc);
+  uint64_t Cc = 0;
+  for (int j = 0; j < p; ++j) Cc |= (uint64_t)128 << (8 * j);
+  uint64_t Y = (uint64_t)(X + (int64_t)Cc); /* 0 < Y < 256^p (p = 8: wraps mod 2^64 only if violated) */
+  for (int t = 0; t < p; ++t) digits[t] = (int8_t)((int)((Y >> (8 * (p - 1 - t))) & 255u) - 128);
+}
+
 static void slice_one(double a, int e, int p, int8_t *digits /* [p] */) {
+  if (g_slice_bits == 8) { slice_one_balanced(a, e, p, digits); return; }
   /* |a| * 2^(beta p - e): a power-of-two scaling, exact in __float128. */
   __float128 sc = scalbnq(fabsq((__float128)a), ORACLE_BETA * p - e);
   uint64_t X = (uint64_t)truncq(sc); /* X < 2^(beta p) <= 2^56 */
@@ -197,6 +218,11 @@ void oracle_oz1_accumulators(int64_t m, int64_t n, int64_t k, int p, const int8_
 /* beta_ == 0 => C_in is not read (BLAS rule).                                 */
 /* ------------------------------------------------------------------------- */
 static __float128 oz1_value(const int64_t *cs /* [p] */, int p, int eAi, int eBj) {
+  if (g_slice_bits == 8) { /* balanced base 256: v = S 2^(eA + eB + 4 - 8 (p+1)), the +4 are the guard bits */
+    i128 S8 = 0;
+    for (int s = 0; s < p; ++s) S8 += (i128)cs[s] * ((i128)1 << (8 * (p - 1 - s)));
+    return scalbnq((__float128)S8, eAi + eBj + 4 - 8 * (p + 1));
+  }
   i128 S = 0;
   for (int s = 0; s < p; ++s) S += (i128)cs[s] * ((i128)1 << (ORACLE_BETA * (p - 1 - s)));
   return scalbnq((__float128)S, eAi + eBj - ORACLE_BETA * (p + 1));

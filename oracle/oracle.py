@@ -34,6 +34,15 @@ def set_threads(t):
 
 
 # ---------------------------------------------------------------- exponents
+def set_slice_bits(bits):
+    """7 (default, R1): sign-magnitude 7-bit digits; 8: balanced signed base-256 digits (R23)."""
+    _lib.oracle_set_slice_bits(C.c_int(bits))
+
+
+def get_slice_bits():
+    return int(_lib.oracle_get_slice_bits())
+
+
 def row_exponents(A):
     A = _f64(A)
     m, k = A.shape
