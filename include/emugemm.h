@@ -57,6 +57,12 @@ int emugemm_create(emugemm_handle_t *h);  /* host-only state; checks the device 
 int emugemm_destroy(emugemm_handle_t h);
 int emugemm_set_stream(emugemm_handle_t h, void *cuda_stream /* cudaStream_t */);
 int emugemm_set_workspace(emugemm_handle_t h, void *dev_ptr, size_t bytes);
+/* Scheme I digit format of this handle.  7 (default; R1): sign-magnitude digits of
+ * 7 bits, |d| <= 127.  8 (R23; "slices of beta <= 8
+ * bits"): balanced signed base-256 digits, d in [-128, 127], two guard bits under the row /
+ * column exponent -- 8p - 2 bits per operand, so p = 7 reaches the accuracy of p = 8 at 7 bits
+ * with 28 instead of 36 slice products.  Applies to dgemm_oz1, sgemm_oz1 and the Scheme I hooks. */
+int emugemm_set_slice_bits(emugemm_handle_t h, int bits);
 /* Bytes of workspace a call with these arguments needs.  elem = bytes per
  * matrix element: 4 (float), 8 (double), 16 (complex128).  p_or_nmoduli = p for
  * Scheme I, n_moduli for Scheme II / 3M.  Returns 0 for invalid arguments. */
@@ -143,7 +149,8 @@ int emugemm_dbg_oz2_crt(emugemm_handle_t h, int64_t m, int64_t n, int n_moduli, 
                         double beta, double *C, int64_t ldc);
 /* Host-side helpers (no GPU): bit budget (returns T or < 0), overflow-safe chunk length. */
 int emugemm_oz2_budget(int n_moduli, int64_t k, int is3m, int *tA, int *tB);
-int64_t emugemm_oz1_chunk_k(int p);
+int64_t emugemm_oz1_chunk_k(int p);                       /* 7-bit digits */
+int64_t emugemm_oz1_chunk_k_bits(int p, int slice_bits);   /* p k_c dmax^2 <= 2^31 - 1, dmax = 127 / 128 */
 /* Issue-bound tcgen05.mma kind::i8 probe (operands resident in shared memory, no
  * loads in the loop), one CTA per SM.  ops = HOST array of n_ops (<= 64) MMAs, five
  * ints each: {TMEM column of D, width N (multiple of 16, <= 256), A slot 0..7

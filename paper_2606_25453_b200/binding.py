@@ -35,6 +35,7 @@ def load_library():
         lib.emugemm_workspace_bytes.restype = _sz
         lib.emugemm_workspace_bytes.argtypes = [_int, _int, _i64, _i64, _i64, _int]
         lib.emugemm_oz1_chunk_k.restype = _i64
+        lib.emugemm_oz1_chunk_k_bits.restype = _i64
         _lib = lib
     return _lib
 
@@ -51,8 +52,8 @@ def oz2_budget(n_moduli, k, is3m=False):
     return int(T), a.value, b.value
 
 
-def oz1_chunk_k(p):
-    return int(load_library().emugemm_oz1_chunk_k(_int(p)))
+def oz1_chunk_k(p, slice_bits=7):
+    return int(load_library().emugemm_oz1_chunk_k_bits(_int(p), _int(slice_bits)))
 
 
 def _ptr(t):
@@ -71,6 +72,7 @@ class EmuGemm:
         self._h = _vp(None)
         self._check(self._lib.emugemm_create(C.byref(self._h)))
         self._ws = None
+        self.slice_bits = 7
         self.set_stream(torch.cuda.current_stream())
 
     def close(self):
@@ -91,6 +93,11 @@ class EmuGemm:
     # ---- handle ------------------------------------------------------------
     def set_stream(self, stream):
         self._check(self._lib.emugemm_set_stream(self._h, _vp(stream.cuda_stream)))
+
+    def set_slice_bits(self, bits):
+        """Scheme I digits: 7 = sign-magnitude (default), 8 = balanced base 256 (see include/emugemm.h)."""
+        self._check(self._lib.emugemm_set_slice_bits(self._h, _int(bits)))
+        self.slice_bits = bits
 
     def workspace_bytes(self, scheme, elem, m, n, k, pn):
         return int(self._lib.emugemm_workspace_bytes(scheme, elem, m, n, k, pn))
@@ -195,8 +202,8 @@ class EmuGemm:
         n = B.shape[1]
         self._reserve_for(OZ1, self._elem(A), m, n, k, p)
         kpad = (k + 127) // 128 * 128
-        ck = chunk_k if chunk_k > 0 else oz1_chunk_k(p)
-        ck = min((ck + 127) // 128 * 128, oz1_chunk_k(p))
+        ck = chunk_k if chunk_k > 0 else oz1_chunk_k(p, self.slice_bits)
+        ck = min((ck + 127) // 128 * 128, oz1_chunk_k(p, self.slice_bits))
         nch = max(1, -(-kpad // ck))
         out = torch.empty((nch, p, m, n), dtype=torch.int32, device="cuda")
         got = _int(0)

@@ -48,9 +48,9 @@ struct Carver {
 };
 static size_t granule(size_t bytes) { return static_cast<size_t>(round_up(static_cast<int64_t>(bytes), 1024)); }
 
-static int oz1_chunks(int p, int64_t kpad, int64_t chunk_override, int64_t *chunk_len) {
-  int64_t c = chunk_override > 0 ? round_up(chunk_override, kBlockK) : oz1_chunk_k_host(p);
-  if (c > oz1_chunk_k_host(p)) c = oz1_chunk_k_host(p);
+static int oz1_chunks(int p, int bits, int64_t kpad, int64_t chunk_override, int64_t *chunk_len) {
+  int64_t c = chunk_override > 0 ? round_up(chunk_override, kBlockK) : oz1_chunk_k_host(p, bits);
+  if (c > oz1_chunk_k_host(p, bits)) c = oz1_chunk_k_host(p, bits);
   int n = static_cast<int>((kpad + c - 1) / c);
   if (n < 1) n = 1;
   // equalise the chunks (same number, balanced length, still <= the safe bound)
@@ -123,7 +123,8 @@ static int run_oz1(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k, do
   }
   const int64_t kpad = round_up(k, kBlockK);
   int64_t clen;
-  const int nch = oz1_chunks(p, kpad, chunk_override, &clen);
+  const int bits = h->slice_bits;
+  const int nch = oz1_chunks(p, bits, kpad, chunk_override, &clen);
   if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
   Carver cv(h->ws, h->ws_bytes);
   auto *diag = cv.take<unsigned long long>(1);
@@ -139,12 +140,12 @@ static int run_oz1(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k, do
   EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
 
   EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB));
-  EMU_TRY(launch_oz1_slice(h, elem, 0, m, k, kpad, A, lda, nullptr, eA, p, SA));
-  EMU_TRY(launch_oz1_slice(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, p, SB));
+  EMU_TRY(launch_oz1_slice(h, elem, 0, m, k, kpad, A, lda, nullptr, eA, p, bits, SA));
+  EMU_TRY(launch_oz1_slice(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, p, bits, SB));
   EMU_TRY(mark(h, 1));
 
   Oz1GemmArgs g;
-  g.m = m; g.n = n; g.kpad = kpad; g.p = p; g.SA = SA; g.SB = SB; g.eA = eA; g.eB = eB;
+  g.m = m; g.n = n; g.kpad = kpad; g.p = p; g.slice_bits = bits; g.SA = SA; g.SB = SB; g.eA = eA; g.eB = eB;
   g.alpha = alpha; g.beta = beta; g.C = C; g.ldc = ldc; g.cycles = diag;
   const int final_kind = (elem == kF32) ? 1 : 0;
   for (int c = 0; c < nch; ++c) {
@@ -255,6 +256,12 @@ int emugemm_set_stream(emugemm_handle_t h, void *s) {
   return EMUGEMM_OK;
 }
 
+int emugemm_set_slice_bits(emugemm_handle_t h, int bits) {
+  if (!h || (bits != 7 && bits != 8)) return EMUGEMM_ERR_ARG;
+  h->slice_bits = bits;
+  return EMUGEMM_OK;
+}
+
 int emugemm_set_workspace(emugemm_handle_t h, void *p, size_t bytes) {
   if (!h) return EMUGEMM_ERR_ARG;
   if (reinterpret_cast<uintptr_t>(p) & 1023) return EMUGEMM_ERR_ALIGNMENT;
@@ -272,7 +279,7 @@ size_t emugemm_workspace_bytes(int scheme, int elem, int64_t m, int64_t n, int64
     if (pn > 8 || (elem != 4 && elem != 8)) return 0;
     total += granule(static_cast<size_t>(pn) * m * kpad) + granule(static_cast<size_t>(pn) * n * kpad);
     int64_t clen;
-    const int nch = oz1_chunks(pn, kpad, 0, &clen);
+    const int nch = oz1_chunks(pn, 8, kpad, 0, &clen);  // the 8-bit mode has the shorter chunks: size for it
     if (nch > 1) total += granule(static_cast<size_t>(nch) * m * n * 16);
   } else if (scheme == EMUGEMM_OZ2 || scheme == EMUGEMM_OZ2_3M) {
     if (pn > kMaxModuli) return 0;
@@ -371,7 +378,7 @@ int emugemm_dbg_oz1_slices(emugemm_handle_t h, int elem, int by_cols, int64_t ro
   auto *S = cv.take<int8_t>(static_cast<size_t>(p) * rows * kpad);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   if (by_cols) EMU_TRY(launch_colmax(h, elem, rows, k, X, ldx, mb));
-  EMU_TRY(launch_oz1_slice(h, elem, by_cols, rows, k, kpad, X, ldx, mb, e_out, p, S));
+  EMU_TRY(launch_oz1_slice(h, elem, by_cols, rows, k, kpad, X, ldx, mb, e_out, p, h->slice_bits, S));
   return unpad_planes(h, out, S, static_cast<int64_t>(p) * rows, k, kpad);
 }
 
@@ -437,7 +444,10 @@ int emugemm_oz2_budget(int n_moduli, int64_t k, int is3m, int *tA, int *tB) {
   return T;
 }
 
-int64_t emugemm_oz1_chunk_k(int p) { return (p >= 1 && p <= 8) ? oz1_chunk_k_host(p) : 0; }
+int64_t emugemm_oz1_chunk_k(int p) { return (p >= 1 && p <= 8) ? oz1_chunk_k_host(p, 7) : 0; }
+int64_t emugemm_oz1_chunk_k_bits(int p, int slice_bits) {
+  return (p >= 1 && p <= 8 && (slice_bits == 7 || slice_bits == 8)) ? oz1_chunk_k_host(p, slice_bits) : 0;
+}
 
 int emugemm_dbg_i8_probe(emugemm_handle_t h, int n_ops, const int *ops, int iters, float *ms, int *ctas,
                          long long *cycles) {

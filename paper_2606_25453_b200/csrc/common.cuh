@@ -30,6 +30,7 @@ struct emugemm_ctx {
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   int launches = 0;
   int dbg_flags = 0;
+  int slice_bits = 7;  // Scheme I digits: 7 = sign-magnitude (R1, default), 8 = balanced base 256 (R23)
   unsigned long long *diag = nullptr;  // device: [0] = GEMM-kernel SM cycles of the last call (inside the workspace)
   PFN_cuTensorMapEncodeTiled_v12000 encode = nullptr;
 };
@@ -74,7 +75,8 @@ int launch_colmax(emugemm_ctx *ctx, int elem, int64_t rows, int64_t k, const voi
 // by_cols = 0: one fused kernel scans each row and slices it (maxbits unused); by_cols = 1: maxbits[rows] from
 // launch_colmax, the kernel derives and publishes the exponents.
 int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
-                     const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int p, int8_t *out);
+                     const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int p, int slice_bits,
+                     int8_t *out);
 
 // Scheme II residues: elem 8: out[N][rows][kpad]; elem 16: out[3][N][rows][kpad] (re, im, Sigma); e as above.
 int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
@@ -85,6 +87,7 @@ struct Oz1GemmArgs {
   int64_t m, n, kpad;          // kpad: padded k of the slice planes (multiple of kBlockK)
   int64_t k0, k1;              // k-chunk [k0, k1) handled by this launch (multiples of kBlockK)
   int p;
+  int slice_bits;              // 7 or 8 (weights 2^(bits (p-1-s)), scaling 2^(eA + eB - bits (p+1) [+ 4 guard bits]))
   const int8_t *SA, *SB;       // [p][m][kpad], [p][n][kpad]
   const int32_t *eA, *eB;
   int out_kind;                // 0: final FP64 C, 1: final FP32 C, 2: INT32 dump [p][m][n], 3: double-double partial [m][n][2]
@@ -127,6 +130,6 @@ int launch_i8_probe(emugemm_ctx *ctx, int n_ops, const int *ops, int iters, floa
 // host helpers shared by api.cu and the drivers
 int oz2_moduli_host(int n, int *mod);                  // greedy coprime list, descending from 256
 int oz2_budget_host(int n, int64_t k, int is3m, int *tA, int *tB);
-int64_t oz1_chunk_k_host(int p);
+int64_t oz1_chunk_k_host(int p, int slice_bits = 7);
 
 }  // namespace emu

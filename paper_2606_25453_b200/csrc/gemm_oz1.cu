@@ -151,6 +151,7 @@ struct Oz1Dev {
   void *C;
   int64_t ldc;
   unsigned long long *cycles;
+  int slice_bits;  // 7 or 8
   int dbg;  // experiment flags (emugemm_dbg_set_flags): 1 = no TMA after the ring is first filled, 2 = no epilogue math
 };
 
@@ -180,19 +181,35 @@ template <int P, int OUT>
 struct Oz1Epi {
   static constexpr int NG = (P + 2) / 3;  // groups, most significant first; the last may hold 1 or 2 accumulators
   bool vec_c, vec_e;
+  int w1, w2;             // 2^bits, 2^(2 bits): weights inside a group (bits = 7 or 8, run-time: same code for R1 and R23)
+  long long bias[NG];     // exponent-bias constants per group
+  double unb[NG];
+  int e_off;              // exponent of the scaling besides eA_i + eB_j
   __device__ __forceinline__ void init(const Oz1Dev &a) {
     vec_c = (a.ldc % 4 == 0) && ((reinterpret_cast<uintptr_t>(a.C) & 31) == 0);
     vec_e = (reinterpret_cast<uintptr_t>(a.eB) & 15) == 0;
-  }
-  // group g covers accumulators s = 3g .. min(3g+2, P-1); its weight is 2^(7 (P-1-last))
-  __device__ __forceinline__ static double group(const uint32_t (&v)[P][8], int c, int g) {
-    const int s0 = 3 * g, s1 = (3 * g + 2 < P - 1) ? 3 * g + 2 : P - 1;
-    const int sh = kBeta * (P - 1 - s1);
-    long long G = magic_bias(sh);
+    const int bits = a.slice_bits;
+    w1 = 1 << bits;
+    w2 = 1 << (2 * bits);
 #pragma unroll
-    for (int s = s0; s <= s1; ++s)  // IMAD.WIDE: sign-extending 32 x 32 -> 64 multiply-add
-      G += static_cast<long long>(static_cast<int32_t>(v[s][c])) * static_cast<long long>(1 << (kBeta * (s1 - s)));
-    return unbias(G, sh);
+    for (int g = 0; g < NG; ++g) {
+      const int s1 = (3 * g + 2 < P - 1) ? 3 * g + 2 : P - 1;
+      const int sh = bits * (P - 1 - s1);
+      bias[g] = (static_cast<long long>(0x433 + sh) << 52) + (1LL << 51);
+      unb[g] = __longlong_as_double(bias[g]);
+    }
+    e_off = (bits == 8 ? 4 : 0) - bits * (P + 1);  // R23: two guard bits per operand
+  }
+  // group g covers accumulators s = 3g .. min(3g+2, P-1); its weight is 2^(bits (P-1-last)); |G| < 2^49 < 2^51
+  __device__ __forceinline__ double group(const uint32_t (&v)[P][8], int c, int g) const {
+    const int s0 = 3 * g, s1 = (3 * g + 2 < P - 1) ? 3 * g + 2 : P - 1;
+    long long G = bias[g];
+#pragma unroll
+    for (int s = s0; s <= s1; ++s) {  // IMAD.WIDE: sign-extending 32 x 32 -> 64 multiply-add
+      const int w = (s1 - s == 0) ? 1 : (s1 - s == 1) ? w1 : w2;
+      G += static_cast<long long>(static_cast<int32_t>(v[s][c])) * static_cast<long long>(w);
+    }
+    return __longlong_as_double(G) - unb[g];
   }
   // column exponents of one 8-column chunk (issued one chunk ahead of their use: the load latency is hidden)
   __device__ __forceinline__ void load_eb(const Oz1Dev &a, int64_t gcol, int (&eb)[8]) const {
@@ -461,7 +478,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       if constexpr (MC) nb = 2 * nb + static_cast<int>(cta);
       const int64_t grow = static_cast<int64_t>(mb) * kTileRows + (PAIR ? cta * kTileM : 0u) + row;
       const bool row_ok = grow < a.m;
-      const int eArow = row_ok ? __ldg(a.eA + grow) - kBeta * (P + 1) : 0;
+      const int eArow = row_ok ? __ldg(a.eA + grow) + epi.e_off : 0;
       const int64_t gcol0 = static_cast<int64_t>(nb) * NT + half * (NT / 2);
       int ea[8], eb[8];
       epi.load_eb(a, gcol0, ea);  // first chunk's column exponents: in flight while the tile's MMAs finish
@@ -551,6 +568,7 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   d.eA = g.eA; d.eB = g.eB;
   d.out_kind = g.out_kind; d.alpha = g.alpha; d.beta = g.beta; d.C = g.C; d.ldc = g.ldc;
   d.cycles = g.cycles;
+  d.slice_bits = g.slice_bits;
   d.dbg = ctx->dbg_flags;
   constexpr bool CL2 = PAIR || MC;
   const int tiles = d.mt * d.nt_tiles;
@@ -610,8 +628,9 @@ int launch_oz1_gemm(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
 
 // Overflow-safe k-chunk (R7): the fullest accumulator C_{p-1} sums p products of k_c
 // terms each bounded by 127^2, so p k_c 127^2 <= 2^31 - 1; rounded down to a multiple of 128.
-int64_t oz1_chunk_k_host(int p) {
-  const int64_t bound = 2147483647LL / (static_cast<int64_t>(p) * 127 * 127);
+int64_t oz1_chunk_k_host(int p, int slice_bits) {
+  const int64_t dmax = (slice_bits == 8) ? 128 : 127;  // largest digit magnitude
+  const int64_t bound = 2147483647LL / (static_cast<int64_t>(p) * dmax * dmax);
   return bound / kBlockK * kBlockK;
 }
 

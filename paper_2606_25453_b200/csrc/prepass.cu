@@ -263,6 +263,31 @@ __device__ __forceinline__ unsigned int pack4(int a, int b, int c, int d) {
          ((static_cast<unsigned int>(c) & 0xFFu) << 16) | ((static_cast<unsigned int>(d) & 0xFFu) << 24);
 }
 
+// Balanced base-256 digits (R23): X = +-|X| (|X| < 2^(8P-2)), Y = X + sum_j 128 256^j; digit t = byte (P-1-t) of Y
+// minus 128 = that byte XOR 0x80 as int8.  One 64-bit add per element, then byte permutes only.
+template <int P, typename Sink>
+__device__ __forceinline__ void emit_oz1_b8(const Prep (&q)[4], Sink sink) {
+  constexpr unsigned long long kC = (P == 8) ? 0x8080808080808080ull : ((0x8080808080808080ull) & ((1ull << (8 * (P & 7))) - 1ull));
+  unsigned int lo[4], hi[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const long long mag = static_cast<long long>((static_cast<unsigned long long>(q[i].w1) << 32) | q[i].w0);
+    const unsigned long long Y = (static_cast<unsigned long long>(q[i].neg ? -mag : mag) + kC) ^ kC;  // bytes = int8 digits
+    lo[i] = static_cast<unsigned int>(Y);
+    hi[i] = static_cast<unsigned int>(Y >> 32);
+  }
+#pragma unroll
+  for (int t = 0; t < P; ++t) {
+    const int byte = P - 1 - t;  // byte index inside Y
+    // selector: result byte 0 = byte (byte & 3) of the first operand, result byte 1 = the same byte of the second
+    const unsigned int sel = static_cast<unsigned int>(byte & 3) | (static_cast<unsigned int>(4 + (byte & 3)) << 4);
+    const unsigned int w = (byte < 4)
+        ? __byte_perm(__byte_perm(lo[0], lo[1], sel), __byte_perm(lo[2], lo[3], sel), 0x5410)
+        : __byte_perm(__byte_perm(hi[0], hi[1], sel), __byte_perm(hi[2], hi[3], sel), 0x5410);
+    sink(t, w);
+  }
+}
+
 template <int P, typename Sink>
 __device__ __forceinline__ void emit_oz1(const Prep (&q)[4], Sink sink) {
 #pragma unroll
@@ -306,7 +331,8 @@ __device__ __forceinline__ void emit_quad(const T (&v)[4][W], int e_row, int par
 #pragma unroll
   for (int i = 0; i < 4; ++i) a[i] = prepare<T, NW>(v[i][0], e_row, scale_bits);
   if constexpr (MODE == 0) {
-    emit_oz1<PARAM>(a, sink);
+    if constexpr (PARAM >= 16) emit_oz1_b8<PARAM - 16>(a, sink);  // PARAM = 16 + p: balanced 8-bit digits
+    else emit_oz1<PARAM>(a, sink);
   } else if constexpr (W == 1) {
     emit_oz2_real_from<0>(a, param, sink);
   } else {
@@ -444,13 +470,16 @@ static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k,
 
 template <typename T, int P>
 static int slice_p(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
-                   const unsigned long long *maxbits, int32_t *e, int8_t *out) {
+                   const unsigned long long *maxbits, int32_t *e, int slice_bits, int8_t *out) {
+  if (slice_bits == 8)  // |X| = trunc(|x| 2^(8p - 2 - e)): two guard bits
+    return launch_planes<T, 1, 0, 16 + P>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, 8 * P - 2, P, out);
   return launch_planes<T, 1, 0, P>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, kBeta * P, P, out);
 }
 
 int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
-                     const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int p, int8_t *out) {
-#define EMU_SLICE_CASE(T, PP) case PP: return slice_p<T, PP>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, out)
+                     const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int p, int slice_bits,
+                     int8_t *out) {
+#define EMU_SLICE_CASE(T, PP) case PP: return slice_p<T, PP>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out)
   if (elem == kF64) {
     switch (p) {
       EMU_SLICE_CASE(double, 1); EMU_SLICE_CASE(double, 2); EMU_SLICE_CASE(double, 3); EMU_SLICE_CASE(double, 4);
