@@ -85,10 +85,11 @@ static void crt_constants(int N, CrtConst &c) {
 // (108 %) by the first version of this kernel at 1 conversion / clk / SM; both are replaced by exponent-bias
 // additions on the FP64 pipe (profiles/).
 __device__ __forceinline__ double pow2_dev(int e) { return __hiloint2double((1023 + e) << 20, 0); }
-// exact double of a residue byte b (two's complement int8 in the low 8 bits of w >> sh)
-__device__ __forceinline__ double residue_to_double(unsigned w, int sh) {
-  const unsigned biased = ((w >> sh) & 0xFFu) ^ 0x80u;  // c + 128 in [0, 255]
-  return __hiloint2double(0x43300000, static_cast<int>(biased)) - 4503599627370624.0;  // (2^52 + c + 128) - (2^52 + 128)
+// exact double of residue byte i of wx, where wx = w ^ 0x80808080 holds c + 128 in [0, 255] per byte:
+// one byte permute + one FP64 addition: (2^52 + c + 128) - (2^52 + 128)
+__device__ __forceinline__ double residue_to_double(unsigned wx, int i) {
+  const unsigned biased = __byte_perm(wx, 0u, 0x4440u | static_cast<unsigned>(i));
+  return __hiloint2double(0x43300000, static_cast<int>(biased)) - 4503599627370624.0;
 }
 __device__ __forceinline__ double round_nearest(double x) {  // |x| < 2^51: round to nearest even without F2F
   const double big = 6755399441055744.0;  // 1.5 * 2^52
@@ -117,9 +118,11 @@ __device__ __forceinline__ void crt_accumulate(const CrtConst &k, const int8_t *
           if (j0 + 4 + e < n) w1 |= static_cast<unsigned>(static_cast<uint8_t>(src[l * plane + 4 + e])) << (8 * e);
         }
       }
+      w0 ^= 0x80808080u;
+      w1 ^= 0x80808080u;
 #pragma unroll
       for (int e = 0; e < kCrtVec; ++e) {
-        const double cl = residue_to_double(e < 4 ? w0 : w1, 8 * (e & 3));
+        const double cl = residue_to_double(e < 4 ? w0 : w1, e & 3);
         shi[e] = fma(k.whi[l], cl, shi[e]);
         slo[e] = fma(k.wlo[l], cl, slo[e]);
       }

@@ -232,19 +232,27 @@ __host__ __device__ constexpr unsigned int magic32(int m) {  // ceil(2^32 / m)
                                    static_cast<unsigned long long>(m));
 }
 
-// symmetric residue of sign * (w2:w1:w0) modulo the L-th modulus (L compile-time)
+// symmetric residue of sign * (w2:w1:w0) modulo the L-th modulus (L compile-time).
+// Odd m, hm = (m-1)/2: t = sum_j byte_j (256^j mod m) + hm == |a'| + hm (mod m), t < 2^20; q = floor(t / m) by one
+// multiply-high (exact: t (M m - 2^32) / (m 2^32) < 2^-12 < 1/m); (t - q m) - hm lies in [-hm, hm] and is congruent
+// to |a'|: the symmetric residue of the magnitude (R11), and sym(-x) = -sym(x) for odd m (R13).  m = 256: the low
+// byte of the two's complement value.
 template <int L>
 __device__ __forceinline__ int oz2_residue(const Prep &q) {  // q.w2 == 0 is a compile-time constant on the two-word path
   constexpr int m = h_moduli[L];
-  constexpr unsigned int c0 = pack_w(0, m), c1 = pack_w(1, m), c2 = pack_w(2, m), mg = magic32(m);
-  unsigned int s = __dp4a(q.w0, c0, 0u);
-  s = __dp4a(q.w1, c1, s);
-  s = __dp4a(q.w2, c2, s);                       // < 12 * 255 * 255 < 2^20, congruent to |a'| mod m
-  const unsigned int qq = __umulhi(s, mg);       // floor(s / m): error s / 2^32 < 2^-12 < 1/m
-  int r = static_cast<int>(s - qq * static_cast<unsigned int>(m));  // [0, m)
-  if (q.neg && r) r = m - r;                     // floored mod of the signed value (R13)
-  if (r >= (m + 1) / 2) r -= m;                  // symmetric range (R11)
-  return r;
+  if constexpr (m == 256) {
+    const unsigned int v = q.neg ? 0u - q.w0 : q.w0;
+    return static_cast<int>(static_cast<signed char>(v & 0xFFu));
+  } else {
+    constexpr unsigned int c0 = pack_w(0, m), c1 = pack_w(1, m), c2 = pack_w(2, m), mg = magic32(m);
+    constexpr unsigned int hm = (m - 1) / 2;
+    unsigned int t = __dp4a(q.w0, c0, hm);
+    t = __dp4a(q.w1, c1, t);
+    t = __dp4a(q.w2, c2, t);
+    const unsigned int qq = __umulhi(t, mg);
+    const int r = static_cast<int>(t - qq * static_cast<unsigned int>(m)) - static_cast<int>(hm);
+    return q.neg ? -r : r;
+  }
 }
 template <int L>
 __device__ __forceinline__ int sym_small(int t) {  // t in (-m, m): re-reduce to the symmetric range (R15)
@@ -258,9 +266,9 @@ __device__ __forceinline__ int sym_small(int t) {  // t in (-m, m): re-reduce to
 // plane emission.  Each thread owns 4 consecutive k of one row/column ("quad")
 // and emits one packed 32-bit word per plane through `sink(plane, word)`.
 // ----------------------------------------------------------------------------
-__device__ __forceinline__ unsigned int pack4(int a, int b, int c, int d) {
-  return (static_cast<unsigned int>(a) & 0xFFu) | ((static_cast<unsigned int>(b) & 0xFFu) << 8) |
-         ((static_cast<unsigned int>(c) & 0xFFu) << 16) | ((static_cast<unsigned int>(d) & 0xFFu) << 24);
+__device__ __forceinline__ unsigned int pack4(int a, int b, int c, int d) {  // low bytes -> one word (3 PRMT)
+  return __byte_perm(__byte_perm(static_cast<unsigned int>(a), static_cast<unsigned int>(b), 0x0040),
+                     __byte_perm(static_cast<unsigned int>(c), static_cast<unsigned int>(d), 0x0040), 0x5410);
 }
 
 // Balanced base-256 digits (R23): X = +-|X| (|X| < 2^(8P-2)), Y = X + sum_j 128 256^j; digit t = byte (P-1-t) of Y
