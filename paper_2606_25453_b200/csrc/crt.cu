@@ -101,28 +101,36 @@ constexpr int kCrtVec = 8;  // columns per thread on the vector path (one 8-byte
 template <bool VEC>
 __device__ __forceinline__ void crt_accumulate(const CrtConst &k, const int8_t *__restrict__ src, int64_t plane, int64_t j0,
                                                int64_t n, double (&shi)[kCrtVec], double (&slo)[kCrtVec]) {
+  // all residue planes are requested before any is consumed: up to 20 independent 8-byte loads in flight per
+  // thread (the first version interleaved load and use and stalled on the long scoreboard, ncu)
+  unsigned w0[kMaxModuli], w1[kMaxModuli];
+#pragma unroll
+  for (int l = 0; l < kMaxModuli; ++l) {
+    w0[l] = w1[l] = 0x80808080u;
+    if (l < k.N) {
+      if (VEC) {
+        const uint2 w = __ldg(reinterpret_cast<const uint2 *>(src + l * plane));
+        w0[l] = w.x; w1[l] = w.y;
+      } else {
+        unsigned a = 0, b = 0;
+#pragma unroll
+        for (int e = 0; e < 4; ++e) {
+          if (j0 + e < n) a |= static_cast<unsigned>(static_cast<uint8_t>(src[l * plane + e])) << (8 * e);
+          if (j0 + 4 + e < n) b |= static_cast<unsigned>(static_cast<uint8_t>(src[l * plane + 4 + e])) << (8 * e);
+        }
+        w0[l] = a; w1[l] = b;
+      }
+    }
+  }
 #pragma unroll
   for (int e = 0; e < kCrtVec; ++e) { shi[e] = 0.0; slo[e] = 0.0; }
 #pragma unroll
   for (int l = 0; l < kMaxModuli; ++l) {
     if (l < k.N) {
-      unsigned w0, w1;
-      if (VEC) {
-        const uint2 w = __ldg(reinterpret_cast<const uint2 *>(src + l * plane));
-        w0 = w.x; w1 = w.y;
-      } else {
-        w0 = w1 = 0;
-#pragma unroll
-        for (int e = 0; e < 4; ++e) {
-          if (j0 + e < n) w0 |= static_cast<unsigned>(static_cast<uint8_t>(src[l * plane + e])) << (8 * e);
-          if (j0 + 4 + e < n) w1 |= static_cast<unsigned>(static_cast<uint8_t>(src[l * plane + 4 + e])) << (8 * e);
-        }
-      }
-      w0 ^= 0x80808080u;
-      w1 ^= 0x80808080u;
+      const unsigned x0 = w0[l] ^ 0x80808080u, x1 = w1[l] ^ 0x80808080u;
 #pragma unroll
       for (int e = 0; e < kCrtVec; ++e) {
-        const double cl = residue_to_double(e < 4 ? w0 : w1, e & 3);
+        const double cl = residue_to_double(e < 4 ? x0 : x1, e & 3);
         shi[e] = fma(k.whi[l], cl, shi[e]);
         slo[e] = fma(k.wlo[l], cl, slo[e]);
       }
