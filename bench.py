@@ -347,7 +347,7 @@ def main():
             roof["frac_of_probe"] = achieved / tops
         except Exception as ex:  # the probe is context, never the product
             detail["i8_issue_probe_error"] = str(ex)
-    if a.scheme == "oz1" and w["p"] == 8 and a.slice_bits == 7:
+    if a.scheme == "oz1" and w["p"] == 8 and a.slice_bits == 7 and not a.no_probe:
         # NEXT item f1 (R23): the same problem with 7 balanced 8-bit slices (28 instead of 36 products),
         # which reaches the accuracy of 8 slices of 7 bits; context only, the headline stays BASELINE's p = 8
         h.set_slice_bits(8)
