@@ -25,9 +25,11 @@ namespace emu {
 
 constexpr int kOz2NT = 256;                   // tile columns
 constexpr int kOz2PairM = 2 * kTileM;         // tile rows of a CTA pair
-constexpr int kOz2Stages = 6;
+constexpr int kOz2KPerStage = 2;              // 128-byte k-blocks per ring stage: 8 MMAs per barrier wait / commit
+constexpr int kOz2Stages = 3;
 constexpr int kOz2BStage = (kOz2NT / 2) * kBlockK;  // 16 KB: this CTA's half of the B rows
-constexpr int kOz2StageBytes = kAStageBytes + kOz2BStage;
+constexpr int kOz2KbBytes = kAStageBytes + kOz2BStage;         // one k-block: A 16 KB + this CTA's B half 16 KB
+constexpr int kOz2StageBytes = kOz2KPerStage * kOz2KbBytes;
 constexpr int kOz2Smem = kOz2Stages * kOz2StageBytes + 1024 + 256;
 
 struct Oz2Dev {
@@ -125,13 +127,16 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         const int brow = nb * kOz2NT + static_cast<int>(cta) * (kOz2NT / 2);
         for (int q = 0; q < NPROD; ++q) {
           const int plane = q * a.n_moduli + l;
-          for (int kb = 0; kb < a.kblocks; ++kb) {
+          for (int kb = 0; kb < a.kblocks; kb += kOz2KPerStage) {
+            const int nkb = (a.kblocks - kb < kOz2KPerStage) ? a.kblocks - kb : kOz2KPerStage;
             mbar_wait(&empty[st], ph ^ 1);
             const uint32_t full_leader = mapa_u32(&full[st], 0);
-            if (cta == 0) mbar_arrive_expect_tx(&full[st], 2 * kOz2StageBytes);
-            uint8_t *dst = smem + st * kOz2StageBytes;
-            tma_load_3d_cg2(dst, &tmA, full_leader, kb * kBlockK, arow, plane);
-            tma_load_3d_cg2(dst + kAStageBytes, &tmB, full_leader, kb * kBlockK, brow, plane);
+            if (cta == 0) mbar_arrive_expect_tx(&full[st], 2 * nkb * kOz2KbBytes);
+            for (int i = 0; i < nkb; ++i) {
+              uint8_t *dst = smem + st * kOz2StageBytes + i * kOz2KbBytes;
+              tma_load_3d_cg2(dst, &tmA, full_leader, (kb + i) * kBlockK, arow, plane);
+              tma_load_3d_cg2(dst + kAStageBytes, &tmB, full_leader, (kb + i) * kBlockK, brow, plane);
+            }
             if (++st == kOz2Stages) { st = 0; ph ^= 1; }
           }
         }
@@ -151,17 +156,24 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
           const uint32_t slot = item & 1, tph = (item >> 1) & 1;
           mbar_wait(&tempty[slot], tph ^ 1);
           tc_fence_after();
-          for (int kb = 0; kb < a.kblocks; ++kb) {
+          for (int kb = 0; kb < a.kblocks; kb += kOz2KPerStage) {
+            const int nkb = (a.kblocks - kb < kOz2KPerStage) ? a.kblocks - kb : kOz2KPerStage;
             if (!ready) mbar_wait(&full[st], ph);
             tc_fence_after();
-            const uint32_t a_base = smem_u32(smem + st * kOz2StageBytes), b_base = a_base + kAStageBytes;
+            const uint32_t s_base = smem_u32(smem + st * kOz2StageBytes);
             const int st_cur = st;
             if (++st == kOz2Stages) { st = 0; ph ^= 1; }
             ready = mbar_try_wait(&full[st], ph);
 #pragma unroll
-            for (int ks = 0; ks < kBlockK / 32; ++ks)
-              umma_i8_cg2(tmem_base + slot * kOz2NT, make_sdesc_sw128(a_base + ks * 32), make_sdesc_sw128(b_base + ks * 32),
-                          idesc, (kb | ks) ? 1u : 0u);
+            for (int i = 0; i < kOz2KPerStage; ++i) {
+              if (i < nkb) {
+                const uint32_t a_base = s_base + i * kOz2KbBytes, b_base = a_base + kAStageBytes;
+#pragma unroll
+                for (int ks = 0; ks < kBlockK / 32; ++ks)
+                  umma_i8_cg2(tmem_base + slot * kOz2NT, make_sdesc_sw128(a_base + ks * 32), make_sdesc_sw128(b_base + ks * 32),
+                              idesc, (kb | i | ks) ? 1u : 0u);
+              }
+            }
             umma_commit_cg2(&empty[st_cur], 3);  // both CTAs' producers may refill the stage
           }
           umma_commit_cg2(&tfull[slot], 3);      // both CTAs' epilogues may drain their 128 rows
