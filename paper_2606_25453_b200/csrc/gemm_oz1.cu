@@ -36,14 +36,16 @@ struct Oz1Cfg {
   // PAIR (cta_group::2, P <= 4): a CTA pair owns a 256 x NT tile; each CTA stages only NT/2 rows of every B slice
   static constexpr int kBRows = PAIR ? NT / 2 : NT;
   static constexpr int kBStageBytes = P * kBRows * kBlockK;
-  static constexpr int SB = 2;
+  // B ring depth.  A k-block of B is released only when all P slices have used it, so its refill has one k-block of
+  // MMA time to arrive: 4,608 clk at P = 8 but 1,536 clk at P = 2 -- pairs (small P, small stages) get three stages.
+  static constexpr int SB = PAIR ? 3 : 2;
   // A ring: one stage = the slice PAIR (j, P-1-j) of a k-block (2 x 16 KB).  Pairing the widest with the
   // narrowest slice gives every stage the same MMA time ((P+1) NT/2 clk per k32), so the single issuing thread
   // pays one barrier wait + one commit per ~constant amount of tensor work and the MMA queue never drains
   // on the narrow slices (measured: +11 % tensor-pipe activity over one barrier per slice).
   static constexpr int NPAIR = (P + 1) / 2;
   static constexpr int kAPairBytes = 2 * kAStageBytes;
-  static constexpr int kSAMax = PAIR ? 5 : 4;
+  static constexpr int kSAMax = 4;
   static constexpr int SA = (kSmemLimit - 2048 - SB * kBStageBytes) / kAPairBytes > kSAMax
                                 ? kSAMax
                                 : (kSmemLimit - 2048 - SB * kBStageBytes) / kAPairBytes;
