@@ -99,6 +99,27 @@ int emugemm_zgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, co
                          const double *A, int64_t lda, const double *B, int64_t ldb,
                          const double beta[2], double *C, int64_t ldc, int n_moduli);
 
+/* ---- transposed operands (SURVEY 8(b) "NEXT": transposes / column-major) -- *
+ * C = alpha op(A) op(B) + beta C with op(X) = X (trans = 0) or X^T (trans = 1, no
+ * conjugation).  op(A) is m x k: A is stored m x k (lda >= k) or, transposed, k x m
+ * (lda >= m); op(B) is k x n: B is stored k x n (ldb >= n) or n x k (ldb >= k).  All
+ * row-major.  A column-major BLAS call C = A B is the row-major call C^T = B^T A^T on
+ * the same buffers: swap the operands and m <-> n, every transposition flag keeps its
+ * meaning.  The pre-pass reads a k-contiguous operand with its row kernel and a
+ * k-strided one with its column (transposing) kernel; nothing else changes.        */
+int emugemm_dgemm_oz1_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha,
+                        const double *A, int64_t lda, const double *B, int64_t ldb, double beta, double *C,
+                        int64_t ldc, int p);
+int emugemm_sgemm_oz1_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, float alpha,
+                        const float *A, int64_t lda, const float *B, int64_t ldb, float beta, float *C,
+                        int64_t ldc, int p);
+int emugemm_dgemm_oz2_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha,
+                        const double *A, int64_t lda, const double *B, int64_t ldb, double beta, double *C,
+                        int64_t ldc, int n_moduli);
+int emugemm_zgemm_oz2_3m_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k,
+                           const double alpha[2], const double *A, int64_t lda, const double *B, int64_t ldb,
+                           const double beta[2], double *C, int64_t ldc, int n_moduli);
+
 /* ---- per-stage timing of the last call (bench only) --------------------- *
  * When enabled, compute calls bracket their stages with CUDA events on the
  * handle's stream; emugemm_stage_ms() synchronises and returns milliseconds of

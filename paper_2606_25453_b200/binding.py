@@ -136,39 +136,46 @@ class EmuGemm:
         assert t.stride(-1) == 1, "row-major tensors with a contiguous last dimension are required"
         return t.stride(0)
 
-    def dgemm_oz1(self, A, B, C_, p, alpha=1.0, beta=0.0):
-        m, k = A.shape
-        n = B.shape[1]
+    # transa / transb: the tensor holds the TRANSPOSE of the operand (A: k x m, B: n x k), row-major
+    @staticmethod
+    def _dims(A, B, transa, transb):
+        m, k = (A.shape[1], A.shape[0]) if transa else A.shape
+        n = B.shape[0] if transb else B.shape[1]
+        return m, n, k
+
+    def dgemm_oz1(self, A, B, C_, p, alpha=1.0, beta=0.0, transa=False, transb=False):
+        m, n, k = self._dims(A, B, transa, transb)
         self._reserve_for(OZ1, 8, m, n, k, p)
-        self._check(self._lib.emugemm_dgemm_oz1(self._h, _i64(m), _i64(n), _i64(k), _dbl(alpha), _ptr(A), _i64(self._ld(A)),
-                                                 _ptr(B), _i64(self._ld(B)), _dbl(beta), _ptr(C_), _i64(self._ld(C_)), _int(p)))
+        self._check(self._lib.emugemm_dgemm_oz1_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), _dbl(alpha),
+                                                   _ptr(A), _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), _dbl(beta), _ptr(C_),
+                                                   _i64(self._ld(C_)), _int(p)))
         return C_
 
-    def sgemm_oz1(self, A, B, C_, p, alpha=1.0, beta=0.0):
-        m, k = A.shape
-        n = B.shape[1]
+    def sgemm_oz1(self, A, B, C_, p, alpha=1.0, beta=0.0, transa=False, transb=False):
+        m, n, k = self._dims(A, B, transa, transb)
         self._reserve_for(OZ1, 4, m, n, k, p)
-        self._check(self._lib.emugemm_sgemm_oz1(self._h, _i64(m), _i64(n), _i64(k), _flt(alpha), _ptr(A), _i64(self._ld(A)),
-                                                 _ptr(B), _i64(self._ld(B)), _flt(beta), _ptr(C_), _i64(self._ld(C_)), _int(p)))
+        self._check(self._lib.emugemm_sgemm_oz1_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), _flt(alpha),
+                                                   _ptr(A), _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), _flt(beta), _ptr(C_),
+                                                   _i64(self._ld(C_)), _int(p)))
         return C_
 
-    def dgemm_oz2(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0):
-        m, k = A.shape
-        n = B.shape[1]
+    def dgemm_oz2(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0, transa=False, transb=False):
+        m, n, k = self._dims(A, B, transa, transb)
         self._reserve_for(OZ2, 8, m, n, k, n_moduli)
-        self._check(self._lib.emugemm_dgemm_oz2(self._h, _i64(m), _i64(n), _i64(k), _dbl(alpha), _ptr(A), _i64(self._ld(A)),
-                                                 _ptr(B), _i64(self._ld(B)), _dbl(beta), _ptr(C_), _i64(self._ld(C_)), _int(n_moduli)))
+        self._check(self._lib.emugemm_dgemm_oz2_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), _dbl(alpha),
+                                                   _ptr(A), _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), _dbl(beta), _ptr(C_),
+                                                   _i64(self._ld(C_)), _int(n_moduli)))
         return C_
 
-    def zgemm_oz2_3m(self, A, B, C_, n_moduli, alpha=1.0 + 0j, beta=0j):
+    def zgemm_oz2_3m(self, A, B, C_, n_moduli, alpha=1.0 + 0j, beta=0j, transa=False, transb=False):
         """A, B, C_: complex128 CUDA tensors."""
-        m, k = A.shape
-        n = B.shape[1]
+        m, n, k = self._dims(A, B, transa, transb)
         self._reserve_for(OZ2_3M, 16, m, n, k, n_moduli)
         al = (_dbl * 2)(complex(alpha).real, complex(alpha).imag)
         be = (_dbl * 2)(complex(beta).real, complex(beta).imag)
-        self._check(self._lib.emugemm_zgemm_oz2_3m(self._h, _i64(m), _i64(n), _i64(k), al, _ptr(A), _i64(self._ld(A)),
-                                                    _ptr(B), _i64(self._ld(B)), be, _ptr(C_), _i64(self._ld(C_)), _int(n_moduli)))
+        self._check(self._lib.emugemm_zgemm_oz2_3m_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), al, _ptr(A),
+                                                      _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), be, _ptr(C_),
+                                                      _i64(self._ld(C_)), _int(n_moduli)))
         return C_
 
     # ---- test hooks -----------------------------------------------------------

@@ -93,13 +93,14 @@ static int mark(emugemm_ctx *h, int i) {
   return EMUGEMM_OK;
 }
 
-static int check_gemm_args(emugemm_ctx *h, int64_t m, int64_t n, int64_t k, const void *A, int64_t lda, const void *B,
-                           int64_t ldb, const void *C, int64_t ldc) {
+static int check_gemm_args(emugemm_ctx *h, int ta, int tb, int64_t m, int64_t n, int64_t k, const void *A, int64_t lda,
+                           const void *B, int64_t ldb, const void *C, int64_t ldc) {
   if (!h) return EMUGEMM_ERR_ARG;
-  if (m < 0 || n < 0 || k < 0) return EMUGEMM_ERR_ARG;
+  if (m < 0 || n < 0 || k < 0 || (ta & ~1) || (tb & ~1)) return EMUGEMM_ERR_ARG;
   if (m == 0 || n == 0) return EMUGEMM_OK;
   if (!C || ldc < n) return EMUGEMM_ERR_ARG;
-  if (k > 0 && (!A || !B || lda < k || ldb < n)) return EMUGEMM_ERR_ARG;
+  // op(A) is m x k: stored m x k (lda >= k) or, transposed, k x m (lda >= m); op(B) is k x n likewise
+  if (k > 0 && (!A || !B || lda < (ta ? m : k) || ldb < (tb ? k : n))) return EMUGEMM_ERR_ARG;
   if ((reinterpret_cast<uintptr_t>(A) | reinterpret_cast<uintptr_t>(B) | reinterpret_cast<uintptr_t>(C)) & 15)
     return EMUGEMM_ERR_ALIGNMENT;
   if (k >= (1LL << 31) - 256 || m >= (1LL << 31) - 256 || n >= (1LL << 31) - 256) return EMUGEMM_ERR_ARG;
@@ -107,10 +108,10 @@ static int check_gemm_args(emugemm_ctx *h, int64_t m, int64_t n, int64_t k, cons
 }
 
 // Scheme I call sequence; out_mode: 0 final, 2 = INT32 dump per chunk into `dump`
-static int run_oz1(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k, double alpha, const void *A, int64_t lda,
+static int run_oz1(emugemm_ctx *h, int ta, int tb, int elem, int64_t m, int64_t n, int64_t k, double alpha, const void *A, int64_t lda,
                    const void *B, int64_t ldb, double beta, void *C, int64_t ldc, int p, int32_t *dump,
                    int64_t chunk_override, int *n_chunks_out) {
-  EMU_TRY(check_gemm_args(h, m, n, k, A, lda, B, ldb, dump ? static_cast<const void *>(dump) : C, dump ? n : ldc));
+  EMU_TRY(check_gemm_args(h, ta, tb, m, n, k, A, lda, B, ldb, dump ? static_cast<const void *>(dump) : C, dump ? n : ldc));
   if (p < 1 || p > (elem == kF32 ? 4 : 8)) return EMUGEMM_ERR_ARG;
   h->launches = 0;
   if (m == 0 || n == 0) return EMUGEMM_OK;
@@ -139,9 +140,12 @@ static int run_oz1(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k, do
   h->diag = diag;
   EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
 
-  EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB));
-  EMU_TRY(launch_oz1_slice(h, elem, 0, m, k, kpad, A, lda, nullptr, eA, p, bits, SA));
-  EMU_TRY(launch_oz1_slice(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, p, bits, SB));
+  // planes are indexed [row of op(A)] / [column of op(B)] with k contiguous: a k-major stored operand (A^T stored
+  // k x m, B stored k x n) goes through the column kernels, an operand whose k is contiguous through the row kernel
+  if (ta) EMU_TRY(launch_colmax(h, elem, m, k, A, lda, mbA));
+  if (!tb) EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB));
+  EMU_TRY(launch_oz1_slice(h, elem, ta, m, k, kpad, A, lda, mbA, eA, p, bits, SA));
+  EMU_TRY(launch_oz1_slice(h, elem, !tb, n, k, kpad, B, ldb, mbB, eB, p, bits, SB));
   EMU_TRY(mark(h, 1));
 
   Oz1GemmArgs g;
@@ -164,9 +168,9 @@ static int run_oz1(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k, do
 }
 
 // Scheme II call sequence (real and 3M)
-static int run_oz2(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_t k, const double alpha[2], const void *A,
+static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t n, int64_t k, const double alpha[2], const void *A,
                    int64_t lda, const void *B, int64_t ldb, const double beta[2], double *C, int64_t ldc, int N) {
-  EMU_TRY(check_gemm_args(h, m, n, k, A, lda, B, ldb, C, ldc));
+  EMU_TRY(check_gemm_args(h, ta, tb, m, n, k, A, lda, B, ldb, C, ldc));
   if (N < 2 || N > kMaxModuli) return EMUGEMM_ERR_ARG;
   h->launches = 0;
   if (m == 0 || n == 0) return EMUGEMM_OK;
@@ -196,9 +200,10 @@ static int run_oz2(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_t k, co
   h->diag = diag;
   EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
 
-  EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB));
-  EMU_TRY(launch_oz2_residues(h, elem, 0, m, k, kpad, A, lda, nullptr, eA, N, tA, RA));
-  EMU_TRY(launch_oz2_residues(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, N, tB, RB));
+  if (ta) EMU_TRY(launch_colmax(h, elem, m, k, A, lda, mbA));
+  if (!tb) EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB));
+  EMU_TRY(launch_oz2_residues(h, elem, ta, m, k, kpad, A, lda, mbA, eA, N, tA, RA));
+  EMU_TRY(launch_oz2_residues(h, elem, !tb, n, k, kpad, B, ldb, mbB, eB, N, tB, RB));
   EMU_TRY(mark(h, 1));
   Oz2GemmArgs g;
   g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = N; g.is3m = is3m; g.RA = RA; g.RB = RB; g.CR = CR; g.cycles = diag;
@@ -306,27 +311,46 @@ const char *emugemm_status_string(int s) {
 
 int emugemm_last_cuda_error(emugemm_handle_t h) { return h ? h->last_cuda : 0; }
 
+int emugemm_dgemm_oz1_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha,
+                        const double *A, int64_t lda, const double *B, int64_t ldb, double beta, double *C, int64_t ldc, int p) {
+  return run_oz1(h, transa, transb, kF64, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, p, nullptr, 0, nullptr);
+}
+int emugemm_sgemm_oz1_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, float alpha,
+                        const float *A, int64_t lda, const float *B, int64_t ldb, float beta, float *C, int64_t ldc, int p) {
+  return run_oz1(h, transa, transb, kF32, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, p, nullptr, 0, nullptr);
+}
+int emugemm_dgemm_oz2_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha,
+                        const double *A, int64_t lda, const double *B, int64_t ldb, double beta, double *C, int64_t ldc,
+                        int n_moduli) {
+  const double al[2] = {alpha, 0.0}, be[2] = {beta, 0.0};
+  return run_oz2(h, transa, transb, 0, m, n, k, al, A, lda, B, ldb, be, C, ldc, n_moduli);
+}
+int emugemm_zgemm_oz2_3m_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, const double alpha[2],
+                           const double *A, int64_t lda, const double *B, int64_t ldb, const double beta[2], double *C,
+                           int64_t ldc, int n_moduli) {
+  if (!alpha || !beta) return EMUGEMM_ERR_ARG;
+  return run_oz2(h, transa, transb, 1, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, n_moduli);
+}
+
 int emugemm_dgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,
                       const double *B, int64_t ldb, double beta, double *C, int64_t ldc, int p) {
-  return run_oz1(h, kF64, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, p, nullptr, 0, nullptr);
+  return emugemm_dgemm_oz1_t(h, 0, 0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, p);
 }
 
 int emugemm_sgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda,
                       const float *B, int64_t ldb, float beta, float *C, int64_t ldc, int p) {
-  return run_oz1(h, kF32, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, p, nullptr, 0, nullptr);
+  return emugemm_sgemm_oz1_t(h, 0, 0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, p);
 }
 
 int emugemm_dgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,
                       const double *B, int64_t ldb, double beta, double *C, int64_t ldc, int n_moduli) {
-  const double al[2] = {alpha, 0.0}, be[2] = {beta, 0.0};
-  return run_oz2(h, 0, m, n, k, al, A, lda, B, ldb, be, C, ldc, n_moduli);
+  return emugemm_dgemm_oz2_t(h, 0, 0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, n_moduli);
 }
 
 int emugemm_zgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2], const double *A,
                          int64_t lda, const double *B, int64_t ldb, const double beta[2], double *C, int64_t ldc,
                          int n_moduli) {
-  if (!alpha || !beta) return EMUGEMM_ERR_ARG;
-  return run_oz2(h, 1, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, n_moduli);
+  return emugemm_zgemm_oz2_3m_t(h, 0, 0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, n_moduli);
 }
 
 int emugemm_last_gemm_cycles(emugemm_handle_t h, unsigned long long *cycles) {
@@ -385,7 +409,7 @@ int emugemm_dbg_oz1_slices(emugemm_handle_t h, int elem, int by_cols, int64_t ro
 int emugemm_dbg_oz1_accumulators(emugemm_handle_t h, int elem, int64_t m, int64_t n, int64_t k, const void *A, int64_t lda,
                                  const void *B, int64_t ldb, int p, int64_t chunk_k, int32_t *out, int *n_chunks_out) {
   if (!out) return EMUGEMM_ERR_ARG;
-  return run_oz1(h, elem, m, n, k, 1.0, A, lda, B, ldb, 0.0, nullptr, n, p, out, chunk_k, n_chunks_out);
+  return run_oz1(h, 0, 0, elem, m, n, k, 1.0, A, lda, B, ldb, 0.0, nullptr, n, p, out, chunk_k, n_chunks_out);
 }
 
 int emugemm_dbg_oz2_residues(emugemm_handle_t h, int elem, int by_cols, int64_t rows, int64_t k, const void *X, int64_t ldx,
