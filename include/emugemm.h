@@ -120,6 +120,35 @@ int emugemm_zgemm_oz2_3m_t(emugemm_handle_t h, int transa, int transb, int64_t m
                            const double alpha[2], const double *A, int64_t lda, const double *B, int64_t ldb,
                            const double beta[2], double *C, int64_t ldc, int n_moduli);
 
+/* ---- pre-decomposed operands ---------- *
+ * An operand that takes part in several products is decomposed ONCE (slices or
+ * residues + exponents, in the library's private layout, inside a caller-owned device
+ * buffer) and then multiplied any number of times with emugemm_gemm_pre(), which
+ * runs only the fused GEMM and the reconstruction.  Results are bit-identical to the
+ * one-shot calls.  The struct is plain data owned by the caller; the buffer must
+ * outlive its uses, be 1024-byte aligned and hold emugemm_operand_bytes() bytes.
+ *   scheme : EMUGEMM_OZ1 (elem 4 / 8), EMUGEMM_OZ2 (elem 8), EMUGEMM_OZ2_3M (elem 16)
+ *   role   : 0 = left operand op(A) (rows x k), 1 = right operand op(B) (k x rows)
+ *   trans  : as in the _t calls (role 0: X stored k x rows; role 1: X stored rows x k)
+ * Scheme II scales an operand with a bit budget that depends on k, n_moduli and the
+ * role, so a handle is tied to them; Scheme I handles are tied to p and the digit
+ * format of the handle at decomposition time.                                      */
+typedef struct emugemm_operand {
+  int scheme, role, elem, pn, slice_bits, t_bits;
+  int64_t rows, k, kpad;
+  void *buf;       /* device: int8 planes [planes][rows][kpad], then int32 exponents [rows] */
+  size_t bytes;
+} emugemm_operand_t;
+size_t emugemm_operand_bytes(int scheme, int64_t rows, int64_t k, int p_or_nmoduli);
+int emugemm_decompose(emugemm_handle_t h, int scheme, int role, int trans, int elem, int64_t rows, int64_t k,
+                      const void *X, int64_t ldx, int p_or_nmoduli, void *dev_buf, size_t bytes,
+                      emugemm_operand_t *out);
+/* C (m x n, type by elem: float / double / complex128) = alpha A B + beta C; alpha, beta point to
+ * HOST {re, im} (im ignored for real).  A->rows = m, B->rows = n, both with the same scheme, elem,
+ * k, p / n_moduli (and digit format).  Needs the workspace of the corresponding one-shot call. */
+int emugemm_gemm_pre(emugemm_handle_t h, const emugemm_operand_t *A, const emugemm_operand_t *B, const double alpha[2],
+                     const double beta[2], void *C, int64_t ldc);
+
 /* ---- per-stage timing of the last call (bench only) --------------------- *
  * When enabled, compute calls bracket their stages with CUDA events on the
  * handle's stream; emugemm_stage_ms() synchronises and returns milliseconds of

@@ -14,6 +14,13 @@ OZ1, OZ2, OZ2_3M = 1, 2, 3
 _i64, _int, _dbl, _flt, _vp, _sz = C.c_int64, C.c_int, C.c_double, C.c_float, C.c_void_p, C.c_size_t
 
 
+class Operand(C.Structure):
+    """emugemm_operand_t (include/emugemm.h): a pre-decomposed operand; `tensor` keeps the device buffer alive."""
+    _fields_ = [("scheme", C.c_int), ("role", C.c_int), ("elem", C.c_int), ("pn", C.c_int), ("slice_bits", C.c_int),
+                ("t_bits", C.c_int), ("rows", C.c_int64), ("k", C.c_int64), ("kpad", C.c_int64), ("buf", C.c_void_p),
+                ("bytes", C.c_size_t)]
+
+
 class EmuGemmError(RuntimeError):
     def __init__(self, status, msg):
         super().__init__(f"emugemm status {status}: {msg}")
@@ -34,6 +41,8 @@ def load_library():
         lib.emugemm_status_string.restype = C.c_char_p
         lib.emugemm_workspace_bytes.restype = _sz
         lib.emugemm_workspace_bytes.argtypes = [_int, _int, _i64, _i64, _i64, _int]
+        lib.emugemm_operand_bytes.restype = _sz
+        lib.emugemm_operand_bytes.argtypes = [_int, _i64, _i64, _int]
         lib.emugemm_oz1_chunk_k.restype = _i64
         lib.emugemm_oz1_chunk_k_bits.restype = _i64
         _lib = lib
@@ -176,6 +185,35 @@ class EmuGemm:
         self._check(self._lib.emugemm_zgemm_oz2_3m_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), al, _ptr(A),
                                                       _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), be, _ptr(C_),
                                                       _i64(self._ld(C_)), _int(n_moduli)))
+        return C_
+
+    # ---- pre-decomposed operands (emugemm_decompose / emugemm_gemm_pre) --------
+    def decompose(self, scheme, role, X, pn, trans=False):
+        """-> Operand for the left (role 0) or right (role 1) operand; X as in the _t calls."""
+        torch = self._torch
+        elem = self._elem(X)
+        stored_rows, stored_cols = X.shape
+        by_cols = bool(trans) if role == 0 else not trans
+        rows, k = (stored_cols, stored_rows) if by_cols else (stored_rows, stored_cols)
+        nbytes = int(self._lib.emugemm_operand_bytes(scheme, rows, k, pn))
+        assert nbytes > 0, "invalid operand arguments"
+        raw = torch.empty(nbytes + 1024, dtype=torch.uint8, device="cuda")
+        off = (-raw.data_ptr()) % 1024
+        if self._ws is None or self._ws.numel() < 8 * rows + 4096:
+            self.reserve(max(8 * rows + 4096, 1 << 20))
+        op = Operand()
+        self._check(self._lib.emugemm_decompose(self._h, _int(scheme), _int(role), _int(int(trans)), _int(elem), _i64(rows), _i64(k),
+                                                 _ptr(X), _i64(self._ld(X)), _int(pn), _vp(raw.data_ptr() + off), _sz(nbytes),
+                                                 C.byref(op)))
+        op.tensor = raw
+        return op
+
+    def gemm_pre(self, opA, opB, C_, alpha=1.0, beta=0.0):
+        scheme_elem = {(OZ1, 4): 4, (OZ1, 8): 8, (OZ2, 8): 8, (OZ2_3M, 16): 16}[(opA.scheme, opA.elem)]
+        self._reserve_for(opA.scheme, scheme_elem, opA.rows, opB.rows, opA.k, opA.pn)
+        al = (_dbl * 2)(complex(alpha).real, complex(alpha).imag)
+        be = (_dbl * 2)(complex(beta).real, complex(beta).imag)
+        self._check(self._lib.emugemm_gemm_pre(self._h, C.byref(opA), C.byref(opB), al, be, _ptr(C_), _i64(self._ld(C_))))
         return C_
 
     # ---- test hooks -----------------------------------------------------------

@@ -107,6 +107,29 @@ static int check_gemm_args(emugemm_ctx *h, int ta, int tb, int64_t m, int64_t n,
   return EMUGEMM_OK;
 }
 
+// Fused GEMM (one launch per overflow-safe k-chunk) + chunk reduction from sliced operands (shared by the one-shot
+// calls and the pre-decomposed operand path).
+static int oz1_gemm_phase(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t kpad, int p, int bits, const int8_t *SA,
+                          const int8_t *SB, const int32_t *eA, const int32_t *eB, double alpha, double beta, void *C,
+                          int64_t ldc, int32_t *dump, int nch, int64_t clen, double *part, unsigned long long *diag) {
+  Oz1GemmArgs g;
+  g.m = m; g.n = n; g.kpad = kpad; g.p = p; g.slice_bits = bits; g.SA = SA; g.SB = SB; g.eA = eA; g.eB = eB;
+  g.alpha = alpha; g.beta = beta; g.C = C; g.ldc = ldc; g.cycles = diag;
+  const int final_kind = (elem == kF32) ? 1 : 0;
+  for (int c = 0; c < nch; ++c) {
+    g.k0 = c * clen;
+    g.k1 = (g.k0 + clen < kpad) ? g.k0 + clen : kpad;
+    if (dump) { g.out_kind = 2; g.C = dump + static_cast<int64_t>(c) * p * m * n; }
+    else if (nch == 1) g.out_kind = final_kind;
+    else { g.out_kind = 3; g.C = part + static_cast<int64_t>(c) * m * n * 2; }
+    EMU_TRY(launch_oz1_gemm(h, g));
+  }
+  EMU_TRY(mark(h, 2));
+  if (nch > 1 && !dump) EMU_TRY(launch_oz1_chunk_reduce(h, m, n, nch, part, final_kind, alpha, beta, C, ldc));
+  EMU_TRY(mark(h, 3));
+  return EMUGEMM_OK;
+}
+
 // Scheme I call sequence; out_mode: 0 final, 2 = INT32 dump per chunk into `dump`
 static int run_oz1(emugemm_ctx *h, int ta, int tb, int elem, int64_t m, int64_t n, int64_t k, double alpha, const void *A, int64_t lda,
                    const void *B, int64_t ldb, double beta, void *C, int64_t ldc, int p, int32_t *dump,
@@ -147,23 +170,25 @@ static int run_oz1(emugemm_ctx *h, int ta, int tb, int elem, int64_t m, int64_t 
   EMU_TRY(launch_oz1_slice(h, elem, ta, m, k, kpad, A, lda, mbA, eA, p, bits, SA));
   EMU_TRY(launch_oz1_slice(h, elem, !tb, n, k, kpad, B, ldb, mbB, eB, p, bits, SB));
   EMU_TRY(mark(h, 1));
-
-  Oz1GemmArgs g;
-  g.m = m; g.n = n; g.kpad = kpad; g.p = p; g.slice_bits = bits; g.SA = SA; g.SB = SB; g.eA = eA; g.eB = eB;
-  g.alpha = alpha; g.beta = beta; g.C = C; g.ldc = ldc; g.cycles = diag;
-  const int final_kind = (elem == kF32) ? 1 : 0;
-  for (int c = 0; c < nch; ++c) {
-    g.k0 = c * clen;
-    g.k1 = (g.k0 + clen < kpad) ? g.k0 + clen : kpad;
-    if (dump) { g.out_kind = 2; g.C = dump + static_cast<int64_t>(c) * p * m * n; }
-    else if (nch == 1) g.out_kind = final_kind;
-    else { g.out_kind = 3; g.C = part + static_cast<int64_t>(c) * m * n * 2; }
-    EMU_TRY(launch_oz1_gemm(h, g));
-  }
-  EMU_TRY(mark(h, 2));
-  if (nch > 1 && !dump) EMU_TRY(launch_oz1_chunk_reduce(h, m, n, nch, part, final_kind, alpha, beta, C, ldc));
-  EMU_TRY(mark(h, 3));
+  EMU_TRY(oz1_gemm_phase(h, elem, m, n, kpad, p, bits, SA, SB, eA, eB, alpha, beta, C, ldc, dump, nch, clen, part, diag));
   if (n_chunks_out) *n_chunks_out = nch;
+  return EMUGEMM_OK;
+}
+
+// Per-modulus GEMMs with fused reduction + CRT from residue planes (one-shot calls and pre-decomposed operands).
+static int oz2_gemm_phase(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_t kpad, int N, const int8_t *RA,
+                          const int8_t *RB, int8_t *CR, const int32_t *eA, const int32_t *eB, int tA, int tB,
+                          const double alpha[2], const double beta[2], double *C, int64_t ldc, unsigned long long *diag) {
+  Oz2GemmArgs g;
+  g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = N; g.is3m = is3m; g.RA = RA; g.RB = RB; g.CR = CR; g.cycles = diag;
+  EMU_TRY(launch_oz2_gemm(h, g));
+  EMU_TRY(mark(h, 2));
+  Oz2CrtArgs c;
+  c.m = m; c.n = n; c.n_moduli = N; c.CR = CR; c.eA = eA; c.eB = eB; c.tA = tA; c.tB = tB; c.is_complex = is3m;
+  c.alpha[0] = alpha[0]; c.alpha[1] = alpha[1]; c.beta[0] = beta[0]; c.beta[1] = beta[1];
+  c.C = C; c.ldc = ldc;
+  EMU_TRY(launch_oz2_crt(h, c));
+  EMU_TRY(mark(h, 3));
   return EMUGEMM_OK;
 }
 
@@ -205,17 +230,7 @@ static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t 
   EMU_TRY(launch_oz2_residues(h, elem, ta, m, k, kpad, A, lda, mbA, eA, N, tA, RA));
   EMU_TRY(launch_oz2_residues(h, elem, !tb, n, k, kpad, B, ldb, mbB, eB, N, tB, RB));
   EMU_TRY(mark(h, 1));
-  Oz2GemmArgs g;
-  g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = N; g.is3m = is3m; g.RA = RA; g.RB = RB; g.CR = CR; g.cycles = diag;
-  EMU_TRY(launch_oz2_gemm(h, g));
-  EMU_TRY(mark(h, 2));
-  Oz2CrtArgs c;
-  c.m = m; c.n = n; c.n_moduli = N; c.CR = CR; c.eA = eA; c.eB = eB; c.tA = tA; c.tB = tB; c.is_complex = is3m;
-  c.alpha[0] = alpha[0]; c.alpha[1] = alpha[1]; c.beta[0] = beta[0]; c.beta[1] = beta[1];
-  c.C = C; c.ldc = ldc;
-  EMU_TRY(launch_oz2_crt(h, c));
-  EMU_TRY(mark(h, 3));
-  return EMUGEMM_OK;
+  return oz2_gemm_phase(h, is3m, m, n, kpad, N, RA, RB, CR, eA, eB, tA, tB, alpha, beta, C, ldc, diag);
 }
 
 }  // namespace emu
@@ -351,6 +366,92 @@ int emugemm_zgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, co
                          int64_t lda, const double *B, int64_t ldb, const double beta[2], double *C, int64_t ldc,
                          int n_moduli) {
   return emugemm_zgemm_oz2_3m_t(h, 0, 0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, n_moduli);
+}
+
+// ---- pre-decomposed operands ---------------------------------------------------
+static int operand_planes(int scheme, int pn) { return scheme == EMUGEMM_OZ2_3M ? 3 * pn : pn; }
+
+size_t emugemm_operand_bytes(int scheme, int64_t rows, int64_t k, int pn) {
+  if (rows < 0 || k < 0 || pn < 1) return 0;
+  if (scheme == EMUGEMM_OZ1 ? pn > 8 : (scheme == EMUGEMM_OZ2 || scheme == EMUGEMM_OZ2_3M) ? pn > kMaxModuli : true) return 0;
+  const int64_t kpad = round_up(k, kBlockK);
+  return granule(static_cast<size_t>(operand_planes(scheme, pn)) * rows * kpad) + granule(4 * static_cast<size_t>(rows)) + 1024;
+}
+
+int emugemm_decompose(emugemm_handle_t h, int scheme, int role, int trans, int elem, int64_t rows, int64_t k, const void *X,
+                      int64_t ldx, int pn, void *dev_buf, size_t bytes, emugemm_operand_t *out) {
+  if (!h || !out || !dev_buf || !X || rows <= 0 || k <= 0 || (role & ~1) || (trans & ~1)) return EMUGEMM_ERR_ARG;
+  const bool oz1 = scheme == EMUGEMM_OZ1, oz2 = scheme == EMUGEMM_OZ2, z3m = scheme == EMUGEMM_OZ2_3M;
+  if (!(oz1 || oz2 || z3m)) return EMUGEMM_ERR_ARG;
+  if (oz1 ? !((elem == kF64 && pn >= 1 && pn <= 8) || (elem == kF32 && pn >= 1 && pn <= 4))
+          : !(elem == (z3m ? kZ128 : kF64) && pn >= 2 && pn <= kMaxModuli))
+    return EMUGEMM_ERR_ARG;
+  const int by_cols = role == 0 ? trans : !trans;  // is k the strided dimension of the stored operand?
+  if (ldx < (by_cols ? rows : k)) return EMUGEMM_ERR_ARG;
+  if ((reinterpret_cast<uintptr_t>(X) & 15) || (reinterpret_cast<uintptr_t>(dev_buf) & 1023)) return EMUGEMM_ERR_ALIGNMENT;
+  if (bytes < emugemm_operand_bytes(scheme, rows, k, pn)) return EMUGEMM_ERR_WORKSPACE;
+  int t_bits = 0;
+  if (!oz1) {
+    int tA, tB;
+    if (oz2_budget_host(pn, k, z3m, &tA, &tB) < 2 || k > 131071) return EMUGEMM_ERR_PRECISION;
+    t_bits = role == 0 ? tA : tB;
+  }
+  const int64_t kpad = round_up(k, kBlockK);
+  Carver ob(dev_buf, bytes);
+  auto *planes = ob.take<int8_t>(static_cast<size_t>(operand_planes(scheme, pn)) * rows * kpad);
+  auto *e = ob.take<int32_t>(rows);
+  unsigned long long *mb = nullptr;
+  if (by_cols) {  // column maxima scratch comes from the handle's workspace
+    if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
+    Carver cv(h->ws, h->ws_bytes);
+    mb = cv.take<unsigned long long>(rows);
+    if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+    EMU_TRY(launch_colmax(h, elem, rows, k, X, ldx, mb));
+  }
+  h->launches = 0;
+  if (oz1) EMU_TRY(launch_oz1_slice(h, elem, by_cols, rows, k, kpad, X, ldx, mb, e, pn, h->slice_bits, planes));
+  else EMU_TRY(launch_oz2_residues(h, elem, by_cols, rows, k, kpad, X, ldx, mb, e, pn, t_bits, planes));
+  out->scheme = scheme; out->role = role; out->elem = elem; out->pn = pn;
+  out->slice_bits = oz1 ? h->slice_bits : 0; out->t_bits = t_bits;
+  out->rows = rows; out->k = k; out->kpad = kpad; out->buf = dev_buf; out->bytes = bytes;
+  return EMUGEMM_OK;
+}
+
+int emugemm_gemm_pre(emugemm_handle_t h, const emugemm_operand_t *A, const emugemm_operand_t *B, const double alpha[2],
+                     const double beta[2], void *C, int64_t ldc) {
+  if (!h || !A || !B || !alpha || !beta || !C) return EMUGEMM_ERR_ARG;
+  if (A->role != 0 || B->role != 1 || A->scheme != B->scheme || A->elem != B->elem || A->pn != B->pn || A->k != B->k ||
+      A->slice_bits != B->slice_bits || !A->buf || !B->buf || ldc < B->rows)
+    return EMUGEMM_ERR_ARG;
+  if (reinterpret_cast<uintptr_t>(C) & 15) return EMUGEMM_ERR_ALIGNMENT;
+  const int64_t m = A->rows, n = B->rows, kpad = A->kpad;
+  const int scheme = A->scheme, pn = A->pn, planes = operand_planes(scheme, pn);
+  const int8_t *PA = static_cast<const int8_t *>(A->buf), *PB = static_cast<const int8_t *>(B->buf);
+  const int32_t *eA = reinterpret_cast<const int32_t *>(PA + granule(static_cast<size_t>(planes) * m * kpad));
+  const int32_t *eB = reinterpret_cast<const int32_t *>(PB + granule(static_cast<size_t>(planes) * n * kpad));
+  if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
+  h->launches = 0;
+  Carver cv(h->ws, h->ws_bytes);
+  auto *diag = cv.take<unsigned long long>(1);
+  EMU_TRY(mark(h, 0));
+  EMU_TRY(mark(h, 1));
+  if (scheme == EMUGEMM_OZ1) {
+    int64_t clen;
+    const int nch = oz1_chunks(pn, A->slice_bits, kpad, 0, &clen);
+    double *part = nch > 1 ? cv.take<double>(static_cast<size_t>(nch) * m * n * 2) : nullptr;
+    if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+    h->diag = diag;
+    EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+    return oz1_gemm_phase(h, A->elem, m, n, kpad, pn, A->slice_bits, PA, PB, eA, eB, alpha[0], beta[0], C, ldc, nullptr, nch,
+                          clen, part, diag);
+  }
+  const int is3m = scheme == EMUGEMM_OZ2_3M;
+  auto *CR = cv.take<int8_t>(static_cast<size_t>(is3m ? 2 : 1) * pn * m * n);
+  if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+  h->diag = diag;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+  return oz2_gemm_phase(h, is3m, m, n, kpad, pn, PA, PB, CR, eA, eB, A->t_bits, B->t_bits, alpha, beta, static_cast<double *>(C),
+                        ldc, diag);
 }
 
 int emugemm_last_gemm_cycles(emugemm_handle_t h, unsigned long long *cycles) {
