@@ -696,6 +696,44 @@ int oracle_dgemm_oz2(int64_t m, int64_t n, int64_t k, double alpha, const double
 
 /* Whole Scheme II ZGEMM via 3M (R15, R16).  alpha, beta_ are
  * complex (re, im); A, B, C complex (re, im) pairs, strides in complex elements. */
+/* FP32 entry point of Scheme II ("EmuGEMM-II SGEMM (p8-p11)"): the same
+ * algorithm on 24-bit inputs widened exactly to double, one rounding to float from the __float128 value. */
+int oracle_sgemm_oz2(int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda, const float *B,
+                     int64_t ldb, float beta_, float *C, int64_t ldc, int N) {
+  if (N < 2 || N > ORACLE_MAX_MODULI || m < 0 || n < 0 || k < 1) return -1;
+  if (m == 0 || n == 0) return 0;
+  int32_t tA, tB;
+  if (oracle_oz2_budget(N, k, 0, &tA, &tB) < 2) return -2;
+  double *Ad = malloc(sizeof(double) * (size_t)m * k), *Bd = malloc(sizeof(double) * (size_t)k * n);
+  for (int64_t i = 0; i < m; ++i) for (int64_t h = 0; h < k; ++h) Ad[i * k + h] = A[i * lda + h];
+  for (int64_t h = 0; h < k; ++h) for (int64_t j = 0; j < n; ++j) Bd[h * n + j] = B[h * ldb + j];
+  int32_t *eA = malloc(sizeof(int32_t) * (size_t)m), *eB = malloc(sizeof(int32_t) * (size_t)n);
+  int8_t *RA = malloc((size_t)N * m * k), *RB = malloc((size_t)N * n * k), *CR = malloc((size_t)N * m * n);
+  oracle_row_exponents(m, k, Ad, k, eA);
+  oracle_col_exponents(k, n, Bd, n, eB);
+  oracle_oz2_residues_rows(m, k, Ad, k, eA, tA, N, RA);
+  oracle_oz2_residues_cols(k, n, Bd, n, eB, tB, N, RB);
+  (void)oracle_oz2_modprod(m, n, k, N, RA, RB, CR, NULL);
+  int32_t mod[ORACLE_MAX_MODULI];
+  oracle_oz2_moduli(N, mod);
+  u256 P = oz2_P(N, mod), w[ORACLE_MAX_MODULI];
+  oz2_weights(N, mod, &P, w);
+  for (int64_t i = 0; i < m; ++i)
+    for (int64_t j = 0; j < n; ++j) {
+      int c[ORACLE_MAX_MODULI];
+      for (int l = 0; l < N; ++l) c[l] = CR[((int64_t)l * m + i) * n + j];
+      u256 mag;
+      int sg = oz2_crt_one(N, mod, &P, w, c, &mag);
+      __float128 v = scalbnq(u256_to_q(&mag), eA[i] + eB[j] - tA - tB);
+      if (sg < 0) v = -v;
+      __float128 r = (__float128)alpha * v;
+      if (beta_ != 0.0f) r += (__float128)beta_ * (__float128)C[i * ldc + j];
+      C[i * ldc + j] = (float)r;
+    }
+  free(Ad); free(Bd); free(eA); free(eB); free(RA); free(RB); free(CR);
+  return 0;
+}
+
 int oracle_zgemm_oz2_3m(int64_t m, int64_t n, int64_t k, const double *alpha, const double *A, int64_t lda,
                         const double *B, int64_t ldb, const double *beta_, double *C, int64_t ldc, int N) {
   if (N < 2 || N > ORACLE_MAX_MODULI || m < 0 || n < 0 || k < 1) return -1;

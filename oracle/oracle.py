@@ -318,6 +318,21 @@ def dgemm_oz2(A, B, N, alpha=1.0, beta=0.0, Cin=None):
     return out
 
 
+def sgemm_oz2(A, B, N, alpha=1.0, beta=0.0, Cin=None):
+    """Scheme II on float32 inputs, float32 output (oracle_sgemm_oz2)."""
+    A = np.ascontiguousarray(A, np.float32)
+    B = np.ascontiguousarray(B, np.float32)
+    m, k = A.shape
+    _, n = B.shape
+    out = np.zeros((m, n), np.float32) if Cin is None else np.ascontiguousarray(Cin, np.float32).copy()
+    _lib.oracle_sgemm_oz2.restype = C.c_int
+    rc = _lib.oracle_sgemm_oz2(_i64(m), _i64(n), _i64(k), C.c_float(alpha), _ptr(A), _i64(k), _ptr(B), _i64(n),
+                               C.c_float(beta), _ptr(out), _i64(n), C.c_int(N))
+    if rc:
+        raise ValueError(f"oracle_sgemm_oz2 rc={rc}")
+    return out
+
+
 def zgemm_oz2_3m(A, B, N, alpha=1.0 + 0j, beta=0j, Cin=None):
     A, Af = _zview(A)
     B, Bf = _zview(B)

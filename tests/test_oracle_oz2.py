@@ -220,3 +220,37 @@ def test_sampled_equals_full_oz2():
     assert np.array_equal(O.oz2_sampled(A, B, 14, rows, cols), O.dgemm_oz2(A, B, 14)[np.ix_(rows, cols)])
     Az, Bz = G.complex_pair(8, 9, 30, 1.0, 6)
     assert np.array_equal(O.oz2_sampled(Az, Bz, 14, rows[:1], cols[:1], is3m=True), O.zgemm_oz2_3m(Az, Bz, 14)[np.ix_(rows[:1], cols[:1])])
+
+
+# ---- Scheme II on FP32 inputs ("EmuGEMM-II SGEMM (p8-p11)") ----
+def test_sgemm_oz2_is_correctly_rounded_when_the_budget_covers_the_inputs():
+    """k = 64, N = 10: tA = tB >= 24 + the spread of a narrow-range row, so the integer product is the exact
+    product of the float inputs and the result is the correctly rounded float of A.B (float64 matmul of
+    24-bit inputs with k = 64 is exact enough to round to the same float except at ties: compare via
+    __float128 brute force)."""
+    rng = np.random.default_rng(5)
+    A = (1.0 + rng.random((24, 64))).astype(np.float32)
+    B = (1.0 + rng.random((64, 16))).astype(np.float32)
+    T, tA, tB = O.oz2_budget(10, 64)
+    assert tA >= 25 and tB >= 25
+    C = O.sgemm_oz2(A, B, 10)
+    exact, _ = O.bf128_dgemm(A.astype(np.float64), B.astype(np.float64))
+    assert np.array_equal(C, exact.astype(np.float32))
+
+
+def test_sgemm_oz2_small_integers_and_alpha_beta():
+    rng = np.random.default_rng(7)
+    A = rng.integers(-63, 64, size=(20, 30)).astype(np.float32)
+    B = rng.integers(-63, 64, size=(30, 10)).astype(np.float32)
+    Cin = rng.integers(-5, 6, size=(20, 10)).astype(np.float32)
+    want = 2.0 * (A.astype(np.float64) @ B.astype(np.float64)) - 3.0 * Cin
+    assert np.array_equal(O.sgemm_oz2(A, B, 8, alpha=2.0, beta=-3.0, Cin=Cin), want.astype(np.float32))
+
+
+def test_sgemm_oz2_matches_dgemm_oz2_rounded_once():
+    """Same integers as the FP64 entry point on the widened inputs: the float result is within one float ulp of the
+    rounded double result (double rounding) and inside the method's bound against the exact product."""
+    A, B = G.real_pair(40, 30, 200, 1.0, 3, dtype=np.float32)
+    C32 = O.sgemm_oz2(A, B, 9)
+    C64 = O.dgemm_oz2(A.astype(np.float64), B.astype(np.float64), 9)
+    assert (np.abs(C32.astype(np.float64) - C64) <= np.spacing(np.abs(C64).astype(np.float32)).astype(np.float64)).all()
