@@ -93,6 +93,11 @@ int emugemm_dgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, doubl
                       const double *A, int64_t lda, const double *B, int64_t ldb, double beta,
                       double *C, int64_t ldc, int n_moduli);
 
+/* FP32 inputs and output ("EmuGEMM-II SGEMM (p8-p11)"): the same kernels on
+ * 24-bit inputs; 8-11 moduli cover FP32 accuracy at k = 8192.                  */
+int emugemm_sgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda,
+                      const float *B, int64_t ldb, float beta, float *C, int64_t ldc, int n_moduli);
+
 /* ---- Scheme II complex via 3M ------------------------ *
  * A, B, C hold complex128 as (re, im) pairs; alpha, beta point to HOST {re, im}. */
 int emugemm_zgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2],
@@ -116,6 +121,9 @@ int emugemm_sgemm_oz1_t(emugemm_handle_t h, int transa, int transb, int64_t m, i
 int emugemm_dgemm_oz2_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha,
                         const double *A, int64_t lda, const double *B, int64_t ldb, double beta, double *C,
                         int64_t ldc, int n_moduli);
+int emugemm_sgemm_oz2_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, float alpha,
+                        const float *A, int64_t lda, const float *B, int64_t ldb, float beta, float *C,
+                        int64_t ldc, int n_moduli);
 int emugemm_zgemm_oz2_3m_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k,
                            const double alpha[2], const double *A, int64_t lda, const double *B, int64_t ldb,
                            const double beta[2], double *C, int64_t ldc, int n_moduli);
@@ -127,7 +135,7 @@ int emugemm_zgemm_oz2_3m_t(emugemm_handle_t h, int transa, int transb, int64_t m
  * runs only the fused GEMM and the reconstruction.  Results are bit-identical to the
  * one-shot calls.  The struct is plain data owned by the caller; the buffer must
  * outlive its uses, be 1024-byte aligned and hold emugemm_operand_bytes() bytes.
- *   scheme : EMUGEMM_OZ1 (elem 4 / 8), EMUGEMM_OZ2 (elem 8), EMUGEMM_OZ2_3M (elem 16)
+ *   scheme : EMUGEMM_OZ1 (elem 4 / 8), EMUGEMM_OZ2 (elem 4 / 8), EMUGEMM_OZ2_3M (elem 16)
  *   role   : 0 = left operand op(A) (rows x k), 1 = right operand op(B) (k x rows)
  *   trans  : as in the _t calls (role 0: X stored k x rows; role 1: X stored rows x k)
  * Scheme II scales an operand with a bit budget that depends on k, n_moduli and the

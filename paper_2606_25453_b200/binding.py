@@ -176,6 +176,14 @@ class EmuGemm:
                                                    _i64(self._ld(C_)), _int(n_moduli)))
         return C_
 
+    def sgemm_oz2(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0, transa=False, transb=False):
+        m, n, k = self._dims(A, B, transa, transb)
+        self._reserve_for(OZ2, 8, m, n, k, n_moduli)
+        self._check(self._lib.emugemm_sgemm_oz2_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), _flt(alpha),
+                                                   _ptr(A), _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), _flt(beta), _ptr(C_),
+                                                   _i64(self._ld(C_)), _int(n_moduli)))
+        return C_
+
     def zgemm_oz2_3m(self, A, B, C_, n_moduli, alpha=1.0 + 0j, beta=0j, transa=False, transb=False):
         """A, B, C_: complex128 CUDA tensors."""
         m, n, k = self._dims(A, B, transa, transb)
@@ -209,7 +217,7 @@ class EmuGemm:
         return op
 
     def gemm_pre(self, opA, opB, C_, alpha=1.0, beta=0.0):
-        scheme_elem = {(OZ1, 4): 4, (OZ1, 8): 8, (OZ2, 8): 8, (OZ2_3M, 16): 16}[(opA.scheme, opA.elem)]
+        scheme_elem = {(OZ1, 4): 4, (OZ1, 8): 8, (OZ2, 4): 8, (OZ2, 8): 8, (OZ2_3M, 16): 16}[(opA.scheme, opA.elem)]
         self._reserve_for(opA.scheme, scheme_elem, opA.rows, opB.rows, opA.k, opA.pn)
         al = (_dbl * 2)(complex(alpha).real, complex(alpha).imag)
         be = (_dbl * 2)(complex(beta).real, complex(beta).imag)

@@ -178,13 +178,14 @@ static int run_oz1(emugemm_ctx *h, int ta, int tb, int elem, int64_t m, int64_t 
 // Per-modulus GEMMs with fused reduction + CRT from residue planes (one-shot calls and pre-decomposed operands).
 static int oz2_gemm_phase(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_t kpad, int N, const int8_t *RA,
                           const int8_t *RB, int8_t *CR, const int32_t *eA, const int32_t *eB, int tA, int tB,
-                          const double alpha[2], const double beta[2], double *C, int64_t ldc, unsigned long long *diag) {
+                          const double alpha[2], const double beta[2], double *C, int64_t ldc, unsigned long long *diag,
+                          int out_f32 = 0) {
   Oz2GemmArgs g;
   g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = N; g.is3m = is3m; g.RA = RA; g.RB = RB; g.CR = CR; g.cycles = diag;
   EMU_TRY(launch_oz2_gemm(h, g));
   EMU_TRY(mark(h, 2));
   Oz2CrtArgs c;
-  c.m = m; c.n = n; c.n_moduli = N; c.CR = CR; c.eA = eA; c.eB = eB; c.tA = tA; c.tB = tB; c.is_complex = is3m;
+  c.m = m; c.n = n; c.n_moduli = N; c.CR = CR; c.eA = eA; c.eB = eB; c.tA = tA; c.tB = tB; c.is_complex = is3m; c.out_f32 = out_f32;
   c.alpha[0] = alpha[0]; c.alpha[1] = alpha[1]; c.beta[0] = beta[0]; c.beta[1] = beta[1];
   c.C = C; c.ldc = ldc;
   EMU_TRY(launch_oz2_crt(h, c));
@@ -194,12 +195,12 @@ static int oz2_gemm_phase(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_
 
 // Scheme II call sequence (real and 3M)
 static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t n, int64_t k, const double alpha[2], const void *A,
-                   int64_t lda, const void *B, int64_t ldb, const double beta[2], double *C, int64_t ldc, int N) {
+                   int64_t lda, const void *B, int64_t ldb, const double beta[2], double *C, int64_t ldc, int N, int f32 = 0) {
   EMU_TRY(check_gemm_args(h, ta, tb, m, n, k, A, lda, B, ldb, C, ldc));
   if (N < 2 || N > kMaxModuli) return EMUGEMM_ERR_ARG;
   h->launches = 0;
   if (m == 0 || n == 0) return EMUGEMM_OK;
-  const int elem = is3m ? kZ128 : kF64;
+  const int elem = is3m ? kZ128 : (f32 ? kF32 : kF64);
   EMU_TRY(mark(h, 0));
   if (k == 0) {
     EMU_TRY(scale_c(h, m, n, beta[0], beta[1], C, ldc, elem));
@@ -230,7 +231,7 @@ static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t 
   EMU_TRY(launch_oz2_residues(h, elem, ta, m, k, kpad, A, lda, mbA, eA, N, tA, RA));
   EMU_TRY(launch_oz2_residues(h, elem, !tb, n, k, kpad, B, ldb, mbB, eB, N, tB, RB));
   EMU_TRY(mark(h, 1));
-  return oz2_gemm_phase(h, is3m, m, n, kpad, N, RA, RB, CR, eA, eB, tA, tB, alpha, beta, C, ldc, diag);
+  return oz2_gemm_phase(h, is3m, m, n, kpad, N, RA, RB, CR, eA, eB, tA, tB, alpha, beta, C, ldc, diag, f32);
 }
 
 }  // namespace emu
@@ -340,6 +341,16 @@ int emugemm_dgemm_oz2_t(emugemm_handle_t h, int transa, int transb, int64_t m, i
   const double al[2] = {alpha, 0.0}, be[2] = {beta, 0.0};
   return run_oz2(h, transa, transb, 0, m, n, k, al, A, lda, B, ldb, be, C, ldc, n_moduli);
 }
+int emugemm_sgemm_oz2_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, float alpha,
+                        const float *A, int64_t lda, const float *B, int64_t ldb, float beta, float *C, int64_t ldc,
+                        int n_moduli) {
+  const double al[2] = {alpha, 0.0}, be[2] = {beta, 0.0};
+  return run_oz2(h, transa, transb, 0, m, n, k, al, A, lda, B, ldb, be, reinterpret_cast<double *>(C), ldc, n_moduli, 1);
+}
+int emugemm_sgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda,
+                      const float *B, int64_t ldb, float beta, float *C, int64_t ldc, int n_moduli) {
+  return emugemm_sgemm_oz2_t(h, 0, 0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, n_moduli);
+}
 int emugemm_zgemm_oz2_3m_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, const double alpha[2],
                            const double *A, int64_t lda, const double *B, int64_t ldb, const double beta[2], double *C,
                            int64_t ldc, int n_moduli) {
@@ -384,7 +395,7 @@ int emugemm_decompose(emugemm_handle_t h, int scheme, int role, int trans, int e
   const bool oz1 = scheme == EMUGEMM_OZ1, oz2 = scheme == EMUGEMM_OZ2, z3m = scheme == EMUGEMM_OZ2_3M;
   if (!(oz1 || oz2 || z3m)) return EMUGEMM_ERR_ARG;
   if (oz1 ? !((elem == kF64 && pn >= 1 && pn <= 8) || (elem == kF32 && pn >= 1 && pn <= 4))
-          : !(elem == (z3m ? kZ128 : kF64) && pn >= 2 && pn <= kMaxModuli))
+          : !((z3m ? elem == kZ128 : (elem == kF64 || elem == kF32)) && pn >= 2 && pn <= kMaxModuli))
     return EMUGEMM_ERR_ARG;
   const int by_cols = role == 0 ? trans : !trans;  // is k the strided dimension of the stored operand?
   if (ldx < (by_cols ? rows : k)) return EMUGEMM_ERR_ARG;
@@ -451,7 +462,7 @@ int emugemm_gemm_pre(emugemm_handle_t h, const emugemm_operand_t *A, const emuge
   h->diag = diag;
   EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
   return oz2_gemm_phase(h, is3m, m, n, kpad, pn, PA, PB, CR, eA, eB, A->t_bits, B->t_bits, alpha, beta, static_cast<double *>(C),
-                        ldc, diag);
+                        ldc, diag, A->elem == kF32);
 }
 
 int emugemm_last_gemm_cycles(emugemm_handle_t h, unsigned long long *cycles) {

@@ -118,6 +118,7 @@ struct Oz2CrtArgs {
   const int32_t *eA, *eB;
   int tA, tB;
   int is_complex;              // 0: real alpha/beta; 1: complex, C is (re, im) pairs
+  int out_f32;                 // real only: C is float (Scheme II SGEMM)
   double alpha[2], beta[2];
   double *C;
   int64_t ldc;

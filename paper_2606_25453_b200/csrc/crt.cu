@@ -144,7 +144,8 @@ __device__ __forceinline__ double crt_finish(const CrtConst &k, double shi, doub
 }
 
 // one thread per 8 consecutive columns of one row
-template <bool VEC, bool CPLX>
+// KIND: 0 = FP64 C, 1 = complex128 C, 2 = FP32 C (Scheme II SGEMM: one more rounding, double -> float)
+template <bool VEC, int KIND>
 __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const int8_t *__restrict__ CR,
                                                   const int32_t *__restrict__ eA, const int32_t *__restrict__ eB,
                                                   int tsum, double ar, double ai, double br, double bi,
@@ -166,7 +167,24 @@ __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const in
   crt_accumulate<VEC>(k, CR + i * n + j0, plane, j0, n, shi, slo);
 #pragma unroll
   for (int e = 0; e < kCrtVec; ++e) vr[e] = crt_finish(k, shi[e], slo[e]) * sc1[e] * sc2[e];
-  if (!CPLX) {
+  if (KIND == 2) {
+    float *o = reinterpret_cast<float *>(C) + i * ldc + j0;
+    float f[kCrtVec];
+#pragma unroll
+    for (int e = 0; e < kCrtVec; ++e) {
+      double x = ar * vr[e];
+      if (br != 0.0 && j0 + e < n) x = fma(br, static_cast<double>(o[e]), x);
+      f[e] = static_cast<float>(x);
+    }
+    if (VEC && (ldc % 4 == 0) && ((reinterpret_cast<uintptr_t>(C) & 15) == 0)) {
+      reinterpret_cast<float4 *>(o)[0] = make_float4(f[0], f[1], f[2], f[3]);
+      reinterpret_cast<float4 *>(o)[1] = make_float4(f[4], f[5], f[6], f[7]);
+    } else {
+#pragma unroll
+      for (int e = 0; e < kCrtVec; ++e)
+        if (j0 + e < n) o[e] = f[e];
+    }
+  } else if (KIND == 0) {
     double *o = C + i * ldc + j0;
     if (br != 0.0) {
 #pragma unroll
@@ -218,10 +236,13 @@ int launch_oz2_crt(emugemm_ctx *ctx, const Oz2CrtArgs &a) {
 #define EMU_CRT_LAUNCH(V, Z)                                                                                              \
   crt_kernel<V, Z><<<grid, 256, 0, ctx->stream>>>(a.m, a.n, a.CR, a.eA, a.eB, tsum, a.alpha[0], a.alpha[1], a.beta[0], \
                                                    a.beta[1], a.C, a.ldc, k)
-  if (vec && a.is_complex) EMU_CRT_LAUNCH(true, true);
-  else if (vec) EMU_CRT_LAUNCH(true, false);
-  else if (a.is_complex) EMU_CRT_LAUNCH(false, true);
-  else EMU_CRT_LAUNCH(false, false);
+  const int kind = a.is_complex ? 1 : (a.out_f32 ? 2 : 0);
+  if (vec && kind == 1) EMU_CRT_LAUNCH(true, 1);
+  else if (vec && kind == 2) EMU_CRT_LAUNCH(true, 2);
+  else if (vec) EMU_CRT_LAUNCH(true, 0);
+  else if (kind == 1) EMU_CRT_LAUNCH(false, 1);
+  else if (kind == 2) EMU_CRT_LAUNCH(false, 2);
+  else EMU_CRT_LAUNCH(false, 0);
 #undef EMU_CRT_LAUNCH
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());

@@ -514,6 +514,9 @@ int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, i
   if (elem == kF64)
     return two ? launch_planes<double, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out)
                : launch_planes<double, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out);
+  if (elem == kF32)  // 24-bit inputs (Scheme II SGEMM)
+    return two ? launch_planes<float, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out)
+               : launch_planes<float, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out);
   if (elem == kZ128)
     return two ? launch_planes<double, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out)
                : launch_planes<double, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out);

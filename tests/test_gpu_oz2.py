@@ -147,3 +147,30 @@ def test_zgemm_alpha_beta(env):
     got = C.cpu().numpy()
     assert_within_ulps(got.real, want.real, scale, 2)
     assert_within_ulps(got.imag, want.imag, scale, 2)
+
+
+# ---- Scheme II on FP32 inputs (emugemm_sgemm_oz2) ----
+@pytest.mark.parametrize("N,shape", [(8, (256, 256, 256)), (11, (200, 300, 333)), (9, (129, 513, 140))])
+def test_sgemm_oz2(env, N, shape):
+    torch, O, h, E = env
+    m, n, k = shape
+    A, B = G.real_pair(m, n, k, 1.0, 4, dtype=np.float32)
+    C = torch.full((m, n), float("nan"), dtype=torch.float32, device="cuda")
+    h.sgemm_oz2(dev(torch, A), dev(torch, B), C, N)
+    _, absAB = O.bf128_dgemm(A.astype(np.float64), B.astype(np.float64))
+    assert_within_ulps(C.cpu().numpy(), O.sgemm_oz2(A, B, N), absAB, 2, bits=23, what=f"sgemm_oz2 N={N}")
+
+
+def test_sgemm_oz2_residues_alpha_beta_transposed(env):
+    torch, O, h, E = env
+    m, n, k, N = 140, 90, 260, 10
+    A, B, Cin = G.real_pair(m, n, k, 1.0, 6, dtype=np.float32, with_c=True)
+    _, tA, tB = O.oz2_budget(N, k)
+    RA, _ = h.dbg_oz2_residues(dev(torch, A), False, N, tA)
+    A64 = A.astype(np.float64)
+    assert np.array_equal(RA.cpu().numpy(), O.oz2_residues_rows(A64, O.row_exponents(A64), tA, N))
+    C = dev(torch, Cin)
+    h.sgemm_oz2(dev(torch, A.T), dev(torch, B), C, N, alpha=2.5, beta=-0.5, transa=True)
+    _, absAB = O.bf128_dgemm(A64, B.astype(np.float64))
+    assert_within_ulps(C.cpu().numpy(), O.sgemm_oz2(A, B, N, alpha=2.5, beta=-0.5, Cin=Cin), 2.5 * absAB + 0.5 * np.abs(Cin), 2,
+                       bits=23, what="sgemm_oz2 alpha/beta")
