@@ -164,6 +164,27 @@ def oz1_sampled(A, B, p, rows, cols, alpha=1.0, is_f32=False):
     return out
 
 
+def zgemm_oz1_4m(A, B, p, alpha=1.0 + 0j, beta=0j, Cin=None):
+    """Scheme I complex GEMM by the 4M formulation ("EmuGEMM-I uses the 4M formulation"; SURVEY 8(f)
+    item 3): the four real products are ONE real Scheme I GEMM on the real embedding
+        A' = [[Re A, -Im A], [Im A, Re A]]  (2m x 2k),   B' = [[Re B], [Im B]]  (2k x n),
+    whose rows i and m + i give Re and Im of A B.  Rows i and m + i of A' hold the same magnitudes, so they share
+    their exponent (the max over Re and Im of row i of A, as R16 does for 3M); column j of B' covers Re and Im of
+    column j of B.  T = dgemm_oz1(A', B', p) (one rounding per component), then C = alpha (T_re + i T_im) + beta C_in
+    in complex double arithmetic."""
+    A = np.ascontiguousarray(A, np.complex128)
+    B = np.ascontiguousarray(B, np.complex128)
+    m = A.shape[0]
+    Ae = np.block([[A.real, -A.imag], [A.imag, A.real]])
+    Be = np.vstack([B.real, B.imag])
+    T = dgemm_oz1(np.ascontiguousarray(Ae), np.ascontiguousarray(Be), p)
+    Tc = T[:m] + 1j * T[m:]
+    out = complex(alpha) * Tc
+    if complex(beta) != 0:
+        out = out + complex(beta) * np.ascontiguousarray(Cin, np.complex128)
+    return out
+
+
 # ---------------------------------------------------------------- brute force
 def bf128_dgemm(A, B):
     """(C, absAB): __float128 product of the original operands and (|A||B|)_ij."""

@@ -1,0 +1,40 @@
+"""Pins for the Scheme I 4M complex oracle (-m "not gpu"): the embedding
+identity against numpy's complex product on small integers (exact), and the __float128 complex brute force
+inside the Scheme I truncation bound of the embedded real problem."""
+import numpy as np
+
+import emugemm_inputs as G
+from oracle import oracle as O
+from test_oracle_oz1 import oz1_error_bound
+
+
+def test_small_gaussian_integers_exact():
+    rng = np.random.default_rng(3)
+    A = rng.integers(-31, 32, size=(12, 20)) + 1j * rng.integers(-31, 32, size=(12, 20))
+    B = rng.integers(-31, 32, size=(20, 9)) + 1j * rng.integers(-31, 32, size=(20, 9))
+    Cin = rng.integers(-5, 6, size=(12, 9)) + 1j * rng.integers(-5, 6, size=(12, 9))
+    for p in (3, 8):
+        assert np.array_equal(O.zgemm_oz1_4m(A, B, p), A @ B)
+    assert np.array_equal(O.zgemm_oz1_4m(A, B, 4, alpha=2 - 1j, beta=1j, Cin=Cin), (2 - 1j) * (A @ B) + 1j * Cin)
+
+
+def test_vs_float128_complex_bruteforce_within_bound():
+    m, n, k, p = 48, 40, 96, 6
+    A, B = G.complex_pair(m, n, k, 0.5, 3)
+    C = O.zgemm_oz1_4m(A, B, p)
+    exact, _ = O.bf128_zgemm(A, B)
+    Ae = np.block([[A.real, -A.imag], [A.imag, A.real]])
+    Be = np.vstack([B.real, B.imag])
+    bound = oz1_error_bound(Ae, Be, p)  # bound of the embedded real Scheme I problem, rows i / m + i = Re / Im
+    assert (np.abs(C.real - exact.real) < bound[:m] + np.spacing(np.abs(exact.real))).all()
+    assert (np.abs(C.imag - exact.imag) < bound[m:] + np.spacing(np.abs(exact.imag))).all()
+    # one slice fewer is visibly worse: the bound is not vacuous
+    C5 = O.zgemm_oz1_4m(A, B, p - 1)
+    assert np.median(np.abs(C5 - exact)) > 20 * np.median(np.abs(C - exact))
+
+
+def test_rows_of_the_embedding_share_exponents():
+    A, _ = G.complex_pair(9, 4, 33, 2.0, 11)
+    Ae = np.block([[A.real, -A.imag], [A.imag, A.real]])
+    e = O.row_exponents(np.ascontiguousarray(Ae))
+    assert np.array_equal(e[:9], e[9:]) and np.array_equal(e[:9], O.row_exponents_z(A))
