@@ -50,7 +50,7 @@ enum emugemm_status {
   EMUGEMM_ERR_CUDA = -6       /* a CUDA call failed; see emugemm_last_cuda_error() */
 };
 
-enum emugemm_scheme { EMUGEMM_OZ1 = 1, EMUGEMM_OZ2 = 2, EMUGEMM_OZ2_3M = 3 };
+enum emugemm_scheme { EMUGEMM_OZ1 = 1, EMUGEMM_OZ2 = 2, EMUGEMM_OZ2_3M = 3, EMUGEMM_OZ1_4M = 4 };
 
 /* ---- handle ------------------------------------------------------------- */
 int emugemm_create(emugemm_handle_t *h);  /* host-only state; checks the device */
@@ -83,6 +83,14 @@ int emugemm_dgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, doubl
 int emugemm_sgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, float alpha,
                       const float *A, int64_t lda, const float *B, int64_t ldb, float beta,
                       float *C, int64_t ldc, int p);
+
+/* Scheme I complex GEMM by the 4M formulation ("EmuGEMM-I uses the 4M formulation"; SURVEY 8(f)
+ * item 3).  A, B, C hold complex128 as (re, im) pairs, strides in complex elements; alpha, beta point to HOST
+ * {re, im}.  The four real products run as ONE fused Scheme I GEMM of size 2m x n x 2k on the real embedding
+ * A' = [[Re A, -Im A], [Im A, Re A]], B' = [[Re B], [Im B]] (rows i and m + i share the exponent of row i of A).
+ * Workspace: emugemm_workspace_bytes(EMUGEMM_OZ1_4M, 16, m, n, k, p).  1 <= p <= 8.                            */
+int emugemm_zgemm_oz1_4m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2], const double *A,
+                         int64_t lda, const double *B, int64_t ldb, const double beta[2], double *C, int64_t ldc, int p);
 
 /* ---- Scheme II ---------------------------------------- *
  * n_moduli pairwise-coprime moduli <= 256 (256, 255, 253, 251, 247, ... greedy

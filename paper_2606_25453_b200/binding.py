@@ -10,7 +10,7 @@ import re
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libemugemm.so")
 _HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "emugemm.h")
 
-OZ1, OZ2, OZ2_3M = 1, 2, 3
+OZ1, OZ2, OZ2_3M, OZ1_4M = 1, 2, 3, 4
 _i64, _int, _dbl, _flt, _vp, _sz = C.c_int64, C.c_int, C.c_double, C.c_float, C.c_void_p, C.c_size_t
 
 
@@ -174,6 +174,17 @@ class EmuGemm:
         self._check(self._lib.emugemm_dgemm_oz2_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), _dbl(alpha),
                                                    _ptr(A), _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), _dbl(beta), _ptr(C_),
                                                    _i64(self._ld(C_)), _int(n_moduli)))
+        return C_
+
+    def zgemm_oz1_4m(self, A, B, C_, p, alpha=1.0 + 0j, beta=0j):
+        """A, B, C_: complex128 CUDA tensors (Scheme I, 4M)."""
+        m, k = A.shape
+        n = B.shape[1]
+        self._reserve_for(OZ1_4M, 16, m, n, k, p)
+        al = (_dbl * 2)(complex(alpha).real, complex(alpha).imag)
+        be = (_dbl * 2)(complex(beta).real, complex(beta).imag)
+        self._check(self._lib.emugemm_zgemm_oz1_4m(self._h, _i64(m), _i64(n), _i64(k), al, _ptr(A), _i64(self._ld(A)), _ptr(B),
+                                                    _i64(self._ld(B)), be, _ptr(C_), _i64(self._ld(C_)), _int(p)))
         return C_
 
     def sgemm_oz2(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0, transa=False, transb=False):

@@ -81,6 +81,24 @@ __global__ void scale_c_kernel(int64_t m, int64_t n, double br, double bi, void 
   }
 }
 
+// C = alpha (T[i][j] + i T[m + i][j]) + beta C: the complex combination of the 4M real embedding result T (2m x n)
+__global__ void zcombine_4m_kernel(int64_t m, int64_t n, const double *__restrict__ T, double ar, double ai, double br, double bi,
+                                   double *__restrict__ C, int64_t ldc) {
+  const int64_t idx = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
+  if (idx >= m * n) return;
+  const int64_t i = idx / n, j = idx - i * n;
+  const double tr = T[idx], ti = T[idx + m * n];
+  double re = ar * tr - ai * ti, im = ar * ti + ai * tr;
+  double *o = C + 2 * (i * ldc + j);
+  if (br != 0.0 || bi != 0.0) {
+    const double cr = o[0], ci = o[1];
+    re += br * cr - bi * ci;
+    im += br * ci + bi * cr;
+  }
+  o[0] = re;
+  o[1] = im;
+}
+
 static int scale_c(emugemm_ctx *h, int64_t m, int64_t n, double br, double bi, void *C, int64_t ldc, int elem) {
   scale_c_kernel<<<static_cast<unsigned>((m * n + 255) / 256), 256, 0, h->stream>>>(m, n, br, bi, C, ldc, elem);
   h->launches++;
@@ -302,6 +320,14 @@ size_t emugemm_workspace_bytes(int scheme, int elem, int64_t m, int64_t n, int64
     int64_t clen;
     const int nch = oz1_chunks(pn, 8, kpad, 0, &clen);  // the 8-bit mode has the shorter chunks: size for it
     if (nch > 1) total += granule(static_cast<size_t>(nch) * m * n * 16);
+  } else if (scheme == EMUGEMM_OZ1_4M) {
+    if (pn > 8 || elem != 16) return 0;
+    const int64_t kk = 2 * kpad, mm = 2 * m;
+    total += granule(4 * mm) + granule(static_cast<size_t>(pn) * mm * kk) + granule(static_cast<size_t>(pn) * n * kk) +
+             granule(static_cast<size_t>(mm) * n * 8);
+    int64_t clen;
+    const int nch = oz1_chunks(pn, 8, kk, 0, &clen);
+    if (nch > 1) total += granule(static_cast<size_t>(nch) * mm * n * 16);
   } else if (scheme == EMUGEMM_OZ2 || scheme == EMUGEMM_OZ2_3M) {
     if (pn > kMaxModuli) return 0;
     const size_t pi = scheme == EMUGEMM_OZ2_3M ? 3 : 1, po = scheme == EMUGEMM_OZ2_3M ? 2 : 1;
@@ -326,6 +352,51 @@ const char *emugemm_status_string(int s) {
 }
 
 int emugemm_last_cuda_error(emugemm_handle_t h) { return h ? h->last_cuda : 0; }
+
+// Scheme I ZGEMM by 4M: one real Scheme I GEMM of size 2m x n x 2k on the real embedding
+// A' = [[Re A, -Im A], [Im A, Re A]], B' = [[Re B], [Im B]], then the complex alpha / beta combination.
+int emugemm_zgemm_oz1_4m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2], const double *A, int64_t lda,
+                         const double *B, int64_t ldb, const double beta[2], double *C, int64_t ldc, int p) {
+  if (!alpha || !beta) return EMUGEMM_ERR_ARG;
+  EMU_TRY(check_gemm_args(h, 0, 0, m, n, k, A, lda, B, ldb, C, ldc));
+  if (p < 1 || p > 8) return EMUGEMM_ERR_ARG;
+  h->launches = 0;
+  if (m == 0 || n == 0) return EMUGEMM_OK;
+  EMU_TRY(mark(h, 0));
+  if (k == 0) {
+    EMU_TRY(scale_c(h, m, n, beta[0], beta[1], C, ldc, kZ128));
+    EMU_TRY(mark(h, 1)); EMU_TRY(mark(h, 2)); EMU_TRY(mark(h, 3));
+    return EMUGEMM_OK;
+  }
+  const int64_t kpad = round_up(k, kBlockK), kk = 2 * kpad, mm = 2 * m;
+  const int bits = h->slice_bits;
+  int64_t clen;
+  const int nch = oz1_chunks(p, bits, kk, 0, &clen);
+  if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
+  Carver cv(h->ws, h->ws_bytes);
+  auto *diag = cv.take<unsigned long long>(1);
+  auto *mbB = cv.take<unsigned long long>(n);
+  auto *eA = cv.take<int32_t>(mm);
+  auto *eB = cv.take<int32_t>(n);
+  auto *SA = cv.take<int8_t>(static_cast<size_t>(p) * mm * kk);
+  auto *SB = cv.take<int8_t>(static_cast<size_t>(p) * n * kk);
+  auto *T = cv.take<double>(static_cast<size_t>(mm) * n);
+  double *part = nch > 1 ? cv.take<double>(static_cast<size_t>(nch) * mm * n * 2) : nullptr;
+  if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+  h->diag = diag;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+  EMU_TRY(launch_colmax(h, kZ128, n, k, B, ldb, mbB));
+  EMU_TRY(launch_oz1_4m_slice(h, 0, m, k, kpad, A, lda, nullptr, eA, p, bits, SA));
+  EMU_TRY(launch_oz1_4m_slice(h, 1, n, k, kpad, B, ldb, mbB, eB, p, bits, SB));
+  EMU_TRY(mark(h, 1));
+  EMU_TRY(oz1_gemm_phase(h, kF64, mm, n, kk, p, bits, SA, SB, eA, eB, 1.0, 0.0, T, n, nullptr, nch, clen, part, diag));
+  zcombine_4m_kernel<<<static_cast<unsigned>((m * n + 255) / 256), 256, 0, h->stream>>>(m, n, T, alpha[0], alpha[1], beta[0],
+                                                                                      beta[1], C, ldc);
+  h->launches++;
+  EMU_CUDA(h, cudaGetLastError());
+  EMU_TRY(mark(h, 3));
+  return EMUGEMM_OK;
+}
 
 int emugemm_dgemm_oz1_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha,
                         const double *A, int64_t lda, const double *B, int64_t ldb, double beta, double *C, int64_t ldc, int p) {

@@ -83,6 +83,10 @@ int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, i
                         const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int n_moduli,
                         int t_bits, int8_t *out);
 
+// Scheme I complex by 4M: digit planes of the real embedding (prepass.cu) and the final complex combination.
+int launch_oz1_4m_slice(emugemm_ctx *ctx, int is_b, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
+                        const unsigned long long *maxbits, int32_t *e, int p, int slice_bits, int8_t *out);
+
 struct Oz1GemmArgs {
   int64_t m, n, kpad;          // kpad: padded k of the slice planes (multiple of kBlockK)
   int64_t k0, k1;              // k-chunk [k0, k1) handled by this launch (multiples of kBlockK)

@@ -523,6 +523,148 @@ int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, i
   return EMUGEMM_ERR_ARG;
 }
 
+// ---- Scheme I complex (4M): digit planes of the REAL EMBEDDING ------------
+//   A' = [[Re A, -Im A], [Im A, Re A]] (2m x 2k),  B' = [[Re B], [Im B]] (2k x n)
+// written directly from the complex operands: every digit word of Re A / Im A is stored twice (rows i and m + i),
+// the negated imaginary part is digitised from the sign-flipped value (exact in both digit formats).
+// Embedded k index: [0, kpad) = first half, [kpad, 2 kpad) = second half (each half zero-padded to kpad).
+template <int PARAM, typename Sink>
+__device__ __forceinline__ void emit_oz1_any(const Prep (&q)[4], Sink sink) {
+  if constexpr (PARAM >= 16) emit_oz1_b8<PARAM - 16>(q, sink);
+  else emit_oz1<PARAM>(q, sink);
+}
+
+template <int PARAM>
+__global__ void __launch_bounds__(256) oz1_4m_rows_kernel(const double *__restrict__ X, int64_t ldx, int64_t m, int64_t k,
+                                                          int64_t kpad, int32_t *__restrict__ e_out, int scale_bits,
+                                                          int8_t *__restrict__ out) {
+  const int64_t row = blockIdx.x;
+  const double *src = X + row * ldx * 2;
+  unsigned long long mx = 0;
+  for (int64_t h = static_cast<int64_t>(threadIdx.x) * 4; h < 2 * k; h += 1024)
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+      if (h + i < 2 * k) {
+        const unsigned long long b = abs_bits(src[h + i]);
+        mx = b > mx ? b : mx;
+      }
+  for (int o = 16; o > 0; o >>= 1) {
+    const unsigned long long y = __shfl_xor_sync(0xffffffffu, mx, o);
+    mx = y > mx ? y : mx;
+  }
+  __shared__ unsigned long long red[8];
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
+  __syncthreads();
+#pragma unroll
+  for (int w = 0; w < 8; ++w) mx = red[w] > mx ? red[w] : mx;
+  const int e_row = exponent_of_maxbits<double>(mx);
+  if (threadIdx.x == 0) { e_out[row] = e_row; e_out[m + row] = e_row; }
+
+  const int64_t kk = 2 * kpad, plane_stride = 2 * m * kk;
+  for (int64_t h0 = static_cast<int64_t>(threadIdx.x) * 4; h0 < kpad; h0 += 1024) {
+    Prep re[4], im[4], nim[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const bool in = h0 + i < k;
+      re[i] = prepare<double, 2>(in ? src[(h0 + i) * 2] : 0.0, e_row, scale_bits);
+      im[i] = prepare<double, 2>(in ? src[(h0 + i) * 2 + 1] : 0.0, e_row, scale_bits);
+      nim[i] = im[i];
+      nim[i].neg = !im[i].neg;
+    }
+    int8_t *top = out + row * kk + h0, *bot = out + (m + row) * kk + h0;
+    emit_oz1_any<PARAM>(re, [&](int t, unsigned int w) {
+      *reinterpret_cast<unsigned int *>(top + t * plane_stride) = w;
+      *reinterpret_cast<unsigned int *>(bot + t * plane_stride + kpad) = w;
+    });
+    emit_oz1_any<PARAM>(im, [&](int t, unsigned int w) { *reinterpret_cast<unsigned int *>(bot + t * plane_stride) = w; });
+    emit_oz1_any<PARAM>(nim, [&](int t, unsigned int w) { *reinterpret_cast<unsigned int *>(top + t * plane_stride + kpad) = w; });
+  }
+}
+
+// B (k x n complex, ldx in complex elements): planes out[t][j][2 kpad] = [digits of Re B(:, j) | digits of Im B(:, j)];
+// tile = 32 columns x 128 k, transposed through shared memory ("virtual plane" P + t = imaginary half).
+template <int PARAM>
+__global__ void __launch_bounds__(256) oz1_4m_cols_kernel(const double *__restrict__ X, int64_t ldx, int64_t n, int64_t k,
+                                                          int64_t kpad, const unsigned long long *__restrict__ maxbits,
+                                                          int32_t *__restrict__ e_out, int scale_bits, int P,
+                                                          int8_t *__restrict__ out) {
+  extern __shared__ unsigned int tile[];  // [2 P][32][33]
+  constexpr int TH = 128, PW = TH / 4 + 1;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const int64_t j = static_cast<int64_t>(blockIdx.x) * 32 + lane;
+  const int64_t hb = static_cast<int64_t>(blockIdx.y) * TH;
+  const int e_row = (j < n) ? exponent_of_maxbits<double>(maxbits[j]) : 0;
+  if (blockIdx.y == 0 && warp == 0 && j < n) e_out[j] = e_row;
+  for (int hw = warp; hw < TH / 4; hw += 8) {
+    const int64_t h0 = hb + hw * 4;
+    Prep re[4], im[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      const bool in = j < n && h0 + i < k;
+      re[i] = prepare<double, 2>(in ? X[((h0 + i) * ldx + j) * 2] : 0.0, e_row, scale_bits);
+      im[i] = prepare<double, 2>(in ? X[((h0 + i) * ldx + j) * 2 + 1] : 0.0, e_row, scale_bits);
+    }
+    emit_oz1_any<PARAM>(re, [&](int t, unsigned int w) { tile[(t * 32 + lane) * PW + hw] = w; });
+    emit_oz1_any<PARAM>(im, [&](int t, unsigned int w) { tile[((P + t) * 32 + lane) * PW + hw] = w; });
+  }
+  __syncthreads();
+  const int64_t kk = 2 * kpad;
+  for (int r = warp; r < 2 * P * 32; r += 8) {  // one warp writes one 128-byte row segment
+    const int vp = r >> 5, jj = r & 31;
+    const int64_t jg = static_cast<int64_t>(blockIdx.x) * 32 + jj;
+    if (jg < n) {
+      const int t = vp % P, halfsel = vp / P;
+      *reinterpret_cast<unsigned int *>(out + (static_cast<int64_t>(t) * n + jg) * kk + halfsel * kpad + hb + lane * 4) =
+          tile[(vp * 32 + jj) * PW + lane];
+    }
+  }
+}
+
+template <int P>
+static int slice4m_p(emugemm_ctx *ctx, int is_b, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
+                     const unsigned long long *maxbits, int32_t *e, int slice_bits, int8_t *out) {
+  cudaStream_t st = ctx->stream;
+  const double *x = static_cast<const double *>(X);
+  const int scale_bits = slice_bits == 8 ? 8 * P - 2 : kBeta * P;
+  if (!is_b) {
+    if (slice_bits == 8) oz1_4m_rows_kernel<16 + P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out);
+    else oz1_4m_rows_kernel<P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out);
+  } else {
+    const size_t smem = static_cast<size_t>(2 * P) * 32 * 33 * 4;
+    const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / 128));
+    if (slice_bits == 8) {
+      auto kern = oz1_4m_cols_kernel<16 + P>;
+      EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 32 * 33 * 4));
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, scale_bits, P, out);
+    } else {
+      auto kern = oz1_4m_cols_kernel<P>;
+      EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 32 * 33 * 4));
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, scale_bits, P, out);
+    }
+  }
+  ctx->launches++;
+  EMU_CUDA(ctx, cudaGetLastError());
+  return EMUGEMM_OK;
+}
+
+// is_b = 0: A (rows x k complex) -> out[p][2 rows][2 kpad], e[2 rows];  is_b = 1: B (k x rows complex) ->
+// out[p][rows][2 kpad], e[rows], maxbits from launch_colmax(kZ128).
+int launch_oz1_4m_slice(emugemm_ctx *ctx, int is_b, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
+                        const unsigned long long *maxbits, int32_t *e, int p, int slice_bits, int8_t *out) {
+  if (rows == 0 || kpad == 0) return EMUGEMM_OK;
+  switch (p) {
+    case 1: return slice4m_p<1>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
+    case 2: return slice4m_p<2>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
+    case 3: return slice4m_p<3>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
+    case 4: return slice4m_p<4>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
+    case 5: return slice4m_p<5>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
+    case 6: return slice4m_p<6>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
+    case 7: return slice4m_p<7>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
+    case 8: return slice4m_p<8>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
+    default: return EMUGEMM_ERR_ARG;
+  }
+}
+
 // ---- host helpers -----------------------------------------------------------
 int oz2_moduli_host(int n, int *mod) {
   if (n < 1 || n > 24) return -1;
