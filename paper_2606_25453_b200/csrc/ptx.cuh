@@ -53,6 +53,9 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   const long long t0 = clock64();
   const long long limit = threadIdx.x >= 64 ? 8000000000LL : 4000000000LL;
   while (!mbar_try_wait(bar, parity)) {
+    // epilogue warps wait for a whole k-loop (~10^5 cycles): back off instead of polling shared memory and the issue
+    // slots the MMA / TMA threads share with them (costs <= 0.3 us of wake-up latency per tile)
+    if (threadIdx.x >= 64) __nanosleep(256);
     if (clock64() - t0 > limit) {
       printf("emugemm: mbarrier timeout block %d thread %d bar %u parity %u\n", blockIdx.x, threadIdx.x,
              smem_u32(bar), parity);
