@@ -92,6 +92,15 @@ int emugemm_sgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, float
 int emugemm_zgemm_oz1_4m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2], const double *A,
                          int64_t lda, const double *B, int64_t ldb, const double beta[2], double *C, int64_t ldc, int p);
 
+/* CGEMM: complex64 operands and result as (re, im) float pairs (PAPER.md:299 CGEMM by 4M), the
+ * same kernels on 24-bit inputs, one more rounding to float at the end; alpha, beta HOST {re, im} doubles.
+ * 1 <= p <= 4; 2 <= n_moduli <= 20 (8-11 cover FP32 accuracy).  Workspace as for the complex128 calls.        */
+int emugemm_cgemm_oz1_4m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2], const float *A,
+                         int64_t lda, const float *B, int64_t ldb, const double beta[2], float *C, int64_t ldc, int p);
+int emugemm_cgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2], const float *A,
+                         int64_t lda, const float *B, int64_t ldb, const double beta[2], float *C, int64_t ldc,
+                         int n_moduli);
+
 /* ---- Scheme II ---------------------------------------- *
  * n_moduli pairwise-coprime moduli <= 256 (256, 255, 253, 251, 247, ... greedy
  * descending); symmetric INT8 residues; one INT8 GEMM per modulus with the

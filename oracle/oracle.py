@@ -185,6 +185,24 @@ def zgemm_oz1_4m(A, B, p, alpha=1.0 + 0j, beta=0j, Cin=None):
     return out
 
 
+def cgemm_oz1_4m(A, B, p, alpha=1.0 + 0j, beta=0j, Cin=None):
+    """CGEMM by Scheme I / 4M: complex64 inputs widened exactly to complex128, the complex128 oracle, then each
+    component rounded to float (a second rounding after the double one: at most 2^-29 relative beyond 1/2 ulp of
+    float, far inside the 2-ulp FP32 tolerance)."""
+    A = np.ascontiguousarray(A, np.complex64).astype(np.complex128)
+    B = np.ascontiguousarray(B, np.complex64).astype(np.complex128)
+    C0 = None if Cin is None else np.ascontiguousarray(Cin, np.complex64).astype(np.complex128)
+    return zgemm_oz1_4m(A, B, p, alpha=alpha, beta=beta, Cin=C0).astype(np.complex64)
+
+
+def cgemm_oz2_3m(A, B, N, alpha=1.0 + 0j, beta=0j, Cin=None):
+    """CGEMM by Scheme II / 3M on complex64 inputs: as cgemm_oz1_4m, through zgemm_oz2_3m."""
+    A = np.ascontiguousarray(A, np.complex64).astype(np.complex128)
+    B = np.ascontiguousarray(B, np.complex64).astype(np.complex128)
+    C0 = None if Cin is None else np.ascontiguousarray(Cin, np.complex64).astype(np.complex128)
+    return zgemm_oz2_3m(A, B, N, alpha=alpha, beta=beta, Cin=C0).astype(np.complex64)
+
+
 # ---------------------------------------------------------------- brute force
 def bf128_dgemm(A, B):
     """(C, absAB): __float128 product of the original operands and (|A||B|)_ij."""

@@ -187,6 +187,28 @@ class EmuGemm:
                                                     _i64(self._ld(B)), be, _ptr(C_), _i64(self._ld(C_)), _int(p)))
         return C_
 
+    def cgemm_oz1_4m(self, A, B, C_, p, alpha=1.0 + 0j, beta=0j):
+        """A, B, C_: complex64 CUDA tensors (Scheme I, 4M)."""
+        m, k = A.shape
+        n = B.shape[1]
+        self._reserve_for(OZ1_4M, 16, m, n, k, p)
+        al = (_dbl * 2)(complex(alpha).real, complex(alpha).imag)
+        be = (_dbl * 2)(complex(beta).real, complex(beta).imag)
+        self._check(self._lib.emugemm_cgemm_oz1_4m(self._h, _i64(m), _i64(n), _i64(k), al, _ptr(A), _i64(self._ld(A)), _ptr(B),
+                                                    _i64(self._ld(B)), be, _ptr(C_), _i64(self._ld(C_)), _int(p)))
+        return C_
+
+    def cgemm_oz2_3m(self, A, B, C_, n_moduli, alpha=1.0 + 0j, beta=0j):
+        """A, B, C_: complex64 CUDA tensors (Scheme II, 3M)."""
+        m, k = A.shape
+        n = B.shape[1]
+        self._reserve_for(OZ2_3M, 16, m, n, k, n_moduli)
+        al = (_dbl * 2)(complex(alpha).real, complex(alpha).imag)
+        be = (_dbl * 2)(complex(beta).real, complex(beta).imag)
+        self._check(self._lib.emugemm_cgemm_oz2_3m(self._h, _i64(m), _i64(n), _i64(k), al, _ptr(A), _i64(self._ld(A)), _ptr(B),
+                                                    _i64(self._ld(B)), be, _ptr(C_), _i64(self._ld(C_)), _int(n_moduli)))
+        return C_
+
     def sgemm_oz2(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0, transa=False, transb=False):
         m, n, k = self._dims(A, B, transa, transb)
         self._reserve_for(OZ2, 8, m, n, k, n_moduli)

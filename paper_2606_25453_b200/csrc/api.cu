@@ -73,6 +73,11 @@ __global__ void scale_c_kernel(int64_t m, int64_t n, double br, double bi, void 
   } else if (elem == 4) {
     float *o = static_cast<float *>(C) + i * ldc + j;
     *o = (br == 0.0) ? 0.0f : static_cast<float>(br) * *o;
+  } else if (elem == 64) {  // complex64
+    float *o = static_cast<float *>(C) + 2 * (i * ldc + j);
+    const double re = o[0], im = o[1];
+    if (br == 0.0 && bi == 0.0) { o[0] = 0.0f; o[1] = 0.0f; }
+    else { o[0] = static_cast<float>(br * re - bi * im); o[1] = static_cast<float>(br * im + bi * re); }
   } else {
     double *o = static_cast<double *>(C) + 2 * (i * ldc + j);
     const double re = o[0], im = o[1];
@@ -82,21 +87,22 @@ __global__ void scale_c_kernel(int64_t m, int64_t n, double br, double bi, void 
 }
 
 // C = alpha (T[i][j] + i T[m + i][j]) + beta C: the complex combination of the 4M real embedding result T (2m x n)
+template <typename TC /* double or float: component type of C */>
 __global__ void zcombine_4m_kernel(int64_t m, int64_t n, const double *__restrict__ T, double ar, double ai, double br, double bi,
-                                   double *__restrict__ C, int64_t ldc) {
+                                   TC *__restrict__ C, int64_t ldc) {
   const int64_t idx = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
   if (idx >= m * n) return;
   const int64_t i = idx / n, j = idx - i * n;
   const double tr = T[idx], ti = T[idx + m * n];
   double re = ar * tr - ai * ti, im = ar * ti + ai * tr;
-  double *o = C + 2 * (i * ldc + j);
+  TC *o = C + 2 * (i * ldc + j);
   if (br != 0.0 || bi != 0.0) {
     const double cr = o[0], ci = o[1];
     re += br * cr - bi * ci;
     im += br * ci + bi * cr;
   }
-  o[0] = re;
-  o[1] = im;
+  o[0] = static_cast<TC>(re);
+  o[1] = static_cast<TC>(im);
 }
 
 static int scale_c(emugemm_ctx *h, int64_t m, int64_t n, double br, double bi, void *C, int64_t ldc, int elem) {
@@ -218,7 +224,7 @@ static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t 
   if (N < 2 || N > kMaxModuli) return EMUGEMM_ERR_ARG;
   h->launches = 0;
   if (m == 0 || n == 0) return EMUGEMM_OK;
-  const int elem = is3m ? kZ128 : (f32 ? kF32 : kF64);
+  const int elem = is3m ? (f32 ? kC64 : kZ128) : (f32 ? kF32 : kF64);
   EMU_TRY(mark(h, 0));
   if (k == 0) {
     EMU_TRY(scale_c(h, m, n, beta[0], beta[1], C, ldc, elem));
@@ -355,16 +361,16 @@ int emugemm_last_cuda_error(emugemm_handle_t h) { return h ? h->last_cuda : 0; }
 
 // Scheme I ZGEMM by 4M: one real Scheme I GEMM of size 2m x n x 2k on the real embedding
 // A' = [[Re A, -Im A], [Im A, Re A]], B' = [[Re B], [Im B]], then the complex alpha / beta combination.
-int emugemm_zgemm_oz1_4m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2], const double *A, int64_t lda,
-                         const double *B, int64_t ldb, const double beta[2], double *C, int64_t ldc, int p) {
+static int run_oz1_4m(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k, const double alpha[2], const void *A, int64_t lda,
+                      const void *B, int64_t ldb, const double beta[2], void *C, int64_t ldc, int p) {
   if (!alpha || !beta) return EMUGEMM_ERR_ARG;
   EMU_TRY(check_gemm_args(h, 0, 0, m, n, k, A, lda, B, ldb, C, ldc));
-  if (p < 1 || p > 8) return EMUGEMM_ERR_ARG;
+  if (p < 1 || p > (elem == kC64 ? 4 : 8)) return EMUGEMM_ERR_ARG;
   h->launches = 0;
   if (m == 0 || n == 0) return EMUGEMM_OK;
   EMU_TRY(mark(h, 0));
   if (k == 0) {
-    EMU_TRY(scale_c(h, m, n, beta[0], beta[1], C, ldc, kZ128));
+    EMU_TRY(scale_c(h, m, n, beta[0], beta[1], C, ldc, elem));
     EMU_TRY(mark(h, 1)); EMU_TRY(mark(h, 2)); EMU_TRY(mark(h, 3));
     return EMUGEMM_OK;
   }
@@ -385,17 +391,35 @@ int emugemm_zgemm_oz1_4m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, co
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   h->diag = diag;
   EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
-  EMU_TRY(launch_colmax(h, kZ128, n, k, B, ldb, mbB));
-  EMU_TRY(launch_oz1_4m_slice(h, 0, m, k, kpad, A, lda, nullptr, eA, p, bits, SA));
-  EMU_TRY(launch_oz1_4m_slice(h, 1, n, k, kpad, B, ldb, mbB, eB, p, bits, SB));
+  EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB));
+  EMU_TRY(launch_oz1_4m_slice(h, elem, 0, m, k, kpad, A, lda, nullptr, eA, p, bits, SA));
+  EMU_TRY(launch_oz1_4m_slice(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, p, bits, SB));
   EMU_TRY(mark(h, 1));
   EMU_TRY(oz1_gemm_phase(h, kF64, mm, n, kk, p, bits, SA, SB, eA, eB, 1.0, 0.0, T, n, nullptr, nch, clen, part, diag));
-  zcombine_4m_kernel<<<static_cast<unsigned>((m * n + 255) / 256), 256, 0, h->stream>>>(m, n, T, alpha[0], alpha[1], beta[0],
-                                                                                      beta[1], C, ldc);
+  const unsigned cgrid = static_cast<unsigned>((m * n + 255) / 256);
+  if (elem == kC64)
+    zcombine_4m_kernel<float><<<cgrid, 256, 0, h->stream>>>(m, n, T, alpha[0], alpha[1], beta[0], beta[1], static_cast<float *>(C), ldc);
+  else
+    zcombine_4m_kernel<double><<<cgrid, 256, 0, h->stream>>>(m, n, T, alpha[0], alpha[1], beta[0], beta[1], static_cast<double *>(C), ldc);
   h->launches++;
   EMU_CUDA(h, cudaGetLastError());
   EMU_TRY(mark(h, 3));
   return EMUGEMM_OK;
+}
+
+int emugemm_zgemm_oz1_4m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2], const double *A, int64_t lda,
+                         const double *B, int64_t ldb, const double beta[2], double *C, int64_t ldc, int p) {
+  return run_oz1_4m(h, kZ128, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, p);
+}
+// complex64 operands and result (CGEMM): alpha, beta stay HOST double pairs
+int emugemm_cgemm_oz1_4m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2], const float *A, int64_t lda,
+                         const float *B, int64_t ldb, const double beta[2], float *C, int64_t ldc, int p) {
+  return run_oz1_4m(h, kC64, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, p);
+}
+int emugemm_cgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, const double alpha[2], const float *A, int64_t lda,
+                         const float *B, int64_t ldb, const double beta[2], float *C, int64_t ldc, int n_moduli) {
+  if (!alpha || !beta) return EMUGEMM_ERR_ARG;
+  return run_oz2(h, 0, 0, 1, m, n, k, alpha, A, lda, B, ldb, beta, reinterpret_cast<double *>(C), ldc, n_moduli, 1);
 }
 
 int emugemm_dgemm_oz1_t(emugemm_handle_t h, int transa, int transb, int64_t m, int64_t n, int64_t k, double alpha,

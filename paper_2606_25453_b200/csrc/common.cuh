@@ -60,7 +60,7 @@ int encode_planes_tmap(emugemm_ctx *ctx, CUtensorMap *tm, const void *base, int6
                        int64_t planes, int box_rows, int box_planes);
 
 // ---- stage drivers (all asynchronous on ctx->stream) ------------------------
-enum ElemKind { kF32 = 4, kF64 = 8, kZ128 = 16 };
+enum ElemKind { kF32 = 4, kF64 = 8, kZ128 = 16, kC64 = 64 /* complex64: internal id, not a byte count */ };
 
 // Max-|x| bit pattern per row (by_cols = 0) or column (by_cols = 1) -> frexp exponent e_out[rows];
 // maxbits is a rows x u64 scratch (zeroed inside).  For kZ128 the exponent covers re and im.
@@ -84,7 +84,7 @@ int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, i
                         int t_bits, int8_t *out);
 
 // Scheme I complex by 4M: digit planes of the real embedding (prepass.cu) and the final complex combination.
-int launch_oz1_4m_slice(emugemm_ctx *ctx, int is_b, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
+int launch_oz1_4m_slice(emugemm_ctx *ctx, int elem /* kZ128 or kC64 */, int is_b, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
                         const unsigned long long *maxbits, int32_t *e, int p, int slice_bits, int8_t *out);
 
 struct Oz1GemmArgs {
@@ -122,7 +122,7 @@ struct Oz2CrtArgs {
   const int32_t *eA, *eB;
   int tA, tB;
   int is_complex;              // 0: real alpha/beta; 1: complex, C is (re, im) pairs
-  int out_f32;                 // real only: C is float (Scheme II SGEMM)
+  int out_f32;                 // C holds float (real: SGEMM) or float pairs (complex: CGEMM)
   double alpha[2], beta[2];
   double *C;
   int64_t ldc;

@@ -144,7 +144,7 @@ __device__ __forceinline__ double crt_finish(const CrtConst &k, double shi, doub
 }
 
 // one thread per 8 consecutive columns of one row
-// KIND: 0 = FP64 C, 1 = complex128 C, 2 = FP32 C (Scheme II SGEMM: one more rounding, double -> float)
+// KIND: 0 = FP64 C, 1 = complex128 C, 2 = FP32 C (SGEMM), 3 = complex64 C (CGEMM); 2 and 3 round once more to float
 template <bool VEC, int KIND>
 __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const int8_t *__restrict__ CR,
                                                   const int32_t *__restrict__ eA, const int32_t *__restrict__ eB,
@@ -207,20 +207,36 @@ __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const in
     crt_accumulate<VEC>(k, CR + static_cast<int64_t>(k.N) * plane + i * n + j0, plane, j0, n, shi, slo);
 #pragma unroll
     for (int e = 0; e < kCrtVec; ++e) vi[e] = crt_finish(k, shi[e], slo[e]) * sc1[e] * sc2[e];
-    double *o = C + 2 * (i * ldc + j0);
     const bool has_beta = (br != 0.0 || bi != 0.0);
+    if (KIND == 3) {  // complex64 C: float pairs
+      float *o = reinterpret_cast<float *>(C) + 2 * (i * ldc + j0);
 #pragma unroll
-    for (int e = 0; e < kCrtVec; ++e) {
-      if (j0 + e >= n) break;
-      double re = ar * vr[e] - ai * vi[e];
-      double im = ar * vi[e] + ai * vr[e];
-      if (has_beta) {
-        const double cr = o[2 * e], ci = o[2 * e + 1];
-        re += br * cr - bi * ci;
-        im += br * ci + bi * cr;
+      for (int e = 0; e < kCrtVec; ++e) {
+        if (j0 + e >= n) break;
+        double re = ar * vr[e] - ai * vi[e];
+        double im = ar * vi[e] + ai * vr[e];
+        if (has_beta) {
+          const double cr = o[2 * e], ci = o[2 * e + 1];
+          re += br * cr - bi * ci;
+          im += br * ci + bi * cr;
+        }
+        *reinterpret_cast<float2 *>(o + 2 * e) = make_float2(static_cast<float>(re), static_cast<float>(im));
       }
-      if ((reinterpret_cast<uintptr_t>(C) & 15) == 0) *reinterpret_cast<double2 *>(o + 2 * e) = make_double2(re, im);
-      else { o[2 * e] = re; o[2 * e + 1] = im; }
+    } else {
+      double *o = C + 2 * (i * ldc + j0);
+#pragma unroll
+      for (int e = 0; e < kCrtVec; ++e) {
+        if (j0 + e >= n) break;
+        double re = ar * vr[e] - ai * vi[e];
+        double im = ar * vi[e] + ai * vr[e];
+        if (has_beta) {
+          const double cr = o[2 * e], ci = o[2 * e + 1];
+          re += br * cr - bi * ci;
+          im += br * ci + bi * cr;
+        }
+        if ((reinterpret_cast<uintptr_t>(C) & 15) == 0) *reinterpret_cast<double2 *>(o + 2 * e) = make_double2(re, im);
+        else { o[2 * e] = re; o[2 * e + 1] = im; }
+      }
     }
   }
 }
@@ -236,8 +252,10 @@ int launch_oz2_crt(emugemm_ctx *ctx, const Oz2CrtArgs &a) {
 #define EMU_CRT_LAUNCH(V, Z)                                                                                              \
   crt_kernel<V, Z><<<grid, 256, 0, ctx->stream>>>(a.m, a.n, a.CR, a.eA, a.eB, tsum, a.alpha[0], a.alpha[1], a.beta[0], \
                                                    a.beta[1], a.C, a.ldc, k)
-  const int kind = a.is_complex ? 1 : (a.out_f32 ? 2 : 0);
-  if (vec && kind == 1) EMU_CRT_LAUNCH(true, 1);
+  const int kind = a.is_complex ? (a.out_f32 ? 3 : 1) : (a.out_f32 ? 2 : 0);
+  if (vec && kind == 3) EMU_CRT_LAUNCH(true, 3);
+  else if (kind == 3) EMU_CRT_LAUNCH(false, 3);
+  else if (vec && kind == 1) EMU_CRT_LAUNCH(true, 1);
   else if (vec && kind == 2) EMU_CRT_LAUNCH(true, 2);
   else if (vec) EMU_CRT_LAUNCH(true, 0);
   else if (kind == 1) EMU_CRT_LAUNCH(false, 1);

@@ -122,6 +122,7 @@ int launch_colmax(emugemm_ctx *ctx, int elem, int64_t rows, int64_t k, const voi
   const dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>((k + kseg - 1) / kseg));
   if (elem == kF64) colmax_kernel<double, 1><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits);
   else if (elem == kF32) colmax_kernel<float, 1><<<grid, 256, 0, st>>>(static_cast<const float *>(X), ldx, rows, k, kseg, maxbits);
+  else if (elem == kC64) colmax_kernel<float, 2><<<grid, 256, 0, st>>>(static_cast<const float *>(X), ldx, rows, k, kseg, maxbits);
   else colmax_kernel<double, 2><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits);
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
@@ -517,6 +518,9 @@ int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, i
   if (elem == kF32)  // 24-bit inputs (Scheme II SGEMM)
     return two ? launch_planes<float, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out)
                : launch_planes<float, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out);
+  if (elem == kC64)
+    return two ? launch_planes<float, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out)
+               : launch_planes<float, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out);
   if (elem == kZ128)
     return two ? launch_planes<double, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out)
                : launch_planes<double, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out);
@@ -534,12 +538,12 @@ __device__ __forceinline__ void emit_oz1_any(const Prep (&q)[4], Sink sink) {
   else emit_oz1<PARAM>(q, sink);
 }
 
-template <int PARAM>
-__global__ void __launch_bounds__(256) oz1_4m_rows_kernel(const double *__restrict__ X, int64_t ldx, int64_t m, int64_t k,
+template <typename T, int PARAM>
+__global__ void __launch_bounds__(256) oz1_4m_rows_kernel(const T *__restrict__ X, int64_t ldx, int64_t m, int64_t k,
                                                           int64_t kpad, int32_t *__restrict__ e_out, int scale_bits,
                                                           int8_t *__restrict__ out) {
   const int64_t row = blockIdx.x;
-  const double *src = X + row * ldx * 2;
+  const T *src = X + row * ldx * 2;
   unsigned long long mx = 0;
   for (int64_t h = static_cast<int64_t>(threadIdx.x) * 4; h < 2 * k; h += 1024)
 #pragma unroll
@@ -557,7 +561,7 @@ __global__ void __launch_bounds__(256) oz1_4m_rows_kernel(const double *__restri
   __syncthreads();
 #pragma unroll
   for (int w = 0; w < 8; ++w) mx = red[w] > mx ? red[w] : mx;
-  const int e_row = exponent_of_maxbits<double>(mx);
+  const int e_row = exponent_of_maxbits<T>(mx);
   if (threadIdx.x == 0) { e_out[row] = e_row; e_out[m + row] = e_row; }
 
   const int64_t kk = 2 * kpad, plane_stride = 2 * m * kk;
@@ -566,8 +570,8 @@ __global__ void __launch_bounds__(256) oz1_4m_rows_kernel(const double *__restri
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       const bool in = h0 + i < k;
-      re[i] = prepare<double, 2>(in ? src[(h0 + i) * 2] : 0.0, e_row, scale_bits);
-      im[i] = prepare<double, 2>(in ? src[(h0 + i) * 2 + 1] : 0.0, e_row, scale_bits);
+      re[i] = prepare<T, 2>(in ? src[(h0 + i) * 2] : T(0), e_row, scale_bits);
+      im[i] = prepare<T, 2>(in ? src[(h0 + i) * 2 + 1] : T(0), e_row, scale_bits);
       nim[i] = im[i];
       nim[i].neg = !im[i].neg;
     }
@@ -583,8 +587,8 @@ __global__ void __launch_bounds__(256) oz1_4m_rows_kernel(const double *__restri
 
 // B (k x n complex, ldx in complex elements): planes out[t][j][2 kpad] = [digits of Re B(:, j) | digits of Im B(:, j)];
 // tile = 32 columns x 128 k, transposed through shared memory ("virtual plane" P + t = imaginary half).
-template <int PARAM>
-__global__ void __launch_bounds__(256) oz1_4m_cols_kernel(const double *__restrict__ X, int64_t ldx, int64_t n, int64_t k,
+template <typename T, int PARAM>
+__global__ void __launch_bounds__(256) oz1_4m_cols_kernel(const T *__restrict__ X, int64_t ldx, int64_t n, int64_t k,
                                                           int64_t kpad, const unsigned long long *__restrict__ maxbits,
                                                           int32_t *__restrict__ e_out, int scale_bits, int P,
                                                           int8_t *__restrict__ out) {
@@ -593,7 +597,7 @@ __global__ void __launch_bounds__(256) oz1_4m_cols_kernel(const double *__restri
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t j = static_cast<int64_t>(blockIdx.x) * 32 + lane;
   const int64_t hb = static_cast<int64_t>(blockIdx.y) * TH;
-  const int e_row = (j < n) ? exponent_of_maxbits<double>(maxbits[j]) : 0;
+  const int e_row = (j < n) ? exponent_of_maxbits<T>(maxbits[j]) : 0;
   if (blockIdx.y == 0 && warp == 0 && j < n) e_out[j] = e_row;
   for (int hw = warp; hw < TH / 4; hw += 8) {
     const int64_t h0 = hb + hw * 4;
@@ -601,8 +605,8 @@ __global__ void __launch_bounds__(256) oz1_4m_cols_kernel(const double *__restri
 #pragma unroll
     for (int i = 0; i < 4; ++i) {
       const bool in = j < n && h0 + i < k;
-      re[i] = prepare<double, 2>(in ? X[((h0 + i) * ldx + j) * 2] : 0.0, e_row, scale_bits);
-      im[i] = prepare<double, 2>(in ? X[((h0 + i) * ldx + j) * 2 + 1] : 0.0, e_row, scale_bits);
+      re[i] = prepare<T, 2>(in ? X[((h0 + i) * ldx + j) * 2] : T(0), e_row, scale_bits);
+      im[i] = prepare<T, 2>(in ? X[((h0 + i) * ldx + j) * 2 + 1] : T(0), e_row, scale_bits);
     }
     emit_oz1_any<PARAM>(re, [&](int t, unsigned int w) { tile[(t * 32 + lane) * PW + hw] = w; });
     emit_oz1_any<PARAM>(im, [&](int t, unsigned int w) { tile[((P + t) * 32 + lane) * PW + hw] = w; });
@@ -620,24 +624,24 @@ __global__ void __launch_bounds__(256) oz1_4m_cols_kernel(const double *__restri
   }
 }
 
-template <int P>
+template <typename T, int P>
 static int slice4m_p(emugemm_ctx *ctx, int is_b, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
                      const unsigned long long *maxbits, int32_t *e, int slice_bits, int8_t *out) {
   cudaStream_t st = ctx->stream;
-  const double *x = static_cast<const double *>(X);
+  const T *x = static_cast<const T *>(X);
   const int scale_bits = slice_bits == 8 ? 8 * P - 2 : kBeta * P;
   if (!is_b) {
-    if (slice_bits == 8) oz1_4m_rows_kernel<16 + P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out);
-    else oz1_4m_rows_kernel<P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out);
+    if (slice_bits == 8) oz1_4m_rows_kernel<T, 16 + P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out);
+    else oz1_4m_rows_kernel<T, P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out);
   } else {
     const size_t smem = static_cast<size_t>(2 * P) * 32 * 33 * 4;
     const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / 128));
     if (slice_bits == 8) {
-      auto kern = oz1_4m_cols_kernel<16 + P>;
+      auto kern = oz1_4m_cols_kernel<T, 16 + P>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 32 * 33 * 4));
       kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, scale_bits, P, out);
     } else {
-      auto kern = oz1_4m_cols_kernel<P>;
+      auto kern = oz1_4m_cols_kernel<T, P>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 32 * 33 * 4));
       kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, scale_bits, P, out);
     }
@@ -648,21 +652,23 @@ static int slice4m_p(emugemm_ctx *ctx, int is_b, int64_t rows, int64_t k, int64_
 }
 
 // is_b = 0: A (rows x k complex) -> out[p][2 rows][2 kpad], e[2 rows];  is_b = 1: B (k x rows complex) ->
-// out[p][rows][2 kpad], e[rows], maxbits from launch_colmax(kZ128).
-int launch_oz1_4m_slice(emugemm_ctx *ctx, int is_b, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
+// out[p][rows][2 kpad], e[rows], maxbits from launch_colmax.  elem: kZ128 (complex128) or kC64 (complex64, p <= 4).
+int launch_oz1_4m_slice(emugemm_ctx *ctx, int elem, int is_b, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
                         const unsigned long long *maxbits, int32_t *e, int p, int slice_bits, int8_t *out) {
   if (rows == 0 || kpad == 0) return EMUGEMM_OK;
+#define EMU_4M_CASE(T, PP) case PP: return slice4m_p<T, PP>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out)
+  if (elem == kC64) {
+    switch (p) {
+      EMU_4M_CASE(float, 1); EMU_4M_CASE(float, 2); EMU_4M_CASE(float, 3); EMU_4M_CASE(float, 4);
+      default: return EMUGEMM_ERR_ARG;
+    }
+  }
   switch (p) {
-    case 1: return slice4m_p<1>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
-    case 2: return slice4m_p<2>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
-    case 3: return slice4m_p<3>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
-    case 4: return slice4m_p<4>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
-    case 5: return slice4m_p<5>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
-    case 6: return slice4m_p<6>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
-    case 7: return slice4m_p<7>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
-    case 8: return slice4m_p<8>(ctx, is_b, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out);
+    EMU_4M_CASE(double, 1); EMU_4M_CASE(double, 2); EMU_4M_CASE(double, 3); EMU_4M_CASE(double, 4);
+    EMU_4M_CASE(double, 5); EMU_4M_CASE(double, 6); EMU_4M_CASE(double, 7); EMU_4M_CASE(double, 8);
     default: return EMUGEMM_ERR_ARG;
   }
+#undef EMU_4M_CASE
 }
 
 // ---- host helpers -----------------------------------------------------------

@@ -38,3 +38,17 @@ def test_rows_of_the_embedding_share_exponents():
     Ae = np.block([[A.real, -A.imag], [A.imag, A.real]])
     e = O.row_exponents(np.ascontiguousarray(Ae))
     assert np.array_equal(e[:9], e[9:]) and np.array_equal(e[:9], O.row_exponents_z(A))
+
+
+def test_cgemm_oracles_exact_on_gaussian_integers_and_close_to_truth():
+    rng = np.random.default_rng(9)
+    A = (rng.integers(-31, 32, size=(10, 24)) + 1j * rng.integers(-31, 32, size=(10, 24))).astype(np.complex64)
+    B = (rng.integers(-31, 32, size=(24, 7)) + 1j * rng.integers(-31, 32, size=(24, 7))).astype(np.complex64)
+    want = (A.astype(np.complex128) @ B.astype(np.complex128)).astype(np.complex64)
+    assert np.array_equal(O.cgemm_oz1_4m(A, B, 3), want)
+    assert np.array_equal(O.cgemm_oz2_3m(A, B, 9), want)
+    Az, Bz = G.complex_pair(20, 16, 64, 0.5, 4)
+    Ac, Bc = Az.astype(np.complex64), Bz.astype(np.complex64)
+    exact, absZ = O.bf128_zgemm(Ac.astype(np.complex128), Bc.astype(np.complex128))
+    for got in (O.cgemm_oz1_4m(Ac, Bc, 4), O.cgemm_oz2_3m(Ac, Bc, 11)):
+        assert (np.abs(got.astype(np.complex128) - exact) <= 8 * 2.0 ** -23 * absZ).all()
