@@ -33,7 +33,7 @@ template <int P, bool PAIR = false>
 struct Oz1Cfg {
   // NT: tile width; P * NT <= 512 TMEM columns, every MMA width a multiple of 16
   static constexpr int NT = (P <= 2) ? 256 : (P == 3) ? 160 : (P == 4) ? 128 : (P == 5) ? 96 : (P == 6) ? 80 : 64;
-  // PAIR (cta_group::2, P <= 4): a CTA pair owns a 256 x NT tile; each CTA stages only NT/2 rows of every B slice
+  // PAIR (cta_group::2, P <= 3): a CTA pair owns a 256 x NT tile; each CTA stages only NT/2 rows of every B slice
   static constexpr int kBRows = PAIR ? NT / 2 : NT;
   static constexpr int kBStageBytes = P * kBRows * kBlockK;
   // B ring depth.  A k-block of B is released only when all P slices have used it, so its refill has one k-block of
@@ -117,7 +117,7 @@ __device__ __forceinline__ void oz1_issue_slice_per_product(int t, uint32_t tmem
   }
 }
 
-// CTA-pair schedule (cta_group::2, P <= 4 where NT >= 128): one 256 x NT x 32 MMA per product, issued by the leader
+// CTA-pair schedule (cta_group::2, used for P <= 3; needs NT >= 128): one 256 x NT x 32 MMA per product, issued by the leader
 // CTA for both SMs; CTA r supplies rows 128 r .. of A_t and rows NT/2 r .. of B_u from its own shared memory, so the
 // columns of D come out in natural order and land on C_{t+u}.  A_t stays in the collector across its P - t MMAs.
 template <int P>
@@ -551,8 +551,9 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   if (blockIdx.x == 0 && threadIdx.x == 0 && a.cycles) atomicAdd(a.cycles, static_cast<unsigned long long>(clock64() - t_start));
 }
 
-// P <= 4 (NT >= 128) runs as CTA pairs (cta_group::2); P >= 5 needs N-concatenated MMAs, whose columns a pair
-// would split between the two CTAs' B halves, and stays one CTA per tile.
+// P <= 3 runs as CTA pairs (cta_group::2, one MMA per product, NT >= 160); P >= 4 uses N-concatenated MMAs, whose
+// columns a pair would split between the two CTAs' B halves, so it stays one CTA per tile, two N-adjacent tiles per
+// cluster sharing A by TMA multicast.  Same-run A/B at 8192^3: p = 3 pairs +6 %, p = 4 one-CTA +4 %.
 template <int P, bool PAIR, bool MC>
 static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   using Cfg = Oz1Cfg<P, PAIR>;
@@ -605,11 +606,11 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
 
 template <int P>
 static int launch_p(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
-  if constexpr (P <= 4) {
+  if constexpr (P <= 3) {
     if (!(ctx->dbg_flags & 8)) return launch_pp<P, true, false>(ctx, g);  // dbg bit 3: force the one-CTA N-concatenated kernel (A/B timing)
   }
-  // A multicast pays where A dominates the operand traffic (NT = 64: +2-4 % at p = 8; within noise at p = 5, 6)
-  if (P >= 7 && !(ctx->dbg_flags & 16)) return launch_pp<P, false, true>(ctx, g);  // dbg bit 4: no multicast clusters (A/B timing)
+  // A multicast: +2-4 % at p = 8 (NT = 64, A dominates the operand traffic), +2 % at p = 4, within noise at p = 5, 6
+  if (P >= 4 && !(ctx->dbg_flags & 16)) return launch_pp<P, false, true>(ctx, g);  // dbg bit 4: no multicast clusters (A/B timing)
   return launch_pp<P, false, false>(ctx, g);
 }
 
