@@ -140,14 +140,13 @@ static int oz1_gemm_phase(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_
   g.m = m; g.n = n; g.kpad = kpad; g.p = p; g.slice_bits = bits; g.SA = SA; g.SB = SB; g.eA = eA; g.eB = eB;
   g.alpha = alpha; g.beta = beta; g.C = C; g.ldc = ldc; g.cycles = diag;
   const int final_kind = (elem == kF32) ? 1 : 0;
-  for (int c = 0; c < nch; ++c) {
-    g.k0 = c * clen;
-    g.k1 = (g.k0 + clen < kpad) ? g.k0 + clen : kpad;
-    if (dump) { g.out_kind = 2; g.C = dump + static_cast<int64_t>(c) * p * m * n; }
-    else if (nch == 1) g.out_kind = final_kind;
-    else { g.out_kind = 3; g.C = part + static_cast<int64_t>(c) * m * n * 2; }
-    EMU_TRY(launch_oz1_gemm(h, g));
-  }
+  // ONE launch: with several overflow-safe k-chunks a work item of the persistent kernel is (chunk, tile), so short
+  // chunks of a long-k problem still fill the machine
+  g.k0 = 0; g.k1 = kpad; g.n_chunks = nch; g.chunk_k = clen;
+  if (dump) { g.out_kind = 2; g.C = dump; g.chunk_stride = static_cast<int64_t>(p) * m * n * 4; }
+  else if (nch == 1) { g.out_kind = final_kind; g.chunk_stride = 0; }
+  else { g.out_kind = 3; g.C = part; g.chunk_stride = m * n * 16; }
+  EMU_TRY(launch_oz1_gemm(h, g));
   EMU_TRY(mark(h, 2));
   if (nch > 1 && !dump) EMU_TRY(launch_oz1_chunk_reduce(h, m, n, nch, part, final_kind, alpha, beta, C, ldc));
   EMU_TRY(mark(h, 3));

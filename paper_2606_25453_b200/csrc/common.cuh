@@ -89,7 +89,9 @@ int launch_oz1_4m_slice(emugemm_ctx *ctx, int elem /* kZ128 or kC64 */, int is_b
 
 struct Oz1GemmArgs {
   int64_t m, n, kpad;          // kpad: padded k of the slice planes (multiple of kBlockK)
-  int64_t k0, k1;              // k-chunk [k0, k1) handled by this launch (multiples of kBlockK)
+  int64_t k0, k1;              // k range [k0, k1) handled by this launch (multiples of kBlockK)
+  int n_chunks;                // > 1: the range is cut into overflow-safe chunks of chunk_k, one output per chunk
+  int64_t chunk_k, chunk_stride;  // chunk length (multiple of kBlockK), bytes between the chunks' outputs
   int p;
   int slice_bits;              // 7 or 8 (weights 2^(bits (p-1-s)), scaling 2^(eA + eB - bits (p+1) [+ 4 guard bits]))
   const int8_t *SA, *SB;       // [p][m][kpad], [p][n][kpad]

@@ -146,6 +146,8 @@ __device__ __forceinline__ void oz1_issue_slice_pair(int t, uint32_t tmem_base, 
 struct Oz1Dev {
   int64_t m, n;
   int kb0, kb1;       // k-blocks [kb0, kb1) of 128
+  int chunk_kb, nch;  // overflow-safe k-chunks of chunk_kb k-blocks each: a work item is (chunk, tile)
+  int64_t chunk_stride;  // bytes between the outputs of consecutive chunks (OUT = 2 dump, OUT = 3 partials)
   int mt, nt_tiles;   // tile grid
   const int32_t *eA, *eB;
   int out_kind;
@@ -330,6 +332,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int num_tiles = a.mt * a.nt_tiles;
+  const int num_items = num_tiles * a.nch;  // chunk-major: consecutive items share the k-range of their operands
   // PAIR: the two CTAs of a cluster work on one 256-row tile; rank 0 (leader) issues the MMAs for both
   static_assert(!(PAIR && MC), "pairs already share operands");
   constexpr bool CL2 = PAIR || MC;  // launched as clusters of 2
@@ -367,11 +370,13 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       // L2 eviction hints were measured and dropped: EVICT_LAST on A changes nothing (15.1 vs 15.2 GB DRAM reads per
       // 8192^3 p = 8 launch), EVICT_FIRST on B raises them to 21.9 GB
       constexpr uint64_t polA = kEvictNormal, polB = kEvictNormal;
-      for (int tile = work_id; tile < num_tiles; tile += num_workers) {
+      for (int item = work_id; item < num_items; item += num_workers) {
+        const int chunk = item / num_tiles, tile = item - chunk * num_tiles;
+        const int kb0 = a.kb0 + chunk * a.chunk_kb, kb1 = (kb0 + a.chunk_kb < a.kb1) ? kb0 + a.chunk_kb : a.kb1;
         int mb, nb;
         tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
         if constexpr (MC) nb = 2 * nb + static_cast<int>(cta);  // a.nt_tiles counts PAIRS of N-tiles
-        for (int kb = a.kb0; kb < a.kb1; ++kb) {
+        for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait(&bempty[sb], pb ^ 1);
           if constexpr (PAIR) {
             if (cta == 0) mbar_arrive_expect_tx(&bfull[sb], kTxMul * Cfg::kBStageBytes);
@@ -425,10 +430,12 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       // look-ahead: the barrier of the NEXT stage is probed (non-blocking) before the MMAs of the current stage are
       // issued, so the ~90-cycle try_wait latency overlaps tensor work instead of draining the MMA queue
       bool a_ready = false, b_ready = false;
-      for (int tile = work_id; tile < num_tiles; tile += num_workers) {
+      for (int item = work_id; item < num_items; item += num_workers) {
+        const int chunk = item / num_tiles, tile = item - chunk * num_tiles;
+        const int kb0 = a.kb0 + chunk * a.chunk_kb, kb1 = (kb0 + a.chunk_kb < a.kb1) ? kb0 + a.chunk_kb : a.kb1;
         mbar_wait(tempty, pt ^ 1);  // epilogue has drained the accumulators of the previous tile
         tc_fence_after();
-        for (int kb = a.kb0; kb < a.kb1; ++kb) {
+        for (int kb = kb0; kb < kb1; ++kb) {
           if (!b_ready) mbar_wait(&bfull[sb], pb);
           const uint32_t b_base = smem_u32(sB + sb * Cfg::kBStageBytes);
           const int sb_next = (sb + 1 == SB) ? 0 : sb + 1;
@@ -444,11 +451,11 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             a_ready = mbar_try_wait(&afull[sa], pa);
             if (j == Cfg::NPAIR - 1) b_ready = mbar_try_wait(&bfull[sb_next], pb_next);
             if constexpr (PAIR) {
-              oz1_issue_slice_pair<P>(lo, tmem_base, a_base, b_base, kb != a.kb0 || lo != 0);
+              oz1_issue_slice_pair<P>(lo, tmem_base, a_base, b_base, kb != kb0 || lo != 0);
               if (hi != lo) oz1_issue_slice_pair<P>(hi, tmem_base, a_base + kAStageBytes, b_base, true);
               umma_commit_cg2(&aempty[sa_cur], 3);  // both CTAs' stages reusable once these MMAs have read them
             } else {
-              oz1_issue_slice<P, kUseCollector>(lo, tmem_base, a_base, b_base, kb != a.kb0 || lo != 0);
+              oz1_issue_slice<P, kUseCollector>(lo, tmem_base, a_base, b_base, kb != kb0 || lo != 0);
               if (hi != lo) oz1_issue_slice<P, kUseCollector>(hi, tmem_base, a_base + kAStageBytes, b_base, true);
               if constexpr (MC) umma_commit_mc(&aempty[sa_cur], 3);  // both CTAs must be done before either refills
               else umma_commit(&aempty[sa_cur]);                     // stage reusable once these MMAs have read it
@@ -474,7 +481,10 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     epi.init(a);
     constexpr int kChunks = NT / 2 / 8;  // 8-column chunks per thread
     constexpr bool kDoubleBuffer = (P <= 6);  // two register sets of P x 8 accumulator values fit without spilling
-    for (int tile = work_id; tile < num_tiles; tile += num_workers) {
+    Oz1Dev ac = a;  // per-item copy: the output of chunk c starts c * chunk_stride bytes further
+    for (int item = work_id; item < num_items; item += num_workers) {
+      const int chunk = item / num_tiles, tile = item - chunk * num_tiles;
+      ac.C = static_cast<char *>(a.C) + chunk * a.chunk_stride;
       int mb, nb;
       tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
       if constexpr (MC) nb = 2 * nb + static_cast<int>(cta);
@@ -502,7 +512,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
               for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + (i + 1) * 8, vb[s]);
               epi.load_eb(a, gcol0 + (i + 1) * 8, eb);
             }
-            epi.chunk(a, va, ea, grow, row_ok, eArow, gcol0 + i * 8);
+            epi.chunk(ac, va, ea, grow, row_ok, eArow, gcol0 + i * 8);
             if (i + 1 < kChunks) {
               tmem_ld_wait();
               if (i + 2 < kChunks) {
@@ -510,7 +520,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + (i + 2) * 8, va[s]);
                 epi.load_eb(a, gcol0 + (i + 2) * 8, ea);
               }
-              epi.chunk(a, vb, eb, grow, row_ok, eArow, gcol0 + (i + 1) * 8);
+              epi.chunk(ac, vb, eb, grow, row_ok, eArow, gcol0 + (i + 1) * 8);
             }
           }
         } else {
@@ -522,13 +532,13 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + i * 8, v[s]);
             if (i + 1 < kChunks) epi.load_eb(a, gcol0 + (i + 1) * 8, eb);
             tmem_ld_wait();
-            epi.chunk(a, v, ea, grow, row_ok, eArow, gcol0 + i * 8);
+            epi.chunk(ac, v, ea, grow, row_ok, eArow, gcol0 + i * 8);
             if (i + 1 < kChunks) {
 #pragma unroll
               for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + (i + 1) * 8, v[s]);
               if (i + 2 < kChunks) epi.load_eb(a, gcol0 + (i + 2) * 8, ea);
               tmem_ld_wait();
-              epi.chunk(a, v, eb, grow, row_ok, eArow, gcol0 + (i + 1) * 8);
+              epi.chunk(ac, v, eb, grow, row_ok, eArow, gcol0 + (i + 1) * 8);
             }
           }
         }
@@ -565,6 +575,9 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   d.m = g.m; d.n = g.n;
   d.kb0 = static_cast<int>(g.k0 / kBlockK);
   d.kb1 = static_cast<int>(g.k1 / kBlockK);
+  d.nch = g.n_chunks > 0 ? g.n_chunks : 1;
+  d.chunk_kb = g.n_chunks > 1 ? static_cast<int>(g.chunk_k / kBlockK) : d.kb1 - d.kb0;
+  d.chunk_stride = g.chunk_stride;
   d.mt = static_cast<int>((g.m + kTileRows - 1) / kTileRows);
   d.nt_tiles = static_cast<int>((g.n + Cfg::NT - 1) / Cfg::NT);
   if (MC) d.nt_tiles = (d.nt_tiles + 1) / 2;  // pairs of N-adjacent tiles, one per CTA of the cluster
@@ -574,9 +587,9 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   d.slice_bits = g.slice_bits;
   d.dbg = ctx->dbg_flags;
   constexpr bool CL2 = PAIR || MC;
-  const int tiles = d.mt * d.nt_tiles;
+  const int64_t tiles = static_cast<int64_t>(d.mt) * d.nt_tiles * d.nch;
   const int workers = CL2 ? ctx->num_sms / 2 : ctx->num_sms;
-  const int grid = (CL2 ? 2 : 1) * (tiles < workers ? tiles : workers);
+  const int grid = (CL2 ? 2 : 1) * static_cast<int>(tiles < workers ? tiles : workers);
   void (*kern)(CUtensorMap, CUtensorMap, Oz1Dev) = nullptr;
   switch (g.out_kind) {
     case 0: kern = oz1_gemm_kernel<P, 0, PAIR, MC>; break;
