@@ -14,12 +14,19 @@
 //  * "N-concatenation": the accumulators C_0..C_{p-1} are consecutive NT-column
 //    blocks of TMEM and the B slices are consecutive NT-row blocks of one SMEM
 //    operand, so A_t x [B_0 | ... | B_{p-1-t}] is ONE tcgen05.mma of width
-//    (p-t) NT (split at 256) writing columns [t NT, p NT): exactly the products
-//    A_t B_u -> C_{t+u}.  A_t is read from shared memory once per <= 256 columns
-//    instead of once per product (12 instead of 36 MMAs per k32 at p = 8), which
-//    keeps the SMEM read rate under the 128 B/clk/SM port.
+//    (p-t) NT (two near-equal halves when > 256) writing columns [t NT, p NT):
+//    exactly the products A_t B_u -> C_{t+u}.  A_t is fetched from shared memory
+//    once per (t, k32) (A-operand collector across the two halves) instead of once
+//    per product (12 instead of 36 MMAs per k32 at p = 8).
+//  * A ring of slice PAIRS (j, p-1-j): every stage carries the same MMA time;
+//    the issuing thread probes the next stage's barrier before issuing.
 //  * Warp-specialised persistent CTA: warp 0 = TMA producer, warp 1 = MMA issuer
-//    (one elected thread) + TMEM allocator, warps 2-9 = epilogue.
+//    (one elected thread) + TMEM allocator, warps 2-9 = epilogue (accumulator
+//    triples folded into exact int64, exponent-bias conversion, FP64 scaling).
+//  * Clusters of 2: p >= 4 one tile per CTA, two N-adjacent tiles share A by TMA
+//    multicast; p <= 3 a cta_group::2 pair owns one 256 x NT tile (one MMA per
+//    product).  k-chunks that cannot overflow INT32 are work items of the same
+//    launch.
 #include "common.cuh"
 #include "ptx.cuh"
 #include "gemm_common.cuh"
