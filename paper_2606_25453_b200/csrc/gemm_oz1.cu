@@ -74,17 +74,18 @@ __device__ __forceinline__ void oz1_issue_slice(int t, uint32_t tmem_base, uint3
   const int cols = (P - t) * NT;
   const int n0 = (cols <= 256) ? cols : ((cols / 2 + 15) / 16) * 16;
   const int n1 = cols - n0;
+  const uint32_t a_lo = sdesc_lo(a_base), b_lo = sdesc_lo(b_base);  // per MMA: one add on the address field
 #pragma unroll
   for (int ks = 0; ks < kBlockK / 32; ++ks) {
-    const uint64_t adesc = make_sdesc_sw128(a_base + ks * 32);
+    const uint64_t adesc = sdesc_from_lo(a_lo + ((ks * 32) >> 4));
     const uint32_t acc = (accumulate || ks != 0) ? 1u : 0u;
     const uint32_t d = tmem_base + t * NT;
-    const uint64_t bdesc0 = make_sdesc_sw128(b_base + ks * 32);
+    const uint64_t bdesc0 = sdesc_from_lo(b_lo + ((ks * 32) >> 4));
     if (n1 == 0) {
       umma_i8<0>(d, adesc, bdesc0, make_idesc_i8(kTileM, n0), acc);
     } else {
       // the two MMAs share A_t: the first keeps it in the collector, the second drops it
-      const uint64_t bdesc1 = make_sdesc_sw128(b_base + n0 * kBlockK + ks * 32);
+      const uint64_t bdesc1 = sdesc_from_lo(b_lo + ((n0 * kBlockK + ks * 32) >> 4));
       if (COLL) {
         umma_i8<1>(d, adesc, bdesc0, make_idesc_i8(kTileM, n0), acc);
         umma_i8<3>(d + n0, adesc, bdesc1, make_idesc_i8(kTileM, n1), acc);
@@ -105,15 +106,16 @@ __device__ __forceinline__ void oz1_issue_slice_per_product(int t, uint32_t tmem
                                                             bool accumulate) {
   constexpr int NT = Oz1Cfg<P>::NT;
   constexpr uint32_t idesc = make_idesc_i8(kTileM, NT);
+  const uint32_t a_lo = sdesc_lo(a_base), b_lo = sdesc_lo(b_base);
 #pragma unroll
   for (int ks = 0; ks < kBlockK / 32; ++ks) {
-    const uint64_t adesc = make_sdesc_sw128(a_base + ks * 32);
+    const uint64_t adesc = sdesc_from_lo(a_lo + ((ks * 32) >> 4));
 #pragma unroll
     for (int u = 0; u < P; ++u) {
       if (u < P - t) {
         const uint32_t acc = (accumulate || ks != 0) ? 1u : 0u;
         const uint32_t d = tmem_base + (t + u) * NT;
-        const uint64_t bdesc = make_sdesc_sw128(b_base + u * NT * kBlockK + ks * 32);
+        const uint64_t bdesc = sdesc_from_lo(b_lo + ((u * NT * kBlockK + ks * 32) >> 4));
         const bool first = (u == 0), last = (u == P - t - 1);
         if (COLL && first && !last) umma_i8<1>(d, adesc, bdesc, idesc, acc);
         else if (COLL && !first && last) umma_i8<3>(d, adesc, bdesc, idesc, acc);
@@ -131,15 +133,16 @@ template <int P>
 __device__ __forceinline__ void oz1_issue_slice_pair(int t, uint32_t tmem_base, uint32_t a_base, uint32_t b_base, bool accumulate) {
   constexpr int NT = Oz1Cfg<P, true>::NT;
   constexpr uint32_t idesc = make_idesc_i8(2 * kTileM, NT);
+  const uint32_t a_lo = sdesc_lo(a_base), b_lo = sdesc_lo(b_base);
 #pragma unroll
   for (int ks = 0; ks < kBlockK / 32; ++ks) {
-    const uint64_t adesc = make_sdesc_sw128(a_base + ks * 32);
+    const uint64_t adesc = sdesc_from_lo(a_lo + ((ks * 32) >> 4));
 #pragma unroll
     for (int u = 0; u < P; ++u) {
       if (u < P - t) {
         const uint32_t acc = (accumulate || ks != 0) ? 1u : 0u;
         const uint32_t d = tmem_base + (t + u) * NT;
-        const uint64_t bdesc = make_sdesc_sw128(b_base + u * (NT / 2) * kBlockK + ks * 32);
+        const uint64_t bdesc = sdesc_from_lo(b_lo + ((u * (NT / 2) * kBlockK + ks * 32) >> 4));
         const bool first = (u == 0), last = (u == P - t - 1);
         if (first && !last) umma_i8_cg2<1>(d, adesc, bdesc, idesc, acc);
         else if (!first && last) umma_i8_cg2<3>(d, adesc, bdesc, idesc, acc);

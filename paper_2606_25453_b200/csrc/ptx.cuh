@@ -258,4 +258,13 @@ __device__ __forceinline__ uint64_t make_sdesc_sw128(uint32_t smem_addr) {
          (1ull << 46) | (2ull << 61);
 }
 
+// The descriptor above split for cheap per-MMA arithmetic: only the 14-bit address field (low word) changes
+// between the MMAs of a stage, so the issuer keeps the low word of the stage base and adds (bytes >> 4); the
+// operand must stay below 256 KB of shared memory (no carry out of the field), offsets are multiples of 16 B.
+__device__ __forceinline__ uint32_t sdesc_lo(uint32_t smem_addr) { return ((smem_addr & 0x3FFFFu) >> 4) | (1u << 16); }
+__device__ __forceinline__ uint64_t sdesc_from_lo(uint32_t lo) {
+  constexpr uint32_t kHi = (1024u >> 4) | (1u << 14) | (2u << 29);  // SBO 1024 B, version 1, SWIZZLE_128B
+  return (static_cast<uint64_t>(kHi) << 32) | lo;
+}
+
 }  // namespace emu
