@@ -84,6 +84,24 @@ int emugemm_sgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, float
                       const float *A, int64_t lda, const float *B, int64_t ldb, float beta,
                       float *C, int64_t ldc, int p);
 
+/* Strided batched Scheme I ("a batched implementation is possible through a
+ * single interleaved tensor per batch entry"): C_b = alpha*A_b*B_b + beta*C_b for b = 0..batch-1, all of one
+ * shape, X_b = X + b*strideX (strides in elements, >= 0; strideA / strideB = 0 shares one operand; the C_b must
+ * not overlap: strideC >= (m-1)*ldc + n).  Row-major, no transposes.  Every entry is bit-identical to the
+ * single call on it.  The digit planes of all entries are stacked entry-major and ONE fused launch walks
+ * (entry, tile) work items, so many small products fill the machine; entries whose k needs several
+ * overflow-safe chunks (k > emugemm_oz1_chunk_k) run one by one.  Workspace: emugemm_workspace_bytes(
+ * EMUGEMM_OZ1, elem, batch*m, batch*n, k, p).  Limits: batch <= 65535, batch*m and batch*n < 2^31 - 256;
+ * with batch > 1 every stride must keep the entries 16-byte aligned (EMUGEMM_ERR_ALIGNMENT).               */
+int emugemm_dgemm_oz1_strided_batched(emugemm_handle_t h, int64_t batch, int64_t m, int64_t n, int64_t k,
+                                      double alpha, const double *A, int64_t lda, int64_t strideA,
+                                      const double *B, int64_t ldb, int64_t strideB, double beta, double *C,
+                                      int64_t ldc, int64_t strideC, int p);
+int emugemm_sgemm_oz1_strided_batched(emugemm_handle_t h, int64_t batch, int64_t m, int64_t n, int64_t k,
+                                      float alpha, const float *A, int64_t lda, int64_t strideA,
+                                      const float *B, int64_t ldb, int64_t strideB, float beta, float *C,
+                                      int64_t ldc, int64_t strideC, int p);
+
 /* Scheme I complex GEMM by the 4M formulation ("EmuGEMM-I uses the 4M formulation"; SURVEY 8(f)
  * item 3).  A, B, C hold complex128 as (re, im) pairs, strides in complex elements; alpha, beta point to HOST
  * {re, im}.  The four real products run as ONE fused Scheme I GEMM of size 2m x n x 2k on the real embedding

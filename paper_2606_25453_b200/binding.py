@@ -168,6 +168,31 @@ class EmuGemm:
                                                    _i64(self._ld(C_)), _int(p)))
         return C_
 
+    def _batched(self, fn, cvt, elem, A, B, C_, p, alpha, beta):
+        # A: (batch, m, k) or (m, k) shared by all entries; B: (batch, k, n) or (k, n); C_: (batch, m, n).
+        # The last dimension is contiguous, dimension -2 carries the leading dimension, dimension 0 the batch stride.
+        batch, m, n = C_.shape
+        k = A.shape[-1]
+        for X, shp in ((A, (m, k)), (B, (k, n))):
+            if tuple(X.shape[-2:]) != shp or X.stride(-1) != 1 or (X.dim() == 3 and X.shape[0] != batch):
+                raise ValueError("batched operands: A (batch, m, k), B (batch, k, n), C (batch, m, n), last dimension contiguous")
+        if C_.stride(-1) != 1:
+            raise ValueError("C must be contiguous in its last dimension")
+        sa = A.stride(0) if A.dim() == 3 else 0
+        sb = B.stride(0) if B.dim() == 3 else 0
+        self._reserve_for(OZ1, elem, batch * m, batch * n, k, p)
+        self._check(fn(self._h, _i64(batch), _i64(m), _i64(n), _i64(k), cvt(alpha), _ptr(A), _i64(A.stride(-2)), _i64(sa),
+                       _ptr(B), _i64(B.stride(-2)), _i64(sb), cvt(beta), _ptr(C_), _i64(C_.stride(-2)), _i64(C_.stride(0)),
+                       _int(p)))
+        return C_
+
+    def dgemm_oz1_strided_batched(self, A, B, C_, p, alpha=1.0, beta=0.0):
+        """C_[b] = alpha A[b] B[b] + beta C_[b] (float64 CUDA tensors; a 2-D A or B is shared by all entries)."""
+        return self._batched(self._lib.emugemm_dgemm_oz1_strided_batched, _dbl, 8, A, B, C_, p, alpha, beta)
+
+    def sgemm_oz1_strided_batched(self, A, B, C_, p, alpha=1.0, beta=0.0):
+        return self._batched(self._lib.emugemm_sgemm_oz1_strided_batched, _flt, 4, A, B, C_, p, alpha, beta)
+
     def dgemm_oz2(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0, transa=False, transb=False):
         m, n, k = self._dims(A, B, transa, transb)
         self._reserve_for(OZ2, 8, m, n, k, n_moduli)

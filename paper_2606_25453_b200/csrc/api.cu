@@ -135,8 +135,10 @@ static int check_gemm_args(emugemm_ctx *h, int ta, int tb, int64_t m, int64_t n,
 // calls and the pre-decomposed operand path).
 static int oz1_gemm_phase(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t kpad, int p, int bits, const int8_t *SA,
                           const int8_t *SB, const int32_t *eA, const int32_t *eB, double alpha, double beta, void *C,
-                          int64_t ldc, int32_t *dump, int nch, int64_t clen, double *part, unsigned long long *diag) {
+                          int64_t ldc, int32_t *dump, int nch, int64_t clen, double *part, unsigned long long *diag,
+                          int batch = 1, int64_t batch_stride_c = 0) {
   Oz1GemmArgs g;
+  g.batch = batch; g.batch_stride_c = batch_stride_c;
   g.m = m; g.n = n; g.kpad = kpad; g.p = p; g.slice_bits = bits; g.SA = SA; g.SB = SB; g.eA = eA; g.eB = eB;
   g.alpha = alpha; g.beta = beta; g.C = C; g.ldc = ldc; g.cycles = diag;
   const int final_kind = (elem == kF32) ? 1 : 0;
@@ -196,6 +198,62 @@ static int run_oz1(emugemm_ctx *h, int ta, int tb, int elem, int64_t m, int64_t 
   EMU_TRY(oz1_gemm_phase(h, elem, m, n, kpad, p, bits, SA, SB, eA, eB, alpha, beta, C, ldc, dump, nch, clen, part, diag));
   if (n_chunks_out) *n_chunks_out = nch;
   return EMUGEMM_OK;
+}
+
+// Strided batched Scheme I: `batch` independent products of one shape.  The digit
+// planes of all entries are stacked entry-major ([p][batch m][kpad], [p][batch n][kpad]), the pre-pass kernels take
+// the entry from a grid dimension and ONE persistent fused launch walks (entry, tile) work items, so many small
+// products fill the machine.  Entries whose k needs several overflow-safe chunks, and k = 0, run one by one.
+static int run_oz1_batched(emugemm_ctx *h, int elem, int64_t batch, int64_t m, int64_t n, int64_t k, double alpha,
+                           const void *A, int64_t lda, int64_t strideA, const void *B, int64_t ldb, int64_t strideB,
+                           double beta, void *C, int64_t ldc, int64_t strideC, int p) {
+  if (!h || batch < 0 || strideA < 0 || strideB < 0 || strideC < 0) return EMUGEMM_ERR_ARG;
+  EMU_TRY(check_gemm_args(h, 0, 0, m, n, k, A, lda, B, ldb, C, ldc));
+  if (p < 1 || p > (elem == kF32 ? 4 : 8)) return EMUGEMM_ERR_ARG;
+  h->launches = 0;
+  if (batch == 0 || m == 0 || n == 0) return EMUGEMM_OK;
+  const int64_t es = (elem == kF32) ? 4 : 8;
+  if (batch > 1) {
+    if (((strideA * es) | (strideB * es) | (strideC * es)) & 15) return EMUGEMM_ERR_ALIGNMENT;
+    if (strideC < (m - 1) * ldc + n) return EMUGEMM_ERR_ARG;  // the outputs must not overlap (inputs may: stride 0 shares one)
+    if (batch > 65535 || batch * m >= (1LL << 31) - 256 || batch * n >= (1LL << 31) - 256) return EMUGEMM_ERR_ARG;
+  }
+  const int64_t kpad = round_up(k, kBlockK);
+  int64_t clen = 0;
+  const int bits = h->slice_bits;
+  const int nch = k > 0 ? oz1_chunks(p, bits, kpad, 0, &clen) : 0;
+  if (batch == 1 || k == 0 || nch > 1) {
+    int launches = 0;
+    for (int64_t b = 0; b < batch; ++b) {
+      EMU_TRY(run_oz1(h, 0, 0, elem, m, n, k, alpha, static_cast<const char *>(A) + b * strideA * es, lda,
+                      static_cast<const char *>(B) + b * strideB * es, ldb, beta, static_cast<char *>(C) + b * strideC * es, ldc, p,
+                      nullptr, 0, nullptr));
+      launches += h->launches;
+    }
+    h->launches = launches;
+    return EMUGEMM_OK;
+  }
+  EMU_TRY(mark(h, 0));
+  if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
+  const int64_t M = batch * m, N = batch * n;
+  Carver cv(h->ws, h->ws_bytes);  // the layout of a single M x N x k call: emugemm_workspace_bytes(1, elem, batch m, batch n, k, p)
+  auto *diag = cv.take<unsigned long long>(1);
+  auto *mbA = cv.take<unsigned long long>(M);
+  auto *mbB = cv.take<unsigned long long>(N);
+  auto *eA = cv.take<int32_t>(M);
+  auto *eB = cv.take<int32_t>(N);
+  auto *SA = cv.take<int8_t>(static_cast<size_t>(p) * M * kpad);
+  auto *SB = cv.take<int8_t>(static_cast<size_t>(p) * N * kpad);
+  if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+  h->diag = diag;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+  const int nb = static_cast<int>(batch);
+  EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB, nb, strideB));
+  EMU_TRY(launch_oz1_slice(h, elem, 0, m, k, kpad, A, lda, mbA, eA, p, bits, SA, nb, strideA));
+  EMU_TRY(launch_oz1_slice(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, p, bits, SB, nb, strideB));
+  EMU_TRY(mark(h, 1));
+  return oz1_gemm_phase(h, elem, m, n, kpad, p, bits, SA, SB, eA, eB, alpha, beta, C, ldc, nullptr, 1, clen, nullptr, diag, nb,
+                        strideC * es);
 }
 
 // Per-modulus GEMMs with fused reduction + CRT from residue planes (one-shot calls and pre-decomposed operands).
@@ -460,6 +518,17 @@ int emugemm_dgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, doubl
 int emugemm_sgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, float alpha, const float *A, int64_t lda,
                       const float *B, int64_t ldb, float beta, float *C, int64_t ldc, int p) {
   return emugemm_sgemm_oz1_t(h, 0, 0, m, n, k, alpha, A, lda, B, ldb, beta, C, ldc, p);
+}
+
+int emugemm_dgemm_oz1_strided_batched(emugemm_handle_t h, int64_t batch, int64_t m, int64_t n, int64_t k, double alpha,
+                                      const double *A, int64_t lda, int64_t strideA, const double *B, int64_t ldb,
+                                      int64_t strideB, double beta, double *C, int64_t ldc, int64_t strideC, int p) {
+  return run_oz1_batched(h, kF64, batch, m, n, k, alpha, A, lda, strideA, B, ldb, strideB, beta, C, ldc, strideC, p);
+}
+int emugemm_sgemm_oz1_strided_batched(emugemm_handle_t h, int64_t batch, int64_t m, int64_t n, int64_t k, float alpha,
+                                      const float *A, int64_t lda, int64_t strideA, const float *B, int64_t ldb,
+                                      int64_t strideB, float beta, float *C, int64_t ldc, int64_t strideC, int p) {
+  return run_oz1_batched(h, kF32, batch, m, n, k, alpha, A, lda, strideA, B, ldb, strideB, beta, C, ldc, strideC, p);
 }
 
 int emugemm_dgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,

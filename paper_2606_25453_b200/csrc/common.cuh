@@ -68,15 +68,17 @@ int launch_exponent_scan(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, 
                          int64_t ldx, unsigned long long *maxbits, int32_t *e_out);
 
 // Column maxima (|x| bit patterns) of X (k x rows): the input of the by_cols = 1 plane kernels.
+// batch > 1 (strided batched calls): entry b of X starts b * xstride elements further, its maxima are
+// maxbits[b rows .. (b + 1) rows).
 int launch_colmax(emugemm_ctx *ctx, int elem, int64_t rows, int64_t k, const void *X, int64_t ldx,
-                  unsigned long long *maxbits);
+                  unsigned long long *maxbits, int batch = 1, int64_t xstride = 0);
 
 // Scheme I slicing: out[p][rows][kpad] int8 (zero padded to kpad) AND the exponents e[rows] (output).
 // by_cols = 0: one fused kernel scans each row and slices it (maxbits unused); by_cols = 1: maxbits[rows] from
 // launch_colmax, the kernel derives and publishes the exponents.
 int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
                      const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int p, int slice_bits,
-                     int8_t *out);
+                     int8_t *out, int batch = 1, int64_t xstride = 0);  // batch: out[p][batch rows][kpad], e[batch rows]
 
 // Scheme II residues: elem 8: out[N][rows][kpad]; elem 16: out[3][N][rows][kpad] (re, im, Sigma); e as above.
 int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
@@ -96,6 +98,8 @@ struct Oz1GemmArgs {
   int slice_bits;              // 7 or 8 (weights 2^(bits (p-1-s)), scaling 2^(eA + eB - bits (p+1) [+ 4 guard bits]))
   const int8_t *SA, *SB;       // [p][m][kpad], [p][n][kpad]
   const int32_t *eA, *eB;
+  int batch = 1;               // strided batched call: planes / exponents hold batch * m (n) rows, entry-major
+  int64_t batch_stride_c = 0;  // bytes between the C matrices of consecutive entries
   int out_kind;                // 0: final FP64 C, 1: final FP32 C, 2: INT32 dump [p][m][n], 3: double-double partial [m][n][2]
   double alpha, beta;
   void *C;

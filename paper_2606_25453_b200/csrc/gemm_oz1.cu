@@ -159,6 +159,8 @@ struct Oz1Dev {
   int chunk_kb, nch;  // overflow-safe k-chunks of chunk_kb k-blocks each: a work item is (chunk, tile)
   int64_t chunk_stride;  // bytes between the outputs of consecutive chunks (OUT = 2 dump, OUT = 3 partials)
   int mt, nt_tiles;   // tile grid
+  int nbatch;         // strided batched call: entry b uses plane rows [b m, (b+1) m) / [b n, (b+1) n), exponents likewise
+  int64_t batch_stride_c;  // bytes between the C matrices of consecutive entries
   const int32_t *eA, *eB;
   int out_kind;
   double alpha, beta;
@@ -199,9 +201,13 @@ struct Oz1Epi {
   long long bias[NG];     // exponent-bias constants per group
   double unb[NG];
   int e_off;              // exponent of the scaling besides eA_i + eB_j
-  __device__ __forceinline__ void init(const Oz1Dev &a) {
+  // vector access flags of the current work item (its C and column exponents may start anywhere in a batch)
+  __device__ __forceinline__ void set_item(const Oz1Dev &a) {
     vec_c = (a.ldc % 4 == 0) && ((reinterpret_cast<uintptr_t>(a.C) & 31) == 0);
     vec_e = (reinterpret_cast<uintptr_t>(a.eB) & 15) == 0;
+  }
+  __device__ __forceinline__ void init(const Oz1Dev &a) {
+    set_item(a);
     const int bits = a.slice_bits;
     w1 = 1 << bits;
     w2 = 1 << (2 * bits);
@@ -342,7 +348,8 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const int num_tiles = a.mt * a.nt_tiles;
-  const int num_items = num_tiles * a.nch;  // chunk-major: consecutive items share the k-range of their operands
+  const int per_entry = num_tiles * a.nch;  // chunk-major: consecutive items share the k-range of their operands
+  const int num_items = per_entry * a.nbatch;  // entry-major: item = (batch entry, chunk, tile)
   // PAIR: the two CTAs of a cluster work on one 256-row tile; rank 0 (leader) issues the MMAs for both
   static_assert(!(PAIR && MC), "pairs already share operands");
   constexpr bool CL2 = PAIR || MC;  // launched as clusters of 2
@@ -381,22 +388,24 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       // 8192^3 p = 8 launch), EVICT_FIRST on B raises them to 21.9 GB
       constexpr uint64_t polA = kEvictNormal, polB = kEvictNormal;
       for (int item = work_id; item < num_items; item += num_workers) {
-        const int chunk = item / num_tiles, tile = item - chunk * num_tiles;
+        const int bidx = item / per_entry, rem = item - bidx * per_entry;
+        const int chunk = rem / num_tiles, tile = rem - chunk * num_tiles;
         const int kb0 = a.kb0 + chunk * a.chunk_kb, kb1 = (kb0 + a.chunk_kb < a.kb1) ? kb0 + a.chunk_kb : a.kb1;
         int mb, nb;
         tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
         if constexpr (MC) nb = 2 * nb + static_cast<int>(cta);  // a.nt_tiles counts PAIRS of N-tiles
+        const int rowA0 = static_cast<int>(bidx * a.m), rowB0 = static_cast<int>(bidx * a.n);  // this entry's plane rows
         for (int kb = kb0; kb < kb1; ++kb) {
           mbar_wait(&bempty[sb], pb ^ 1);
           if constexpr (PAIR) {
             if (cta == 0) mbar_arrive_expect_tx(&bfull[sb], kTxMul * Cfg::kBStageBytes);
             tma_load_3d_cg2(sB + sb * Cfg::kBStageBytes, &tmB, mapa_u32(&bfull[sb], 0), kb * kBlockK,
-                            nb * NT + static_cast<int>(cta) * Cfg::kBRows, 0, polB);
+                            rowB0 + nb * NT + static_cast<int>(cta) * Cfg::kBRows, 0, polB);
           } else if ((a.dbg & 1) && nloadb >= SB) {
             mbar_arrive(&bfull[sb]);
           } else {
             mbar_arrive_expect_tx(&bfull[sb], Cfg::kBStageBytes);
-            tma_load_3d(sB + sb * Cfg::kBStageBytes, &tmB, &bfull[sb], kb * kBlockK, nb * NT, 0, polB);
+            tma_load_3d(sB + sb * Cfg::kBStageBytes, &tmB, &bfull[sb], kb * kBlockK, rowB0 + nb * NT, 0, polB);
           }
           ++nloadb;
           if (++sb == SB) { sb = 0; pb ^= 1; }
@@ -407,14 +416,14 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             uint8_t *dst = sA + sa * Cfg::kAPairBytes;
             if constexpr (PAIR) {
               const uint32_t bar = mapa_u32(&afull[sa], 0);
-              const int arow = mb * kTileRows + static_cast<int>(cta) * kTileM;
+              const int arow = rowA0 + mb * kTileRows + static_cast<int>(cta) * kTileM;
               if (cta == 0) mbar_arrive_expect_tx(&afull[sa], kTxMul * (lo == hi ? kAStageBytes : Cfg::kAPairBytes));
               tma_load_3d_cg2(dst, &tmA, bar, kb * kBlockK, arow, lo, polA);
               if (hi != lo) tma_load_3d_cg2(dst + kAStageBytes, &tmA, bar, kb * kBlockK, arow, hi, polA);
             } else if constexpr (MC) {
               // this CTA fetches rows [64 cta, 64 cta + 64) of both slices and multicasts them to the pair
               constexpr int kHalf = kAStageBytes / 2;
-              const int arow = mb * kTileM + static_cast<int>(cta) * (kTileM / 2);
+              const int arow = rowA0 + mb * kTileM + static_cast<int>(cta) * (kTileM / 2);
               mbar_arrive_expect_tx(&afull[sa], lo == hi ? kAStageBytes : Cfg::kAPairBytes);
               tma_load_3d_mc(dst + cta * kHalf, &tmA, &afull[sa], kb * kBlockK, arow, lo, 3, polA);
               if (hi != lo) tma_load_3d_mc(dst + kAStageBytes + cta * kHalf, &tmA, &afull[sa], kb * kBlockK, arow, hi, 3, polA);
@@ -422,8 +431,8 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
               mbar_arrive(&afull[sa]);
             } else {
               mbar_arrive_expect_tx(&afull[sa], lo == hi ? kAStageBytes : Cfg::kAPairBytes);
-              tma_load_3d(dst, &tmA, &afull[sa], kb * kBlockK, mb * kTileM, lo, polA);
-              if (hi != lo) tma_load_3d(dst + kAStageBytes, &tmA, &afull[sa], kb * kBlockK, mb * kTileM, hi, polA);
+              tma_load_3d(dst, &tmA, &afull[sa], kb * kBlockK, rowA0 + mb * kTileM, lo, polA);
+              if (hi != lo) tma_load_3d(dst + kAStageBytes, &tmA, &afull[sa], kb * kBlockK, rowA0 + mb * kTileM, hi, polA);
             }
             ++nloada;
             if (++sa == SA) { sa = 0; pa ^= 1; }
@@ -441,7 +450,8 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       // issued, so the ~90-cycle try_wait latency overlaps tensor work instead of draining the MMA queue
       bool a_ready = false, b_ready = false;
       for (int item = work_id; item < num_items; item += num_workers) {
-        const int chunk = item / num_tiles, tile = item - chunk * num_tiles;
+        const int bidx = item / per_entry, rem = item - bidx * per_entry;
+        const int chunk = rem / num_tiles, tile = rem - chunk * num_tiles;
         const int kb0 = a.kb0 + chunk * a.chunk_kb, kb1 = (kb0 + a.chunk_kb < a.kb1) ? kb0 + a.chunk_kb : a.kb1;
         mbar_wait(tempty, pt ^ 1);  // epilogue has drained the accumulators of the previous tile
         tc_fence_after();
@@ -493,17 +503,21 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     constexpr bool kDoubleBuffer = (P <= 6);  // two register sets of P x 8 accumulator values fit without spilling
     Oz1Dev ac = a;  // per-item copy: the output of chunk c starts c * chunk_stride bytes further
     for (int item = work_id; item < num_items; item += num_workers) {
-      const int chunk = item / num_tiles, tile = item - chunk * num_tiles;
-      ac.C = static_cast<char *>(a.C) + chunk * a.chunk_stride;
+      const int bidx = item / per_entry, rem = item - bidx * per_entry;
+      const int chunk = rem / num_tiles, tile = rem - chunk * num_tiles;
+      ac.C = static_cast<char *>(a.C) + chunk * a.chunk_stride + bidx * a.batch_stride_c;
+      ac.eA = a.eA + bidx * a.m;
+      ac.eB = a.eB + bidx * a.n;
+      epi.set_item(ac);
       int mb, nb;
       tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
       if constexpr (MC) nb = 2 * nb + static_cast<int>(cta);
       const int64_t grow = static_cast<int64_t>(mb) * kTileRows + (PAIR ? cta * kTileM : 0u) + row;
       const bool row_ok = grow < a.m;
-      const int eArow = row_ok ? __ldg(a.eA + grow) + epi.e_off : 0;
+      const int eArow = row_ok ? __ldg(ac.eA + grow) + epi.e_off : 0;
       const int64_t gcol0 = static_cast<int64_t>(nb) * NT + half * (NT / 2);
       int ea[8], eb[8];
-      epi.load_eb(a, gcol0, ea);  // first chunk's column exponents: in flight while the tile's MMAs finish
+      epi.load_eb(ac, gcol0, ea);  // first chunk's column exponents: in flight while the tile's MMAs finish
       mbar_wait(tfull, pt);
       tc_fence_after();
       if (!(a.dbg & 2)) {
@@ -520,7 +534,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             if (i + 1 < kChunks) {
 #pragma unroll
               for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + (i + 1) * 8, vb[s]);
-              epi.load_eb(a, gcol0 + (i + 1) * 8, eb);
+              epi.load_eb(ac, gcol0 + (i + 1) * 8, eb);
             }
             epi.chunk(ac, va, ea, grow, row_ok, eArow, gcol0 + i * 8);
             if (i + 1 < kChunks) {
@@ -528,7 +542,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
               if (i + 2 < kChunks) {
 #pragma unroll
                 for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + (i + 2) * 8, va[s]);
-                epi.load_eb(a, gcol0 + (i + 2) * 8, ea);
+                epi.load_eb(ac, gcol0 + (i + 2) * 8, ea);
               }
               epi.chunk(ac, vb, eb, grow, row_ok, eArow, gcol0 + (i + 1) * 8);
             }
@@ -540,13 +554,13 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
           for (int i = 0; i < kChunks; i += 2) {
 #pragma unroll
             for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + i * 8, v[s]);
-            if (i + 1 < kChunks) epi.load_eb(a, gcol0 + (i + 1) * 8, eb);
+            if (i + 1 < kChunks) epi.load_eb(ac, gcol0 + (i + 1) * 8, eb);
             tmem_ld_wait();
             epi.chunk(ac, v, ea, grow, row_ok, eArow, gcol0 + i * 8);
             if (i + 1 < kChunks) {
 #pragma unroll
               for (int s = 0; s < P; ++s) tmem_ld8(tcol + s * NT + (i + 1) * 8, v[s]);
-              if (i + 2 < kChunks) epi.load_eb(a, gcol0 + (i + 2) * 8, ea);
+              if (i + 2 < kChunks) epi.load_eb(ac, gcol0 + (i + 2) * 8, ea);
               tmem_ld_wait();
               epi.chunk(ac, v, eb, grow, row_ok, eArow, gcol0 + (i + 1) * 8);
             }
@@ -579,8 +593,10 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   using Cfg = Oz1Cfg<P, PAIR>;
   constexpr int kTileRows = PAIR ? 2 * kTileM : kTileM;
   CUtensorMap tmA, tmB;
-  EMU_TRY(encode_planes_tmap(ctx, &tmA, g.SA, g.kpad, g.m, P, MC ? kTileM / 2 : kTileM, 1));
-  EMU_TRY(encode_planes_tmap(ctx, &tmB, g.SB, g.kpad, g.n, P, Cfg::kBRows, P));
+  const int batch = g.batch > 0 ? g.batch : 1;
+  if (batch > 1 && g.n_chunks > 1) return EMUGEMM_ERR_ARG;  // the API runs chunked entries one by one
+  EMU_TRY(encode_planes_tmap(ctx, &tmA, g.SA, g.kpad, g.m * batch, P, MC ? kTileM / 2 : kTileM, 1));
+  EMU_TRY(encode_planes_tmap(ctx, &tmB, g.SB, g.kpad, g.n * batch, P, Cfg::kBRows, P));
   Oz1Dev d;
   d.m = g.m; d.n = g.n;
   d.kb0 = static_cast<int>(g.k0 / kBlockK);
@@ -591,13 +607,15 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   d.mt = static_cast<int>((g.m + kTileRows - 1) / kTileRows);
   d.nt_tiles = static_cast<int>((g.n + Cfg::NT - 1) / Cfg::NT);
   if (MC) d.nt_tiles = (d.nt_tiles + 1) / 2;  // pairs of N-adjacent tiles, one per CTA of the cluster
+  d.nbatch = batch; d.batch_stride_c = g.batch_stride_c;
   d.eA = g.eA; d.eB = g.eB;
   d.out_kind = g.out_kind; d.alpha = g.alpha; d.beta = g.beta; d.C = g.C; d.ldc = g.ldc;
   d.cycles = g.cycles;
   d.slice_bits = g.slice_bits;
   d.dbg = ctx->dbg_flags;
   constexpr bool CL2 = PAIR || MC;
-  const int64_t tiles = static_cast<int64_t>(d.mt) * d.nt_tiles * d.nch;
+  const int64_t tiles = static_cast<int64_t>(d.mt) * d.nt_tiles * d.nch * batch;
+  if (tiles >= (1LL << 31)) return EMUGEMM_ERR_ARG;
   const int workers = CL2 ? ctx->num_sms / 2 : ctx->num_sms;
   const int grid = (CL2 ? 2 : 1) * static_cast<int>(tiles < workers ? tiles : workers);
   void (*kern)(CUtensorMap, CUtensorMap, Oz1Dev) = nullptr;

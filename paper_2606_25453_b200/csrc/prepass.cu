@@ -70,9 +70,12 @@ __global__ void __launch_bounds__(256) rowmax_kernel(const T *__restrict__ X, in
 // X is k x rows (ldx), one thread per column, grid.y splits k; atomicMax merges.
 template <typename T, int W>
 __global__ void __launch_bounds__(256) colmax_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows, int64_t k,
-                                                     int64_t kseg, unsigned long long *__restrict__ maxbits) {
+                                                     int64_t kseg, unsigned long long *__restrict__ maxbits,
+                                                     int64_t xstride) {
   const int64_t j = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
   if (j >= rows) return;
+  X += static_cast<int64_t>(blockIdx.z) * xstride * W;  // batch entry (strided batched calls)
+  maxbits += static_cast<int64_t>(blockIdx.z) * rows;
   const int64_t h0 = static_cast<int64_t>(blockIdx.y) * kseg;
   const int64_t h1 = (h0 + kseg < k) ? h0 + kseg : k;
   unsigned long long mx = 0;
@@ -108,22 +111,22 @@ __global__ void bits_to_exponent_kernel(const unsigned long long *__restrict__ m
 // Column maxima of X (k x rows, ldx) as |x| bit patterns -> maxbits[rows] (zeroed here); the column kernels turn them
 // into exponents.
 int launch_colmax(emugemm_ctx *ctx, int elem, int64_t rows, int64_t k, const void *X, int64_t ldx,
-                  unsigned long long *maxbits) {
-  if (rows == 0) return EMUGEMM_OK;
+                  unsigned long long *maxbits, int batch, int64_t xstride) {
+  if (rows == 0 || batch == 0) return EMUGEMM_OK;
   cudaStream_t st = ctx->stream;
-  EMU_CUDA(ctx, cudaMemsetAsync(maxbits, 0, sizeof(unsigned long long) * rows, st));
+  EMU_CUDA(ctx, cudaMemsetAsync(maxbits, 0, sizeof(unsigned long long) * rows * batch, st));
   if (k == 0) return EMUGEMM_OK;
   // enough k-segments to fill the machine: ~8 CTAs per SM
   const int64_t gx = (rows + 255) / 256;
-  int64_t segs = (static_cast<int64_t>(ctx->num_sms) * 8 + gx - 1) / gx;
+  int64_t segs = (static_cast<int64_t>(ctx->num_sms) * 8 + gx * batch - 1) / (gx * batch);
   if (segs > (k + 63) / 64) segs = (k + 63) / 64;
   if (segs < 1) segs = 1;
   const int64_t kseg = (k + segs - 1) / segs;
-  const dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>((k + kseg - 1) / kseg));
-  if (elem == kF64) colmax_kernel<double, 1><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits);
-  else if (elem == kF32) colmax_kernel<float, 1><<<grid, 256, 0, st>>>(static_cast<const float *>(X), ldx, rows, k, kseg, maxbits);
-  else if (elem == kC64) colmax_kernel<float, 2><<<grid, 256, 0, st>>>(static_cast<const float *>(X), ldx, rows, k, kseg, maxbits);
-  else colmax_kernel<double, 2><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits);
+  const dim3 grid(static_cast<unsigned>(gx), static_cast<unsigned>((k + kseg - 1) / kseg), static_cast<unsigned>(batch));
+  if (elem == kF64) colmax_kernel<double, 1><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits, xstride);
+  else if (elem == kF32) colmax_kernel<float, 1><<<grid, 256, 0, st>>>(static_cast<const float *>(X), ldx, rows, k, kseg, maxbits, xstride);
+  else if (elem == kC64) colmax_kernel<float, 2><<<grid, 256, 0, st>>>(static_cast<const float *>(X), ldx, rows, k, kseg, maxbits, xstride);
+  else colmax_kernel<double, 2><<<grid, 256, 0, st>>>(static_cast<const double *>(X), ldx, rows, k, kseg, maxbits, xstride);
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
   return EMUGEMM_OK;
@@ -359,9 +362,12 @@ __device__ __forceinline__ void emit_quad(const T (&v)[4][W], int e_row, int par
 template <typename T, int W, int MODE, int PARAM>
 __global__ void __launch_bounds__(256) planes_rows_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows,
                                                           int64_t k, int64_t kpad, int32_t *__restrict__ e_out,
-                                                          int param, int scale_bits, int8_t *__restrict__ out) {
-  const int64_t row = blockIdx.x;
-  const T *src = X + row * ldx * W;
+                                                          int param, int scale_bits, int8_t *__restrict__ out,
+                                                          int64_t xstride, int64_t plane_rows) {
+  // batch entry b = blockIdx.y (strided batched calls: entry b of X starts xstride elements further; its planes are
+  // rows [b rows, (b + 1) rows) of planes that hold plane_rows rows)
+  const int64_t row = static_cast<int64_t>(blockIdx.y) * rows + blockIdx.x;
+  const T *src = X + (static_cast<int64_t>(blockIdx.y) * xstride + static_cast<int64_t>(blockIdx.x) * ldx) * W;
   unsigned long long mx = 0;
   for (int64_t h = static_cast<int64_t>(threadIdx.x) * 4; h < k; h += 1024) {
 #pragma unroll
@@ -385,7 +391,7 @@ __global__ void __launch_bounds__(256) planes_rows_kernel(const T *__restrict__ 
   const int e_row = exponent_of_maxbits<T>(mx);
   if (threadIdx.x == 0) e_out[row] = e_row;
 
-  const int64_t plane_stride = rows * kpad;
+  const int64_t plane_stride = plane_rows * kpad;
   for (int64_t h0 = static_cast<int64_t>(threadIdx.x) * 4; h0 < kpad; h0 += 1024) {
     T v[4][W];
 #pragma unroll
@@ -406,8 +412,13 @@ __global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ 
                                                           int64_t k, int64_t kpad,
                                                           const unsigned long long *__restrict__ maxbits,
                                                           int32_t *__restrict__ e_out, int param, int scale_bits, int nplanes,
-                                                          int8_t *__restrict__ out) {
+                                                          int8_t *__restrict__ out, int64_t xstride, int64_t plane_rows) {
   extern __shared__ unsigned int tile[];  // [plane][32][TH/4 + 1]
+  // batch entry blockIdx.z (see planes_rows_kernel)
+  X += static_cast<int64_t>(blockIdx.z) * xstride * W;
+  maxbits += static_cast<int64_t>(blockIdx.z) * rows;
+  e_out += static_cast<int64_t>(blockIdx.z) * rows;
+  out += static_cast<int64_t>(blockIdx.z) * rows * kpad;
   constexpr int PW = TH / 4 + 1;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t j = static_cast<int64_t>(blockIdx.x) * 32 + lane;
@@ -436,7 +447,7 @@ __global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ 
     const int64_t jg = static_cast<int64_t>(blockIdx.x) * 32 + jj;
     if (jg < rows) {
       const int wd = lane % LPR;
-      *reinterpret_cast<unsigned int *>(out + (static_cast<int64_t>(plane) * rows + jg) * kpad + hb + wd * 4) =
+      *reinterpret_cast<unsigned int *>(out + (static_cast<int64_t>(plane) * plane_rows + jg) * kpad + hb + wd * 4) =
           tile[(plane * 32 + jj) * PW + wd];
     }
   }
@@ -447,13 +458,16 @@ __global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ 
 template <typename T, int W, int MODE, int PARAM>
 static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X,
                          int64_t ldx, const unsigned long long *maxbits, int32_t *e, int param, int scale_bits, int nplanes,
-                         int8_t *out) {
-  if (rows == 0 || kpad == 0) return EMUGEMM_OK;
+                         int8_t *out, int batch = 1, int64_t xstride = 0) {
+  if (rows == 0 || kpad == 0 || batch == 0) return EMUGEMM_OK;
+  if (batch > 65535) return EMUGEMM_ERR_ARG;  // grid.y / grid.z
+  const int64_t plane_rows = rows * batch;
   cudaStream_t st = ctx->stream;
   const T *x = static_cast<const T *>(X);
   if (!by_cols) {
-    planes_rows_kernel<T, W, MODE, PARAM><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, param,
-                                                                                        scale_bits, out);
+    const dim3 grid(static_cast<unsigned>(rows), static_cast<unsigned>(batch));
+    planes_rows_kernel<T, W, MODE, PARAM><<<grid, 256, 0, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, out, xstride,
+                                                                 plane_rows);
     ctx->launches++;
   } else {
     if (nplanes <= 20) {
@@ -461,15 +475,15 @@ static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k,
       const size_t smem = static_cast<size_t>(nplanes) * 32 * (TH / 4 + 1) * 4;
       auto kern = planes_cols_kernel<T, W, MODE, PARAM, TH>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 20 * 32 * (TH / 4 + 1) * 4));
-      const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH));
-      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, param, scale_bits, nplanes, out);
+      const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH), static_cast<unsigned>(batch));
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, param, scale_bits, nplanes, out, xstride, plane_rows);
     } else {
       constexpr int TH = 32;
       const size_t smem = static_cast<size_t>(nplanes) * 32 * (TH / 4 + 1) * 4;
       auto kern = planes_cols_kernel<T, W, MODE, PARAM, TH>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 60 * 32 * (TH / 4 + 1) * 4));
-      const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH));
-      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, param, scale_bits, nplanes, out);
+      const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH), static_cast<unsigned>(batch));
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, param, scale_bits, nplanes, out, xstride, plane_rows);
     }
     ctx->launches++;
   }
@@ -479,16 +493,16 @@ static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k,
 
 template <typename T, int P>
 static int slice_p(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
-                   const unsigned long long *maxbits, int32_t *e, int slice_bits, int8_t *out) {
+                   const unsigned long long *maxbits, int32_t *e, int slice_bits, int8_t *out, int batch, int64_t xstride) {
   if (slice_bits == 8)  // |X| = trunc(|x| 2^(8p - 2 - e)): two guard bits
-    return launch_planes<T, 1, 0, 16 + P>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, 8 * P - 2, P, out);
-  return launch_planes<T, 1, 0, P>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, kBeta * P, P, out);
+    return launch_planes<T, 1, 0, 16 + P>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, 8 * P - 2, P, out, batch, xstride);
+  return launch_planes<T, 1, 0, P>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, kBeta * P, P, out, batch, xstride);
 }
 
 int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
                      const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int p, int slice_bits,
-                     int8_t *out) {
-#define EMU_SLICE_CASE(T, PP) case PP: return slice_p<T, PP>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out)
+                     int8_t *out, int batch, int64_t xstride) {
+#define EMU_SLICE_CASE(T, PP) case PP: return slice_p<T, PP>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out, batch, xstride)
   if (elem == kF64) {
     switch (p) {
       EMU_SLICE_CASE(double, 1); EMU_SLICE_CASE(double, 2); EMU_SLICE_CASE(double, 3); EMU_SLICE_CASE(double, 4);
