@@ -101,3 +101,58 @@ def test_random_complex(env, case):
     got = Cd.cpu().numpy()
     assert_within_ulps(got.real, want.real, scale, 2, what=what + " re")
     assert_within_ulps(got.imag, want.imag, scale, 2, what=what + " im")
+
+
+@pytest.mark.parametrize("case", range(12))
+def test_random_batched(env, case):
+    """strided batched Scheme I: random shapes (sizes that keep every entry 16-byte aligned), counts, digit formats,
+    batch strides with slack, optionally one shared operand."""
+    torch, O, h = env
+    rng = np.random.default_rng(7000 + case)
+    f32 = bool(case % 3 == 2)
+    q = 4 if f32 else 2                                   # elements per 16 bytes
+    m, n, k = (int(rng.choice([2, 8, 30, 64, 66, 128, 130, 160, 258])) for _ in range(3))
+    batch = int(rng.integers(2, 7))
+    p = int(rng.integers(1, 5 if f32 else 9))
+    bits = 8 if rng.integers(0, 2) else 7
+    share_b = bool(rng.integers(0, 2))
+    use_beta = bool(rng.integers(0, 2))
+    alpha = float(rng.choice([1.0, -1.5, 0.25]))
+    beta = float(rng.choice([0.75, -2.0])) if use_beta else 0.0
+    dt = np.float32 if f32 else np.float64
+    tdt = torch.float32 if f32 else torch.float64
+    A = np.stack([G.real_pair(m, n, k, 1.0, 10 * case + b, dtype=dt)[0] for b in range(batch)])
+    Bs = [G.real_pair(m, n, k, 1.0, 500 + 10 * case + b, dtype=dt)[1] for b in range(1 if share_b else batch)]
+    Cin = np.random.default_rng(case).standard_normal((batch, m, n)).astype(dt)
+    rows_pad, pad = int(rng.integers(0, 3)), q * int(rng.integers(0, 3))   # slack rows between entries, ld slack
+    Ab = torch.zeros((batch, m + rows_pad, k + pad), dtype=tdt, device="cuda")
+    Ab[:, :m, :k] = torch.from_numpy(A).cuda()
+    if share_b:
+        Bb = torch.zeros((k, n + pad), dtype=tdt, device="cuda")
+        Bb[:, :n] = torch.from_numpy(Bs[0]).cuda()
+        Bv = Bb[:, :n]
+    else:
+        Bb = torch.zeros((batch, k + rows_pad, n + pad), dtype=tdt, device="cuda")
+        Bb[:, :k, :n] = torch.from_numpy(np.stack(Bs)).cuda()
+        Bv = Bb[:, :k, :n]
+    Cb = torch.zeros((batch, m + rows_pad, n + pad), dtype=tdt, device="cuda")
+    Cb[:, :m, :n] = torch.from_numpy(Cin).cuda()
+    for t in (Ab, Bb, Cb):   # entries must stay 16-byte aligned: skip draws whose batch stride is not
+        if t.dim() == 3 and (t.stride(0) * t.element_size()) % 16:
+            pytest.skip("batch stride not 16-byte aligned for this draw")
+    h.set_slice_bits(bits)
+    O.set_slice_bits(bits)
+    try:
+        call = h.sgemm_oz1_strided_batched if f32 else h.dgemm_oz1_strided_batched
+        call(Ab[:, :m, :k], Bv, Cb[:, :m, :n], p, alpha=alpha, beta=beta)
+        got = Cb.cpu().numpy()
+        for b in range(batch):
+            Bm = Bs[0] if share_b else Bs[b]
+            _, absAB = O.bf128_dgemm(A[b].astype(np.float64), Bm.astype(np.float64))
+            ref = (O.sgemm_oz1 if f32 else O.dgemm_oz1)(A[b], Bm, p, alpha=alpha, beta=beta, Cin=Cin[b] if use_beta else None)
+            scale = abs(alpha) * absAB + abs(beta) * np.abs(Cin[b].astype(np.float64))
+            assert_within_ulps(got[b, :m, :n], ref, scale, 2, bits=23 if f32 else 52,
+                               what=f"case {case} entry {b} {m}x{n}x{k} p={p} bits={bits} f32={f32}")
+    finally:
+        h.set_slice_bits(7)
+        O.set_slice_bits(7)
