@@ -168,7 +168,7 @@ class EmuGemm:
                                                    _i64(self._ld(C_)), _int(p)))
         return C_
 
-    def _batched(self, fn, cvt, elem, A, B, C_, p, alpha, beta):
+    def _batched(self, fn, cvt, elem, A, B, C_, p, alpha, beta, scheme=OZ1):
         # A: (batch, m, k) or (m, k) shared by all entries; B: (batch, k, n) or (k, n); C_: (batch, m, n).
         # The last dimension is contiguous, dimension -2 carries the leading dimension, dimension 0 the batch stride.
         batch, m, n = C_.shape
@@ -180,7 +180,7 @@ class EmuGemm:
             raise ValueError("C must be contiguous in its last dimension")
         sa = A.stride(0) if A.dim() == 3 else 0
         sb = B.stride(0) if B.dim() == 3 else 0
-        self._reserve_for(OZ1, elem, batch * m, batch * n, k, p)
+        self._reserve_for(scheme, elem, batch * m, batch * n, k, p)
         self._check(fn(self._h, _i64(batch), _i64(m), _i64(n), _i64(k), cvt(alpha), _ptr(A), _i64(A.stride(-2)), _i64(sa),
                        _ptr(B), _i64(B.stride(-2)), _i64(sb), cvt(beta), _ptr(C_), _i64(C_.stride(-2)), _i64(C_.stride(0)),
                        _int(p)))
@@ -192,6 +192,12 @@ class EmuGemm:
 
     def sgemm_oz1_strided_batched(self, A, B, C_, p, alpha=1.0, beta=0.0):
         return self._batched(self._lib.emugemm_sgemm_oz1_strided_batched, _flt, 4, A, B, C_, p, alpha, beta)
+
+    def dgemm_oz2_strided_batched(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0):
+        return self._batched(self._lib.emugemm_dgemm_oz2_strided_batched, _dbl, 8, A, B, C_, n_moduli, alpha, beta, OZ2)
+
+    def sgemm_oz2_strided_batched(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0):
+        return self._batched(self._lib.emugemm_sgemm_oz2_strided_batched, _flt, 4, A, B, C_, n_moduli, alpha, beta, OZ2)
 
     def dgemm_oz2(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0, transa=False, transb=False):
         m, n, k = self._dims(A, B, transa, transb)

@@ -260,15 +260,16 @@ static int run_oz1_batched(emugemm_ctx *h, int elem, int64_t batch, int64_t m, i
 static int oz2_gemm_phase(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_t kpad, int N, const int8_t *RA,
                           const int8_t *RB, int8_t *CR, const int32_t *eA, const int32_t *eB, int tA, int tB,
                           const double alpha[2], const double beta[2], double *C, int64_t ldc, unsigned long long *diag,
-                          int out_f32 = 0) {
+                          int out_f32 = 0, int batch = 1, int64_t batch_stride_c = 0) {
   Oz2GemmArgs g;
+  g.batch = batch;
   g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = N; g.is3m = is3m; g.RA = RA; g.RB = RB; g.CR = CR; g.cycles = diag;
   EMU_TRY(launch_oz2_gemm(h, g));
   EMU_TRY(mark(h, 2));
   Oz2CrtArgs c;
   c.m = m; c.n = n; c.n_moduli = N; c.CR = CR; c.eA = eA; c.eB = eB; c.tA = tA; c.tB = tB; c.is_complex = is3m; c.out_f32 = out_f32;
   c.alpha[0] = alpha[0]; c.alpha[1] = alpha[1]; c.beta[0] = beta[0]; c.beta[1] = beta[1];
-  c.C = C; c.ldc = ldc;
+  c.C = C; c.ldc = ldc; c.batch = batch; c.batch_stride_c = batch_stride_c;
   EMU_TRY(launch_oz2_crt(h, c));
   EMU_TRY(mark(h, 3));
   return EMUGEMM_OK;
@@ -313,6 +314,64 @@ static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t 
   EMU_TRY(launch_oz2_residues(h, elem, !tb, n, k, kpad, B, ldb, mbB, eB, N, tB, RB));
   EMU_TRY(mark(h, 1));
   return oz2_gemm_phase(h, is3m, m, n, kpad, N, RA, RB, CR, eA, eB, tA, tB, alpha, beta, C, ldc, diag, f32);
+}
+
+// Strided batched Scheme II, real (DGEMM / SGEMM): as run_oz1_batched -- residue planes of all entries stacked
+// entry-major, the pre-pass kernels take the entry from a grid dimension, ONE persistent launch walks
+// (entry, modulus, tile) work items, one CRT launch covers the batch (grid.y = entry).
+static int run_oz2_batched(emugemm_ctx *h, int f32, int64_t batch, int64_t m, int64_t n, int64_t k, double alpha,
+                           const void *A, int64_t lda, int64_t strideA, const void *B, int64_t ldb, int64_t strideB,
+                           double beta, void *C, int64_t ldc, int64_t strideC, int N) {
+  if (!h || batch < 0 || strideA < 0 || strideB < 0 || strideC < 0) return EMUGEMM_ERR_ARG;
+  EMU_TRY(check_gemm_args(h, 0, 0, m, n, k, A, lda, B, ldb, C, ldc));
+  if (N < 2 || N > kMaxModuli) return EMUGEMM_ERR_ARG;
+  h->launches = 0;
+  if (batch == 0 || m == 0 || n == 0) return EMUGEMM_OK;
+  const int elem = f32 ? kF32 : kF64;
+  const int64_t es = f32 ? 4 : 8;
+  const double al[2] = {alpha, 0.0}, be[2] = {beta, 0.0};
+  if (batch > 1) {
+    if (((strideA * es) | (strideB * es) | (strideC * es)) & 15) return EMUGEMM_ERR_ALIGNMENT;
+    if (strideC < (m - 1) * ldc + n) return EMUGEMM_ERR_ARG;
+    if (batch > 65535 || batch * m >= (1LL << 31) - 256 || batch * n >= (1LL << 31) - 256) return EMUGEMM_ERR_ARG;
+  }
+  if (batch == 1 || k == 0) {
+    int launches = 0;
+    for (int64_t b = 0; b < batch; ++b) {
+      EMU_TRY(run_oz2(h, 0, 0, 0, m, n, k, al, static_cast<const char *>(A) + b * strideA * es, lda,
+                      static_cast<const char *>(B) + b * strideB * es, ldb, be,
+                      reinterpret_cast<double *>(static_cast<char *>(C) + b * strideC * es), ldc, N, f32));
+      launches += h->launches;
+    }
+    h->launches = launches;
+    return EMUGEMM_OK;
+  }
+  int tA, tB;
+  if (oz2_budget_host(N, k, 0, &tA, &tB) < 2) return EMUGEMM_ERR_PRECISION;
+  if (k > 131071) return EMUGEMM_ERR_PRECISION;
+  EMU_TRY(mark(h, 0));
+  const int64_t kpad = round_up(k, kBlockK);
+  if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
+  const int64_t M = batch * m, NN = batch * n;
+  Carver cv(h->ws, h->ws_bytes);  // the layout of a single (batch m) x (batch n) x k call is an upper bound
+  auto *diag = cv.take<unsigned long long>(1);
+  auto *mbA = cv.take<unsigned long long>(M);
+  auto *mbB = cv.take<unsigned long long>(NN);
+  auto *eA = cv.take<int32_t>(M);
+  auto *eB = cv.take<int32_t>(NN);
+  auto *RA = cv.take<int8_t>(static_cast<size_t>(N) * M * kpad);
+  auto *RB = cv.take<int8_t>(static_cast<size_t>(N) * NN * kpad);
+  auto *CR = cv.take<int8_t>(static_cast<size_t>(N) * M * n);
+  if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
+  h->diag = diag;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+  const int nb = static_cast<int>(batch);
+  EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB, nb, strideB));
+  EMU_TRY(launch_oz2_residues(h, elem, 0, m, k, kpad, A, lda, mbA, eA, N, tA, RA, nb, strideA));
+  EMU_TRY(launch_oz2_residues(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, N, tB, RB, nb, strideB));
+  EMU_TRY(mark(h, 1));
+  return oz2_gemm_phase(h, 0, m, n, kpad, N, RA, RB, CR, eA, eB, tA, tB, al, be, static_cast<double *>(C), ldc, diag, f32, nb,
+                        strideC);
 }
 
 }  // namespace emu
@@ -529,6 +588,17 @@ int emugemm_sgemm_oz1_strided_batched(emugemm_handle_t h, int64_t batch, int64_t
                                       const float *A, int64_t lda, int64_t strideA, const float *B, int64_t ldb,
                                       int64_t strideB, float beta, float *C, int64_t ldc, int64_t strideC, int p) {
   return run_oz1_batched(h, kF32, batch, m, n, k, alpha, A, lda, strideA, B, ldb, strideB, beta, C, ldc, strideC, p);
+}
+
+int emugemm_dgemm_oz2_strided_batched(emugemm_handle_t h, int64_t batch, int64_t m, int64_t n, int64_t k, double alpha,
+                                      const double *A, int64_t lda, int64_t strideA, const double *B, int64_t ldb,
+                                      int64_t strideB, double beta, double *C, int64_t ldc, int64_t strideC, int n_moduli) {
+  return run_oz2_batched(h, 0, batch, m, n, k, alpha, A, lda, strideA, B, ldb, strideB, beta, C, ldc, strideC, n_moduli);
+}
+int emugemm_sgemm_oz2_strided_batched(emugemm_handle_t h, int64_t batch, int64_t m, int64_t n, int64_t k, float alpha,
+                                      const float *A, int64_t lda, int64_t strideA, const float *B, int64_t ldb,
+                                      int64_t strideB, float beta, float *C, int64_t ldc, int64_t strideC, int n_moduli) {
+  return run_oz2_batched(h, 1, batch, m, n, k, alpha, A, lda, strideA, B, ldb, strideB, beta, C, ldc, strideC, n_moduli);
 }
 
 int emugemm_dgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,

@@ -83,7 +83,7 @@ int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int6
 // Scheme II residues: elem 8: out[N][rows][kpad]; elem 16: out[3][N][rows][kpad] (re, im, Sigma); e as above.
 int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
                         const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int n_moduli,
-                        int t_bits, int8_t *out);
+                        int t_bits, int8_t *out, int batch = 1, int64_t xstride = 0);
 
 // Scheme I complex by 4M: digit planes of the real embedding (prepass.cu) and the final complex combination.
 int launch_oz1_4m_slice(emugemm_ctx *ctx, int elem /* kZ128 or kC64 */, int is_b, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
@@ -118,6 +118,7 @@ struct Oz2GemmArgs {
   const int8_t *RA, *RB;       // real: [N][rows][kpad]; 3M: [3][N][rows][kpad]
   int8_t *CR;                  // real: [N][m][n]; 3M: [2][N][m][n]
   unsigned long long *cycles;  // as in Oz1GemmArgs
+  int batch = 1;               // strided batched call: residue planes hold batch * m (n) rows entry-major, CR is [N][batch][m][n]
 };
 int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &a);
 
@@ -127,11 +128,13 @@ struct Oz2CrtArgs {
   const int8_t *CR;            // [N][m][n] (3M: second part at CR + N*m*n)
   const int32_t *eA, *eB;
   int tA, tB;
-  int is_complex;              // 0: real alpha/beta; 1: complex, C is (re, im) pairs
-  int out_f32;                 // C holds float (real: SGEMM) or float pairs (complex: CGEMM)
+  int is_complex = 0;          // 0: real alpha/beta; 1: complex, C is (re, im) pairs
+  int out_f32 = 0;               // C holds float (real: SGEMM) or float pairs (complex: CGEMM)
   double alpha[2], beta[2];
   double *C;
   int64_t ldc;
+  int batch = 1;               // CR [N][batch][m][n], eA [batch m], eB [batch n], C_b = C + b * batch_stride_c elements
+  int64_t batch_stride_c = 0;
 };
 int launch_oz2_crt(emugemm_ctx *ctx, const Oz2CrtArgs &a);
 

@@ -149,12 +149,18 @@ template <bool VEC, int KIND>
 __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const int8_t *__restrict__ CR,
                                                   const int32_t *__restrict__ eA, const int32_t *__restrict__ eB,
                                                   int tsum, double ar, double ai, double br, double bi,
-                                                  double *__restrict__ C, int64_t ldc, const CrtConst k) {
+                                                  double *__restrict__ C, int64_t ldc, const CrtConst k,
+                                                  int64_t c_entry_bytes) {
   const int64_t ncolv = (n + kCrtVec - 1) / kCrtVec;
   const int64_t idx = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
   if (idx >= m * ncolv) return;
   const int64_t i = idx / ncolv, j0 = (idx - i * ncolv) * kCrtVec;
-  const int64_t plane = m * n;
+  // batch entry blockIdx.y: CR is [N][batch][m][n], the exponents are stacked entry-major
+  const int64_t plane = m * n * gridDim.y;
+  CR += static_cast<int64_t>(blockIdx.y) * m * n;
+  eA += static_cast<int64_t>(blockIdx.y) * m;
+  eB += static_cast<int64_t>(blockIdx.y) * n;
+  C = reinterpret_cast<double *>(reinterpret_cast<char *>(C) + static_cast<int64_t>(blockIdx.y) * c_entry_bytes);
   const int eAi = eA[i] - tsum;
   double sc1[kCrtVec], sc2[kCrtVec];
 #pragma unroll
@@ -249,9 +255,13 @@ int launch_oz2_crt(emugemm_ctx *ctx, const Oz2CrtArgs &a) {
   const unsigned grid = static_cast<unsigned>((work + 255) / 256);
   const bool vec = (a.n % kCrtVec == 0) && ((reinterpret_cast<uintptr_t>(a.CR) & 7) == 0);
   const int tsum = a.tA + a.tB;
+  const int batch = a.batch > 0 ? a.batch : 1;
+  if (batch > 65535) return EMUGEMM_ERR_ARG;
+  // bytes between the C matrices of consecutive batch entries (element = float / double, x2 for complex)
+  const int64_t c_entry_bytes = a.batch_stride_c * (a.out_f32 ? 4 : 8) * (a.is_complex ? 2 : 1);
 #define EMU_CRT_LAUNCH(V, Z)                                                                                              \
-  crt_kernel<V, Z><<<grid, 256, 0, ctx->stream>>>(a.m, a.n, a.CR, a.eA, a.eB, tsum, a.alpha[0], a.alpha[1], a.beta[0], \
-                                                   a.beta[1], a.C, a.ldc, k)
+  crt_kernel<V, Z><<<dim3(grid, static_cast<unsigned>(batch)), 256, 0, ctx->stream>>>(a.m, a.n, a.CR, a.eA, a.eB, tsum, a.alpha[0], a.alpha[1], a.beta[0], \
+                                                   a.beta[1], a.C, a.ldc, k, c_entry_bytes)
   const int kind = a.is_complex ? (a.out_f32 ? 3 : 1) : (a.out_f32 ? 2 : 0);
   if (vec && kind == 3) EMU_CRT_LAUNCH(true, 3);
   else if (kind == 3) EMU_CRT_LAUNCH(false, 3);

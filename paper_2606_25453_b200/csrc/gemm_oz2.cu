@@ -36,6 +36,7 @@ struct Oz2Dev {
   int64_t m, n;
   int kblocks;
   int mt, nt_tiles, n_moduli;
+  int nbatch;  // strided batched call: entry b uses plane rows [b m, (b+1) m) / [b n, (b+1) n) and CR[l][b]
   int8_t *CR;
   unsigned long long *cycles;
   int dbg;
@@ -93,7 +94,8 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   const uint32_t cta = cluster_ctarank();  // 0 = leader (issues the MMAs), 1 = peer
   const int cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
   const int tiles_per_mod = a.mt * a.nt_tiles;  // a.mt counts PAIR tiles of 256 rows
-  const int num_tiles = tiles_per_mod * a.n_moduli;
+  const int tiles_per_entry = tiles_per_mod * a.n_moduli;
+  const int num_tiles = tiles_per_entry * a.nbatch;  // entry-major: tile = (batch entry, modulus, tile of the modulus)
 
   if (threadIdx.x == 0) {
     // full[s] (leader's is the one used): 1 arrival (leader's expect_tx) + the bytes of BOTH CTAs' loads;
@@ -120,11 +122,12 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       int st = 0;
       uint32_t ph = 0;
       for (int tile = cluster_id; tile < num_tiles; tile += num_clusters) {
-        const int l = tile / tiles_per_mod;
+        const int bidx = tile / tiles_per_entry, te = tile - bidx * tiles_per_entry;
+        const int l = te / tiles_per_mod;
         int mb, nb;
-        tile_coords(tile - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb);
-        const int arow = mb * kOz2PairM + static_cast<int>(cta) * kTileM;
-        const int brow = nb * kOz2NT + static_cast<int>(cta) * (kOz2NT / 2);
+        tile_coords(te - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb);
+        const int arow = static_cast<int>(bidx * a.m) + mb * kOz2PairM + static_cast<int>(cta) * kTileM;
+        const int brow = static_cast<int>(bidx * a.n) + nb * kOz2NT + static_cast<int>(cta) * (kOz2NT / 2);
         for (int q = 0; q < NPROD; ++q) {
           const int plane = q * a.n_moduli + l;
           for (int kb = 0; kb < a.kblocks; kb += kOz2KPerStage) {
@@ -186,14 +189,15 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     const int row = quad * 32 + lane;
     const uint32_t trow = tmem_base + (static_cast<uint32_t>(quad * 32) << 16);
     const bool vec_ok = (a.n % 16 == 0) && ((reinterpret_cast<uintptr_t>(a.CR) & 15) == 0);
-    const int64_t plane_sz = a.m * a.n;
+    const int64_t plane_sz = a.m * a.n * a.nbatch;
     uint32_t item = 0;
     unsigned t1[NPROD == 3 ? 32 : 1], t2[NPROD == 3 ? 32 : 1];  // T1, T2 of this thread's 128 columns as packed INT8 (3M)
     const uint32_t tempty_leader[2] = {mapa_u32(&tempty[0], 0), mapa_u32(&tempty[1], 0)};
     for (int tile = cluster_id; tile < num_tiles; tile += num_clusters) {
-      const int l = tile / tiles_per_mod;
+      const int bidx = tile / tiles_per_entry, te = tile - bidx * tiles_per_entry;
+      const int l = te / tiles_per_mod;
       int mb, nb;
-      tile_coords(tile - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb);
+      tile_coords(te - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb);
       ModK mk;
       mk.cvec = a.cvec[l]; mk.c0 = a.c0[l]; mk.magic = a.magic[l]; mk.m = static_cast<unsigned>(a.mod[l]); mk.half = (mk.m + 1) / 2;
       const int64_t grow = static_cast<int64_t>(mb) * kOz2PairM + cta * kTileM + row;
@@ -222,7 +226,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 w[g] = pack4i(sym_mod_i32(v[4 * g], mk), sym_mod_i32(v[4 * g + 1], mk), sym_mod_i32(v[4 * g + 2], mk),
                               sym_mod_i32(v[4 * g + 3], mk));
               if (row_ok && gcol < a.n && !(a.dbg & 4))
-                store32(a.CR + (static_cast<int64_t>(l) * a.m + grow) * a.n + gcol, w, gcol, a.n, vec_ok);
+                store32(a.CR + ((static_cast<int64_t>(l) * a.nbatch + bidx) * a.m + grow) * a.n + gcol, w, gcol, a.n, vec_ok);
             } else if (q < 2) {
               // T1 / T2 stay on chip as unsigned residues in [0, m), four per register
 #pragma unroll
@@ -252,7 +256,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 wi[g] = pack4i(im[0], im[1], im[2], im[3]);
               }
               if (row_ok && gcol < a.n && !(a.dbg & 4)) {
-                int8_t *o = a.CR + (static_cast<int64_t>(l) * a.m + grow) * a.n + gcol;
+                int8_t *o = a.CR + ((static_cast<int64_t>(l) * a.nbatch + bidx) * a.m + grow) * a.n + gcol;
                 store32(o, wr, gcol, a.n, vec_ok);
                 store32(o + a.n_moduli * plane_sz, wi, gcol, a.n, vec_ok);
               }
@@ -276,14 +280,16 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
   if (g.m == 0 || g.n == 0 || g.kpad == 0) return EMUGEMM_OK;
   const int parts = g.is3m ? 3 : 1;
   CUtensorMap tmA, tmB;
-  EMU_TRY(encode_planes_tmap(ctx, &tmA, g.RA, g.kpad, g.m, static_cast<int64_t>(parts) * g.n_moduli, kTileM, 1));
-  EMU_TRY(encode_planes_tmap(ctx, &tmB, g.RB, g.kpad, g.n, static_cast<int64_t>(parts) * g.n_moduli, kOz2NT / 2, 1));
+  const int batch = g.batch > 0 ? g.batch : 1;
+  EMU_TRY(encode_planes_tmap(ctx, &tmA, g.RA, g.kpad, g.m * batch, static_cast<int64_t>(parts) * g.n_moduli, kTileM, 1));
+  EMU_TRY(encode_planes_tmap(ctx, &tmB, g.RB, g.kpad, g.n * batch, static_cast<int64_t>(parts) * g.n_moduli, kOz2NT / 2, 1));
   Oz2Dev d;
   d.m = g.m; d.n = g.n;
   d.kblocks = static_cast<int>(g.kpad / kBlockK);
   d.mt = static_cast<int>((g.m + kOz2PairM - 1) / kOz2PairM);  // pair tiles
   d.nt_tiles = static_cast<int>((g.n + kOz2NT - 1) / kOz2NT);
   d.n_moduli = g.n_moduli;
+  d.nbatch = batch;
   d.CR = g.CR;
   d.cycles = g.cycles;
   d.dbg = ctx->dbg_flags;
@@ -299,7 +305,8 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
     d.c0[l] = (m - two31) % m;
     d.magic[l] = static_cast<unsigned>(((1ull << 32) + m - 1ull) / m);
   }
-  const int64_t tiles = static_cast<int64_t>(d.mt) * d.nt_tiles * d.n_moduli;
+  const int64_t tiles = static_cast<int64_t>(d.mt) * d.nt_tiles * d.n_moduli * batch;
+  if (tiles >= (1LL << 31)) return EMUGEMM_ERR_ARG;
   const int pairs = ctx->num_sms / 2;
   const int grid = 2 * (tiles < pairs ? static_cast<int>(tiles) : pairs);
   auto kern = g.is3m ? oz2_gemm_kernel<3> : oz2_gemm_kernel<1>;

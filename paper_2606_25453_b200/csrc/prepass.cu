@@ -523,21 +523,21 @@ int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int6
 
 int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
                         const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int n_moduli, int t_bits,
-                        int8_t *out) {
+                        int8_t *out, int batch, int64_t xstride) {
   if (t_bits < 1 || t_bits > 95) return EMUGEMM_ERR_ARG;  // three 32-bit words hold |a'| < 2^t (t = 77 at most: N = 20, k = 1)
   const bool two = t_bits <= 64;  // |a'| < 2^t fits two 32-bit words: one byte dot product less per residue
   if (elem == kF64)
-    return two ? launch_planes<double, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out)
-               : launch_planes<double, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out);
+    return two ? launch_planes<double, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride)
+               : launch_planes<double, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride);
   if (elem == kF32)  // 24-bit inputs (Scheme II SGEMM)
-    return two ? launch_planes<float, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out)
-               : launch_planes<float, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out);
+    return two ? launch_planes<float, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride)
+               : launch_planes<float, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride);
   if (elem == kC64)
-    return two ? launch_planes<float, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out)
-               : launch_planes<float, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out);
+    return two ? launch_planes<float, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride)
+               : launch_planes<float, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride);
   if (elem == kZ128)
-    return two ? launch_planes<double, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out)
-               : launch_planes<double, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out);
+    return two ? launch_planes<double, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride)
+               : launch_planes<double, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride);
   return EMUGEMM_ERR_ARG;
 }
 

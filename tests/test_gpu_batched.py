@@ -140,3 +140,56 @@ def test_batched_degenerate_and_errors(env):
                                                ct.c_void_p(B.data_ptr()), ct.c_int64(8), ct.c_int64(128), ct.c_double(0.0),
                                                ct.c_void_p(C.data_ptr()), ct.c_int64(8), ct.c_int64(64), ct.c_int(4))
     assert st == -2  # EMUGEMM_ERR_ALIGNMENT
+
+
+# ---- Scheme II ---------------------------------------------------------------------------------------------------
+@pytest.mark.parametrize("N,batch,shape", [(16, 4, (100, 80, 300)), (12, 3, (257, 272, 130)), (20, 2, (300, 200, 333)),
+                                           (14, 5, (64, 64, 128))])
+def test_dgemm_oz2_batched_vs_oracle_and_single(env, N, batch, shape):
+    torch, O, h = env
+    m, n, k = shape
+    A, B = entries(batch, m, n, k, 1.0, 300 + N)
+    Ad, Bd = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
+    C = torch.full((batch, m, n), float("nan"), dtype=torch.float64, device="cuda")  # beta = 0: C not read
+    h.dgemm_oz2_strided_batched(Ad, Bd, C, N)
+    got = C.cpu().numpy()
+    for b in range(batch):
+        _, absAB = O.bf128_dgemm(A[b], B[b])
+        assert_within_ulps(got[b], O.dgemm_oz2(A[b], B[b], N), absAB, 2, what=f"entry {b} N={N} {shape}")
+        single = torch.zeros((m, n), dtype=torch.float64, device="cuda")
+        h.dgemm_oz2(Ad[b], Bd[b], single, N)
+        assert np.array_equal(got[b], single.cpu().numpy()), f"entry {b} differs from the single call"
+
+
+def test_oz2_batched_alpha_beta_strides_shared_a(env):
+    """alpha / beta, padded leading dimensions and batch strides, ONE A shared by all entries (strideA = 0)."""
+    torch, O, h = env
+    batch, m, n, k, N = 3, 90, 72, 200, 15
+    A, _ = G.real_pair(m, n, k, 2.0, 77)
+    _, B = entries(batch, m, n, k, 2.0, 5)
+    Cin = np.random.default_rng(6).standard_normal((batch, m, n))
+    Abuf = torch.zeros((m, k + 6), dtype=torch.float64, device="cuda")
+    Abuf[:, :k] = torch.from_numpy(A).cuda()
+    Bbuf = torch.zeros((batch, k + 2, n + 10), dtype=torch.float64, device="cuda")
+    Bbuf[:, :k, :n] = torch.from_numpy(B).cuda()
+    Cbuf = torch.full((batch, m + 1, n + 4), 7.0, dtype=torch.float64, device="cuda")
+    Cbuf[:, :m, :n] = torch.from_numpy(Cin).cuda()
+    h.dgemm_oz2_strided_batched(Abuf[:, :k], Bbuf[:, :k, :n], Cbuf[:, :m, :n], N, alpha=-1.5, beta=0.75)
+    got = Cbuf.cpu().numpy()
+    assert (got[:, m:, :] == 7.0).all() and (got[:, :, n:] == 7.0).all(), "wrote outside C"
+    for b in range(batch):
+        _, absAB = O.bf128_dgemm(A, B[b])
+        want = O.dgemm_oz2(A, B[b], N, alpha=-1.5, beta=0.75, Cin=Cin[b])
+        assert_within_ulps(got[b, :m, :n], want, 1.5 * absAB + 0.75 * np.abs(Cin[b]), 2, what=f"entry {b}")
+
+
+def test_sgemm_oz2_batched(env):
+    torch, O, h = env
+    batch, m, n, k, N = 3, 130, 96, 260, 9
+    A, B = entries(batch, m, n, k, 1.0, 18, dtype=np.float32)
+    C = torch.zeros((batch, m, n), dtype=torch.float32, device="cuda")
+    h.sgemm_oz2_strided_batched(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, N)
+    got = C.cpu().numpy()
+    for b in range(batch):
+        _, absAB = O.bf128_dgemm(A[b].astype(np.float64), B[b].astype(np.float64))
+        assert_within_ulps(got[b], O.sgemm_oz2(A[b], B[b], N), absAB, 2, bits=23, what=f"entry {b}")
