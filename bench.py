@@ -412,6 +412,26 @@ def main():
         ms8 = q0.elapsed_time(q1) / 5
         detail["f1_8bit_slices_p7"] = {"ms_per_step": ms8, "emulated_tflops": w["flops"] / (ms8 * 1e-3) / 1e12,
                                        "int8_tops": 56.0 * w["m"] * w["n"] * w["k"] / (ms8 * 1e-3) / 1e12}
+        # NEXT item f2: 64 products of 512^3 through ONE strided batched call; context only
+        try:
+            gb = torch.Generator(device="cuda")
+            gb.manual_seed(w["seed"] + 7)
+            Ab = torch.rand((64, 512, 512), device="cuda", dtype=torch.float64, generator=gb) - 0.5
+            Bb = torch.rand((64, 512, 512), device="cuda", dtype=torch.float64, generator=gb) - 0.5
+            Cb = torch.empty((64, 512, 512), device="cuda", dtype=torch.float64)
+            for _ in range(3):
+                h.dgemm_oz1_strided_batched(Ab, Bb, Cb, 8)
+            q0.record(stream)
+            for _ in range(10):
+                h.dgemm_oz1_strided_batched(Ab, Bb, Cb, 8)
+            q1.record(stream)
+            torch.cuda.synchronize()
+            msb = q0.elapsed_time(q1) / 10
+            detail["f2_strided_batched_64x512_p8"] = {"ms_per_call": msb,
+                                                      "emulated_tflops": 2.0 * 64 * 512 ** 3 / (msb * 1e-3) / 1e12}
+            del Ab, Bb, Cb
+        except Exception as ex:  # context, never the product
+            detail["f2_strided_batched_error"] = str(ex)
     detail["paper_context"] = "paper: 3654 Top/s (81% of 4500) EmuGEMM-I end-to-end on B200, other machine (PAPER.md:293)"
 
     line = {"metric": METRIC, "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
