@@ -136,7 +136,8 @@ int emugemm_sgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, float
 /* Strided batched Scheme II, real: conventions, limits and alignment rule as
  * emugemm_dgemm_oz1_strided_batched.  Residue planes of all entries are stacked entry-major; ONE fused launch walks
  * (entry, modulus, tile) work items and ONE CRT launch covers the batch.  Every entry is bit-identical to the single
- * call on it.  Workspace: emugemm_workspace_bytes(EMUGEMM_OZ2, elem, batch*m, batch*n, k, n_moduli).          */
+ * call on it.  Workspace: emugemm_workspace_bytes(EMUGEMM_OZ2 / EMUGEMM_OZ2_3M, elem, batch*m, batch*n, k,
+ * n_moduli).                                                                                                */
 int emugemm_dgemm_oz2_strided_batched(emugemm_handle_t h, int64_t batch, int64_t m, int64_t n, int64_t k,
                                       double alpha, const double *A, int64_t lda, int64_t strideA,
                                       const double *B, int64_t ldb, int64_t strideB, double beta, double *C,
@@ -145,6 +146,12 @@ int emugemm_sgemm_oz2_strided_batched(emugemm_handle_t h, int64_t batch, int64_t
                                       float alpha, const float *A, int64_t lda, int64_t strideA,
                                       const float *B, int64_t ldb, int64_t strideB, float beta, float *C,
                                       int64_t ldc, int64_t strideC, int n_moduli);
+
+/* complex128 by 3M, batched: strides in complex elements, alpha / beta point to HOST {re, im}.            */
+int emugemm_zgemm_oz2_3m_strided_batched(emugemm_handle_t h, int64_t batch, int64_t m, int64_t n, int64_t k,
+                                         const double alpha[2], const double *A, int64_t lda, int64_t strideA,
+                                         const double *B, int64_t ldb, int64_t strideB, const double beta[2],
+                                         double *C, int64_t ldc, int64_t strideC, int n_moduli);
 
 /* ---- Scheme II complex via 3M ------------------------ *
  * A, B, C hold complex128 as (re, im) pairs; alpha, beta point to HOST {re, im}. */

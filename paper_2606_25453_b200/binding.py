@@ -259,6 +259,11 @@ class EmuGemm:
                                                       _i64(self._ld(C_)), _int(n_moduli)))
         return C_
 
+    def zgemm_oz2_3m_strided_batched(self, A, B, C_, n_moduli, alpha=1.0 + 0j, beta=0j):
+        """complex128 CUDA tensors: A (batch, m, k) or (m, k), B (batch, k, n) or (k, n), C_ (batch, m, n)."""
+        cvt = lambda z: (_dbl * 2)(complex(z).real, complex(z).imag)  # noqa: E731
+        return self._batched(self._lib.emugemm_zgemm_oz2_3m_strided_batched, cvt, 16, A, B, C_, n_moduli, alpha, beta, OZ2_3M)
+
     # ---- pre-decomposed operands (emugemm_decompose / emugemm_gemm_pre) --------
     def decompose(self, scheme, role, X, pn, trans=False):
         """-> Operand for the left (role 0) or right (role 1) operand; X as in the _t calls."""

@@ -316,20 +316,21 @@ static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t 
   return oz2_gemm_phase(h, is3m, m, n, kpad, N, RA, RB, CR, eA, eB, tA, tB, alpha, beta, C, ldc, diag, f32);
 }
 
-// Strided batched Scheme II, real (DGEMM / SGEMM): as run_oz1_batched -- residue planes of all entries stacked
+// Strided batched Scheme II (DGEMM / SGEMM / ZGEMM-3M): as run_oz1_batched -- residue planes of all entries stacked
 // entry-major, the pre-pass kernels take the entry from a grid dimension, ONE persistent launch walks
 // (entry, modulus, tile) work items, one CRT launch covers the batch (grid.y = entry).
-static int run_oz2_batched(emugemm_ctx *h, int f32, int64_t batch, int64_t m, int64_t n, int64_t k, double alpha,
-                           const void *A, int64_t lda, int64_t strideA, const void *B, int64_t ldb, int64_t strideB,
-                           double beta, void *C, int64_t ldc, int64_t strideC, int N) {
+static int run_oz2_batched(emugemm_ctx *h, int is3m, int f32, int64_t batch, int64_t m, int64_t n, int64_t k,
+                           const double al[2], const void *A, int64_t lda, int64_t strideA, const void *B, int64_t ldb,
+                           int64_t strideB, const double be[2], void *C, int64_t ldc, int64_t strideC, int N) {
   if (!h || batch < 0 || strideA < 0 || strideB < 0 || strideC < 0) return EMUGEMM_ERR_ARG;
   EMU_TRY(check_gemm_args(h, 0, 0, m, n, k, A, lda, B, ldb, C, ldc));
   if (N < 2 || N > kMaxModuli) return EMUGEMM_ERR_ARG;
   h->launches = 0;
   if (batch == 0 || m == 0 || n == 0) return EMUGEMM_OK;
-  const int elem = f32 ? kF32 : kF64;
-  const int64_t es = f32 ? 4 : 8;
-  const double al[2] = {alpha, 0.0}, be[2] = {beta, 0.0};
+  if (is3m && f32) return EMUGEMM_ERR_ARG;
+  const int elem = is3m ? kZ128 : (f32 ? kF32 : kF64);
+  const int64_t es = is3m ? 16 : (f32 ? 4 : 8);
+  const int parts_in = is3m ? 3 : 1, parts_out = is3m ? 2 : 1;
   if (batch > 1) {
     if (((strideA * es) | (strideB * es) | (strideC * es)) & 15) return EMUGEMM_ERR_ALIGNMENT;
     if (strideC < (m - 1) * ldc + n) return EMUGEMM_ERR_ARG;
@@ -338,7 +339,7 @@ static int run_oz2_batched(emugemm_ctx *h, int f32, int64_t batch, int64_t m, in
   if (batch == 1 || k == 0) {
     int launches = 0;
     for (int64_t b = 0; b < batch; ++b) {
-      EMU_TRY(run_oz2(h, 0, 0, 0, m, n, k, al, static_cast<const char *>(A) + b * strideA * es, lda,
+      EMU_TRY(run_oz2(h, 0, 0, is3m, m, n, k, al, static_cast<const char *>(A) + b * strideA * es, lda,
                       static_cast<const char *>(B) + b * strideB * es, ldb, be,
                       reinterpret_cast<double *>(static_cast<char *>(C) + b * strideC * es), ldc, N, f32));
       launches += h->launches;
@@ -347,7 +348,7 @@ static int run_oz2_batched(emugemm_ctx *h, int f32, int64_t batch, int64_t m, in
     return EMUGEMM_OK;
   }
   int tA, tB;
-  if (oz2_budget_host(N, k, 0, &tA, &tB) < 2) return EMUGEMM_ERR_PRECISION;
+  if (oz2_budget_host(N, k, is3m, &tA, &tB) < 2) return EMUGEMM_ERR_PRECISION;
   if (k > 131071) return EMUGEMM_ERR_PRECISION;
   EMU_TRY(mark(h, 0));
   const int64_t kpad = round_up(k, kBlockK);
@@ -359,9 +360,9 @@ static int run_oz2_batched(emugemm_ctx *h, int f32, int64_t batch, int64_t m, in
   auto *mbB = cv.take<unsigned long long>(NN);
   auto *eA = cv.take<int32_t>(M);
   auto *eB = cv.take<int32_t>(NN);
-  auto *RA = cv.take<int8_t>(static_cast<size_t>(N) * M * kpad);
-  auto *RB = cv.take<int8_t>(static_cast<size_t>(N) * NN * kpad);
-  auto *CR = cv.take<int8_t>(static_cast<size_t>(N) * M * n);
+  auto *RA = cv.take<int8_t>(static_cast<size_t>(parts_in) * N * M * kpad);
+  auto *RB = cv.take<int8_t>(static_cast<size_t>(parts_in) * N * NN * kpad);
+  auto *CR = cv.take<int8_t>(static_cast<size_t>(parts_out) * N * M * n);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   h->diag = diag;
   EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
@@ -370,7 +371,7 @@ static int run_oz2_batched(emugemm_ctx *h, int f32, int64_t batch, int64_t m, in
   EMU_TRY(launch_oz2_residues(h, elem, 0, m, k, kpad, A, lda, mbA, eA, N, tA, RA, nb, strideA));
   EMU_TRY(launch_oz2_residues(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, N, tB, RB, nb, strideB));
   EMU_TRY(mark(h, 1));
-  return oz2_gemm_phase(h, 0, m, n, kpad, N, RA, RB, CR, eA, eB, tA, tB, al, be, static_cast<double *>(C), ldc, diag, f32, nb,
+  return oz2_gemm_phase(h, is3m, m, n, kpad, N, RA, RB, CR, eA, eB, tA, tB, al, be, static_cast<double *>(C), ldc, diag, f32, nb,
                         strideC);
 }
 
@@ -593,12 +594,21 @@ int emugemm_sgemm_oz1_strided_batched(emugemm_handle_t h, int64_t batch, int64_t
 int emugemm_dgemm_oz2_strided_batched(emugemm_handle_t h, int64_t batch, int64_t m, int64_t n, int64_t k, double alpha,
                                       const double *A, int64_t lda, int64_t strideA, const double *B, int64_t ldb,
                                       int64_t strideB, double beta, double *C, int64_t ldc, int64_t strideC, int n_moduli) {
-  return run_oz2_batched(h, 0, batch, m, n, k, alpha, A, lda, strideA, B, ldb, strideB, beta, C, ldc, strideC, n_moduli);
+  const double al[2] = {alpha, 0.0}, be[2] = {beta, 0.0};
+  return run_oz2_batched(h, 0, 0, batch, m, n, k, al, A, lda, strideA, B, ldb, strideB, be, C, ldc, strideC, n_moduli);
 }
 int emugemm_sgemm_oz2_strided_batched(emugemm_handle_t h, int64_t batch, int64_t m, int64_t n, int64_t k, float alpha,
                                       const float *A, int64_t lda, int64_t strideA, const float *B, int64_t ldb,
                                       int64_t strideB, float beta, float *C, int64_t ldc, int64_t strideC, int n_moduli) {
-  return run_oz2_batched(h, 1, batch, m, n, k, alpha, A, lda, strideA, B, ldb, strideB, beta, C, ldc, strideC, n_moduli);
+  const double al[2] = {alpha, 0.0}, be[2] = {beta, 0.0};
+  return run_oz2_batched(h, 0, 1, batch, m, n, k, al, A, lda, strideA, B, ldb, strideB, be, C, ldc, strideC, n_moduli);
+}
+int emugemm_zgemm_oz2_3m_strided_batched(emugemm_handle_t h, int64_t batch, int64_t m, int64_t n, int64_t k,
+                                         const double alpha[2], const double *A, int64_t lda, int64_t strideA,
+                                         const double *B, int64_t ldb, int64_t strideB, const double beta[2], double *C,
+                                         int64_t ldc, int64_t strideC, int n_moduli) {
+  if (!alpha || !beta) return EMUGEMM_ERR_ARG;
+  return run_oz2_batched(h, 1, 0, batch, m, n, k, alpha, A, lda, strideA, B, ldb, strideB, beta, C, ldc, strideC, n_moduli);
 }
 
 int emugemm_dgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha, const double *A, int64_t lda,

@@ -193,3 +193,26 @@ def test_sgemm_oz2_batched(env):
     for b in range(batch):
         _, absAB = O.bf128_dgemm(A[b].astype(np.float64), B[b].astype(np.float64))
         assert_within_ulps(got[b], O.sgemm_oz2(A[b], B[b], N), absAB, 2, bits=23, what=f"entry {b}")
+
+
+@pytest.mark.parametrize("N,batch,shape", [(14, 3, (100, 80, 200)), (18, 2, (257, 272, 130))])
+def test_zgemm_3m_batched(env, N, batch, shape):
+    """complex128 by 3M: every entry against the oracle, bit-identical to the single call; alpha / beta complex."""
+    torch, O, h = env
+    m, n, k = shape
+    trip = [G.complex_pair(m, n, k, 1.0, 60 + 7 * b, with_c=True) for b in range(batch)]
+    A, B, Cin = (np.stack([t[i] for t in trip]) for i in range(3))
+    al, be = 0.5 - 2j, 1.5 + 0.25j
+    Ad, Bd = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
+    C = torch.from_numpy(Cin).cuda()
+    h.zgemm_oz2_3m_strided_batched(Ad, Bd, C, N, alpha=al, beta=be)
+    got = C.cpu().numpy()
+    for b in range(batch):
+        want = O.zgemm_oz2_3m(A[b], B[b], N, alpha=al, beta=be, Cin=Cin[b])
+        _, absZ = O.bf128_zgemm(A[b], B[b])
+        scale = abs(al) * 2 * absZ + abs(be) * 2 * np.abs(Cin[b])
+        assert_within_ulps(got[b].real, want.real, scale, 2, what=f"entry {b} re")
+        assert_within_ulps(got[b].imag, want.imag, scale, 2, what=f"entry {b} im")
+        single = torch.from_numpy(Cin[b]).cuda()
+        h.zgemm_oz2_3m(Ad[b], Bd[b], single, N, alpha=al, beta=be)
+        assert np.array_equal(got[b], single.cpu().numpy()), f"entry {b} differs from the single call"
