@@ -291,7 +291,9 @@ int emugemm_dbg_oz1_issue_probe(emugemm_handle_t h, int p, int use_collector, in
  * once (barrier traffic unchanged), bit 1 = the epilogue skips its TMEM reads, math
  * and stores, bit 2 = only the stores are skipped, bit 3 = Scheme I with p <= 3 runs
  * the one-CTA N-concatenated kernel instead of the CTA-pair kernel, bit 4 = Scheme I
- * with p >= 4 runs without the 2-CTA multicast of A (A/B timing).
+ * with p >= 4 runs without the 2-CTA multicast of A (A/B timing), bit 5 = the Scheme I
+ * row pre-pass runs its two-phase form (row re-read) instead of the register-resident
+ * single-read kernel.
  * Used to attribute tensor-pipe idle time.                        */
 int emugemm_dbg_set_flags(emugemm_handle_t h, int flags);
 

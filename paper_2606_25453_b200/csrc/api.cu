@@ -190,8 +190,6 @@ static int run_oz1(emugemm_ctx *h, int ta, int tb, int elem, int64_t m, int64_t 
 
   // planes are indexed [row of op(A)] / [column of op(B)] with k contiguous: a k-major stored operand (A^T stored
   // k x m, B stored k x n) goes through the column kernels, an operand whose k is contiguous through the row kernel
-  if (ta) EMU_TRY(launch_colmax(h, elem, m, k, A, lda, mbA));
-  if (!tb) EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB));
   EMU_TRY(launch_oz1_slice(h, elem, ta, m, k, kpad, A, lda, mbA, eA, p, bits, SA));
   EMU_TRY(launch_oz1_slice(h, elem, !tb, n, k, kpad, B, ldb, mbB, eB, p, bits, SB));
   EMU_TRY(mark(h, 1));
@@ -248,7 +246,6 @@ static int run_oz1_batched(emugemm_ctx *h, int elem, int64_t batch, int64_t m, i
   h->diag = diag;
   EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
   const int nb = static_cast<int>(batch);
-  EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB, nb, strideB));
   EMU_TRY(launch_oz1_slice(h, elem, 0, m, k, kpad, A, lda, mbA, eA, p, bits, SA, nb, strideA));
   EMU_TRY(launch_oz1_slice(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, p, bits, SB, nb, strideB));
   EMU_TRY(mark(h, 1));
@@ -308,8 +305,6 @@ static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t 
   h->diag = diag;
   EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
 
-  if (ta) EMU_TRY(launch_colmax(h, elem, m, k, A, lda, mbA));
-  if (!tb) EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB));
   EMU_TRY(launch_oz2_residues(h, elem, ta, m, k, kpad, A, lda, mbA, eA, N, tA, RA));
   EMU_TRY(launch_oz2_residues(h, elem, !tb, n, k, kpad, B, ldb, mbB, eB, N, tB, RB));
   EMU_TRY(mark(h, 1));
@@ -367,7 +362,6 @@ static int run_oz2_batched(emugemm_ctx *h, int is3m, int f32, int64_t batch, int
   h->diag = diag;
   EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
   const int nb = static_cast<int>(batch);
-  EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB, nb, strideB));
   EMU_TRY(launch_oz2_residues(h, elem, 0, m, k, kpad, A, lda, mbA, eA, N, tA, RA, nb, strideA));
   EMU_TRY(launch_oz2_residues(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, N, tB, RB, nb, strideB));
   EMU_TRY(mark(h, 1));
@@ -660,7 +654,6 @@ int emugemm_decompose(emugemm_handle_t h, int scheme, int role, int trans, int e
     Carver cv(h->ws, h->ws_bytes);
     mb = cv.take<unsigned long long>(rows);
     if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
-    EMU_TRY(launch_colmax(h, elem, rows, k, X, ldx, mb));
   }
   h->launches = 0;
   if (oz1) EMU_TRY(launch_oz1_slice(h, elem, by_cols, rows, k, kpad, X, ldx, mb, e, pn, h->slice_bits, planes));
@@ -756,7 +749,6 @@ int emugemm_dbg_oz1_slices(emugemm_handle_t h, int elem, int by_cols, int64_t ro
   auto *mb = cv.take<unsigned long long>(rows);
   auto *S = cv.take<int8_t>(static_cast<size_t>(p) * rows * kpad);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
-  if (by_cols) EMU_TRY(launch_colmax(h, elem, rows, k, X, ldx, mb));
   EMU_TRY(launch_oz1_slice(h, elem, by_cols, rows, k, kpad, X, ldx, mb, e_out, p, h->slice_bits, S));
   return unpad_planes(h, out, S, static_cast<int64_t>(p) * rows, k, kpad);
 }
@@ -777,7 +769,6 @@ int emugemm_dbg_oz2_residues(emugemm_handle_t h, int elem, int by_cols, int64_t 
   auto *mb = cv.take<unsigned long long>(rows);
   auto *R = cv.take<int8_t>(static_cast<size_t>(parts) * n_moduli * rows * kpad);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
-  if (by_cols) EMU_TRY(launch_colmax(h, elem, rows, k, X, ldx, mb));
   EMU_TRY(launch_oz2_residues(h, elem, by_cols, rows, k, kpad, X, ldx, mb, e_out, n_moduli, t_bits, R));
   return unpad_planes(h, out, R, static_cast<int64_t>(parts) * n_moduli * rows, k, kpad);
 }

@@ -74,15 +74,15 @@ int launch_colmax(emugemm_ctx *ctx, int elem, int64_t rows, int64_t k, const voi
                   unsigned long long *maxbits, int batch = 1, int64_t xstride = 0);
 
 // Scheme I slicing: out[p][rows][kpad] int8 (zero padded to kpad) AND the exponents e[rows] (output).
-// by_cols = 0: one fused kernel scans each row and slices it (maxbits unused); by_cols = 1: maxbits[rows] from
-// launch_colmax, the kernel derives and publishes the exponents.
+// by_cols = 0: one kernel scans each row and slices it (maxbits unused); by_cols = 1: maxbits is a scratch of
+// batch * rows words: launch_colmax fills it, the column kernel derives and publishes the exponents and slices.
 int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
-                     const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int p, int slice_bits,
+                     const void *X, int64_t ldx, unsigned long long *maxbits, int32_t *e, int p, int slice_bits,
                      int8_t *out, int batch = 1, int64_t xstride = 0);  // batch: out[p][batch rows][kpad], e[batch rows]
 
 // Scheme II residues: elem 8: out[N][rows][kpad]; elem 16: out[3][N][rows][kpad] (re, im, Sigma); e as above.
 int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
-                        const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int n_moduli,
+                        const void *X, int64_t ldx, unsigned long long *maxbits, int32_t *e, int n_moduli,
                         int t_bits, int8_t *out, int batch = 1, int64_t xstride = 0);
 
 // Scheme I complex by 4M: digit planes of the real embedding (prepass.cu) and the final complex combination.

@@ -209,13 +209,6 @@ __device__ __forceinline__ Prep prepare(T v, int e_row, int scale_bits) {
   return r;
 }
 
-template <int P>
-__device__ __forceinline__ int oz1_digit(const Prep &q, int t) {
-  const unsigned long long X = (static_cast<unsigned long long>(q.w1) << 32) | q.w0;
-  const int d = static_cast<int>(static_cast<unsigned int>(X >> (kBeta * (P - 1 - t))) & 127u);
-  return q.neg ? -d : d;
-}
-
 // moduli: greedy pairwise-coprime list descending from 256 (R10)
 __device__ __constant__ int c_moduli[24] = {256, 255, 253, 251, 247, 241, 239, 233, 229, 227, 223, 217,
                                             211, 199, 197, 193, 191, 181, 179, 173, 167, 163, 157, 151};
@@ -236,45 +229,10 @@ __host__ __device__ constexpr unsigned int magic32(int m) {  // ceil(2^32 / m)
                                    static_cast<unsigned long long>(m));
 }
 
-// symmetric residue of sign * (w2:w1:w0) modulo the L-th modulus (L compile-time).
-// Odd m, hm = (m-1)/2: t = sum_j byte_j (256^j mod m) + hm == |a'| + hm (mod m), t < 2^20; q = floor(t / m) by one
-// multiply-high (exact: t (M m - 2^32) / (m 2^32) < 2^-12 < 1/m); (t - q m) - hm lies in [-hm, hm] and is congruent
-// to |a'|: the symmetric residue of the magnitude (R11), and sym(-x) = -sym(x) for odd m (R13).  m = 256: the low
-// byte of the two's complement value.
-template <int L>
-__device__ __forceinline__ int oz2_residue(const Prep &q) {  // q.w2 == 0 is a compile-time constant on the two-word path
-  constexpr int m = h_moduli[L];
-  if constexpr (m == 256) {
-    const unsigned int v = q.neg ? 0u - q.w0 : q.w0;
-    return static_cast<int>(static_cast<signed char>(v & 0xFFu));
-  } else {
-    constexpr unsigned int c0 = pack_w(0, m), c1 = pack_w(1, m), c2 = pack_w(2, m), mg = magic32(m);
-    constexpr unsigned int hm = (m - 1) / 2;
-    unsigned int t = __dp4a(q.w0, c0, hm);
-    t = __dp4a(q.w1, c1, t);
-    t = __dp4a(q.w2, c2, t);
-    const unsigned int qq = __umulhi(t, mg);
-    const int r = static_cast<int>(t - qq * static_cast<unsigned int>(m)) - static_cast<int>(hm);
-    return q.neg ? -r : r;
-  }
-}
-template <int L>
-__device__ __forceinline__ int sym_small(int t) {  // t in (-m, m): re-reduce to the symmetric range (R15)
-  constexpr int m = h_moduli[L];
-  if (t >= (m + 1) / 2) t -= m;
-  else if (t < (m + 1) / 2 - m) t += m;
-  return t;
-}
-
 // ----------------------------------------------------------------------------
 // plane emission.  Each thread owns 4 consecutive k of one row/column ("quad")
 // and emits one packed 32-bit word per plane through `sink(plane, word)`.
 // ----------------------------------------------------------------------------
-__device__ __forceinline__ unsigned int pack4(int a, int b, int c, int d) {  // low bytes -> one word (3 PRMT)
-  return __byte_perm(__byte_perm(static_cast<unsigned int>(a), static_cast<unsigned int>(b), 0x0040),
-                     __byte_perm(static_cast<unsigned int>(c), static_cast<unsigned int>(d), 0x0040), 0x5410);
-}
-
 // Balanced base-256 digits (R23): X = +-|X| (|X| < 2^(8P-2)), Y = X + sum_j 128 256^j; digit t = byte (P-1-t) of Y
 // minus 128 = that byte XOR 0x80 as int8.  One 64-bit add per element, then byte permutes only.
 template <int P, typename Sink>
@@ -300,38 +258,144 @@ __device__ __forceinline__ void emit_oz1_b8(const Prep (&q)[4], Sink sink) {
   }
 }
 
+// Sign-magnitude 7-bit digits (R1) of four elements, one packed word per plane.  Per plane: one funnel shift per
+// element brings digit t to byte 0, three byte permutes gather the four bytes, one AND keeps 7 bits, and the signs
+// are applied to the whole word at once: for a byte d in [0, 127] of a negative element
+// ((d ^ 0x7F) + 1) ^ 0x80 = (128 - d) ^ 0x80 = -d (mod 256) without a carry into the next byte ((d ^ 0x7F) + 1 <= 128).
+// 11 integer instructions per word instead of 19 (shift + mask + negate + select per digit, then the pack).
 template <int P, typename Sink>
 __device__ __forceinline__ void emit_oz1(const Prep (&q)[4], Sink sink) {
+  const unsigned int m1 = (q[0].neg ? 0x1u : 0u) | (q[1].neg ? 0x100u : 0u) | (q[2].neg ? 0x10000u : 0u) | (q[3].neg ? 0x1000000u : 0u);
+  const unsigned int m7 = m1 * 0x7Fu, m8 = m1 << 7;
 #pragma unroll
-  for (int t = 0; t < P; ++t)
-    sink(t, pack4(oz1_digit<P>(q[0], t), oz1_digit<P>(q[1], t), oz1_digit<P>(q[2], t), oz1_digit<P>(q[3], t)));
+  for (int t = 0; t < P; ++t) {
+    const int sh = kBeta * (P - 1 - t);  // compile-time after unrolling
+    unsigned int b[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+      b[i] = (sh == 0) ? q[i].w0 : (sh < 32) ? __funnelshift_r(q[i].w0, q[i].w1, sh) : (sh == 32) ? q[i].w1 : (q[i].w1 >> (sh - 32));
+    const unsigned int w = __byte_perm(__byte_perm(b[0], b[1], 0x0040), __byte_perm(b[2], b[3], 0x0040), 0x5410) & 0x7F7F7F7Fu;
+    sink(t, ((w ^ m7) + m1) ^ m8);
+  }
 }
 
-template <int L, typename Sink>
-__device__ __forceinline__ void emit_oz2_real_from(const Prep (&q)[4], int N, Sink sink) {
+// Scheme II residues of real operands (Eq. 5; R11 / R13).  The element is first turned into its
+// two's complement over NW words (U = a' + neg 2^(32 NW), neg only for a nonzero negative a'), then per modulus
+//   t = sum_j byte_j(U) (256^j mod m) + hm + neg ((-2^(32 NW)) mod m)  ==  a' + hm (mod m),   t < 2^20,
+//   u = t - floor(t / m) m in [0, m): q = floor(t / m) by ONE multiply-high with ceil(2^32 / m) (exact:
+//       t (M m - 2^32) / (m 2^32) < 2^-12 < 1/m), hm = (m - 1) / 2,
+// so u - hm in [-hm, hm] is the symmetric residue of the SIGNED value.  The four u of a quad are packed and hm is
+// subtracted from all four bytes at once: (u + (128 - hm)) ^ 0x80 is u - hm as int8 (u + 128 - hm lies in [1, 255]:
+// no carry).  m = 256: the low byte of U.  6.25 integer instructions per residue (first version: sign-magnitude
+// residue, negate / select and -hm per element: 7.75).
+struct PrepS {
+  unsigned int w0, w1, w2;
+  unsigned int neg;  // all ones for a nonzero negative value, else 0
+};
+template <int NW>
+__device__ __forceinline__ PrepS twos_complement(const Prep &q) {
+  PrepS r;
+  const bool nz = (q.w0 | q.w1 | (NW == 3 ? q.w2 : 0u)) != 0u;
+  r.neg = (q.neg && nz) ? 0xFFFFFFFFu : 0u;
+  if (NW == 2) {
+    const unsigned long long X = (static_cast<unsigned long long>(q.w1) << 32) | q.w0;
+    const unsigned long long U = r.neg ? 0ull - X : X;
+    r.w0 = static_cast<unsigned int>(U);
+    r.w1 = static_cast<unsigned int>(U >> 32);
+    r.w2 = 0u;
+  } else {
+    // 96-bit negate: ~x + 1
+    const unsigned int n0 = ~q.w0 + 1u;
+    const unsigned int c0 = (q.w0 == 0u) ? 1u : 0u;
+    const unsigned int n1 = ~q.w1 + c0;
+    const unsigned int c1 = (c0 && q.w1 == 0u) ? 1u : 0u;
+    const unsigned int n2 = ~q.w2 + c1;
+    r.w0 = r.neg ? n0 : q.w0;
+    r.w1 = r.neg ? n1 : q.w1;
+    r.w2 = r.neg ? n2 : q.w2;
+  }
+  return r;
+}
+__host__ __device__ constexpr unsigned int neg_pow_mod(int nw, int m) {  // (-2^(32 nw)) mod m
+  const unsigned int r = pow256_mod(4 * nw, m);
+  return r == 0u ? 0u : static_cast<unsigned int>(m) - r;
+}
+template <int L, int NW, typename Sink>
+__device__ __forceinline__ void emit_oz2_real_lean(const PrepS (&q)[4], int N, Sink sink) {
   if constexpr (L < kMaxModuli) {
     if (L < N) {
-      sink(L, pack4(oz2_residue<L>(q[0]), oz2_residue<L>(q[1]), oz2_residue<L>(q[2]), oz2_residue<L>(q[3])));
-      emit_oz2_real_from<L + 1>(q, N, sink);
+      constexpr int m = h_moduli[L];
+      if constexpr (m == 256) {
+        sink(L, __byte_perm(__byte_perm(q[0].w0, q[1].w0, 0x0040), __byte_perm(q[2].w0, q[3].w0, 0x0040), 0x5410));
+      } else {
+        constexpr unsigned int c0 = pack_w(0, m), c1 = pack_w(1, m), c2 = pack_w(2, m), mg = magic32(m);
+        constexpr unsigned int hm = (m - 1) / 2, kneg = neg_pow_mod(NW, m);
+        unsigned int u[4];
+#pragma unroll
+        for (int i = 0; i < 4; ++i) {
+          unsigned int t = __dp4a(q[i].w0, c0, (q[i].neg & kneg) + hm);
+          t = __dp4a(q[i].w1, c1, t);
+          if (NW == 3) t = __dp4a(q[i].w2, c2, t);
+          u[i] = t - __umulhi(t, mg) * static_cast<unsigned int>(m);
+        }
+        const unsigned int w = __byte_perm(__byte_perm(u[0], u[1], 0x0040), __byte_perm(u[2], u[3], 0x0040), 0x5410);
+        sink(L, (w + (128u - hm) * 0x01010101u) ^ 0x80808080u);
+      }
+      emit_oz2_real_lean<L + 1, NW>(q, N, sink);
     }
   }
 }
-template <int L, typename Sink>
-__device__ __forceinline__ void emit_oz2_cplx_from(const Prep (&re)[4], const Prep (&im)[4], int N, Sink sink) {
-  if constexpr (L < kMaxModuli) {
-    if (L < N) {
-      int a[4], b[4], s[4];
+// Complex operands (3M): residues of re, im and the Sigma plane sym(r_re + r_im) (R15), four elements
+// per word.  The moduli are walked by a run-time loop over a constant-memory table (the compile-time recursion of
+// the first version kept the addresses and constants of all 3N planes live: 252 registers, 12.5 % occupancy).  With
+// u_re == re + hm, u_im == im + hm (as in emit_oz2_real_lean; hm = floor(m / 2), so m = 256 runs through the same
+// code), t = u_re + u_im + (m - hm) == re + im + hm (mod m) and one more multiply-high reduction gives the Sigma
+// residue: no compares.
+struct ModC {
+  unsigned int c0, c1, c2, mg, negm, hm, kneg2, kneg3;  // negm = -m (mod 2^32)
+};
+#define EMU_MODC(L)                                                                                              \
+  {pack_w(0, h_moduli[L]), pack_w(1, h_moduli[L]), pack_w(2, h_moduli[L]), magic32(h_moduli[L]),                  \
+   0u - static_cast<unsigned int>(h_moduli[L]), static_cast<unsigned int>(h_moduli[L] / 2), neg_pow_mod(2, h_moduli[L]), \
+   neg_pow_mod(3, h_moduli[L])}
+__device__ __constant__ ModC c_modc[24] = {EMU_MODC(0),  EMU_MODC(1),  EMU_MODC(2),  EMU_MODC(3),  EMU_MODC(4),  EMU_MODC(5),
+                                           EMU_MODC(6),  EMU_MODC(7),  EMU_MODC(8),  EMU_MODC(9),  EMU_MODC(10), EMU_MODC(11),
+                                           EMU_MODC(12), EMU_MODC(13), EMU_MODC(14), EMU_MODC(15), EMU_MODC(16), EMU_MODC(17),
+                                           EMU_MODC(18), EMU_MODC(19), EMU_MODC(20), EMU_MODC(21), EMU_MODC(22), EMU_MODC(23)};
+#undef EMU_MODC
+
+// The integer multiplier ("fmaheavy": IDP.4A, IMAD, IMAD.HI) is the pipe these kernels saturate (ncu: 85 %), so the
+// reduction spends exactly NW + 2 instructions there: the start constant is added by ONE three-input add on the ALU
+// pipe (a two-input add tends to be emitted as IMAD.IADD) and t - q m is one multiply-add with -m.
+template <int NW>
+__device__ __forceinline__ unsigned int oz2_u(const PrepS &q, const ModC &mc) {  // (value + hm) mod m in [0, m)
+  unsigned int t = __dp4a(q.w0, mc.c0, 0u);
+  t = __dp4a(q.w1, mc.c1, t);
+  if (NW == 3) t = __dp4a(q.w2, mc.c2, t);
+  t = t + mc.hm + (q.neg & (NW == 2 ? mc.kneg2 : mc.kneg3));
+  return __umulhi(t, mc.mg) * mc.negm + t;
+}
+__device__ __forceinline__ unsigned int pack4u(const unsigned int (&u)[4]) {
+  return __byte_perm(__byte_perm(u[0], u[1], 0x0040), __byte_perm(u[2], u[3], 0x0040), 0x5410);
+}
+template <int NW, typename Sink>
+__device__ __forceinline__ void emit_oz2_cplx_lean(const PrepS (&re)[4], const PrepS (&im)[4], int N, Sink sink) {
+#pragma unroll 1
+  for (int L = 0; L < N; ++L) {
+    const ModC mc = c_modc[L];
+    const unsigned int mhm = 0u - mc.negm - mc.hm;  // m - hm
+    unsigned int ua[4], ub[4], us[4];
 #pragma unroll
-      for (int i = 0; i < 4; ++i) {
-        a[i] = oz2_residue<L>(re[i]);
-        b[i] = oz2_residue<L>(im[i]);
-        s[i] = sym_small<L>(a[i] + b[i]);
-      }
-      sink(L, pack4(a[0], a[1], a[2], a[3]));
-      sink(N + L, pack4(b[0], b[1], b[2], b[3]));
-      sink(2 * N + L, pack4(s[0], s[1], s[2], s[3]));
-      emit_oz2_cplx_from<L + 1>(re, im, N, sink);
+    for (int i = 0; i < 4; ++i) {
+      ua[i] = oz2_u<NW>(re[i], mc);
+      ub[i] = oz2_u<NW>(im[i], mc);
+      const unsigned int t = ua[i] + ub[i] + mhm;
+      us[i] = __umulhi(t, mc.mg) * mc.negm + t;
     }
+    const unsigned int bias = (128u - mc.hm) * 0x01010101u;  // (u + 128 - hm) ^ 0x80 = u - hm as int8, all four bytes at once
+    sink(L, (pack4u(ua) + bias) ^ 0x80808080u);
+    sink(N + L, (pack4u(ub) + bias) ^ 0x80808080u);
+    sink(2 * N + L, (pack4u(us) + bias) ^ 0x80808080u);
   }
 }
 
@@ -346,12 +410,18 @@ __device__ __forceinline__ void emit_quad(const T (&v)[4][W], int e_row, int par
     if constexpr (PARAM >= 16) emit_oz1_b8<PARAM - 16>(a, sink);  // PARAM = 16 + p: balanced 8-bit digits
     else emit_oz1<PARAM>(a, sink);
   } else if constexpr (W == 1) {
-    emit_oz2_real_from<0>(a, param, sink);
-  } else {
-    Prep b[4];
+    PrepS u[4];
 #pragma unroll
-    for (int i = 0; i < 4; ++i) b[i] = prepare<T, NW>(v[i][W - 1], e_row, scale_bits);
-    emit_oz2_cplx_from<0>(a, b, param, sink);
+    for (int i = 0; i < 4; ++i) u[i] = twos_complement<NW>(a[i]);
+    emit_oz2_real_lean<0, NW>(u, param, sink);
+  } else {
+    PrepS re[4], im[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i) {
+      re[i] = twos_complement<NW>(a[i]);
+      im[i] = twos_complement<NW>(prepare<T, NW>(v[i][W - 1], e_row, scale_bits));
+    }
+    emit_oz2_cplx_lean<NW>(re, im, param, sink);
   }
 }
 
@@ -405,6 +475,89 @@ __global__ void __launch_bounds__(256) planes_rows_kernel(const T *__restrict__ 
   }
 }
 
+
+// 4 * W consecutive scalars from a 32-byte (double) / 16-byte (float) aligned address: 256-bit / 128-bit loads
+template <int W>
+__device__ __forceinline__ void load_quad_vec(const double *p, double (&v)[4][W]) {
+  double f[4 * W];
+#pragma unroll
+  for (int i = 0; i < W; ++i)
+    asm("ld.global.nc.v4.f64 {%0,%1,%2,%3}, [%4];" : "=d"(f[4 * i]), "=d"(f[4 * i + 1]), "=d"(f[4 * i + 2]), "=d"(f[4 * i + 3]) : "l"(p + 4 * i));
+#pragma unroll
+  for (int i = 0; i < 4 * W; ++i) v[i / W][i % W] = f[i];
+}
+template <int W>
+__device__ __forceinline__ void load_quad_vec(const float *p, float (&v)[4][W]) {
+#pragma unroll
+  for (int i = 0; i < W; ++i) {
+    const float4 t = __ldg(reinterpret_cast<const float4 *>(p) + i);
+    const float f[4] = {t.x, t.y, t.z, t.w};
+#pragma unroll
+    for (int j = 0; j < 4; ++j) v[(4 * i + j) / W][(4 * i + j) % W] = f[j];
+  }
+}
+
+// ---- rows, register-resident (kpad * W <= 32 NT): ONE read of X -------------------
+// One CTA per row; every thread loads its 8 / W quads (32 scalars) once with vector loads, the row maximum is
+// reduced from the registers, and the digits / residues are computed from the same registers: X is requested from
+// memory exactly once (the two-phase kernel above re-reads the row, which misses L2 at 8192^2: 1.0 GB of DRAM reads
+// for a 0.5 GB operand, profiles/).  Longer rows keep the two-phase kernel.
+template <typename T, int W, int MODE, int PARAM, int NT>
+__global__ void __launch_bounds__(NT) planes_rows_reg_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows,
+                                                              int64_t k, int64_t kpad, int32_t *__restrict__ e_out,
+                                                              int param, int scale_bits, int8_t *__restrict__ out,
+                                                              int64_t xstride, int64_t plane_rows) {
+  constexpr int R = 8 / W;
+  const int64_t row = static_cast<int64_t>(blockIdx.y) * rows + blockIdx.x;
+  const T *src = X + (static_cast<int64_t>(blockIdx.y) * xstride + static_cast<int64_t>(blockIdx.x) * ldx) * W;
+  const bool vec = (reinterpret_cast<uintptr_t>(src) & (sizeof(T) == 8 ? 31 : 15)) == 0;
+  const int kk = static_cast<int>(k);
+  T v[R][4][W];
+  unsigned long long mx = 0;
+#pragma unroll
+  for (int q = 0; q < R; ++q) {
+    const int h0 = (static_cast<int>(threadIdx.x) + q * NT) * 4;
+    if (vec && h0 + 4 <= kk) {
+      load_quad_vec<W>(src + static_cast<int64_t>(h0) * W, v[q]);
+    } else {
+#pragma unroll
+      for (int i = 0; i < 4; ++i)
+#pragma unroll
+        for (int c = 0; c < W; ++c) v[q][i][c] = (h0 + i < kk) ? src[static_cast<int64_t>(h0 + i) * W + c] : T(0);
+    }
+#pragma unroll
+    for (int i = 0; i < 4; ++i)
+#pragma unroll
+      for (int c = 0; c < W; ++c) {
+        const unsigned long long b = abs_bits(v[q][i][c]);
+        mx = b > mx ? b : mx;
+      }
+  }
+  for (int o = 16; o > 0; o >>= 1) {
+    const unsigned long long y = __shfl_xor_sync(0xffffffffu, mx, o);
+    mx = y > mx ? y : mx;
+  }
+  __shared__ unsigned long long red[NT / 32];
+  if ((threadIdx.x & 31) == 0) red[threadIdx.x >> 5] = mx;
+  __syncthreads();
+#pragma unroll
+  for (int w = 0; w < NT / 32; ++w) mx = red[w] > mx ? red[w] : mx;
+  const int e_row = exponent_of_maxbits<T>(mx);
+  if (threadIdx.x == 0) e_out[row] = e_row;
+
+  const int64_t plane_stride = plane_rows * kpad;
+#pragma unroll
+  for (int q = 0; q < R; ++q) {
+    const int h0 = (static_cast<int>(threadIdx.x) + q * NT) * 4;
+    if (h0 < kpad) {
+      int8_t *dst = out + row * kpad + h0;
+      emit_quad<T, W, MODE, PARAM>(v[q], e_row, param, scale_bits, [&](int plane, unsigned int word) {
+        *reinterpret_cast<unsigned int *>(dst + plane * plane_stride) = word;
+      });
+    }
+  }
+}
+
 // ---- columns: X is k x rows (ldx); transposed through shared memory ----------
 // tile = 32 columns x TH k; thread (lane = column, warp = k-quad index).
 template <typename T, int W, int MODE, int PARAM, int TH>
@@ -453,11 +606,12 @@ __global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ 
   }
 }
 
+
 // by_cols = 0: fused scan + planes of the rows of X, exponents written to e.
-// by_cols = 1: planes of the columns of X; maxbits[j] must hold the column maxima (launch_colmax), exponents written to e.
+// by_cols = 1: column maxima (launch_colmax into the scratch maxbits[rows]) + planes of the columns of X, exponents written to e.
 template <typename T, int W, int MODE, int PARAM>
-static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X,
-                         int64_t ldx, const unsigned long long *maxbits, int32_t *e, int param, int scale_bits, int nplanes,
+static int launch_planes(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X,
+                         int64_t ldx, unsigned long long *maxbits, int32_t *e, int param, int scale_bits, int nplanes,
                          int8_t *out, int batch = 1, int64_t xstride = 0) {
   if (rows == 0 || kpad == 0 || batch == 0) return EMUGEMM_OK;
   if (batch > 65535) return EMUGEMM_ERR_ARG;  // grid.y / grid.z
@@ -466,10 +620,33 @@ static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k,
   const T *x = static_cast<const T *>(X);
   if (!by_cols) {
     const dim3 grid(static_cast<unsigned>(rows), static_cast<unsigned>(batch));
-    planes_rows_kernel<T, W, MODE, PARAM><<<grid, 256, 0, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, out, xstride,
-                                                                 plane_rows);
+    const bool two_phase = (ctx->dbg_flags & 32) != 0;  // dbg bit 5: the two-phase kernels (A/B timing)
+    // Scheme I digits: the register-resident single-read kernel when the row fits (p = 2: 0.159 -> 0.111 ms, p = 8: 0.246 ->
+    // 0.218 ms at 8192^2).  Scheme II residues are bound by the integer pipes, not by the second read: there the 80
+    // registers of the resident row cost occupancy (N = 16: 0.431 -> 0.475 ms, 3M N = 18: 1.81 -> 2.89 ms), so they keep
+    // the two-phase kernel.
+    bool done = false;
+    if constexpr (MODE == 0) {
+      if (!two_phase && kpad * W <= 32 * 256) {
+        planes_rows_reg_kernel<T, W, MODE, PARAM, 256><<<grid, 256, 0, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, out,
+                                                                              xstride, plane_rows);
+        done = true;
+      } else if (!two_phase && kpad * W <= 32 * 512) {
+        planes_rows_reg_kernel<T, W, MODE, PARAM, 512><<<grid, 512, 0, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, out,
+                                                                              xstride, plane_rows);
+        done = true;
+      }
+    }
+    if (!done)
+      planes_rows_kernel<T, W, MODE, PARAM><<<grid, 256, 0, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, out, xstride,
+                                                                   plane_rows);
     ctx->launches++;
   } else {
+    // The column maxima are a true dependency: a separate launch reads X once more.  A single-read variant (tile kept in
+    // registers, per-panel arrival counters, tickets) measured SLOWER: the panel barrier re-synchronises the CTAs of
+    // a wave, so the load phase and the digit phase no longer overlap (p = 2: 0.207 -> 0.215 ms, p = 8: 0.30 -> 0.34 ms,
+    // N = 16: 0.64 -> 0.70 ms at 8192^2).
+    EMU_TRY(launch_colmax(ctx, elem, rows, k, X, ldx, maxbits, batch, xstride));
     if (nplanes <= 20) {
       constexpr int TH = 128;
       const size_t smem = static_cast<size_t>(nplanes) * 32 * (TH / 4 + 1) * 4;
@@ -493,14 +670,14 @@ static int launch_planes(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k,
 
 template <typename T, int P>
 static int slice_p(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
-                   const unsigned long long *maxbits, int32_t *e, int slice_bits, int8_t *out, int batch, int64_t xstride) {
+                   unsigned long long *maxbits, int32_t *e, int slice_bits, int8_t *out, int batch, int64_t xstride) {
   if (slice_bits == 8)  // |X| = trunc(|x| 2^(8p - 2 - e)): two guard bits
-    return launch_planes<T, 1, 0, 16 + P>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, 8 * P - 2, P, out, batch, xstride);
-  return launch_planes<T, 1, 0, P>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, kBeta * P, P, out, batch, xstride);
+    return launch_planes<T, 1, 0, 16 + P>(ctx, sizeof(T) == 8 ? kF64 : kF32, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, 8 * P - 2, P, out, batch, xstride);
+  return launch_planes<T, 1, 0, P>(ctx, sizeof(T) == 8 ? kF64 : kF32, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, kBeta * P, P, out, batch, xstride);
 }
 
 int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
-                     const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int p, int slice_bits,
+                     const void *X, int64_t ldx, unsigned long long *maxbits, int32_t *e, int p, int slice_bits,
                      int8_t *out, int batch, int64_t xstride) {
 #define EMU_SLICE_CASE(T, PP) case PP: return slice_p<T, PP>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, slice_bits, out, batch, xstride)
   if (elem == kF64) {
@@ -522,22 +699,22 @@ int launch_oz1_slice(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int6
 }
 
 int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, int64_t k, int64_t kpad,
-                        const void *X, int64_t ldx, const unsigned long long *maxbits, int32_t *e, int n_moduli, int t_bits,
+                        const void *X, int64_t ldx, unsigned long long *maxbits, int32_t *e, int n_moduli, int t_bits,
                         int8_t *out, int batch, int64_t xstride) {
   if (t_bits < 1 || t_bits > 95) return EMUGEMM_ERR_ARG;  // three 32-bit words hold |a'| < 2^t (t = 77 at most: N = 20, k = 1)
   const bool two = t_bits <= 64;  // |a'| < 2^t fits two 32-bit words: one byte dot product less per residue
   if (elem == kF64)
-    return two ? launch_planes<double, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride)
-               : launch_planes<double, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride);
+    return two ? launch_planes<double, 1, 1, 2>(ctx, kF64, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride)
+               : launch_planes<double, 1, 1, 3>(ctx, kF64, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride);
   if (elem == kF32)  // 24-bit inputs (Scheme II SGEMM)
-    return two ? launch_planes<float, 1, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride)
-               : launch_planes<float, 1, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride);
+    return two ? launch_planes<float, 1, 1, 2>(ctx, kF32, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride)
+               : launch_planes<float, 1, 1, 3>(ctx, kF32, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, n_moduli, out, batch, xstride);
   if (elem == kC64)
-    return two ? launch_planes<float, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride)
-               : launch_planes<float, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride);
+    return two ? launch_planes<float, 2, 1, 2>(ctx, kC64, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride)
+               : launch_planes<float, 2, 1, 3>(ctx, kC64, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride);
   if (elem == kZ128)
-    return two ? launch_planes<double, 2, 1, 2>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride)
-               : launch_planes<double, 2, 1, 3>(ctx, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride);
+    return two ? launch_planes<double, 2, 1, 2>(ctx, kZ128, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride)
+               : launch_planes<double, 2, 1, 3>(ctx, kZ128, by_cols, rows, k, kpad, X, ldx, maxbits, e, n_moduli, t_bits, 3 * n_moduli, out, batch, xstride);
   return EMUGEMM_ERR_ARG;
 }
 
