@@ -96,9 +96,10 @@ __device__ __forceinline__ double round_nearest(double x) {  // |x| < 2^51: roun
   return (x + big) - big;
 }
 
-constexpr int kCrtVec = 8;  // columns per thread on the vector path (one 8-byte load per residue plane)
+// columns per thread: 8 (one 8-byte load per residue plane) for real outputs, 4 for complex ones, whose second
+// accumulation pass otherwise pushes the kernel to 153 registers / 12 % occupancy (profiles/r1_prepass_v2.md)
 
-template <bool VEC>
+template <bool VEC, int kCrtVec>
 __device__ __forceinline__ void crt_accumulate(const CrtConst &k, const int8_t *__restrict__ src, int64_t plane, int64_t j0,
                                                int64_t n, double (&shi)[kCrtVec], double (&slo)[kCrtVec]) {
   // all residue planes are requested before any is consumed: up to 20 independent 8-byte loads in flight per
@@ -108,15 +109,17 @@ __device__ __forceinline__ void crt_accumulate(const CrtConst &k, const int8_t *
   for (int l = 0; l < kMaxModuli; ++l) {
     w0[l] = w1[l] = 0x80808080u;
     if (l < k.N) {
-      if (VEC) {
+      if (VEC && kCrtVec == 8) {
         const uint2 w = __ldg(reinterpret_cast<const uint2 *>(src + l * plane));
         w0[l] = w.x; w1[l] = w.y;
+      } else if (VEC) {
+        w0[l] = __ldg(reinterpret_cast<const unsigned *>(src + l * plane));
       } else {
         unsigned a = 0, b = 0;
 #pragma unroll
         for (int e = 0; e < 4; ++e) {
           if (j0 + e < n) a |= static_cast<unsigned>(static_cast<uint8_t>(src[l * plane + e])) << (8 * e);
-          if (j0 + 4 + e < n) b |= static_cast<unsigned>(static_cast<uint8_t>(src[l * plane + 4 + e])) << (8 * e);
+          if (kCrtVec == 8 && j0 + 4 + e < n) b |= static_cast<unsigned>(static_cast<uint8_t>(src[l * plane + 4 + e])) << (8 * e);
         }
         w0[l] = a; w1[l] = b;
       }
@@ -145,7 +148,7 @@ __device__ __forceinline__ double crt_finish(const CrtConst &k, double shi, doub
 
 // one thread per 8 consecutive columns of one row
 // KIND: 0 = FP64 C, 1 = complex128 C, 2 = FP32 C (SGEMM), 3 = complex64 C (CGEMM); 2 and 3 round once more to float
-template <bool VEC, int KIND>
+template <bool VEC, int KIND, int kCrtVec>
 __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const int8_t *__restrict__ CR,
                                                   const int32_t *__restrict__ eA, const int32_t *__restrict__ eB,
                                                   int tsum, double ar, double ai, double br, double bi,
@@ -170,7 +173,7 @@ __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const in
     sc2[e] = pow2_dev(E2 - (E2 >> 1));
   }
   double shi[kCrtVec], slo[kCrtVec], vr[kCrtVec];
-  crt_accumulate<VEC>(k, CR + i * n + j0, plane, j0, n, shi, slo);
+  crt_accumulate<VEC, kCrtVec>(k, CR + i * n + j0, plane, j0, n, shi, slo);
 #pragma unroll
   for (int e = 0; e < kCrtVec; ++e) vr[e] = crt_finish(k, shi[e], slo[e]) * sc1[e] * sc2[e];
   if (KIND == 2) {
@@ -183,8 +186,8 @@ __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const in
       f[e] = static_cast<float>(x);
     }
     if (VEC && (ldc % 4 == 0) && ((reinterpret_cast<uintptr_t>(C) & 15) == 0)) {
-      reinterpret_cast<float4 *>(o)[0] = make_float4(f[0], f[1], f[2], f[3]);
-      reinterpret_cast<float4 *>(o)[1] = make_float4(f[4], f[5], f[6], f[7]);
+#pragma unroll
+      for (int e = 0; e < kCrtVec; e += 4) reinterpret_cast<float4 *>(o)[e / 4] = make_float4(f[e], f[e + 1], f[e + 2], f[e + 3]);
     } else {
 #pragma unroll
       for (int e = 0; e < kCrtVec; ++e)
@@ -210,7 +213,7 @@ __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const in
     }
   } else {
     double vi[kCrtVec];
-    crt_accumulate<VEC>(k, CR + static_cast<int64_t>(k.N) * plane + i * n + j0, plane, j0, n, shi, slo);
+    crt_accumulate<VEC, kCrtVec>(k, CR + static_cast<int64_t>(k.N) * plane + i * n + j0, plane, j0, n, shi, slo);
 #pragma unroll
     for (int e = 0; e < kCrtVec; ++e) vi[e] = crt_finish(k, shi[e], slo[e]) * sc1[e] * sc2[e];
     const bool has_beta = (br != 0.0 || bi != 0.0);
@@ -251,26 +254,27 @@ int launch_oz2_crt(emugemm_ctx *ctx, const Oz2CrtArgs &a) {
   if (a.m == 0 || a.n == 0) return EMUGEMM_OK;
   CrtConst k;
   crt_constants(a.n_moduli, k);
-  const int64_t work = a.m * ((a.n + kCrtVec - 1) / kCrtVec);
+  const int kind = a.is_complex ? (a.out_f32 ? 3 : 1) : (a.out_f32 ? 2 : 0);
+  const int V = a.is_complex ? 4 : 8;  // columns per thread (real outputs with 4: 0.524 -> 0.551 ms, measured)
+  const int64_t work = a.m * ((a.n + V - 1) / V);
   const unsigned grid = static_cast<unsigned>((work + 255) / 256);
-  const bool vec = (a.n % kCrtVec == 0) && ((reinterpret_cast<uintptr_t>(a.CR) & 7) == 0);
+  const bool vec = (a.n % V == 0) && ((reinterpret_cast<uintptr_t>(a.CR) & (V - 1)) == 0);
   const int tsum = a.tA + a.tB;
   const int batch = a.batch > 0 ? a.batch : 1;
   if (batch > 65535) return EMUGEMM_ERR_ARG;
   // bytes between the C matrices of consecutive batch entries (element = float / double, x2 for complex)
   const int64_t c_entry_bytes = a.batch_stride_c * (a.out_f32 ? 4 : 8) * (a.is_complex ? 2 : 1);
-#define EMU_CRT_LAUNCH(V, Z)                                                                                              \
-  crt_kernel<V, Z><<<dim3(grid, static_cast<unsigned>(batch)), 256, 0, ctx->stream>>>(a.m, a.n, a.CR, a.eA, a.eB, tsum, a.alpha[0], a.alpha[1], a.beta[0], \
+#define EMU_CRT_LAUNCH(V_, Z, W_)                                                                                              \
+  crt_kernel<V_, Z, W_><<<dim3(grid, static_cast<unsigned>(batch)), 256, 0, ctx->stream>>>(a.m, a.n, a.CR, a.eA, a.eB, tsum, a.alpha[0], a.alpha[1], a.beta[0], \
                                                    a.beta[1], a.C, a.ldc, k, c_entry_bytes)
-  const int kind = a.is_complex ? (a.out_f32 ? 3 : 1) : (a.out_f32 ? 2 : 0);
-  if (vec && kind == 3) EMU_CRT_LAUNCH(true, 3);
-  else if (kind == 3) EMU_CRT_LAUNCH(false, 3);
-  else if (vec && kind == 1) EMU_CRT_LAUNCH(true, 1);
-  else if (vec && kind == 2) EMU_CRT_LAUNCH(true, 2);
-  else if (vec) EMU_CRT_LAUNCH(true, 0);
-  else if (kind == 1) EMU_CRT_LAUNCH(false, 1);
-  else if (kind == 2) EMU_CRT_LAUNCH(false, 2);
-  else EMU_CRT_LAUNCH(false, 0);
+  if (vec && kind == 3) EMU_CRT_LAUNCH(true, 3, 4);
+  else if (kind == 3) EMU_CRT_LAUNCH(false, 3, 4);
+  else if (vec && kind == 1) EMU_CRT_LAUNCH(true, 1, 4);
+  else if (vec && kind == 2) EMU_CRT_LAUNCH(true, 2, 8);
+  else if (vec) EMU_CRT_LAUNCH(true, 0, 8);
+  else if (kind == 1) EMU_CRT_LAUNCH(false, 1, 4);
+  else if (kind == 2) EMU_CRT_LAUNCH(false, 2, 8);
+  else EMU_CRT_LAUNCH(false, 0, 8);
 #undef EMU_CRT_LAUNCH
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
