@@ -1,4 +1,6 @@
-// prepass.cu -- bandwidth-bound decomposition kernels.
+// prepass.cu -- decomposition kernels: one pass over the operand, one write of
+// the planes; the digit kernels end up bound by the ALU pipe, the residue kernels by the integer multiplier
+// (profiles/r1_prepass_v2.md).
 //
 //  * exponent scan: max |x| bit pattern per row of A / per column of B -> frexp
 //    exponent ("each row of A is scaled by a power-of-two factor";
