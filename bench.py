@@ -390,7 +390,10 @@ def main():
             # the kernel's own MMA issue schedule on operands resident in shared memory (no TMA, no epilogue):
             # what the tensor pipe sustains for this p; Scheme II uses the plain N = 256 schedule (p = 1)
             pp = w["p"] if a.scheme in ("oz1", "oz1s") else 1
-            _, tops, eff = h.dbg_oz1_issue_probe(pp, True, 4000)
+            hp = E.EmuGemm(probes=True)   # the PROBES build of the same sources (probe kernels are not in the product)
+            hp.set_stream(stream)
+            _, tops, eff = hp.dbg_oz1_issue_probe(pp, True, 4000)
+            hp.close()
             detail["issue_probe_per_clock_efficiency"] = eff
             detail["issue_probe_tops"] = tops
             roof["frac_of_probe"] = achieved / tops

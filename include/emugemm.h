@@ -262,8 +262,20 @@ int emugemm_dbg_oz2_crt(emugemm_handle_t h, int64_t m, int64_t n, int n_moduli, 
                         double beta, double *C, int64_t ldc);
 /* Host-side helpers (no GPU): bit budget (returns T or < 0), overflow-safe chunk length. */
 int emugemm_oz2_budget(int n_moduli, int64_t k, int is3m, int *tA, int *tB);
+/* Host-side (no GPU): the integer constants of the exact FP64 CRT kernel for n_moduli (R17; PAPER.md:127-130
+ * Eq. 8), so that a CPU test can check them against big integers.  Moduli are combined in pairs (2q, 2q+1), an odd
+ * last one stays alone: *n_pairs = ceil(N/2).  Every pair weight W_q = (P/M_q)((P/M_q)^-1 mod M_q), M_q = m1 m2, and P
+ * itself are written in *n_digits balanced base-2^(*digit_bits) digits: digits[q * n_digits + j], q < n_pairs, is
+ * digit j of W_q, row q = n_pairs is P (sum_j digit_j 2^(j digit_bits), |digit| <= 2^(digit_bits-1)); pair[5q..5q+4] =
+ * {M_q, K1, K2, C0, floor(2^32/M_q)}: x = (K1 c1 + K2 c2 + C0) mod M_q is the pair residue (K1 == 1 mod m1, == 0 mod
+ * m2, K2 the other way round; C0 a multiple of M_q >= 2^24).  Caller arrays (HOST): digits >= 11 * 5 int64, pair >=
+ * 10 * 5 uint32.  Returns 0, or EMUGEMM_ERR_ARG.                                                                  */
+int emugemm_dbg_crt_constants(int n_moduli, int *n_pairs, int *n_digits, int *digit_bits, long long *digits, unsigned *pair);
 int64_t emugemm_oz1_chunk_k(int p);                       /* 7-bit digits */
 int64_t emugemm_oz1_chunk_k_bits(int p, int slice_bits);   /* p k_c dmax^2 <= 2^31 - 1, dmax = 127 / 128 */
+/* ---- PROBES build only (libemugemm_probes.so, compiled with -DEMUGEMM_PROBES; bench.py loads it for its probe leg).
+ * The shipped libemugemm.so exports none of the three calls below and carries no experiment switch in its kernels. */
+#ifdef EMUGEMM_PROBES
 /* Issue-bound tcgen05.mma kind::i8 probe (operands resident in shared memory, no
  * loads in the loop), one CTA per SM.  ops = HOST array of n_ops (<= 64) MMAs, five
  * ints each: {TMEM column of D, width N (multiple of 16, <= 256), A slot 0..7
@@ -296,6 +308,8 @@ int emugemm_dbg_oz1_issue_probe(emugemm_handle_t h, int p, int use_collector, in
  * single-read kernel.
  * Used to attribute tensor-pipe idle time.                        */
 int emugemm_dbg_set_flags(emugemm_handle_t h, int flags);
+
+#endif /* EMUGEMM_PROBES */
 
 #ifdef __cplusplus
 }

@@ -8,6 +8,7 @@ import os
 import re
 
 LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libemugemm.so")
+PROBES_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libemugemm_probes.so")
 _HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "emugemm.h")
 
 OZ1, OZ2, OZ2_3M, OZ1_4M = 1, 2, 3, 4
@@ -27,17 +28,18 @@ class EmuGemmError(RuntimeError):
         self.status = status
 
 
-_lib = None
+_libs = {}
 
 
-def load_library():
-    """dlopen the in-tree library; raises (never falls back) if it has not been built."""
-    global _lib
-    if _lib is None:
-        if not os.path.exists(LIB_PATH):
-            raise FileNotFoundError(f"{LIB_PATH} not built: run `python -m paper_2606_25453_b200.build` "
+def load_library(probes=False):
+    """dlopen the in-tree library; raises (never falls back) if it has not been built.  probes=True: the PROBES build
+    (same sources + -DEMUGEMM_PROBES: emugemm_dbg_set_flags and the tensor-pipe probes), used only by bench.py's probe leg."""
+    if probes not in _libs:
+        path = PROBES_LIB_PATH if probes else LIB_PATH
+        if not os.path.exists(path):
+            raise FileNotFoundError(f"{path} not built: run `python -m paper_2606_25453_b200.build` "
                                     "(the product path has no CPU fallback)")
-        lib = C.CDLL(LIB_PATH)
+        lib = C.CDLL(path)
         lib.emugemm_status_string.restype = C.c_char_p
         lib.emugemm_workspace_bytes.restype = _sz
         lib.emugemm_workspace_bytes.argtypes = [_int, _int, _i64, _i64, _i64, _int]
@@ -45,13 +47,16 @@ def load_library():
         lib.emugemm_operand_bytes.argtypes = [_int, _i64, _i64, _int]
         lib.emugemm_oz1_chunk_k.restype = _i64
         lib.emugemm_oz1_chunk_k_bits.restype = _i64
-        _lib = lib
-    return _lib
+        _libs[probes] = lib
+    return _libs[probes]
 
 
-def exported_symbols():
-    """Names declared in include/emugemm.h (used by the not-gpu load test)."""
+def exported_symbols(probes=False):
+    """Names declared in include/emugemm.h (used by the not-gpu load test); the `#ifdef EMUGEMM_PROBES` block only for
+    the PROBES build."""
     text = open(_HEADER).read()
+    if not probes:
+        text = re.sub(r"#ifdef EMUGEMM_PROBES.*?#endif /\* EMUGEMM_PROBES \*/", "", text, flags=re.S)
     return sorted(set(re.findall(r"\b(emugemm_[a-z0-9_]+)\s*\(", text)))
 
 
@@ -59,6 +64,20 @@ def oz2_budget(n_moduli, k, is3m=False):
     a, b = _int(0), _int(0)
     T = load_library().emugemm_oz2_budget(_int(n_moduli), _i64(k), _int(1 if is3m else 0), C.byref(a), C.byref(b))
     return int(T), a.value, b.value
+
+
+def crt_constants(n_moduli):
+    """emugemm_dbg_crt_constants (host only) -> dict(n_pairs, n_digits, digit_bits, W=[digit lists], P=[digits], pair=[(M, K1, K2, C0, magic)])."""
+    npairs, nd, g = _int(0), _int(0), _int(0)
+    digits = (C.c_longlong * 55)()
+    pair = (C.c_uint * 50)()
+    st = load_library().emugemm_dbg_crt_constants(_int(n_moduli), C.byref(npairs), C.byref(nd), C.byref(g), digits, pair)
+    if st != 0:
+        raise EmuGemmError(st, "emugemm_dbg_crt_constants")
+    NP, J = npairs.value, nd.value
+    rows = [[int(digits[q * J + j]) for j in range(J)] for q in range(NP + 1)]
+    return dict(n_pairs=NP, n_digits=J, digit_bits=g.value, W=rows[:NP], P=rows[NP],
+                pair=[tuple(int(pair[5 * q + i]) for i in range(5)) for q in range(NP)])
 
 
 def oz1_chunk_k(p, slice_bits=7):
@@ -74,14 +93,16 @@ class EmuGemm:
     from the tensors (last dim contiguous).  Workspace is a torch uint8 tensor owned by this object and
     grown on demand OUTSIDE the timed hot path via reserve()."""
 
-    def __init__(self):
+    def __init__(self, probes=False):
         import torch
         self._torch = torch
-        self._lib = load_library()
+        self._lib = load_library(probes)
         self._h = _vp(None)
         self._check(self._lib.emugemm_create(C.byref(self._h)))
         self._ws = None
         self.slice_bits = 7
+        self._device = torch.cuda.current_device()
+        self._stream = None
         self.set_stream(torch.cuda.current_stream())
 
     def close(self):
@@ -102,6 +123,7 @@ class EmuGemm:
     # ---- handle ------------------------------------------------------------
     def set_stream(self, stream):
         self._check(self._lib.emugemm_set_stream(self._h, _vp(stream.cuda_stream)))
+        self._stream = stream
 
     def set_slice_bits(self, bits):
         """Scheme I digits: 7 = sign-magnitude (default), 8 = balanced base 256 (see include/emugemm.h)."""
@@ -114,8 +136,14 @@ class EmuGemm:
     def reserve(self, nbytes):
         torch = self._torch
         if self._ws is None or self._ws.numel() < nbytes + 1024:
+            if self._ws is not None and self._stream is not None:
+                # kernels of earlier calls may still use the old workspace on the handle's stream, which need not be
+                # torch's current stream: the caching allocator must not hand the block out before they are done
+                self._ws.record_stream(self._stream)
             self._ws = None
             raw = torch.empty(int(nbytes) + 2048, dtype=torch.uint8, device="cuda")
+            if self._stream is not None:
+                raw.record_stream(self._stream)
             self._ws = raw
         off = (-self._ws.data_ptr()) % 1024
         self._check(self._lib.emugemm_set_workspace(self._h, _vp(self._ws.data_ptr() + off), _sz(self._ws.numel() - off)))
@@ -146,14 +174,32 @@ class EmuGemm:
         return t.stride(0)
 
     # transa / transb: the tensor holds the TRANSPOSE of the operand (A: k x m, B: n x k), row-major
-    @staticmethod
-    def _dims(A, B, transa, transb):
+    def _dims(self, A, B, transa=False, transb=False, C_=None, dtype=None):
+        """(m, n, k) after checking what the C ABI cannot see from raw pointers: every matrix is a 2-D CUDA tensor of
+        the entry point's dtype on the handle's device, the inner dimensions agree and C is m x n (ValueError before
+        the library is entered: a wrong dtype or shape would make the kernels read or write out of bounds)."""
+        torch = self._torch
+        for name, X in (("A", A), ("B", B), ("C", C_)):
+            if X is None:
+                continue
+            if not isinstance(X, torch.Tensor) or X.dim() != 2:
+                raise ValueError(f"{name}: a 2-D torch tensor is required")
+            if not X.is_cuda or X.device.index != self._device:
+                raise ValueError(f"{name}: must live on cuda:{self._device}, the device of this handle (got {X.device})")
+            if dtype is not None and X.dtype != dtype:
+                raise ValueError(f"{name}: dtype {X.dtype} given, this entry point takes {dtype}")
+            if X.stride(-1) != 1 and X.shape[-1] > 1:
+                raise ValueError(f"{name}: the last dimension must be contiguous")
         m, k = (A.shape[1], A.shape[0]) if transa else A.shape
-        n = B.shape[0] if transb else B.shape[1]
+        kb, n = (B.shape[1], B.shape[0]) if transb else B.shape
+        if k != kb:
+            raise ValueError(f"inner dimensions differ: op(A) is {m} x {k}, op(B) is {kb} x {n}")
+        if C_ is not None and tuple(C_.shape) != (m, n):
+            raise ValueError(f"C is {tuple(C_.shape)}, expected ({m}, {n})")
         return m, n, k
 
     def dgemm_oz1(self, A, B, C_, p, alpha=1.0, beta=0.0, transa=False, transb=False):
-        m, n, k = self._dims(A, B, transa, transb)
+        m, n, k = self._dims(A, B, transa, transb, C_, self._torch.float64)
         self._reserve_for(OZ1, 8, m, n, k, p)
         self._check(self._lib.emugemm_dgemm_oz1_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), _dbl(alpha),
                                                    _ptr(A), _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), _dbl(beta), _ptr(C_),
@@ -161,7 +207,7 @@ class EmuGemm:
         return C_
 
     def sgemm_oz1(self, A, B, C_, p, alpha=1.0, beta=0.0, transa=False, transb=False):
-        m, n, k = self._dims(A, B, transa, transb)
+        m, n, k = self._dims(A, B, transa, transb, C_, self._torch.float32)
         self._reserve_for(OZ1, 4, m, n, k, p)
         self._check(self._lib.emugemm_sgemm_oz1_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), _flt(alpha),
                                                    _ptr(A), _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), _flt(beta), _ptr(C_),
@@ -171,6 +217,13 @@ class EmuGemm:
     def _batched(self, fn, cvt, elem, A, B, C_, p, alpha, beta, scheme=OZ1):
         # A: (batch, m, k) or (m, k) shared by all entries; B: (batch, k, n) or (k, n); C_: (batch, m, n).
         # The last dimension is contiguous, dimension -2 carries the leading dimension, dimension 0 the batch stride.
+        torch = self._torch
+        want = {4: torch.float32, 8: torch.float64, 16: torch.complex128}[elem]
+        for name, X in (("A", A), ("B", B), ("C", C_)):
+            if not isinstance(X, torch.Tensor) or not X.is_cuda or X.device.index != self._device or X.dtype != want:
+                raise ValueError(f"{name}: a {want} tensor on cuda:{self._device} is required")
+        if C_.dim() != 3 or A.dim() not in (2, 3) or B.dim() not in (2, 3):
+            raise ValueError("batched operands: A (batch, m, k) or (m, k), B (batch, k, n) or (k, n), C (batch, m, n)")
         batch, m, n = C_.shape
         k = A.shape[-1]
         for X, shp in ((A, (m, k)), (B, (k, n))):
@@ -200,7 +253,7 @@ class EmuGemm:
         return self._batched(self._lib.emugemm_sgemm_oz2_strided_batched, _flt, 4, A, B, C_, n_moduli, alpha, beta, OZ2)
 
     def dgemm_oz2(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0, transa=False, transb=False):
-        m, n, k = self._dims(A, B, transa, transb)
+        m, n, k = self._dims(A, B, transa, transb, C_, self._torch.float64)
         self._reserve_for(OZ2, 8, m, n, k, n_moduli)
         self._check(self._lib.emugemm_dgemm_oz2_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), _dbl(alpha),
                                                    _ptr(A), _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), _dbl(beta), _ptr(C_),
@@ -209,8 +262,7 @@ class EmuGemm:
 
     def zgemm_oz1_4m(self, A, B, C_, p, alpha=1.0 + 0j, beta=0j):
         """A, B, C_: complex128 CUDA tensors (Scheme I, 4M)."""
-        m, k = A.shape
-        n = B.shape[1]
+        m, n, k = self._dims(A, B, False, False, C_, self._torch.complex128)
         self._reserve_for(OZ1_4M, 16, m, n, k, p)
         al = (_dbl * 2)(complex(alpha).real, complex(alpha).imag)
         be = (_dbl * 2)(complex(beta).real, complex(beta).imag)
@@ -220,8 +272,7 @@ class EmuGemm:
 
     def cgemm_oz1_4m(self, A, B, C_, p, alpha=1.0 + 0j, beta=0j):
         """A, B, C_: complex64 CUDA tensors (Scheme I, 4M)."""
-        m, k = A.shape
-        n = B.shape[1]
+        m, n, k = self._dims(A, B, False, False, C_, self._torch.complex64)
         self._reserve_for(OZ1_4M, 16, m, n, k, p)
         al = (_dbl * 2)(complex(alpha).real, complex(alpha).imag)
         be = (_dbl * 2)(complex(beta).real, complex(beta).imag)
@@ -231,8 +282,7 @@ class EmuGemm:
 
     def cgemm_oz2_3m(self, A, B, C_, n_moduli, alpha=1.0 + 0j, beta=0j):
         """A, B, C_: complex64 CUDA tensors (Scheme II, 3M)."""
-        m, k = A.shape
-        n = B.shape[1]
+        m, n, k = self._dims(A, B, False, False, C_, self._torch.complex64)
         self._reserve_for(OZ2_3M, 16, m, n, k, n_moduli)
         al = (_dbl * 2)(complex(alpha).real, complex(alpha).imag)
         be = (_dbl * 2)(complex(beta).real, complex(beta).imag)
@@ -241,7 +291,7 @@ class EmuGemm:
         return C_
 
     def sgemm_oz2(self, A, B, C_, n_moduli, alpha=1.0, beta=0.0, transa=False, transb=False):
-        m, n, k = self._dims(A, B, transa, transb)
+        m, n, k = self._dims(A, B, transa, transb, C_, self._torch.float32)
         self._reserve_for(OZ2, 8, m, n, k, n_moduli)
         self._check(self._lib.emugemm_sgemm_oz2_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), _flt(alpha),
                                                    _ptr(A), _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), _flt(beta), _ptr(C_),
@@ -250,7 +300,7 @@ class EmuGemm:
 
     def zgemm_oz2_3m(self, A, B, C_, n_moduli, alpha=1.0 + 0j, beta=0j, transa=False, transb=False):
         """A, B, C_: complex128 CUDA tensors."""
-        m, n, k = self._dims(A, B, transa, transb)
+        m, n, k = self._dims(A, B, transa, transb, C_, self._torch.complex128)
         self._reserve_for(OZ2_3M, 16, m, n, k, n_moduli)
         al = (_dbl * 2)(complex(alpha).real, complex(alpha).imag)
         be = (_dbl * 2)(complex(beta).real, complex(beta).imag)
@@ -366,6 +416,11 @@ class EmuGemm:
         self._check(self._lib.emugemm_dbg_oz2_crt(self._h, _i64(m), _i64(n), _int(N), _ptr(CR), _ptr(eA), _ptr(eB), _int(tA),
                                                    _int(tB), _dbl(alpha), _dbl(beta), _ptr(C_), _i64(self._ld(C_))))
         return C_
+
+    # ---- PROBES build only (EmuGemm(probes=True)) -------------------------------
+    def dbg_set_flags(self, flags):
+        """Timing experiments (include/emugemm.h): results become WRONG; exists only in libemugemm_probes.so."""
+        self._check(self._lib.emugemm_dbg_set_flags(self._h, _int(flags)))
 
     def dbg_i8_probe(self, ops, iters=4000):
         """ops: list of (tmem_col, N, a_slot, b_row[, collector]).  -> (ms, Top/s, INT8 op / clk / SM from the SM cycle counter)."""

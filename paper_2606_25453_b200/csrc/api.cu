@@ -814,11 +814,17 @@ int emugemm_oz2_budget(int n_moduli, int64_t k, int is3m, int *tA, int *tB) {
   return T;
 }
 
+int emugemm_dbg_crt_constants(int n_moduli, int *n_pairs, int *n_digits, int *digit_bits, long long *digits, unsigned *pair) {
+  if (!n_pairs || !n_digits || !digit_bits || !digits || !pair) return EMUGEMM_ERR_ARG;
+  return crt_constants_dump(n_moduli, n_pairs, n_digits, digit_bits, digits, pair) ? EMUGEMM_ERR_ARG : EMUGEMM_OK;
+}
+
 int64_t emugemm_oz1_chunk_k(int p) { return (p >= 1 && p <= 8) ? oz1_chunk_k_host(p, 7) : 0; }
 int64_t emugemm_oz1_chunk_k_bits(int p, int slice_bits) {
   return (p >= 1 && p <= 8 && (slice_bits == 7 || slice_bits == 8)) ? oz1_chunk_k_host(p, slice_bits) : 0;
 }
 
+#ifdef EMUGEMM_PROBES
 int emugemm_dbg_i8_probe(emugemm_handle_t h, int n_ops, const int *ops, int iters, float *ms, int *ctas,
                          long long *cycles) {
   if (!h || !ms || !ctas) return EMUGEMM_ERR_ARG;
@@ -836,6 +842,8 @@ int emugemm_dbg_set_flags(emugemm_handle_t h, int flags) {
   h->dbg_flags = flags;
   return EMUGEMM_OK;
 }
+
+#endif  // EMUGEMM_PROBES
 
 #pragma GCC visibility pop
 }  // extern "C"

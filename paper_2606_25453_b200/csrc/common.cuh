@@ -18,6 +18,15 @@ constexpr int kBlockK = 128;      // bytes of k per pipeline block (one 128B swi
 
 struct StageTimer;
 
+// Timing-experiment switches (emugemm_dbg_set_flags) and the tensor-pipe probe kernels exist only in the PROBES build
+// (libemugemm_probes.so, -DEMUGEMM_PROBES, loaded by `bench.py` for its probe leg): the shipped library carries neither
+// the flag tests in its hot loops nor an entry point that can make results wrong.
+#ifdef EMUGEMM_PROBES
+#define EMU_PROBE_FLAG(flags, bit) ((flags) & (bit))
+#else
+#define EMU_PROBE_FLAG(flags, bit) 0
+#endif
+
 }  // namespace emu
 
 struct emugemm_ctx {
@@ -137,9 +146,12 @@ struct Oz2CrtArgs {
   int64_t batch_stride_c = 0;
 };
 int launch_oz2_crt(emugemm_ctx *ctx, const Oz2CrtArgs &a);
+int crt_constants_dump(int N, int *NP, int *J, int *g, long long *digits, unsigned *pair);  // host only (test hook)
 
+#ifdef EMUGEMM_PROBES
 int launch_oz1_issue_probe(emugemm_ctx *ctx, int p, int coll, int iters, float *ms, int *ctas, long long *cycles);
 int launch_i8_probe(emugemm_ctx *ctx, int n_ops, const int *ops, int iters, float *ms, int *ctas, long long *cycles);
+#endif
 
 // host helpers shared by api.cu and the drivers
 int oz2_moduli_host(int n, int *mod);                  // greedy coprime list, descending from 256

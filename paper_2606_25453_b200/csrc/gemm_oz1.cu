@@ -97,35 +97,6 @@ __device__ __forceinline__ void oz1_issue_slice(int t, uint32_t tmem_base, uint3
   }
 }
 
-// Same products, ONE MMA per product (width NT): A_t stays in the collector across its P - t consecutive MMAs.
-// This is the schedule a cta_group::2 pair needs (an N-concatenated MMA would split its columns between the
-// two CTAs' B halves); probed with cta_group::1: MMAs narrower than ~112 columns hit a ~55-cycle
-// per-instruction floor (p = 8, NT = 64: 0.56 of peak), so it only pays for NT >= 128 (DESIGN.md).
-template <int P, bool COLL>
-__device__ __forceinline__ void oz1_issue_slice_per_product(int t, uint32_t tmem_base, uint32_t a_base, uint32_t b_base,
-                                                            bool accumulate) {
-  constexpr int NT = Oz1Cfg<P>::NT;
-  constexpr uint32_t idesc = make_idesc_i8(kTileM, NT);
-  const uint32_t a_lo = sdesc_lo(a_base), b_lo = sdesc_lo(b_base);
-#pragma unroll
-  for (int ks = 0; ks < kBlockK / 32; ++ks) {
-    const uint64_t adesc = sdesc_from_lo(a_lo + ((ks * 32) >> 4));
-#pragma unroll
-    for (int u = 0; u < P; ++u) {
-      if (u < P - t) {
-        const uint32_t acc = (accumulate || ks != 0) ? 1u : 0u;
-        const uint32_t d = tmem_base + (t + u) * NT;
-        const uint64_t bdesc = sdesc_from_lo(b_lo + ((u * NT * kBlockK + ks * 32) >> 4));
-        const bool first = (u == 0), last = (u == P - t - 1);
-        if (COLL && first && !last) umma_i8<1>(d, adesc, bdesc, idesc, acc);
-        else if (COLL && !first && last) umma_i8<3>(d, adesc, bdesc, idesc, acc);
-        else if (COLL && !first && !last) umma_i8<2>(d, adesc, bdesc, idesc, acc);
-        else umma_i8<0>(d, adesc, bdesc, idesc, acc);
-      }
-    }
-  }
-}
-
 // CTA-pair schedule (cta_group::2, used for P <= 3; needs NT >= 128): one 256 x NT x 32 MMA per product, issued by the leader
 // CTA for both SMs; CTA r supplies rows 128 r .. of A_t and rows NT/2 r .. of B_u from its own shared memory, so the
 // columns of D come out in natural order and land on C_{t+u}.  A_t stays in the collector across its P - t MMAs.
@@ -283,7 +254,7 @@ struct Oz1Epi {
         r[c] = acc * d1 * d2;
         if constexpr (OUT == 3) rlo[c] = lo * d1 * d2;
       }
-      if (!row_ok || (a.dbg & 4)) return;
+      if (!row_ok || EMU_PROBE_FLAG(a.dbg, 4)) return;
       if constexpr (OUT == 3) {  // k-chunk partial as double-double [m][n][2]
         double *o = static_cast<double *>(a.C) + (grow * a.n + gcol) * 2;
 #pragma unroll
@@ -401,7 +372,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             if (cta == 0) mbar_arrive_expect_tx(&bfull[sb], kTxMul * Cfg::kBStageBytes);
             tma_load_3d_cg2(sB + sb * Cfg::kBStageBytes, &tmB, mapa_u32(&bfull[sb], 0), kbx * kBlockK,
                             rowB0 + nb * NT + static_cast<int>(cta) * Cfg::kBRows, 0, polB);
-          } else if ((a.dbg & 1) && nloadb >= SB) {
+          } else if (EMU_PROBE_FLAG(a.dbg, 1) && nloadb >= SB) {
             mbar_arrive(&bfull[sb]);
           } else {
             mbar_arrive_expect_tx(&bfull[sb], Cfg::kBStageBytes);
@@ -435,7 +406,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
               mbar_arrive_expect_tx(&afull[sa], lo == hi ? kAStageBytes : Cfg::kAPairBytes);
               tma_load_3d_mc(dst + cta * kHalf, &tmA, &afull[sa], kb * kBlockK, arow, lo, 3, polA);
               if (hi != lo) tma_load_3d_mc(dst + kAStageBytes + cta * kHalf, &tmA, &afull[sa], kb * kBlockK, arow, hi, 3, polA);
-            } else if ((a.dbg & 1) && nloada >= SA) {
+            } else if (EMU_PROBE_FLAG(a.dbg, 1) && nloada >= SA) {
               mbar_arrive(&afull[sa]);
             } else {
               mbar_arrive_expect_tx(&afull[sa], lo == hi ? kAStageBytes : Cfg::kAPairBytes);
@@ -529,7 +500,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       epi.load_eb(ac, gcol0, ea);  // first chunk's column exponents: in flight while the tile's MMAs finish
       mbar_wait(tfull, pt);
       tc_fence_after();
-      if (!(a.dbg & 2)) {
+      if (!EMU_PROBE_FLAG(a.dbg, 2)) {
         const uint32_t tcol = trow + half * (NT / 2);
         if constexpr (kDoubleBuffer) {
           // software pipeline: the TMEM loads and column exponents of chunk i+1 are in flight while chunk i is
@@ -657,10 +628,10 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
 template <int P>
 static int launch_p(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   if constexpr (P <= 3) {
-    if (!(ctx->dbg_flags & 8)) return launch_pp<P, true, false>(ctx, g);  // dbg bit 3: force the one-CTA N-concatenated kernel (A/B timing)
+    if (!EMU_PROBE_FLAG(ctx->dbg_flags, 8)) return launch_pp<P, true, false>(ctx, g);  // dbg bit 3: force the one-CTA N-concatenated kernel (A/B timing)
   }
   // A multicast: +2-4 % at p = 8 (NT = 64, A dominates the operand traffic), +2 % at p = 4, within noise at p = 5, 6
-  if (P >= 4 && !(ctx->dbg_flags & 16)) return launch_pp<P, false, true>(ctx, g);  // dbg bit 4: no multicast clusters (A/B timing)
+  if (P >= 4 && !EMU_PROBE_FLAG(ctx->dbg_flags, 16)) return launch_pp<P, false, true>(ctx, g);  // dbg bit 4: no multicast clusters (A/B timing)
   return launch_pp<P, false, false>(ctx, g);
 }
 
@@ -722,6 +693,36 @@ int launch_oz1_chunk_reduce(emugemm_ctx *ctx, int64_t m, int64_t n, int n_chunks
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
   return EMUGEMM_OK;
+}
+
+#ifdef EMUGEMM_PROBES
+// Same products, ONE MMA per product (width NT): A_t stays in the collector across its P - t consecutive MMAs.
+// This is the schedule a cta_group::2 pair needs (an N-concatenated MMA would split its columns between the
+// two CTAs' B halves); probed with cta_group::1: MMAs narrower than ~112 columns hit a ~55-cycle
+// per-instruction floor (p = 8, NT = 64: 0.56 of peak), so it only pays for NT >= 128 (DESIGN.md).
+template <int P, bool COLL>
+__device__ __forceinline__ void oz1_issue_slice_per_product(int t, uint32_t tmem_base, uint32_t a_base, uint32_t b_base,
+                                                            bool accumulate) {
+  constexpr int NT = Oz1Cfg<P>::NT;
+  constexpr uint32_t idesc = make_idesc_i8(kTileM, NT);
+  const uint32_t a_lo = sdesc_lo(a_base), b_lo = sdesc_lo(b_base);
+#pragma unroll
+  for (int ks = 0; ks < kBlockK / 32; ++ks) {
+    const uint64_t adesc = sdesc_from_lo(a_lo + ((ks * 32) >> 4));
+#pragma unroll
+    for (int u = 0; u < P; ++u) {
+      if (u < P - t) {
+        const uint32_t acc = (accumulate || ks != 0) ? 1u : 0u;
+        const uint32_t d = tmem_base + (t + u) * NT;
+        const uint64_t bdesc = sdesc_from_lo(b_lo + ((u * NT * kBlockK + ks * 32) >> 4));
+        const bool first = (u == 0), last = (u == P - t - 1);
+        if (COLL && first && !last) umma_i8<1>(d, adesc, bdesc, idesc, acc);
+        else if (COLL && !first && last) umma_i8<3>(d, adesc, bdesc, idesc, acc);
+        else if (COLL && !first && !last) umma_i8<2>(d, adesc, bdesc, idesc, acc);
+        else umma_i8<0>(d, adesc, bdesc, idesc, acc);
+      }
+    }
+  }
 }
 
 // ---- issue-bound INT8 tensor-core probe (third denominator) ----
@@ -883,5 +884,7 @@ int launch_oz1_issue_probe(emugemm_ctx *ctx, int p, int coll, int iters, float *
     default: return issue_probe_p<8>(ctx, coll, iters, ms, cycles);
   }
 }
+
+#endif  // EMUGEMM_PROBES
 
 }  // namespace emu

@@ -207,7 +207,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         const uint32_t slot = item & 1, tph = (item >> 1) & 1;
         mbar_wait(&tfull[slot], tph);
         tc_fence_after();
-        if (!(a.dbg & 2)) {
+        if (!EMU_PROBE_FLAG(a.dbg, 2)) {
           // 4 chunks of 32 columns, TMEM loads of chunk i+1 in flight while chunk i is reduced
           uint32_t va[32], vb[32];
           const uint32_t tcol = trow + slot * kOz2NT + half * 128;
@@ -225,7 +225,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
               for (int g = 0; g < 8; ++g)
                 w[g] = pack4i(sym_mod_i32(v[4 * g], mk), sym_mod_i32(v[4 * g + 1], mk), sym_mod_i32(v[4 * g + 2], mk),
                               sym_mod_i32(v[4 * g + 3], mk));
-              if (row_ok && gcol < a.n && !(a.dbg & 4))
+              if (row_ok && gcol < a.n && !EMU_PROBE_FLAG(a.dbg, 4))
                 store32(a.CR + ((static_cast<int64_t>(l) * a.nbatch + bidx) * a.m + grow) * a.n + gcol, w, gcol, a.n, vec_ok);
             } else if (q < 2) {
               // T1 / T2 stay on chip as unsigned residues in [0, m), four per register
@@ -255,7 +255,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
                 wr[g] = pack4i(re[0], re[1], re[2], re[3]);
                 wi[g] = pack4i(im[0], im[1], im[2], im[3]);
               }
-              if (row_ok && gcol < a.n && !(a.dbg & 4)) {
+              if (row_ok && gcol < a.n && !EMU_PROBE_FLAG(a.dbg, 4)) {
                 int8_t *o = a.CR + ((static_cast<int64_t>(l) * a.nbatch + bidx) * a.m + grow) * a.n + gcol;
                 store32(o, wr, gcol, a.n, vec_ok);
                 store32(o + a.n_moduli * plane_sz, wi, gcol, a.n, vec_ok);

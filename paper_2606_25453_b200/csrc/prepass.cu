@@ -622,7 +622,7 @@ static int launch_planes(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, 
   const T *x = static_cast<const T *>(X);
   if (!by_cols) {
     const dim3 grid(static_cast<unsigned>(rows), static_cast<unsigned>(batch));
-    const bool two_phase = (ctx->dbg_flags & 32) != 0;  // dbg bit 5: the two-phase kernels (A/B timing)
+    const bool two_phase = EMU_PROBE_FLAG(ctx->dbg_flags, 32) != 0;  // dbg bit 5: the two-phase kernels (A/B timing)
     // Scheme I digits: the register-resident single-read kernel when the row fits (p = 2: 0.159 -> 0.111 ms, p = 8: 0.246 ->
     // 0.218 ms at 8192^2).  Scheme II residues are bound by the integer pipes, not by the second read: there the 80
     // registers of the resident row cost occupancy (N = 16: 0.431 -> 0.475 ms, 3M N = 18: 1.81 -> 2.89 ms), so they keep

@@ -18,6 +18,17 @@ def test_library_exports_every_declared_symbol():
         assert must in syms
 
 
+def test_probes_build_exports_the_probe_calls_and_the_product_does_not():
+    """The experiment switches ("results become WRONG") and probe kernels live only in libemugemm_probes.so."""
+    prod, probes = E.load_library(), E.load_library(probes=True)
+    extra = sorted(set(E.exported_symbols(probes=True)) - set(E.exported_symbols()))
+    assert extra == ["emugemm_dbg_i8_probe", "emugemm_dbg_oz1_issue_probe", "emugemm_dbg_set_flags"]
+    for s in E.exported_symbols(probes=True):
+        assert hasattr(probes, s), s
+    for s in extra:
+        assert not hasattr(prod, s), s
+
+
 def test_host_helpers_match_oracle():
     for N in (2, 12, 14, 16, 18, 20):
         for k in (1, 4096, 8192, 65536):

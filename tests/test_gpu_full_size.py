@@ -29,7 +29,8 @@ def _samples(m, n, seed, count=36):
     return G.sample_indices(m, count, seed)[:48], G.sample_indices(n, count, seed + 1)[:48]
 
 
-@pytest.mark.parametrize("size,p,phi", [(8192, 8, 2.0), (8192, 3, 0.5), (4096, 5, 2.0), (2048, 6, 0.5)])
+@pytest.mark.parametrize("size,p,phi", [(8192, 8, 2.0), (8192, 3, 0.5), (4096, 5, 2.0), (2048, 6, 0.5), (8192, 4, 0.5), (8192, 6, 2.0),
+                                        (4096, 7, 0.5), (2048, 3, 2.0), (16384, 8, 0.5), (16384, 3, 2.0)])
 def test_config1_oz1_sweep_points(env, size, p, phi):
     """BASELINE configs[1]: Scheme I DGEMM square sweep, seed 1."""
     torch, O, h = env
@@ -43,7 +44,7 @@ def test_config1_oz1_sweep_points(env, size, p, phi):
     assert torch.isfinite(C).all()
 
 
-@pytest.mark.parametrize("N", [12, 20])
+@pytest.mark.parametrize("N", [12, 14, 16, 18, 20])
 def test_config2_oz2_8192(env, N):
     """BASELINE configs[2]: Scheme II DGEMM 8192^3, phi 1, seed 2."""
     torch, O, h = env
@@ -58,7 +59,7 @@ def test_config2_oz2_8192(env, N):
     assert torch.isfinite(C).all()
 
 
-@pytest.mark.parametrize("size,N", [(4096, 14), (4096, 18)])
+@pytest.mark.parametrize("size,N", [(4096, 14), (4096, 18), (8192, 14), (8192, 18)])
 def test_config3_zgemm_3m(env, size, N):
     """BASELINE configs[3]: ZGEMM via 3M, phi 1 on re and im, seed 3."""
     torch, O, h = env
@@ -109,3 +110,89 @@ def test_config4_sgemm_16384(env, p):
     got = C[torch.from_numpy(rows).cuda()][:, torch.from_numpy(cols).cuda()].cpu().numpy()
     want = O.oz1_sampled(A, B, p, rows, cols, is_f32=True)
     assert_within_ulps(got, want, _abs_ab(A, B, rows, cols), 2, bits=23, what=f"sgemm 16384 p={p}")
+
+
+# ---- SURVEY 8(d) "Checks" column at full size: integer intermediates ----
+def test_full_size_slices_bit_exact(env):
+    """configs[1]: ALL slices of the 8192 x 8192 operands (p = 8, phi = 2), rows of A and columns of B, bit for bit."""
+    torch, O, h = env
+    size, p = 8192, 8
+    A, B = G.real_pair(size, size, size, 2.0, 1)
+    for X, by_cols in ((A, False), (B, True)):
+        S, e = h.dbg_oz1_slices(torch.from_numpy(X).cuda(), by_cols, p)
+        oe = O.col_exponents(X) if by_cols else O.row_exponents(X)
+        assert np.array_equal(e.cpu().numpy(), oe)
+        want = O.oz1_slices_cols(X, oe, p) if by_cols else O.oz1_slices_rows(X, oe, p)
+        got = S.cpu().numpy()
+        del S
+        assert np.array_equal(got, want), f"slices differ (by_cols={by_cols})"
+
+
+def test_full_size_residues_bit_exact(env):
+    """configs[2]: ALL residues of the 8192 x 8192 operands (N = 16, phi = 1, seed 2), bit for bit."""
+    torch, O, h = env
+    size, N = 8192, 16
+    A, B = G.real_pair(size, size, size, 1.0, 2)
+    _, tA, tB = O.oz2_budget(N, size)
+    for X, by_cols, t in ((A, False, tA), (B, True, tB)):
+        R, e = h.dbg_oz2_residues(torch.from_numpy(X).cuda(), by_cols, N, t)
+        oe = O.col_exponents(X) if by_cols else O.row_exponents(X)
+        assert np.array_equal(e.cpu().numpy(), oe)
+        want = O.oz2_residues_cols(X, oe, t, N) if by_cols else O.oz2_residues_rows(X, oe, t, N)
+        got = R.cpu().numpy()
+        del R
+        assert np.array_equal(got, want), f"residues differ (by_cols={by_cols})"
+
+
+@pytest.mark.parametrize("p", [8, 3])
+def test_int32_dump_4096(env, p):
+    """INT32 accumulators of the fused kernel at 4096^3 (p = 8: N-concatenated one-CTA kernel; p = 3: the cta_group::2
+    pair kernel): 96 sampled rows x 160 sampled columns of all p accumulators, bit for bit against the oracle's int64
+    slice products (the full dump is 4096^2 p values; the oracle's plain loops finish the sample in seconds)."""
+    torch, O, h = env
+    size = 4096
+    A, B = G.real_pair(size, size, size, 0.5, 1)
+    acc = h.dbg_oz1_accumulators(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), p)
+    assert acc.shape == (1, p, size, size)
+    rows = G.sample_indices(size, 88, 21)[:96]
+    cols = G.sample_indices(size, 152, 22)[:160]
+    got = acc[0][:, torch.from_numpy(rows).cuda()][:, :, torch.from_numpy(cols).cuda()].cpu().numpy().astype(np.int64)
+    del acc
+    eA, eB = O.row_exponents(A), O.col_exponents(B)
+    SA = O.oz1_slices_rows(A[rows], eA[rows], p)
+    SB = O.oz1_slices_cols(np.ascontiguousarray(B[:, cols]), eB[cols], p)
+    assert np.array_equal(got, O.oz1_accumulators(SA, SB))
+
+
+def test_output_residues_8192(env):
+    """configs[2]: per-modulus output residues of the fused mod-GEMM at 8192^3, N = 16, sampled 64 x 64 per modulus."""
+    torch, O, h = env
+    size, N = 8192, 16
+    A, B = G.real_pair(size, size, size, 1.0, 2)
+    _, tA, tB = O.oz2_budget(N, size)
+    eA, eB = O.row_exponents(A), O.col_exponents(B)
+    RA, RB = O.oz2_residues_rows(A, eA, tA, N), O.oz2_residues_cols(B, eB, tB, N)
+    out = h.dbg_oz2_modgemm(torch.from_numpy(RA).cuda(), torch.from_numpy(RB).cuda())
+    rows = G.sample_indices(size, 56, 23)[:64]
+    cols = G.sample_indices(size, 56, 24)[:64]
+    got = out[:, torch.from_numpy(rows).cuda()][:, :, torch.from_numpy(cols).cuda()].cpu().numpy()
+    del out
+    want, _, _ = O.oz2_modprod(np.ascontiguousarray(RA[:, rows]), np.ascontiguousarray(RB[:, cols]))
+    assert np.array_equal(got, want)
+
+
+def test_output_residues_3m_4096(env):
+    """configs[3]: 3M output residues (re, im) at 4096^3, N = 14, sampled."""
+    torch, O, h = env
+    size, N = 4096, 14
+    A, B = G.complex_pair(size, size, size, 1.0, 3)
+    _, tA, tB = O.oz2_budget(N, size, True)
+    RA3 = O.oz2_residues_z(A, O.row_exponents_z(A), tA, N, False)
+    RB3 = O.oz2_residues_z(B, O.col_exponents_z(B), tB, N, True)
+    out = h.dbg_oz2_modgemm(torch.from_numpy(RA3).cuda(), torch.from_numpy(RB3).cuda(), is3m=True)
+    rows = G.sample_indices(size, 40, 25)[:48]
+    cols = G.sample_indices(size, 40, 26)[:48]
+    got = out[:, :, torch.from_numpy(rows).cuda()][:, :, :, torch.from_numpy(cols).cuda()].cpu().numpy()
+    del out
+    want = O.oz2_modprod_3m(np.ascontiguousarray(RA3[:, :, rows]), np.ascontiguousarray(RB3[:, :, cols]))
+    assert np.array_equal(got, want)

@@ -174,3 +174,118 @@ def test_sgemm_oz2_residues_alpha_beta_transposed(env):
     _, absAB = O.bf128_dgemm(A64, B.astype(np.float64))
     assert_within_ulps(C.cpu().numpy(), O.sgemm_oz2(A, B, N, alpha=2.5, beta=-0.5, Cin=Cin), 2.5 * absAB + 0.5 * np.abs(Cin), 2,
                        bits=23, what="sgemm_oz2 alpha/beta")
+
+
+# ---- the CRT is exact for EVERY residue vector (DESIGN.md R17, round 2; VERDICT r1 weak #1) ----
+@pytest.mark.parametrize("N", [2, 3, 8, 11, 12, 14, 15, 16, 18, 20])
+def test_crt_correctly_rounded_for_any_magnitude(env, N):
+    """X of every magnitude from 0 to P/4 (the budget's range, R12), both signs: the kernel must return the
+    correctly rounded double of the big integer.  The expected value is Python's int -> float conversion (correctly
+    rounded, independent of oracle and kernel); the oracle is held to 1 ulp of it (its __float128 step may round twice)."""
+    torch, O, h, E = env
+    mods = [int(x) for x in O.oz2_moduli(N)]
+    P = O.oz2_P(N)
+    rng = np.random.default_rng(1000 + N)
+    m, n = 37, 52   # ragged: scalar tail path of the kernel
+    Xs = []
+    top = (P // 4).bit_length() - 1
+    for idx in range(m * n):
+        bits = idx % (top + 1)
+        x = int(rng.integers(0, 2**62)) * int(rng.integers(0, 2**62)) * int(rng.integers(0, 2**62))
+        x = (x % (1 << bits)) | (1 << bits) if bits > 0 else idx % 3
+        x = min(x, P // 4 - 1)
+        Xs.append(-x if (idx // (top + 1)) % 2 else x)
+    Xs[0], Xs[1], Xs[2], Xs[3] = 0, 1, -1, P // 4 - 1
+    CR = np.empty((N, m, n), np.int8)
+    for l, mod in enumerate(mods):
+        r = np.array([x % mod for x in Xs], np.int64)
+        r = np.where(r >= (mod + 1) // 2, r - mod, r)
+        CR[l] = r.reshape(m, n)
+    eA = np.zeros(m, np.int32); eB = np.zeros(n, np.int32)
+    want = np.array([float(x) for x in Xs]).reshape(m, n)
+    for (mm, nn) in ((m, n), (m, 48)):   # ragged and vector path
+        C = torch.full((mm, nn), float("nan"), dtype=torch.float64, device="cuda")
+        h.dbg_oz2_crt(dev(torch, CR[:, :mm, :nn]), dev(torch, eA[:mm]), dev(torch, eB[:nn]), 0, 0, C)
+        assert np.array_equal(C.cpu().numpy(), want[:mm, :nn]), f"N={N}: CRT is not the correctly rounded integer"
+    orc = O.oz2_crt(CR, eA, eB, 0, 0)
+    assert (np.abs(orc - want) <= np.spacing(np.abs(want))).all()
+
+
+def _adversarial_pairs(m, n, k):
+    """(|A||B|)_ij << k 2^(eA_i + eB_j): each row / column maximum meets a tiny or zero partner (VERDICT r1 weak #1)."""
+    rng = np.random.default_rng(42)
+    out = {}
+    # one 1.0 per row of A at h = i mod k over 2^-40 noise; column j of B is 1.0 at h = (j + 1) mod k, tiny elsewhere
+    A = rng.uniform(-1, 1, (m, k)) * 2.0 ** -40
+    B = rng.uniform(-1, 1, (k, n)) * 2.0 ** -40
+    A[np.arange(m), np.arange(m) % k] = 1.0
+    B[(np.arange(n) + 1) % k, np.arange(n)] = 1.0
+    out["unit_over_noise"] = (A, B)
+    # B = I (k = n): C = A truncated to tA bits; each column of B has one nonzero
+    A2 = rng.uniform(-1, 1, (m, n)) * np.exp(2.0 * rng.standard_normal((m, n)))
+    out["identity"] = (A2, np.eye(n))
+    # the row maximum of A meets an exact zero of B, the rest of the row is 2^-30 smaller
+    A3 = rng.uniform(-1, 1, (m, k)) * 2.0 ** -30
+    A3[:, 0] = rng.uniform(0.5, 1.0, m)
+    B3 = rng.uniform(-1, 1, (k, n))
+    B3[0, :] = 0.0
+    out["max_meets_zero"] = (A3, B3)
+    # integers: exact products with heavy cancellation (result 0 or tiny against k 2^(eA+eB))
+    A4 = rng.integers(-3, 4, (m, k)).astype(np.float64)
+    A4[:, 1] = 2.0 ** 20
+    B4 = rng.integers(-3, 4, (k, n)).astype(np.float64)
+    B4[1, :] = 0.0
+    B4[2, ::2] = 2.0 ** 20
+    out["integers"] = (A4, B4)
+    return out
+
+
+@pytest.mark.parametrize("N", [12, 16, 20])
+@pytest.mark.parametrize("case", ["unit_over_noise", "identity", "max_meets_zero", "integers"])
+def test_dgemm_oz2_adversarial(env, N, case):
+    torch, O, h, E = env
+    m, n, k = 150, 136, 136 if case == "identity" else 200
+    A, B = _adversarial_pairs(m, n, k)[case]
+    C = torch.full((m, n), float("nan"), dtype=torch.float64, device="cuda")
+    h.dgemm_oz2(dev(torch, A), dev(torch, B), C, N)
+    _, absAB = O.bf128_dgemm(A, B)
+    got, want = C.cpu().numpy(), O.dgemm_oz2(A, B, N)
+    assert_within_ulps(got, want, absAB, 2, what=f"adversarial {case} N={N}")
+    zero = absAB == 0
+    assert (got[zero] == 0).all()   # ulp_of(0) = 0: an exact zero must come out as zero
+
+
+def test_zgemm_oz2_3m_adversarial(env):
+    torch, O, h, E = env
+    m, n, k, N = 100, 96, 128, 18
+    Ar, Br = _adversarial_pairs(m, n, k)["unit_over_noise"]
+    Ai, Bi = _adversarial_pairs(m, n, k)["max_meets_zero"]
+    A, B = Ar + 1j * Ai * 2.0 ** -20, Br + 1j * Bi * 2.0 ** -35
+    C = torch.zeros((m, n), dtype=torch.complex128, device="cuda")
+    h.zgemm_oz2_3m(dev(torch, A), dev(torch, B), C, N)
+    want = O.zgemm_oz2_3m(A, B, N)
+    _, absZ = O.bf128_zgemm(A, B)
+    got = C.cpu().numpy()
+    assert_within_ulps(got.real, want.real, absZ, 2, what="3M adversarial re")
+    assert_within_ulps(got.imag, want.imag, absZ, 2, what="3M adversarial im")
+
+
+def test_dgemm_oz2_extreme_exponents(env):
+    """ADVICE r1: operands near DBL_MIN / DBL_MAX: the power-of-two scaling must flush to zero / subnormals / infinity
+    correctly instead of building a garbage exponent field."""
+    torch, O, h, E = env
+    m, n, k, N = 64, 64, 128, 14
+    A, B = G.real_pair(m, n, k, 1.0, 21)
+    for sa, sb in ((2.0 ** -1000, 2.0 ** -1000), (2.0 ** -1020, 2.0 ** -40), (2.0 ** 500, 2.0 ** 500), (2.0 ** -600, 2.0 ** -440)):
+        As, Bs = A * sa, B * sb
+        C = torch.full((m, n), float("nan"), dtype=torch.float64, device="cuda")
+        h.dgemm_oz2(dev(torch, As), dev(torch, Bs), C, N)
+        want = O.dgemm_oz2(As, Bs, N)
+        got = C.cpu().numpy()
+        with np.errstate(over="ignore", under="ignore"):
+            scale = np.abs(As) @ np.abs(Bs)
+        tiny = scale < 2.0 ** -1021
+        if (~tiny).any():
+            assert_within_ulps(got[~tiny], want[~tiny], scale[~tiny], 2, what=f"scales {sa} {sb}")
+        # results in the subnormal range: absolute error of two subnormal spacings
+        assert (np.abs(got[tiny] - want[tiny]) <= 2 * 2.0 ** -1074).all()
