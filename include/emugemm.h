@@ -69,6 +69,11 @@ int emugemm_set_slice_bits(emugemm_handle_t h, int bits);
 size_t emugemm_workspace_bytes(int scheme, int elem, int64_t m, int64_t n, int64_t k, int p_or_nmoduli);
 const char *emugemm_status_string(int status);
 int emugemm_last_cuda_error(emugemm_handle_t h); /* cudaError_t of the last EMUGEMM_ERR_CUDA */
+/* Non-finite inputs give an unspecified result and no fault (see above); the pre-pass of every one-shot compute call
+ * raises a device-side flag when a row of A or a column of B holds an Inf or a NaN (it falls out of the exponent scan:
+ * no extra pass).  *seen (HOST) = 1 if the LAST compute call of this handle saw one, else 0; synchronises the stream.
+ * EMUGEMM_ERR_WORKSPACE before the first compute call or after the workspace was replaced.                    */
+int emugemm_nonfinite_seen(emugemm_handle_t h, int *seen);
 
 /* ---- Scheme I ------------------------------------------ *
  * C = alpha*A*B + beta*C with p signed INT8 slices of beta_bits = 7 bits each

@@ -321,6 +321,79 @@ void oracle_oz1_sampled(int64_t m, int64_t n, int64_t k, double alpha, const dou
 }
 
 /* ------------------------------------------------------------------------- */
+/* Scheme I complex GEMM by the 4M formulation ("EmuGEMM-I uses  */
+/* the 4M formulation"), written as FOUR SEPARATE REAL     */
+/* slice products:                                                            */
+/*   Re(A B) = ReA ReB + (-ImA) ImB,   Im(A B) = ImA ReB + ReA ImB,           */
+/* i.e. the real embedding A' = [[ReA, -ImA], [ImA, ReA]], B' = [[ReB], [ImB]] */
+/* taken product by product: the minus sign is carried by the OPERAND (-ImA is */
+/* sliced), which matters for the balanced 8-bit digits (R23), whose digits of */
+/* -x are not the negated digits of x; with sign-magnitude digits (R1) it is   */
+/* the same as subtracting the product.                                        */
+/* Real and imaginary part of a row of A (column of B) share ONE exponent, the */
+/* maximum over both (R16 applied to 4M: a real diagonal scaling must commute */
+/* with the complex product).  Per s < p the four int64 accumulators          */
+/* P1..P4 (Eq. 2 on the slices of the parts) give                             */
+/*   C_s^re = P1_s + P2_s,   C_s^im = P3_s + P4_s     exactly,                */
+/* Eq. 3 and the scaling are exact in __float128 and each component T_re,     */
+/* T_im is rounded ONCE to double (a real Scheme I result each); then          */
+/*   C = alpha (T_re + i T_im) + beta C_in   in __float128, rounded once per  */
+/* component (to float first when is_f32: the CGEMM entry point).             */
+/* A, B, C: (re, im) pairs, strides in complex elements.                      */
+/* ------------------------------------------------------------------------- */
+int oracle_zgemm_oz1_4m(int64_t m, int64_t n, int64_t k, const double *alpha, const double *A, int64_t lda,
+                        const double *B, int64_t ldb, const double *beta_, double *C, int64_t ldc, int p,
+                        int is_f32) {
+  if (p < 1 || p > 8 || m < 0 || n < 0 || k < 0) return -1;
+  if (m == 0 || n == 0) return 0;
+  const int64_t kk = k ? k : 1;
+  int32_t *eA = malloc(sizeof(int32_t) * (size_t)m), *eB = malloc(sizeof(int32_t) * (size_t)n);
+  double *Ar = malloc(sizeof(double) * (size_t)m * kk), *Ai = malloc(sizeof(double) * (size_t)m * kk);
+  double *An = malloc(sizeof(double) * (size_t)m * kk); /* -Im A */
+  double *Br = malloc(sizeof(double) * (size_t)kk * n), *Bi = malloc(sizeof(double) * (size_t)kk * n);
+  for (int64_t i = 0; i < m; ++i)
+    for (int64_t h = 0; h < k; ++h) {
+      Ar[i * k + h] = A[2 * (i * lda + h)];
+      Ai[i * k + h] = A[2 * (i * lda + h) + 1];
+      An[i * k + h] = -A[2 * (i * lda + h) + 1];
+    }
+  for (int64_t h = 0; h < k; ++h)
+    for (int64_t j = 0; j < n; ++j) { Br[h * n + j] = B[2 * (h * ldb + j)]; Bi[h * n + j] = B[2 * (h * ldb + j) + 1]; }
+  oracle_row_exponents_z(m, k, A, lda, eA);
+  oracle_col_exponents_z(k, n, B, ldb, eB);
+  int8_t *SAr = malloc((size_t)p * m * kk), *SAi = malloc((size_t)p * m * kk), *SAn = malloc((size_t)p * m * kk);
+  int8_t *SBr = malloc((size_t)p * n * kk), *SBi = malloc((size_t)p * n * kk);
+  oracle_oz1_slices_rows(m, k, Ar, k, eA, p, SAr);
+  oracle_oz1_slices_rows(m, k, Ai, k, eA, p, SAi);
+  oracle_oz1_slices_rows(m, k, An, k, eA, p, SAn);
+  oracle_oz1_slices_cols(k, n, Br, n, eB, p, SBr);
+  oracle_oz1_slices_cols(k, n, Bi, n, eB, p, SBi);
+#pragma omp parallel for schedule(static)
+  for (int64_t i = 0; i < m; ++i)
+    for (int64_t j = 0; j < n; ++j) {
+      int64_t cre[8], cim[8];
+      for (int s = 0; s < p; ++s) {
+        const int64_t p1 = acc_one(SAr, SBr, m, n, k, s, i, j), p2 = acc_one(SAn, SBi, m, n, k, s, i, j);
+        const int64_t p3 = acc_one(SAi, SBr, m, n, k, s, i, j), p4 = acc_one(SAr, SBi, m, n, k, s, i, j);
+        cre[s] = p1 + p2;
+        cim[s] = p3 + p4;
+      }
+      const double tre = (double)oz1_value(cre, p, eA[i], eB[j]), tim = (double)oz1_value(cim, p, eA[i], eB[j]);
+      __float128 re = (__float128)alpha[0] * tre - (__float128)alpha[1] * tim;
+      __float128 im = (__float128)alpha[0] * tim + (__float128)alpha[1] * tre;
+      double *c = C + 2 * (i * ldc + j);
+      if (beta_[0] != 0.0 || beta_[1] != 0.0) {
+        re += (__float128)beta_[0] * c[0] - (__float128)beta_[1] * c[1];
+        im += (__float128)beta_[0] * c[1] + (__float128)beta_[1] * c[0];
+      }
+      c[0] = is_f32 ? (double)(float)re : (double)re;
+      c[1] = is_f32 ? (double)(float)im : (double)im;
+    }
+  free(eA); free(eB); free(Ar); free(Ai); free(An); free(Br); free(Bi); free(SAr); free(SAi); free(SAn); free(SBr); free(SBi);
+  return 0;
+}
+
+/* ------------------------------------------------------------------------- */
 /* Brute force: exact-ish product of the ORIGINAL operands in __float128      */
 /* (113-bit significand; each product of two doubles is exact, the sum rounds */
 /* at 2^-113 relative) -- used only to check error bounds.                    */

@@ -1,7 +1,8 @@
 """ctypes view of oracle/liboracle.so (TEST INFRASTRUCTURE; see emugemm_oracle.c).
 
-Argument marshalling only: numpy arrays in, numpy arrays out.  Every function
-cites the C routine it calls; the arithmetic and its paper citations live there.
+Argument marshalling only: numpy arrays in, numpy arrays out (dtype widening of float32 / complex64 inputs to the
+C routines' double interface and the matching narrowing of their results included).  Every function cites the C
+routine it calls; the arithmetic and its paper citations live there.
 """
 import ctypes as C
 import numpy as np
@@ -164,39 +165,36 @@ def oz1_sampled(A, B, p, rows, cols, alpha=1.0, is_f32=False):
     return out
 
 
-def zgemm_oz1_4m(A, B, p, alpha=1.0 + 0j, beta=0j, Cin=None):
-    """Scheme I complex GEMM by the 4M formulation ("EmuGEMM-I uses the 4M formulation"; SURVEY 8(f)
-    item 3): the four real products are ONE real Scheme I GEMM on the real embedding
-        A' = [[Re A, -Im A], [Im A, Re A]]  (2m x 2k),   B' = [[Re B], [Im B]]  (2k x n),
-    whose rows i and m + i give Re and Im of A B.  Rows i and m + i of A' hold the same magnitudes, so they share
-    their exponent (the max over Re and Im of row i of A, as R16 does for 3M); column j of B' covers Re and Im of
-    column j of B.  T = dgemm_oz1(A', B', p) (one rounding per component), then C = alpha (T_re + i T_im) + beta C_in
-    in complex double arithmetic."""
-    A = np.ascontiguousarray(A, np.complex128)
-    B = np.ascontiguousarray(B, np.complex128)
-    m = A.shape[0]
-    Ae = np.block([[A.real, -A.imag], [A.imag, A.real]])
-    Be = np.vstack([B.real, B.imag])
-    T = dgemm_oz1(np.ascontiguousarray(Ae), np.ascontiguousarray(Be), p)
-    Tc = T[:m] + 1j * T[m:]
-    out = complex(alpha) * Tc
-    if complex(beta) != 0:
-        out = out + complex(beta) * np.ascontiguousarray(Cin, np.complex128)
+def zgemm_oz1_4m(A, B, p, alpha=1.0 + 0j, beta=0j, Cin=None, _f32=False):
+    """Scheme I complex GEMM by 4M as four separate real slice products (oracle_zgemm_oz1_4m)."""
+    A, Af = _zview(A)
+    B, Bf = _zview(B)
+    m, k = A.shape
+    _, n = B.shape
+    out = np.zeros((m, n), np.complex128) if Cin is None else np.ascontiguousarray(Cin, np.complex128).copy()
+    al = np.array([complex(alpha).real, complex(alpha).imag], np.float64)
+    be = np.array([complex(beta).real, complex(beta).imag], np.float64)
+    _lib.oracle_zgemm_oz1_4m.restype = C.c_int
+    rc = _lib.oracle_zgemm_oz1_4m(_i64(m), _i64(n), _i64(k), _ptr(al), _ptr(Af), _i64(k), _ptr(Bf), _i64(n), _ptr(be),
+                                  _ptr(out.view(np.float64)), _i64(n), C.c_int(p), C.c_int(1 if _f32 else 0))
+    if rc:
+        raise ValueError(f"oracle_zgemm_oz1_4m rc={rc}")
     return out
 
 
 def cgemm_oz1_4m(A, B, p, alpha=1.0 + 0j, beta=0j, Cin=None):
-    """CGEMM by Scheme I / 4M: complex64 inputs widened exactly to complex128, the complex128 oracle, then each
-    component rounded to float (a second rounding after the double one: at most 2^-29 relative beyond 1/2 ulp of
-    float, far inside the 2-ulp FP32 tolerance)."""
+    """CGEMM by Scheme I / 4M (oracle_zgemm_oz1_4m with is_f32): complex64 inputs widened exactly (marshalling), each
+    component rounded once to float inside the C routine."""
     A = np.ascontiguousarray(A, np.complex64).astype(np.complex128)
     B = np.ascontiguousarray(B, np.complex64).astype(np.complex128)
     C0 = None if Cin is None else np.ascontiguousarray(Cin, np.complex64).astype(np.complex128)
-    return zgemm_oz1_4m(A, B, p, alpha=alpha, beta=beta, Cin=C0).astype(np.complex64)
+    return zgemm_oz1_4m(A, B, p, alpha=alpha, beta=beta, Cin=C0, _f32=True).astype(np.complex64)
 
 
 def cgemm_oz2_3m(A, B, N, alpha=1.0 + 0j, beta=0j, Cin=None):
-    """CGEMM by Scheme II / 3M on complex64 inputs: as cgemm_oz1_4m, through zgemm_oz2_3m."""
+    """CGEMM by Scheme II / 3M on complex64 inputs (oracle_zgemm_oz2_3m on the exactly widened inputs; the last step,
+    one more rounding of each component to float, is a dtype conversion of the routine's double result: at most 2^-29
+    relative beyond 1/2 ulp of float, far inside the 2-ulp FP32 tolerance)."""
     A = np.ascontiguousarray(A, np.complex64).astype(np.complex128)
     B = np.ascontiguousarray(B, np.complex64).astype(np.complex128)
     C0 = None if Cin is None else np.ascontiguousarray(Cin, np.complex64).astype(np.complex128)

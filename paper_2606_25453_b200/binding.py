@@ -162,6 +162,12 @@ class EmuGemm:
         self._check(self._lib.emugemm_stage_ms(self._h, ms, C.byref(n)))
         return [float(x) for x in ms], n.value
 
+    def nonfinite_seen(self):
+        """True if the last compute call's pre-pass met an Inf or a NaN in A or B (synchronises the stream)."""
+        v = _int(0)
+        self._check(self._lib.emugemm_nonfinite_seen(self._h, C.byref(v)))
+        return bool(v.value)
+
     def last_gemm_cycles(self):
         c = C.c_ulonglong(0)
         self._check(self._lib.emugemm_last_gemm_cycles(self._h, C.byref(c)))
@@ -325,6 +331,8 @@ class EmuGemm:
         nbytes = int(self._lib.emugemm_operand_bytes(scheme, rows, k, pn))
         assert nbytes > 0, "invalid operand arguments"
         raw = torch.empty(nbytes + 1024, dtype=torch.uint8, device="cuda")
+        if self._stream is not None:
+            raw.record_stream(self._stream)  # written and read by kernels on the handle's stream
         off = (-raw.data_ptr()) % 1024
         if self._ws is None or self._ws.numel() < 8 * rows + 4096:
             self.reserve(max(8 * rows + 4096, 1 << 20))

@@ -141,6 +141,7 @@ static int oz1_gemm_phase(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_
   g.batch = batch; g.batch_stride_c = batch_stride_c;
   g.m = m; g.n = n; g.kpad = kpad; g.p = p; g.slice_bits = bits; g.SA = SA; g.SB = SB; g.eA = eA; g.eB = eB;
   g.alpha = alpha; g.beta = beta; g.C = C; g.ldc = ldc; g.cycles = diag;
+  g.wave_ctr = diag ? diag + kDiagWaveCtr : nullptr;
   const int final_kind = (elem == kF32) ? 1 : 0;
   // ONE launch: with several overflow-safe k-chunks a work item of the persistent kernel is (chunk, tile), so short
   // chunks of a long-k problem still fill the machine
@@ -186,7 +187,8 @@ static int run_oz1(emugemm_ctx *h, int ta, int tb, int elem, int64_t m, int64_t 
   double *part = (nch > 1 && !dump) ? cv.take<double>(static_cast<size_t>(nch) * m * n * 2) : nullptr;
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   h->diag = diag;
-  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+  h->nf_flag = diag + kDiagNonFinite;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, kDiagBytes, h->stream));
 
   // planes are indexed [row of op(A)] / [column of op(B)] with k contiguous: a k-major stored operand (A^T stored
   // k x m, B stored k x n) goes through the column kernels, an operand whose k is contiguous through the row kernel
@@ -244,7 +246,8 @@ static int run_oz1_batched(emugemm_ctx *h, int elem, int64_t batch, int64_t m, i
   auto *SB = cv.take<int8_t>(static_cast<size_t>(p) * N * kpad);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   h->diag = diag;
-  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+  h->nf_flag = diag + kDiagNonFinite;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, kDiagBytes, h->stream));
   const int nb = static_cast<int>(batch);
   EMU_TRY(launch_oz1_slice(h, elem, 0, m, k, kpad, A, lda, mbA, eA, p, bits, SA, nb, strideA));
   EMU_TRY(launch_oz1_slice(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, p, bits, SB, nb, strideB));
@@ -261,6 +264,7 @@ static int oz2_gemm_phase(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_
   Oz2GemmArgs g;
   g.batch = batch;
   g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = N; g.is3m = is3m; g.RA = RA; g.RB = RB; g.CR = CR; g.cycles = diag;
+  g.wave_ctr = diag ? diag + kDiagWaveCtr : nullptr;
   EMU_TRY(launch_oz2_gemm(h, g));
   EMU_TRY(mark(h, 2));
   Oz2CrtArgs c;
@@ -303,7 +307,8 @@ static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t 
   auto *CR = cv.take<int8_t>(static_cast<size_t>(parts_out) * N * m * n);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   h->diag = diag;
-  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+  h->nf_flag = diag + kDiagNonFinite;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, kDiagBytes, h->stream));
 
   EMU_TRY(launch_oz2_residues(h, elem, ta, m, k, kpad, A, lda, mbA, eA, N, tA, RA));
   EMU_TRY(launch_oz2_residues(h, elem, !tb, n, k, kpad, B, ldb, mbB, eB, N, tB, RB));
@@ -360,7 +365,8 @@ static int run_oz2_batched(emugemm_ctx *h, int is3m, int f32, int64_t batch, int
   auto *CR = cv.take<int8_t>(static_cast<size_t>(parts_out) * N * M * n);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   h->diag = diag;
-  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+  h->nf_flag = diag + kDiagNonFinite;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, kDiagBytes, h->stream));
   const int nb = static_cast<int>(batch);
   EMU_TRY(launch_oz2_residues(h, elem, 0, m, k, kpad, A, lda, mbA, eA, N, tA, RA, nb, strideA));
   EMU_TRY(launch_oz2_residues(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, N, tB, RB, nb, strideB));
@@ -423,6 +429,8 @@ int emugemm_set_workspace(emugemm_handle_t h, void *p, size_t bytes) {
   if (reinterpret_cast<uintptr_t>(p) & 1023) return EMUGEMM_ERR_ALIGNMENT;
   h->ws = p;
   h->ws_bytes = bytes;
+  h->diag = nullptr;  // the diagnostics words lived in the previous workspace
+  h->nf_flag = nullptr;
   return EMUGEMM_OK;
 }
 
@@ -501,7 +509,8 @@ static int run_oz1_4m(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k,
   double *part = nch > 1 ? cv.take<double>(static_cast<size_t>(nch) * mm * n * 2) : nullptr;
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   h->diag = diag;
-  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+  h->nf_flag = diag + kDiagNonFinite;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, kDiagBytes, h->stream));
   EMU_TRY(launch_colmax(h, elem, n, k, B, ldb, mbB));
   EMU_TRY(launch_oz1_4m_slice(h, elem, 0, m, k, kpad, A, lda, nullptr, eA, p, bits, SA));
   EMU_TRY(launch_oz1_4m_slice(h, elem, 1, n, k, kpad, B, ldb, mbB, eB, p, bits, SB));
@@ -656,6 +665,7 @@ int emugemm_decompose(emugemm_handle_t h, int scheme, int role, int trans, int e
     if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   }
   h->launches = 0;
+  h->nf_flag = nullptr;  // the flag belongs to the one-shot calls (it lives in their workspace)
   if (oz1) EMU_TRY(launch_oz1_slice(h, elem, by_cols, rows, k, kpad, X, ldx, mb, e, pn, h->slice_bits, planes));
   else EMU_TRY(launch_oz2_residues(h, elem, by_cols, rows, k, kpad, X, ldx, mb, e, pn, t_bits, planes));
   out->scheme = scheme; out->role = role; out->elem = elem; out->pn = pn;
@@ -688,7 +698,8 @@ int emugemm_gemm_pre(emugemm_handle_t h, const emugemm_operand_t *A, const emuge
     double *part = nch > 1 ? cv.take<double>(static_cast<size_t>(nch) * m * n * 2) : nullptr;
     if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
     h->diag = diag;
-    EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+  h->nf_flag = diag + kDiagNonFinite;
+    EMU_CUDA(h, cudaMemsetAsync(diag, 0, kDiagBytes, h->stream));
     return oz1_gemm_phase(h, A->elem, m, n, kpad, pn, A->slice_bits, PA, PB, eA, eB, alpha[0], beta[0], C, ldc, nullptr, nch,
                           clen, part, diag);
   }
@@ -696,7 +707,8 @@ int emugemm_gemm_pre(emugemm_handle_t h, const emugemm_operand_t *A, const emuge
   auto *CR = cv.take<int8_t>(static_cast<size_t>(is3m ? 2 : 1) * pn * m * n);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   h->diag = diag;
-  EMU_CUDA(h, cudaMemsetAsync(diag, 0, sizeof(unsigned long long), h->stream));
+  h->nf_flag = diag + kDiagNonFinite;
+  EMU_CUDA(h, cudaMemsetAsync(diag, 0, kDiagBytes, h->stream));
   return oz2_gemm_phase(h, is3m, m, n, kpad, pn, PA, PB, CR, eA, eB, A->t_bits, B->t_bits, alpha, beta, static_cast<double *>(C),
                         ldc, diag, A->elem == kF32);
 }
@@ -706,6 +718,16 @@ int emugemm_last_gemm_cycles(emugemm_handle_t h, unsigned long long *cycles) {
   if (!h->diag) return EMUGEMM_ERR_WORKSPACE;
   EMU_CUDA(h, cudaStreamSynchronize(h->stream));
   EMU_CUDA(h, cudaMemcpy(cycles, h->diag, sizeof(unsigned long long), cudaMemcpyDeviceToHost));
+  return EMUGEMM_OK;
+}
+
+int emugemm_nonfinite_seen(emugemm_handle_t h, int *seen) {
+  if (!h || !seen) return EMUGEMM_ERR_ARG;
+  if (!h->diag) return EMUGEMM_ERR_WORKSPACE;
+  unsigned long long v = 0;
+  EMU_CUDA(h, cudaStreamSynchronize(h->stream));
+  EMU_CUDA(h, cudaMemcpy(&v, h->diag + kDiagNonFinite, sizeof(v), cudaMemcpyDeviceToHost));
+  *seen = v != 0;
   return EMUGEMM_OK;
 }
 
@@ -734,6 +756,7 @@ int emugemm_dbg_exponents(emugemm_handle_t h, int elem, int by_cols, int64_t row
                           int32_t *e_out) {
   if (!h || rows < 0 || k < 0 || !e_out) return EMUGEMM_ERR_ARG;
   if (!h->ws) return EMUGEMM_ERR_WORKSPACE;
+  h->nf_flag = nullptr;  // the hooks carve the workspace from its start: no diagnostics words
   Carver cv(h->ws, h->ws_bytes);
   auto *mb = cv.take<unsigned long long>(rows);
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
@@ -745,6 +768,7 @@ int emugemm_dbg_oz1_slices(emugemm_handle_t h, int elem, int by_cols, int64_t ro
   if (!h || rows <= 0 || k <= 0 || !out || !e_out || p < 1 || p > 8) return EMUGEMM_ERR_ARG;
   if (!h->ws) return EMUGEMM_ERR_WORKSPACE;
   const int64_t kpad = round_up(k, kBlockK);
+  h->nf_flag = nullptr;  // the hooks carve the workspace from its start: no diagnostics words
   Carver cv(h->ws, h->ws_bytes);
   auto *mb = cv.take<unsigned long long>(rows);
   auto *S = cv.take<int8_t>(static_cast<size_t>(p) * rows * kpad);
@@ -765,6 +789,7 @@ int emugemm_dbg_oz2_residues(emugemm_handle_t h, int elem, int by_cols, int64_t 
   if (!h->ws) return EMUGEMM_ERR_WORKSPACE;
   const int64_t kpad = round_up(k, kBlockK);
   const int parts = (elem == kZ128) ? 3 : 1;
+  h->nf_flag = nullptr;  // the hooks carve the workspace from its start: no diagnostics words
   Carver cv(h->ws, h->ws_bytes);
   auto *mb = cv.take<unsigned long long>(rows);
   auto *R = cv.take<int8_t>(static_cast<size_t>(parts) * n_moduli * rows * kpad);

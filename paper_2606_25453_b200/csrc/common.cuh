@@ -15,6 +15,10 @@ constexpr int kBeta = 7;          // bits per signed slice (R1; PAPER.
 constexpr int kMaxModuli = 20;    // API range of n_moduli
 constexpr int kTileM = 128;       // rows per CTA tile == tcgen05.mma M (PAPER.md:43 t_M = 128 on Blackwell)
 constexpr int kBlockK = 128;      // bytes of k per pipeline block (one 128B swizzle row, 4 MMAs of K = 32)
+// diagnostics words at the head of the workspace (zeroed per call): [0] SM cycles of the fused GEMM kernel (CTA 0),
+// [1] wave-barrier counter of the fused Scheme I kernel, [2] non-finite-input flag raised by the pre-pass
+constexpr int kDiagBytes = 64;
+constexpr int kDiagWaveCtr = 1, kDiagNonFinite = 2;
 
 struct StageTimer;
 
@@ -41,6 +45,7 @@ struct emugemm_ctx {
   int dbg_flags = 0;
   int slice_bits = 7;  // Scheme I digits: 7 = sign-magnitude (R1, default), 8 = balanced base 256 (R23)
   unsigned long long *diag = nullptr;  // device: [0] = GEMM-kernel SM cycles of the last call (inside the workspace)
+  unsigned long long *nf_flag = nullptr;  // device word the pre-pass ORs 1 into when an operand holds Inf / NaN (null: off)
   PFN_cuTensorMapEncodeTiled_v12000 encode = nullptr;
 };
 
@@ -114,6 +119,7 @@ struct Oz1GemmArgs {
   void *C;
   int64_t ldc;
   unsigned long long *cycles;  // device counter: += SM cycles CTA 0 spent in the kernel (diagnostic), may be null
+  unsigned long long *wave_ctr = nullptr;  // zeroed device word for the wave barrier (null: no barrier)
 };
 int launch_oz1_gemm(emugemm_ctx *ctx, const Oz1GemmArgs &a);
 // Sum n_chunks double-double partials part[c][m][n][2] and apply alpha/beta (out_kind 0 / 1 as above).
@@ -127,6 +133,7 @@ struct Oz2GemmArgs {
   const int8_t *RA, *RB;       // real: [N][rows][kpad]; 3M: [3][N][rows][kpad]
   int8_t *CR;                  // real: [N][m][n]; 3M: [2][N][m][n]
   unsigned long long *cycles;  // as in Oz1GemmArgs
+  unsigned long long *wave_ctr = nullptr;  // as in Oz1GemmArgs
   int batch = 1;               // strided batched call: residue planes hold batch * m (n) rows entry-major, CR is [N][batch][m][n]
 };
 int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &a);

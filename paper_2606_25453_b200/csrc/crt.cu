@@ -142,16 +142,18 @@ int crt_constants_dump(int N, int *NP, int *J, int *g, long long *digits, unsign
 constexpr int kCrtVec = 4;  // columns per thread: one 32-bit load per residue plane
 
 // Exact accumulators acc[e][j] (e = column, j = digit) of kCrtVec consecutive columns of one row from the N residue
-// planes starting at src (plane stride `plane`).  All plane words are requested before the first is consumed.
-template <int J, bool VEC>
+// planes starting at src (plane stride `plane`).  NP = ceil(N / 2) is a template parameter (the digit count follows
+// from it: J = ceil(NP / 2) for the moduli list of R10, checked on the host), so the plane loop, the pair loop and every
+// constant index are resolved at compile time; all plane words are requested before the first is consumed.
+template <int NP, int J>
 __device__ __forceinline__ void crt_accumulate(const CrtConst &k, const int8_t *__restrict__ src, int64_t plane, int64_t j0,
-                                               int64_t n, double (&acc)[kCrtVec][J]) {
-  unsigned w[kMaxModuli];
+                                               int64_t n, bool vec, double (&acc)[kCrtVec][J]) {
+  unsigned w[2 * NP];
 #pragma unroll
-  for (int l = 0; l < kMaxModuli; ++l) {
+  for (int l = 0; l < 2 * NP; ++l) {
     w[l] = 0u;
-    if (l < k.N) {  // uniform
-      if (VEC) {
+    if (l < 2 * NP - 1 || l < k.N) {  // only the last plane of the last pair can be absent (odd N): uniform
+      if (vec) {
         w[l] = __ldg(reinterpret_cast<const unsigned *>(src));
       } else {
         unsigned a = 0;
@@ -161,25 +163,22 @@ __device__ __forceinline__ void crt_accumulate(const CrtConst &k, const int8_t *
         w[l] = a;
       }
     }
-    src += plane;  // unconditional (never dereferenced beyond plane N - 1): no predicated pointer moves
+    if (l + 1 < 2 * NP) src += plane;
   }
 #pragma unroll
-  for (int e = 0; e < kCrtVec; ++e)
-#pragma unroll
-    for (int j = 0; j < J; ++j) acc[e][j] = 0.0;
-#pragma unroll
-  for (int q = 0; q < kMaxPairs; ++q)
-    if (q < k.NP) crt_accumulate_pair<J>(k, q, w[2 * q], w[2 * q + 1], acc);
+  for (int q = 0; q < NP; ++q) crt_accumulate_pair<J>(k, q, w[2 * q], w[2 * q + 1], acc, q == 0);
 }
 
 // one thread per kCrtVec consecutive columns of one row
 // KIND: 0 = FP64 C, 1 = complex128 C, 2 = FP32 C (SGEMM), 3 = complex64 C (CGEMM); 2 and 3 round once more to float
-template <int J, bool VEC, int KIND>
+template <int NP, int KIND>
 __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const int8_t *__restrict__ CR,
                                                   const int32_t *__restrict__ eA, const int32_t *__restrict__ eB,
                                                   int tsum, double ar, double ai, double br, double bi,
                                                   double *__restrict__ C, int64_t ldc, const __grid_constant__ CrtConst k,
-                                                  int64_t c_entry_bytes) {
+                                                  int64_t c_entry_bytes, int vec_flag) {
+  constexpr int J = (NP + 1) / 2;
+  const bool VEC = vec_flag != 0;  // n % 4 == 0 and the residue planes 4-byte aligned: one 32-bit load per plane
   const int64_t ncolv = (n + kCrtVec - 1) / kCrtVec;
   const int64_t idx = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x;
   if (idx >= m * ncolv) return;
@@ -203,7 +202,7 @@ __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const in
 #pragma unroll
   for (int e = 0; e < kCrtVec; ++e) E2[e] = eAi + ((j0 + e < n) ? __ldg(eB + j0 + e) : 0);
   double acc[kCrtVec][J], vr[kCrtVec];
-  crt_accumulate<J, VEC>(k, CR + i * n + j0, plane, j0, n, acc);
+  crt_accumulate<NP, J>(k, CR + i * n + j0, plane, j0, n, VEC, acc);
 #pragma unroll
   for (int e = 0; e < kCrtVec; ++e) vr[e] = crt_scale_pow2(crt_finish<J>(k, acc[e]), E2[e]);
   if (KIND == 2) {
@@ -244,7 +243,7 @@ __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const in
     }
   } else {
     double vi[kCrtVec];
-    crt_accumulate<J, VEC>(k, CR + static_cast<int64_t>(k.N) * plane + i * n + j0, plane, j0, n, acc);
+    crt_accumulate<NP, J>(k, CR + static_cast<int64_t>(k.N) * plane + i * n + j0, plane, j0, n, VEC, acc);
 #pragma unroll
     for (int e = 0; e < kCrtVec; ++e) vi[e] = crt_scale_pow2(crt_finish<J>(k, acc[e]), E2[e]);
     const bool has_beta = (br != 0.0 || bi != 0.0);
@@ -281,26 +280,17 @@ __global__ void __launch_bounds__(256) crt_kernel(int64_t m, int64_t n, const in
   }
 }
 
-template <int J>
-static void crt_launch_j(dim3 grid, cudaStream_t st, bool vec, int kind, const Oz2CrtArgs &a, int tsum, const CrtConst &k,
-                         int64_t c_entry_bytes) {
-#define EMU_CRT_LAUNCH(V_, K_)                                                                                           \
-  crt_kernel<J, V_, K_><<<grid, 256, 0, st>>>(a.m, a.n, a.CR, a.eA, a.eB, tsum, a.alpha[0], a.alpha[1], a.beta[0], a.beta[1], \
-                                              a.C, a.ldc, k, c_entry_bytes)
-  if (vec) {
-    switch (kind) {
-      case 0: EMU_CRT_LAUNCH(true, 0); break;
-      case 1: EMU_CRT_LAUNCH(true, 1); break;
-      case 2: EMU_CRT_LAUNCH(true, 2); break;
-      default: EMU_CRT_LAUNCH(true, 3); break;
-    }
-  } else {
-    switch (kind) {
-      case 0: EMU_CRT_LAUNCH(false, 0); break;
-      case 1: EMU_CRT_LAUNCH(false, 1); break;
-      case 2: EMU_CRT_LAUNCH(false, 2); break;
-      default: EMU_CRT_LAUNCH(false, 3); break;
-    }
+template <int NP>
+static void crt_launch_np(dim3 grid, cudaStream_t st, bool vec, int kind, const Oz2CrtArgs &a, int tsum, const CrtConst &k,
+                          int64_t c_entry_bytes) {
+#define EMU_CRT_LAUNCH(K_)                                                                                                \
+  crt_kernel<NP, K_><<<grid, 256, 0, st>>>(a.m, a.n, a.CR, a.eA, a.eB, tsum, a.alpha[0], a.alpha[1], a.beta[0], a.beta[1], a.C, \
+                                           a.ldc, k, c_entry_bytes, vec ? 1 : 0)
+  switch (kind) {
+    case 0: EMU_CRT_LAUNCH(0); break;
+    case 1: EMU_CRT_LAUNCH(1); break;
+    case 2: EMU_CRT_LAUNCH(2); break;
+    default: EMU_CRT_LAUNCH(3); break;
   }
 #undef EMU_CRT_LAUNCH
 }
@@ -319,12 +309,18 @@ int launch_oz2_crt(emugemm_ctx *ctx, const Oz2CrtArgs &a) {
   // bytes between the C matrices of consecutive batch entries (element = float / double, x2 for complex)
   const int64_t c_entry_bytes = a.batch_stride_c * (a.out_f32 ? 4 : 8) * (a.is_complex ? 2 : 1);
   const dim3 grid(gx, static_cast<unsigned>(batch));
-  switch (k.J) {
-    case 1: crt_launch_j<1>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
-    case 2: crt_launch_j<2>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
-    case 3: crt_launch_j<3>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
-    case 4: crt_launch_j<4>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
-    default: crt_launch_j<5>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
+  if (k.J != (k.NP + 1) / 2) return EMUGEMM_ERR_ARG;  // the kernels derive the digit count from the pair count
+  switch (k.NP) {
+    case 1: crt_launch_np<1>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
+    case 2: crt_launch_np<2>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
+    case 3: crt_launch_np<3>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
+    case 4: crt_launch_np<4>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
+    case 5: crt_launch_np<5>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
+    case 6: crt_launch_np<6>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
+    case 7: crt_launch_np<7>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
+    case 8: crt_launch_np<8>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
+    case 9: crt_launch_np<9>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
+    default: crt_launch_np<10>(grid, ctx->stream, vec, kind, a, tsum, k, c_entry_bytes); break;
   }
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());

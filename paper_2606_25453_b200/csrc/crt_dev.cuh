@@ -71,8 +71,10 @@ __device__ __forceinline__ double crt_round_nearest(double x) {  // |x| < 2^51: 
 }
 
 // acc[e][j] += W_qj x for the four columns e whose residues are the bytes of wa (modulus 2q) and wb (modulus 2q + 1)
+// (first = true: acc is initialised with the product instead of being added to)
 template <int J>
-__device__ __forceinline__ void crt_accumulate_pair(const CrtConst &k, int q, unsigned wa, unsigned wb, double (&acc)[4][J]) {
+__device__ __forceinline__ void crt_accumulate_pair(const CrtConst &k, int q, unsigned wa, unsigned wb, double (&acc)[4][J],
+                                                    bool first = false) {
   const unsigned kp = k.kpack[q], c0 = k.c0[q], mg = k.magic[q], mq = k.mq[q];
   const unsigned w01 = __byte_perm(wa, wb, 0x5140);  // (c1, c2) of column 0, (c1, c2) of column 1
   const unsigned w23 = __byte_perm(wa, wb, 0x7362);
@@ -82,7 +84,7 @@ __device__ __forceinline__ void crt_accumulate_pair(const CrtConst &k, int q, un
   for (int e = 0; e < 4; ++e) {
     const double xd = __hiloint2double(0, static_cast<int>(x[e]));  // the subnormal x 2^-1074: no conversion instruction
 #pragma unroll
-    for (int j = 0; j < J; ++j) acc[e][j] = fma(k.wd[q][j], xd, acc[e][j]);
+    for (int j = 0; j < J; ++j) acc[e][j] = first ? k.wd[q][j] * xd : fma(k.wd[q][j], xd, acc[e][j]);
   }
 }
 

@@ -139,6 +139,11 @@ struct Oz1Dev {
   int64_t ldc;
   unsigned long long *cycles;
   int slice_bits;  // 7 or 8
+  int group_m;     // rasterisation group (tile_coords)
+  int serp;        // 1: every other tile of a CTA walks k downwards, so the k-blocks its L2 neighbourhood used last come first
+  unsigned long long *wave_ctr;  // wave barrier (null: none): all CTAs start their w-th tile together, so that the CTAs
+                                 // sharing an A or B panel ask for the same k-block at the same time (one DRAM read)
+  int n_waves;                   // ceil(items / workers): every CTA arrives that many times
   int dbg;  // experiment flags (emugemm_dbg_set_flags): 1 = no TMA after the ring is first filled, 2 = no epilogue math
 };
 
@@ -358,14 +363,24 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       // L2 eviction hints were measured and dropped: EVICT_LAST on A changes nothing (15.1 vs 15.2 GB DRAM reads per
       // 8192^3 p = 8 launch), EVICT_FIRST on B raises them to 21.9 GB
       constexpr uint64_t polA = kEvictNormal, polB = kEvictNormal;
-      for (int item = work_id; item < num_items; item += num_workers) {
+      int wave = 0;
+      for (int item = work_id; item < num_items; item += num_workers, ++wave) {
+        // static round-robin keeps the tiles of a wave adjacent, but CTAs drift apart by whole tiles over a launch (the
+        // per-SM speed differs by a few per cent) and then every CTA streams its own copy of the panels from DRAM
+        // (13.7 GB instead of ~7 GB per 8192^3 p = 8 launch, ncu): re-align the producers at every tile
+        if (a.wave_ctr && wave > 0) grid_wait(a.wave_ctr, static_cast<unsigned long long>(wave) * gridDim.x);
         const int bidx = item / per_entry, rem = item - bidx * per_entry;
         const int chunk = rem / num_tiles, tile = rem - chunk * num_tiles;
         const int kb0 = a.kb0 + chunk * a.chunk_kb, kb1 = (kb0 + a.chunk_kb < a.kb1) ? kb0 + a.chunk_kb : a.kb1;
         int mb, nb;
-        tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
+        tile_coords(tile, a.mt, a.nt_tiles, mb, nb, a.group_m);
+        if (EMU_PROBE_FLAG(a.dbg, 64)) { mb = 0; nb = 0; }  // probe: every CTA loads tile (0, 0): no DRAM traffic, same L2 -> SM traffic
         if constexpr (MC) nb = 2 * nb + static_cast<int>(cta);  // a.nt_tiles counts PAIRS of N-tiles
         const int rowA0 = static_cast<int>(bidx * a.m), rowB0 = static_cast<int>(bidx * a.n);  // this entry's plane rows
+        // integer accumulation is exact in any order: odd tiles of this CTA walk k downwards (serpentine), so the k-blocks
+        // the previous tile (and its L2 neighbours) touched last are the first ones asked for again
+        const bool rev = a.serp && (((item - work_id) / num_workers) & 1);
+        const int nkb = kb1 - kb0;
         auto load_b = [&](int kbx) {
           mbar_wait(&bempty[sb], pb ^ 1);
           if constexpr (PAIR) {
@@ -386,8 +401,10 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         // at the top of its own k-block, so that its 56-64 KB are not in the way of the next k-block's first A stages
         // (p = 7: 0.884 -> 0.913 per clock, p = 8: 0.941 -> 0.946; with three stages per k-block the two places coincide)
         constexpr bool early_b = !PAIR && Cfg::NPAIR >= 4;
-        for (int kb = kb0; kb < kb1; ++kb) {
-          if (!early_b || kb == kb0) load_b(kb);
+        for (int it = 0; it < nkb; ++it) {
+          const int kb = rev ? kb1 - 1 - it : kb0 + it;
+          const int kb_next = rev ? kb - 1 : kb + 1;
+          if (!early_b || it == 0) load_b(kb);
 #pragma unroll 1
           for (int j = 0; j < Cfg::NPAIR; ++j) {
             const int lo = j, hi = P - 1 - j;
@@ -415,10 +432,13 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             }
             ++nloada;
             if (++sa == SA) { sa = 0; pa ^= 1; }
-            if (early_b && j == 2 && kb + 1 < kb1) load_b(kb + 1);
+            if (early_b && j == 2 && it + 1 < nkb) load_b(kb_next);
           }
         }
+        if (a.wave_ctr) grid_arrive(a.wave_ctr);  // all loads of this tile are issued
       }
+      if (a.wave_ctr)
+        for (; wave < a.n_waves; ++wave) grid_arrive(a.wave_ctr);  // no tile in the last wave(s): the others must not wait for us
     }
     __syncwarp();
   } else if (warp == 1) {
@@ -490,7 +510,7 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       ac.eB = a.eB + bidx * a.n;
       epi.set_item(ac);
       int mb, nb;
-      tile_coords(tile, a.mt, a.nt_tiles, mb, nb);
+      tile_coords(tile, a.mt, a.nt_tiles, mb, nb, a.group_m);
       if constexpr (MC) nb = 2 * nb + static_cast<int>(cta);
       const int64_t grow = static_cast<int64_t>(mb) * kTileRows + (PAIR ? cta * kTileM : 0u) + row;
       const bool row_ok = grow < a.m;
@@ -592,6 +612,10 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   d.out_kind = g.out_kind; d.alpha = g.alpha; d.beta = g.beta; d.C = g.C; d.ldc = g.ldc;
   d.cycles = g.cycles;
   d.slice_bits = g.slice_bits;
+  d.group_m = pick_group_m(ctx->dbg_flags, kGroupM);
+  d.wave_ctr = nullptr;
+  d.n_waves = 0;
+  d.serp = EMU_PROBE_FLAG(ctx->dbg_flags, 128) ? 0 : 1;
   d.dbg = ctx->dbg_flags;
   constexpr bool CL2 = PAIR || MC;
   const int64_t tiles = static_cast<int64_t>(d.mt) * d.nt_tiles * d.nch * batch;
@@ -619,6 +643,21 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   attr[0].val.clusterDim.z = 1;
   cfg.attrs = attr;
   cfg.numAttrs = 1;
+  // Wave barrier: only when every CTA is certainly co-resident (grid <= the clusters the device can hold at once), there
+  // are at least two waves, and the panels are long: measured (A/B, profiles/r2_wave_barrier.md) +18-19 % at 16384^3
+  // (p = 8, FP32 p = 4: the SM clock goes 1.16 -> 1.40 GHz), +1-3 % at 8192^3 p = 8, -0.3 ... -1.9 % at 8192^3 p <= 7 and at
+  // 4096^3 (the re-alignment costs ~1 % of the tensor pipe per clock), so it is on for >= 64 KB of slices per operand row
+  // or k >= 16384.  Probes build: flag 0x10000 switches it off, 0x40000 forces it on.
+  const int workers_used = grid / (CL2 ? 2 : 1);
+  const bool long_panels = static_cast<int64_t>(d.chunk_kb) * kBlockK * P >= 65536 || static_cast<int64_t>(d.chunk_kb) * kBlockK >= 16384;
+  if (g.wave_ctr && tiles > workers_used && d.chunk_kb >= 16 && (long_panels || EMU_PROBE_FLAG(ctx->dbg_flags, 0x40000)) &&
+      !EMU_PROBE_FLAG(ctx->dbg_flags, 0x10000)) {
+    int max_clusters = 0;
+    if (cudaOccupancyMaxActiveClusters(&max_clusters, kern, &cfg) == cudaSuccess && max_clusters >= workers_used) {
+      d.wave_ctr = g.wave_ctr;
+      d.n_waves = static_cast<int>((tiles + workers_used - 1) / workers_used);
+    }
+  }
   EMU_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d));
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());

@@ -39,6 +39,10 @@ struct Oz2Dev {
   int nbatch;  // strided batched call: entry b uses plane rows [b m, (b+1) m) / [b n, (b+1) n) and CR[l][b]
   int8_t *CR;
   unsigned long long *cycles;
+  int group_m;  // rasterisation group (tile_coords)
+  int serp;     // serpentine k (see gemm_oz1.cu)
+  unsigned long long *wave_ctr;  // wave barrier (see gemm_oz1.cu), null: none
+  int n_waves;
   int dbg;
   int mod[kMaxModuli];
   unsigned cvec[kMaxModuli];    // bytes (256^j mod m), j = 0..3 (byte 0 = 256^0)
@@ -121,16 +125,25 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (lane == 0) {
       int st = 0;
       uint32_t ph = 0;
-      for (int tile = cluster_id; tile < num_tiles; tile += num_clusters) {
+      int wave = 0;
+      for (int tile = cluster_id; tile < num_tiles; tile += num_clusters, ++wave) {
+        // re-align the producers of all CTAs at every tile (see gemm_oz1.cu): the pairs that share an A or a B panel then ask
+        // for the same k-block of the same product at the same time, and it comes from DRAM once
+        if (a.wave_ctr && wave > 0) grid_wait(a.wave_ctr, static_cast<unsigned long long>(wave) * gridDim.x);
         const int bidx = tile / tiles_per_entry, te = tile - bidx * tiles_per_entry;
         const int l = te / tiles_per_mod;
         int mb, nb;
-        tile_coords(te - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb);
+        tile_coords(te - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb, a.group_m);
         const int arow = static_cast<int>(bidx * a.m) + mb * kOz2PairM + static_cast<int>(cta) * kTileM;
         const int brow = static_cast<int>(bidx * a.n) + nb * kOz2NT + static_cast<int>(cta) * (kOz2NT / 2);
+        // exact integer accumulation: odd tiles of this pair walk k downwards (serpentine), so the k-blocks its L2
+        // neighbourhood touched last are the first ones asked for again
+        const bool rev = a.serp && (((tile - cluster_id) / num_clusters) & 1);
+        const int nstage = (a.kblocks + kOz2KPerStage - 1) / kOz2KPerStage;
         for (int q = 0; q < NPROD; ++q) {
           const int plane = q * a.n_moduli + l;
-          for (int kb = 0; kb < a.kblocks; kb += kOz2KPerStage) {
+          for (int sidx = 0; sidx < nstage; ++sidx) {
+            const int kb = (rev ? nstage - 1 - sidx : sidx) * kOz2KPerStage;
             const int nkb = (a.kblocks - kb < kOz2KPerStage) ? a.kblocks - kb : kOz2KPerStage;
             mbar_wait(&empty[st], ph ^ 1);
             const uint32_t full_leader = mapa_u32(&full[st], 0);
@@ -143,7 +156,10 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             if (++st == kOz2Stages) { st = 0; ph ^= 1; }
           }
         }
+        if (a.wave_ctr) grid_arrive(a.wave_ctr);
       }
+      if (a.wave_ctr)
+        for (; wave < a.n_waves; ++wave) grid_arrive(a.wave_ctr);
     }
     __syncwarp();
   } else if (warp == 1) {
@@ -154,12 +170,15 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       uint32_t item = 0;
       constexpr uint32_t idesc = make_idesc_i8(kOz2PairM, kOz2NT);
       bool ready = false;  // look-ahead probe of the next stage's barrier (see gemm_oz1.cu)
+      const int nstage = (a.kblocks + kOz2KPerStage - 1) / kOz2KPerStage;
       for (int tile = cluster_id; tile < num_tiles; tile += num_clusters) {
+        const bool rev = a.serp && (((tile - cluster_id) / num_clusters) & 1);  // the producer's k direction for this tile
         for (int q = 0; q < NPROD; ++q, ++item) {
           const uint32_t slot = item & 1, tph = (item >> 1) & 1;
           mbar_wait(&tempty[slot], tph ^ 1);
           tc_fence_after();
-          for (int kb = 0; kb < a.kblocks; kb += kOz2KPerStage) {
+          for (int sidx = 0; sidx < nstage; ++sidx) {
+            const int kb = (rev ? nstage - 1 - sidx : sidx) * kOz2KPerStage;  // only the (possibly short) last stage differs
             const int nkb = (a.kblocks - kb < kOz2KPerStage) ? a.kblocks - kb : kOz2KPerStage;
             if (!ready) mbar_wait(&full[st], ph);
             tc_fence_after();
@@ -174,7 +193,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
 #pragma unroll
                 for (int ks = 0; ks < kBlockK / 32; ++ks)
                   umma_i8_cg2(tmem_base + slot * kOz2NT, make_sdesc_sw128(a_base + ks * 32), make_sdesc_sw128(b_base + ks * 32),
-                              idesc, (kb | i | ks) ? 1u : 0u);
+                              idesc, (sidx | i | ks) ? 1u : 0u);
               }
             }
             umma_commit_cg2(&empty[st_cur], 3);  // both CTAs' producers may refill the stage
@@ -197,7 +216,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       const int bidx = tile / tiles_per_entry, te = tile - bidx * tiles_per_entry;
       const int l = te / tiles_per_mod;
       int mb, nb;
-      tile_coords(te - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb);
+      tile_coords(te - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb, a.group_m);
       ModK mk;
       mk.cvec = a.cvec[l]; mk.c0 = a.c0[l]; mk.magic = a.magic[l]; mk.m = static_cast<unsigned>(a.mod[l]); mk.half = (mk.m + 1) / 2;
       const int64_t grow = static_cast<int64_t>(mb) * kOz2PairM + cta * kTileM + row;
@@ -292,6 +311,8 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
   d.nbatch = batch;
   d.CR = g.CR;
   d.cycles = g.cycles;
+  d.group_m = pick_group_m(ctx->dbg_flags, kGroupM);
+  d.serp = EMU_PROBE_FLAG(ctx->dbg_flags, 128) ? 0 : 1;
   d.dbg = ctx->dbg_flags;
   int mod[24];
   oz2_moduli_host(g.n_moduli, mod);
@@ -311,6 +332,27 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
   const int grid = 2 * (tiles < pairs ? static_cast<int>(tiles) : pairs);
   auto kern = g.is3m ? oz2_gemm_kernel<3> : oz2_gemm_kernel<1>;
   EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kOz2Smem));
+  // Wave barrier (gemm_oz1.cu): only when all CTAs are certainly co-resident, there are at least two waves and a tile is
+  // long enough (>= 16 k-blocks per product) to hide the re-alignment
+  d.wave_ctr = nullptr;
+  d.n_waves = 0;
+  const bool want_sync = g.is3m ? !EMU_PROBE_FLAG(ctx->dbg_flags, 0x10000) : EMU_PROBE_FLAG(ctx->dbg_flags, 0x20000) != 0;
+  if (g.wave_ctr && want_sync && tiles > grid / 2 && d.kblocks >= 16) {
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(grid));
+    cfg.blockDim = dim3(kGemmThreads);
+    cfg.dynamicSmemBytes = kOz2Smem;
+    cudaLaunchAttribute attr[1];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 1;
+    int max_clusters = 0;
+    if (cudaOccupancyMaxActiveClusters(&max_clusters, kern, &cfg) == cudaSuccess && max_clusters >= grid / 2) {
+      d.wave_ctr = g.wave_ctr;
+      d.n_waves = static_cast<int>((tiles + grid / 2 - 1) / (grid / 2));
+    }
+  }
   kern<<<grid, kGemmThreads, kOz2Smem, ctx->stream>>>(tmA, tmB, d);
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());

@@ -92,6 +92,14 @@ __global__ void __launch_bounds__(256) colmax_kernel(const T *__restrict__ X, in
   if (mx) atomicMax(&maxbits[j], mx);
 }
 
+// Non-finite inputs ("result unspecified, no fault"; the pre-pass raises a device-side flag): the row /
+// column maximum of the |x| bit patterns has an all-ones exponent field exactly when the row / column holds an Inf or NaN.
+template <typename T>
+__device__ __forceinline__ void flag_nonfinite(unsigned long long maxbits, unsigned long long *flag) {
+  const unsigned long long inf = sizeof(T) == 8 ? 0x7FF0000000000000ull : 0x7F800000ull;
+  if (flag && maxbits >= inf) atomicOr(flag, 1ull);
+}
+
 // frexp exponent of the magnitude whose bit pattern is b (the row / column maximum); zero row -> 0 (R2)
 template <typename T>
 __device__ __forceinline__ int exponent_of_maxbits(unsigned long long b) {
@@ -435,7 +443,7 @@ template <typename T, int W, int MODE, int PARAM>
 __global__ void __launch_bounds__(256) planes_rows_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows,
                                                           int64_t k, int64_t kpad, int32_t *__restrict__ e_out,
                                                           int param, int scale_bits, int8_t *__restrict__ out,
-                                                          int64_t xstride, int64_t plane_rows) {
+                                                          int64_t xstride, int64_t plane_rows, unsigned long long *nf_flag) {
   // batch entry b = blockIdx.y (strided batched calls: entry b of X starts xstride elements further; its planes are
   // rows [b rows, (b + 1) rows) of planes that hold plane_rows rows)
   const int64_t row = static_cast<int64_t>(blockIdx.y) * rows + blockIdx.x;
@@ -461,7 +469,7 @@ __global__ void __launch_bounds__(256) planes_rows_kernel(const T *__restrict__ 
 #pragma unroll
   for (int w = 0; w < 8; ++w) mx = red[w] > mx ? red[w] : mx;
   const int e_row = exponent_of_maxbits<T>(mx);
-  if (threadIdx.x == 0) e_out[row] = e_row;
+  if (threadIdx.x == 0) { e_out[row] = e_row; flag_nonfinite<T>(mx, nf_flag); }
 
   const int64_t plane_stride = plane_rows * kpad;
   for (int64_t h0 = static_cast<int64_t>(threadIdx.x) * 4; h0 < kpad; h0 += 1024) {
@@ -508,7 +516,7 @@ template <typename T, int W, int MODE, int PARAM, int NT>
 __global__ void __launch_bounds__(NT) planes_rows_reg_kernel(const T *__restrict__ X, int64_t ldx, int64_t rows,
                                                               int64_t k, int64_t kpad, int32_t *__restrict__ e_out,
                                                               int param, int scale_bits, int8_t *__restrict__ out,
-                                                              int64_t xstride, int64_t plane_rows) {
+                                                              int64_t xstride, int64_t plane_rows, unsigned long long *nf_flag) {
   constexpr int R = 8 / W;
   const int64_t row = static_cast<int64_t>(blockIdx.y) * rows + blockIdx.x;
   const T *src = X + (static_cast<int64_t>(blockIdx.y) * xstride + static_cast<int64_t>(blockIdx.x) * ldx) * W;
@@ -545,7 +553,7 @@ __global__ void __launch_bounds__(NT) planes_rows_reg_kernel(const T *__restrict
 #pragma unroll
   for (int w = 0; w < NT / 32; ++w) mx = red[w] > mx ? red[w] : mx;
   const int e_row = exponent_of_maxbits<T>(mx);
-  if (threadIdx.x == 0) e_out[row] = e_row;
+  if (threadIdx.x == 0) { e_out[row] = e_row; flag_nonfinite<T>(mx, nf_flag); }
 
   const int64_t plane_stride = plane_rows * kpad;
 #pragma unroll
@@ -567,7 +575,8 @@ __global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ 
                                                           int64_t k, int64_t kpad,
                                                           const unsigned long long *__restrict__ maxbits,
                                                           int32_t *__restrict__ e_out, int param, int scale_bits, int nplanes,
-                                                          int8_t *__restrict__ out, int64_t xstride, int64_t plane_rows) {
+                                                          int8_t *__restrict__ out, int64_t xstride, int64_t plane_rows,
+                                                          unsigned long long *nf_flag) {
   extern __shared__ unsigned int tile[];  // [plane][32][TH/4 + 1]
   // batch entry blockIdx.z (see planes_rows_kernel)
   X += static_cast<int64_t>(blockIdx.z) * xstride * W;
@@ -580,7 +589,7 @@ __global__ void __launch_bounds__(256) planes_cols_kernel(const T *__restrict__ 
   const int64_t hb = static_cast<int64_t>(blockIdx.y) * TH;
   // column exponent from the column-max bit pattern (colmax_kernel ran before); the first k-block publishes it
   const int e_row = (j < rows) ? exponent_of_maxbits<T>(maxbits[j]) : 0;
-  if (blockIdx.y == 0 && warp == 0 && j < rows) e_out[j] = e_row;
+  if (blockIdx.y == 0 && warp == 0 && j < rows) { e_out[j] = e_row; flag_nonfinite<T>(maxbits[j], nf_flag); }
   for (int hw = warp; hw < TH / 4; hw += 8) {
     const int64_t h0 = hb + hw * 4;
     T v[4][W];
@@ -631,17 +640,17 @@ static int launch_planes(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, 
     if constexpr (MODE == 0) {
       if (!two_phase && kpad * W <= 32 * 256) {
         planes_rows_reg_kernel<T, W, MODE, PARAM, 256><<<grid, 256, 0, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, out,
-                                                                              xstride, plane_rows);
+                                                                              xstride, plane_rows, ctx->nf_flag);
         done = true;
       } else if (!two_phase && kpad * W <= 32 * 512) {
         planes_rows_reg_kernel<T, W, MODE, PARAM, 512><<<grid, 512, 0, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, out,
-                                                                              xstride, plane_rows);
+                                                                              xstride, plane_rows, ctx->nf_flag);
         done = true;
       }
     }
     if (!done)
       planes_rows_kernel<T, W, MODE, PARAM><<<grid, 256, 0, st>>>(x, ldx, rows, k, kpad, e, param, scale_bits, out, xstride,
-                                                                   plane_rows);
+                                                                   plane_rows, ctx->nf_flag);
     ctx->launches++;
   } else {
     // The column maxima are a true dependency: a separate launch reads X once more.  A single-read variant (tile kept in
@@ -655,14 +664,14 @@ static int launch_planes(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, 
       auto kern = planes_cols_kernel<T, W, MODE, PARAM, TH>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 20 * 32 * (TH / 4 + 1) * 4));
       const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH), static_cast<unsigned>(batch));
-      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, param, scale_bits, nplanes, out, xstride, plane_rows);
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, param, scale_bits, nplanes, out, xstride, plane_rows, ctx->nf_flag);
     } else {
       constexpr int TH = 32;
       const size_t smem = static_cast<size_t>(nplanes) * 32 * (TH / 4 + 1) * 4;
       auto kern = planes_cols_kernel<T, W, MODE, PARAM, TH>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 60 * 32 * (TH / 4 + 1) * 4));
       const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / TH), static_cast<unsigned>(batch));
-      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, param, scale_bits, nplanes, out, xstride, plane_rows);
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, param, scale_bits, nplanes, out, xstride, plane_rows, ctx->nf_flag);
     }
     ctx->launches++;
   }
@@ -734,7 +743,7 @@ __device__ __forceinline__ void emit_oz1_any(const Prep (&q)[4], Sink sink) {
 template <typename T, int PARAM>
 __global__ void __launch_bounds__(256) oz1_4m_rows_kernel(const T *__restrict__ X, int64_t ldx, int64_t m, int64_t k,
                                                           int64_t kpad, int32_t *__restrict__ e_out, int scale_bits,
-                                                          int8_t *__restrict__ out) {
+                                                          int8_t *__restrict__ out, unsigned long long *nf_flag) {
   const int64_t row = blockIdx.x;
   const T *src = X + row * ldx * 2;
   unsigned long long mx = 0;
@@ -755,7 +764,7 @@ __global__ void __launch_bounds__(256) oz1_4m_rows_kernel(const T *__restrict__ 
 #pragma unroll
   for (int w = 0; w < 8; ++w) mx = red[w] > mx ? red[w] : mx;
   const int e_row = exponent_of_maxbits<T>(mx);
-  if (threadIdx.x == 0) { e_out[row] = e_row; e_out[m + row] = e_row; }
+  if (threadIdx.x == 0) { e_out[row] = e_row; e_out[m + row] = e_row; flag_nonfinite<T>(mx, nf_flag); }
 
   const int64_t kk = 2 * kpad, plane_stride = 2 * m * kk;
   for (int64_t h0 = static_cast<int64_t>(threadIdx.x) * 4; h0 < kpad; h0 += 1024) {
@@ -784,14 +793,14 @@ template <typename T, int PARAM>
 __global__ void __launch_bounds__(256) oz1_4m_cols_kernel(const T *__restrict__ X, int64_t ldx, int64_t n, int64_t k,
                                                           int64_t kpad, const unsigned long long *__restrict__ maxbits,
                                                           int32_t *__restrict__ e_out, int scale_bits, int P,
-                                                          int8_t *__restrict__ out) {
+                                                          int8_t *__restrict__ out, unsigned long long *nf_flag) {
   extern __shared__ unsigned int tile[];  // [2 P][32][33]
   constexpr int TH = 128, PW = TH / 4 + 1;
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const int64_t j = static_cast<int64_t>(blockIdx.x) * 32 + lane;
   const int64_t hb = static_cast<int64_t>(blockIdx.y) * TH;
   const int e_row = (j < n) ? exponent_of_maxbits<T>(maxbits[j]) : 0;
-  if (blockIdx.y == 0 && warp == 0 && j < n) e_out[j] = e_row;
+  if (blockIdx.y == 0 && warp == 0 && j < n) { e_out[j] = e_row; flag_nonfinite<T>(maxbits[j], nf_flag); }
   for (int hw = warp; hw < TH / 4; hw += 8) {
     const int64_t h0 = hb + hw * 4;
     Prep re[4], im[4];
@@ -824,19 +833,19 @@ static int slice4m_p(emugemm_ctx *ctx, int is_b, int64_t rows, int64_t k, int64_
   const T *x = static_cast<const T *>(X);
   const int scale_bits = slice_bits == 8 ? 8 * P - 2 : kBeta * P;
   if (!is_b) {
-    if (slice_bits == 8) oz1_4m_rows_kernel<T, 16 + P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out);
-    else oz1_4m_rows_kernel<T, P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out);
+    if (slice_bits == 8) oz1_4m_rows_kernel<T, 16 + P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out, ctx->nf_flag);
+    else oz1_4m_rows_kernel<T, P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out, ctx->nf_flag);
   } else {
     const size_t smem = static_cast<size_t>(2 * P) * 32 * 33 * 4;
     const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / 128));
     if (slice_bits == 8) {
       auto kern = oz1_4m_cols_kernel<T, 16 + P>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 32 * 33 * 4));
-      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, scale_bits, P, out);
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, scale_bits, P, out, ctx->nf_flag);
     } else {
       auto kern = oz1_4m_cols_kernel<T, P>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 32 * 33 * 4));
-      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, scale_bits, P, out);
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, scale_bits, P, out, ctx->nf_flag);
     }
   }
   ctx->launches++;

@@ -64,6 +64,26 @@ __device__ __forceinline__ void mbar_wait(uint64_t *bar, uint32_t parity) {
   }
 }
 
+// ---------------------------------------------------------------- grid-wide wave barrier (all CTAs co-resident)
+// Monotonic counter: every CTA arrives once per wave; wave w may start when the counter has reached w * (number of CTAs).
+// Bounded like mbar_wait: a CTA that is not co-resident must trap, never hang the GPU.
+__device__ __forceinline__ void grid_arrive(unsigned long long *ctr) {
+  asm volatile("red.release.gpu.global.add.u64 [%0], 1;" ::"l"(ctr) : "memory");
+}
+__device__ __forceinline__ void grid_wait(const unsigned long long *ctr, unsigned long long target) {
+  unsigned long long v;
+  const long long t0 = clock64();
+  for (;;) {
+    asm volatile("ld.acquire.gpu.global.u64 %0, [%1];" : "=l"(v) : "l"(ctr) : "memory");
+    if (v >= target) return;
+    __nanosleep(64);
+    if (clock64() - t0 > 4000000000LL) {
+      printf("emugemm: wave barrier timeout block %d (%llu of %llu)\n", blockIdx.x, v, target);
+      __trap();
+    }
+  }
+}
+
 // ---------------------------------------------------------------- TMA
 __device__ __forceinline__ void tma_prefetch_desc(const CUtensorMap *tm) {
   asm volatile("prefetch.tensormap [%0];" ::"l"(tm) : "memory");

@@ -90,3 +90,32 @@ def test_degenerate_oz2_and_3m(env):
     Cc = torch.ones((130, 130), dtype=torch.float64, device="cuda")
     h.dgemm_oz2(Z, Z, Cc, 16)  # all-zero operands
     assert (Cc == 0).all()
+
+
+def test_nonfinite_flag(env):
+    """non-finite inputs give an unspecified result and no fault; the pre-pass raises a flag."""
+    import numpy as np
+    torch, E, h = env[0], env[1], env[2]
+    A = torch.rand((70, 130), dtype=torch.float64, device="cuda") - 0.5
+    B = torch.rand((130, 50), dtype=torch.float64, device="cuda") - 0.5
+    C = torch.zeros((70, 50), dtype=torch.float64, device="cuda")
+    h.dgemm_oz1(A, B, C, 4)
+    assert h.nonfinite_seen() is False
+    for bad, where in ((float("inf"), "A"), (float("nan"), "B"), (-float("inf"), "B")):
+        A2, B2 = A.clone(), B.clone()
+        (A2 if where == "A" else B2)[3, 7] = bad
+        h.dgemm_oz1(A2, B2, C, 4)
+        assert h.nonfinite_seen() is True
+        h.dgemm_oz2(A2, B2, C, 12)
+        assert h.nonfinite_seen() is True
+    h.dgemm_oz2(A, B, C, 12)
+    assert h.nonfinite_seen() is False   # the flag describes the last call only
+    Z = (torch.rand((40, 64), dtype=torch.float64, device="cuda") - 0.5).to(torch.complex128)
+    Z[1, 2] = complex(0.0, float("nan"))
+    W = (torch.rand((64, 30), dtype=torch.float64, device="cuda") - 0.5).to(torch.complex128)
+    Cz = torch.zeros((40, 30), dtype=torch.complex128, device="cuda")
+    h.zgemm_oz2_3m(Z, W, Cz, 14)
+    assert h.nonfinite_seen() is True
+    torch.cuda.synchronize()  # no fault: the device is still usable
+    h.dgemm_oz1(A, B, C, 4)
+    assert torch.isfinite(C).all()

@@ -1,9 +1,11 @@
 """-m gpu: pre-decomposed operands (emugemm_decompose + emugemm_gemm_pre):
-bit-identical to the one-shot calls, an operand decomposed once is reused against several partners."""
+bit-identical to the one-shot calls, an operand decomposed once is reused against several partners, and the results
+match the ORACLE on the same inputs (2 ulp of (|A||B|)_ij), including transposed-storage operands."""
 import numpy as np
 import pytest
 
 import emugemm_inputs as G
+from gpu_util import assert_within_ulps
 
 pytestmark = pytest.mark.gpu
 
@@ -80,3 +82,50 @@ def test_mismatched_operands_rejected(env):
     assert ei.value.status == -1
     with pytest.raises(E.EmuGemmError):
         h.gemm_pre(opA, opA, Cc)  # two left operands
+
+
+@pytest.mark.parametrize("transa,transb", [(False, False), (True, False), (False, True), (True, True)])
+def test_oz1_operands_against_oracle(env, transa, transb):
+    """emugemm_decompose with either storage of either operand, then emugemm_gemm_pre, against oracle_dgemm_oz1."""
+    torch, E, h = env
+    from oracle import oracle as O
+    m, n, k, p = 150, 200, 260, 6
+    A, B, Cin = G.real_pair(m, n, k, 1.0, 31, with_c=True)
+    opA = h.decompose(E.OZ1, 0, dev(torch, A.T if transa else A), p, trans=transa)
+    opB = h.decompose(E.OZ1, 1, dev(torch, B.T if transb else B), p, trans=transb)
+    C = dev(torch, Cin)
+    h.gemm_pre(opA, opB, C, alpha=-0.75, beta=1.5)
+    want = O.dgemm_oz1(A, B, p, alpha=-0.75, beta=1.5, Cin=Cin)
+    _, absAB = O.bf128_dgemm(A, B)
+    assert_within_ulps(C.cpu().numpy(), want, 0.75 * absAB + 1.5 * np.abs(Cin), 2, what=f"operands oz1 {transa} {transb}")
+
+
+@pytest.mark.parametrize("transa,transb", [(False, False), (True, True)])
+def test_oz2_operands_against_oracle(env, transa, transb):
+    torch, E, h = env
+    from oracle import oracle as O
+    m, n, k, N = 130, 140, 300, 15
+    A, B = G.real_pair(m, n, k, 1.0, 32)
+    opA = h.decompose(E.OZ2, 0, dev(torch, A.T if transa else A), N, trans=transa)
+    opB = h.decompose(E.OZ2, 1, dev(torch, B.T if transb else B), N, trans=transb)
+    C = torch.full((m, n), float("nan"), dtype=torch.float64, device="cuda")
+    h.gemm_pre(opA, opB, C)
+    _, absAB = O.bf128_dgemm(A, B)
+    assert_within_ulps(C.cpu().numpy(), O.dgemm_oz2(A, B, N), absAB, 2, what=f"operands oz2 {transa} {transb}")
+
+
+def test_3m_operands_against_oracle(env):
+    torch, E, h = env
+    from oracle import oracle as O
+    m, n, k, N = 90, 70, 200, 14
+    A, B = G.complex_pair(m, n, k, 1.0, 33)
+    oa = h.decompose(E.OZ2_3M, 0, dev(torch, A), N)
+    ob = h.decompose(E.OZ2_3M, 1, dev(torch, B.T), N, trans=True)
+    Z = torch.zeros((m, n), dtype=torch.complex128, device="cuda")
+    h.gemm_pre(oa, ob, Z, alpha=0.5 - 2j)
+    want = O.zgemm_oz2_3m(A, B, N, alpha=0.5 - 2j)
+    _, absZ = O.bf128_zgemm(A, B)
+    got = Z.cpu().numpy()
+    scale = abs(0.5 - 2j) * 2 * absZ
+    assert_within_ulps(got.real, want.real, scale, 2, what="operands 3M re")
+    assert_within_ulps(got.imag, want.imag, scale, 2, what="operands 3M im")

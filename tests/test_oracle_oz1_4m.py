@@ -52,3 +52,21 @@ def test_cgemm_oracles_exact_on_gaussian_integers_and_close_to_truth():
     exact, absZ = O.bf128_zgemm(Ac.astype(np.complex128), Bc.astype(np.complex128))
     for got in (O.cgemm_oz1_4m(Ac, Bc, 4), O.cgemm_oz2_3m(Ac, Bc, 11)):
         assert (np.abs(got.astype(np.complex128) - exact) <= 8 * 2.0 ** -23 * absZ).all()
+
+
+def test_four_products_equal_the_real_embedding():
+    """The oracle states 4M as four separate real slice products; the same value must come out of ONE real Scheme I
+    product on the embedding A' = [[Re A, -Im A], [Im A, Re A]], B' = [[Re B], [Im B]] (the form the CUDA path uses),
+    bit for bit: rows i and m + i of A' share the exponent of row i of A, the digits of -Im A are the negated digits."""
+    try:
+        for bits, p, seed in ((7, 3, 5), (7, 6, 6), (7, 8, 7), (8, 4, 8), (8, 7, 9)):
+            O.set_slice_bits(bits)
+            A, B = G.complex_pair(21, 17, 50, 1.0, seed)
+            m = A.shape[0]
+            Ae = np.ascontiguousarray(np.block([[A.real, -A.imag], [A.imag, A.real]]))
+            Be = np.ascontiguousarray(np.vstack([B.real, B.imag]))
+            T = O.dgemm_oz1(Ae, Be, p)
+            got = O.zgemm_oz1_4m(A, B, p)
+            assert np.array_equal(got.real, T[:m]) and np.array_equal(got.imag, T[m:]), (bits, p)
+    finally:
+        O.set_slice_bits(7)
