@@ -29,7 +29,7 @@ METRIC = "emulated FP64 TFLOP/s (2mnk/t) & INT8 Top/s as % of B200 dense INT8 pe
 def parse():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=20)
+    ap.add_argument("--steps", type=int, default=30)  # median of >= 30 runs
     ap.add_argument("--warmup", type=int, default=5)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--scheme", default="oz1", choices=["oz1", "oz1s", "oz2", "oz2z"])
@@ -44,6 +44,10 @@ def parse():
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-probe", action="store_true")
     ap.add_argument("--cpu-sample", type=int, default=0, help="rows = cols of the oracle sample")
+    ap.add_argument("--probe-flags", type=lambda x: int(x, 0), default=0,
+                    help="A/B experiments only (results may be WRONG): run the PROBES build of the library with these "
+                         "emugemm_dbg_set_flags bits (include/emugemm.h), e.g. 0x10000 = no wave barrier")
+    ap.add_argument("--fusion", action="store_true", help="Scheme II: fused reconstruction inside the GEMM kernel (default: separate CRT kernel)")
     return ap.parse_args()
 
 
@@ -56,16 +60,19 @@ def workload(a):
         seed, phi = (1, 0.5) if a.scheme == "oz1" else (4, 1.0)
         ops = p * (p + 1) * m * n * k  # INT8 ops (p(p+1)/2 products of 2mnk)
         flops = 2.0 * m * n * k
+        alg = p * (m + n) * k + (8 if a.scheme == "oz1" else 4) * m * n  # Eq. 10: fused GEMM bytes
         name = f"{'OZ1 DGEMM' if a.scheme == 'oz1' else 'OZ1 SGEMM'} m={m} n={n} k={k} p={p}"
     else:
         p = a.p or (16 if a.scheme == "oz2" else 14)
         seed, phi = (2, 1.0) if a.scheme == "oz2" else (3, 1.0)
         ops = (1 if a.scheme == "oz2" else 3) * p * 2 * m * n * k
         flops = (2.0 if a.scheme == "oz2" else 8.0) * m * n * k
+        # Eq. 15 / 18: per modulus (m+n)k + mn, 3M 3(m+n)k + 2mn
+        alg = p * ((m + n) * k + m * n) if a.scheme == "oz2" else p * (3 * (m + n) * k + 2 * m * n)
         name = f"{'OZ2 DGEMM' if a.scheme == 'oz2' else 'OZ2 ZGEMM-3M'} m={m} n={n} k={k} N={p}"
     if a.phi >= 0:
         phi = a.phi
-    return dict(m=m, n=n, k=k, p=p, seed=seed, phi=phi, ops=float(ops), flops=float(flops), name=name)
+    return dict(m=m, n=n, k=k, p=p, seed=seed, phi=phi, ops=float(ops), flops=float(flops), name=name, alg_bytes=float(alg))
 
 
 def make_inputs(a, w, seed_offset=0):
@@ -154,18 +161,53 @@ def cpu_oracle_leg(a, w, sample):
             "sample": f"{len(rows)} rows x {len(cols)} cols of the {w['name']} output, full k"}
 
 
+def calibrated_oracle_leg(a, w, target_s=15.0):
+    """cpu_oracle_leg on a sample sized for ~target_s seconds of CPU work: calibrate on 96 x 96 sampled outputs (fixed
+    per-call slicing cost included, so small samples are pessimistic), then run the sized sample.  The SAME routine
+    serves `cpu_baseline` of the main arm and every step of `--impl reference`, so the two figures agree."""
+    cal = cpu_oracle_leg(a, w, 96)
+    per_elem = cal["seconds"] / (96 * 96)
+    side = int(min(w["m"], w["n"], max(96, (2.7 * target_s / max(per_elem, 1e-9)) ** 0.5)))
+    return cpu_oracle_leg(a, w, side), side
+
+
+def oracle_context(a, w):
+    """SURVEY 8(d) / BASELINE.md 3: the oracle single-threaded on a small sample of this workload, and BASELINE config 1
+    (Scheme I DGEMM 256^3, p = 6) IN FULL with one thread and with all threads.  Context beside `cpu_baseline`."""
+    import emugemm_inputs as G
+    from oracle import oracle as O
+    out = {}
+    nthreads = O.threads()
+    try:
+        O.set_threads(1)
+        st = cpu_oracle_leg(a, w, 48)
+        out["single_thread"] = {"value": st["value"], "unit": "TFLOP/s", "cores": 1, "seconds": st["seconds"], "sample": st["sample"]}
+        A, B = G.real_pair(256, 256, 256, 0.5, 0)
+        t0 = time.perf_counter(); O.dgemm_oz1(A, B, 6); t1 = time.perf_counter() - t0
+        O.set_threads(nthreads)
+        t0 = time.perf_counter(); O.dgemm_oz1(A, B, 6); tn = time.perf_counter() - t0
+        fl = 2.0 * 256 ** 3
+        out["config1_full_256_p6"] = {"seconds_1_thread": t1, "gflops_1_thread": fl / t1 / 1e9, "seconds_all": tn,
+                                      "gflops_all": fl / tn / 1e9, "cores": nthreads,
+                                      "int_mac_per_s_all": 21.0 * 256 ** 3 / tn}
+    finally:
+        O.set_threads(nthreads)
+    return out
+
+
 def reference_leg(a, w):
-    """--impl reference: the oracle on host cores; each step = a bounded sample of the workload."""
-    sample = a.cpu_sample or 128
+    """--impl reference: the oracle on host cores; each step = the same bounded sample of the workload that the main
+    arm's `cpu_baseline` uses (calibrated to ~15 s), repeated for `steps` steps or until ~150 s are spent."""
     vals, cb = [], None
-    for _ in range(max(1, min(a.warmup, 1))):
-        cpu_oracle_leg(a, w, min(sample, 32))
+    cpu_oracle_leg(a, w, 32)  # warm-up (library load, page-in)
+    first, side = calibrated_oracle_leg(a, w)
+    vals.append(first["value"]); cb = first
     t_all = time.perf_counter()
-    for _ in range(max(1, a.steps)):
-        cb = cpu_oracle_leg(a, w, sample)
-        vals.append(cb["value"])
-        if time.perf_counter() - t_all > 150:
+    for _ in range(max(0, a.steps - 1)):
+        if time.perf_counter() - t_all + first["seconds"] > 150:
             break
+        cb = cpu_oracle_leg(a, w, side)
+        vals.append(cb["value"])
     v = statistics.median(vals)
     cb["value"] = v
     line = {"impl": "reference", "metric": METRIC, "value": v, "unit": "TFLOP/s", "n_gpus": a.gpus, "steps": len(vals),
@@ -213,10 +255,14 @@ def main():
     hC = torch.empty((w["m"], w["n"]), dtype=cdtype).pin_memory()
     dA, dB = hA.cuda(), hB.cuda()
     dC = torch.empty((w["m"], w["n"]), dtype=cdtype, device="cuda")
-    h = E.EmuGemm()
+    h = E.EmuGemm(probes=bool(a.probe_flags))
     stream = torch.cuda.current_stream()
     h.set_stream(stream)
     h.set_slice_bits(a.slice_bits)
+    if a.probe_flags:
+        h.dbg_set_flags(a.probe_flags)
+    if a.fusion:
+        h.set_oz2_fusion(True)
     call = {"oz1": h.dgemm_oz1, "oz1s": h.sgemm_oz1, "oz2": h.dgemm_oz2, "oz2z": h.zgemm_oz2_3m}[a.scheme]
 
     def step():
@@ -259,14 +305,17 @@ def main():
 
     # a second pass without the per-step synchronisation gives the back-to-back step time
     barrier()
-    f0, f1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
-    f0.record(stream)
-    for _ in range(a.steps):
+    marks = [torch.cuda.Event(enable_timing=True) for _ in range(a.steps + 1)]
+    marks[0].record(stream)
+    for i in range(a.steps):
         step()
-    f1.record(stream)
+        marks[i + 1].record(stream)   # an event record does not synchronise: the steps still run back to back
     barrier()
     clocks = sampler.stop(t_win0, time.time())
-    ms_step = shard.max_over_ranks(f0.elapsed_time(f1) / a.steps, dist, "cuda")
+    per_step = [marks[i].elapsed_time(marks[i + 1]) for i in range(a.steps)]
+    ms_step = shard.max_over_ranks(marks[0].elapsed_time(marks[-1]) / a.steps, dist, "cuda")
+    ms_median = statistics.median(per_step)
+    ms_q = statistics.quantiles(per_step, n=4) if len(per_step) >= 4 else [ms_median] * 3
     value = shard.aggregate_throughput(w["flops"], world, ms_step) / 1e12
 
     # ---- end to end: host (pinned) buffers, H2D + call + D2H inside the timed region ----
@@ -352,19 +401,24 @@ def main():
     peak_src = "measured bf16 burst x2 (guide's nominal int8:bf16 ratio 4.5:2.25)" if peaks else \
         "fallback 1.59 PF bf16 x2 (guide's nominal int8:bf16 ratio)"
     gemm_ms = statistics.median(stage[1])
+    gemm_q = statistics.quantiles(stage[1], n=4) if len(stage[1]) >= 4 else [gemm_ms] * 3
     achieved = w["ops"] / (gemm_ms * 1e-3) / 1e12
     peak = 2.0 * bf16_burst
-    traffic = None  # dram__bytes_read.sum + dram__bytes_write.sum of the GEMM kernel, per launch, from the committed ncu capture
+    # dram__bytes_read.sum + dram__bytes_write.sum of the GEMM kernel, per launch, from the committed ncu capture of this
+    # command at this commit (profiles/traffic.csv: workload, kernel, bytes, capture file); ncu cannot run inside a timed run
+    traffic, traffic_src = None, None
     try:
         for row in open(os.path.join(ROOT, "profiles", "traffic.csv")):
             f = [x.strip() for x in row.split(",")]
             if len(f) >= 3 and f[0] == w["name"]:
                 traffic = float(f[2])
+                traffic_src = f[3] if len(f) > 3 else "profiles/traffic.csv"
     except (OSError, ValueError):
         pass
     roof = {"bound": "tensor", "kernel": "oz1_gemm_kernel" if a.scheme.startswith("oz1") else "oz2_gemm_kernel",
             "achieved": achieved, "peak": peak, "unit": "TFLOP/s", "frac": achieved / peak, "traffic": traffic,
-            "peak_source": peak_src, "kernel_ms": gemm_ms, "int8_ops_per_launch": w["ops"],
+            "traffic_source": traffic_src, "algorithmic_bytes": w["alg_bytes"],
+            "peak_source": peak_src, "kernel_ms": gemm_ms, "kernel_ms_iqr": gemm_q[2] - gemm_q[0], "int8_ops_per_launch": w["ops"],
             "frac_of_nominal_4500": achieved / NOMINAL_INT8_TOPS}
     if peaks.get("bf16_tflops_sustained"):
         roof["frac_of_sustained"] = achieved / (2.0 * peaks["bf16_tflops_sustained"])
@@ -438,20 +492,23 @@ def main():
     detail["paper_context"] = "paper: 3654 Top/s (81% of 4500) EmuGEMM-I end-to-end on B200, other machine (PAPER.md:293)"
 
     line = {"metric": METRIC, "value": value, "unit": "TFLOP/s", "n_gpus": world, "steps": a.steps, "warmup": max(a.warmup, 3),
-            "ms_per_step": ms_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "ms_per_step": ms_step, "ms_per_step_median": ms_median, "ms_per_step_iqr": ms_q[2] - ms_q[0],
+            "value_at_median": w["flops"] / (ms_median * 1e-3) / 1e12,
+            "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "int8", "data": "synthetic",
-            "config": {"workload": w["name"], "phi": w["phi"], "seed": w["seed"], "alpha": 1, "beta": 0, "slice_bits": a.slice_bits,
+            "config": {"workload": w["name"], "phi": w["phi"], "seed": w["seed"], "alpha": 1, "beta": 0, "slice_bits": a.slice_bits, "probe_flags": hex(a.probe_flags), "oz2_fusion": bool(a.fusion),
                        "l2": "inputs (A, B, slices > 1 GB) exceed the 126 MB L2, no flush needed",
                        "parallelism": f"{world} independent problems" if world > 1 else "1 GPU"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "detail": detail}
     if not a.no_cpu:
         if a.cpu_sample:
             line["cpu_baseline"] = cpu_oracle_leg(a, w, a.cpu_sample)
-        else:  # calibrate on 96 x 96 sampled outputs, then size the sample for 10-20 s of CPU work
-            cal = cpu_oracle_leg(a, w, 96)
-            per_elem = cal["seconds"] / (96 * 96)
-            side = int(min(w["m"], w["n"], max(96, (40.0 / max(per_elem, 1e-9)) ** 0.5)))  # fixed costs make 96 x 96 pessimistic: lands at 10-20 s
-            line["cpu_baseline"] = cpu_oracle_leg(a, w, side)
+        else:  # the same calibrated sample `--impl reference` times
+            line["cpu_baseline"], _ = calibrated_oracle_leg(a, w)
+        try:
+            line["cpu_baseline"]["context"] = oracle_context(a, w)
+        except Exception as ex:  # context, never the product
+            line["cpu_baseline"]["context_error"] = str(ex)
     print(json.dumps(line))
     h.close()
     if dist is not None:

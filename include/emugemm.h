@@ -63,6 +63,17 @@ int emugemm_set_workspace(emugemm_handle_t h, void *dev_ptr, size_t bytes);
  * column exponent -- 8p - 2 bits per operand, so p = 7 reaches the accuracy of p = 8 at 7 bits
  * with 28 instead of 36 slice products.  Applies to dgemm_oz1, sgemm_oz1 and the Scheme I hooks. */
 int emugemm_set_slice_bits(emugemm_handle_t h, int bits);
+/* Scheme II real FP64 product (emugemm_dgemm_oz2 and its _t / strided-batched / pre-decomposed forms), SURVEY 8(f) item 4
+ * (the paper keeps the CRT separate and pays the residue workspace): on = 1 runs the reconstruction
+ * INSIDE the per-modulus GEMM kernel -- a work item is an output tile, the moduli are the inner loop, the tile's
+ * residues wait in a per-CTA scratch of 2 x N x 32 KB (the [N][m][n] residue planes are never written), and the epilogue
+ * warps run the exact FP64 CRT of the previous tile between the modulus epilogues of the current one.  Applies when
+ * 7 <= n_moduli and the problem has at least two waves of 256 x 256 tiles (the scratch must fit where the residue planes
+ * would have been); otherwise, and with on = 0, the separate CRT kernel runs.  Both paths give bit-identical C.
+ * DEFAULT: off -- measured on B200 the fused form is slower (8192^3, N = 16: 8.9 ms against 5.3 + 0.6 ms; the eight
+ * epilogue warps cannot hide the FP64 reconstruction and the scratch competes with the operand panels for L2,
+ * DESIGN.md 5.7): it is kept as the measured answer to "can Scheme II be fully fused on this machine".           */
+int emugemm_set_oz2_fusion(emugemm_handle_t h, int on);
 /* Bytes of workspace a call with these arguments needs.  elem = bytes per
  * matrix element: 4 (float), 8 (double), 16 (complex128).  p_or_nmoduli = p for
  * Scheme I, n_moduli for Scheme II / 3M.  Returns 0 for invalid arguments. */

@@ -130,6 +130,10 @@ class EmuGemm:
         self._check(self._lib.emugemm_set_slice_bits(self._h, _int(bits)))
         self.slice_bits = bits
 
+    def set_oz2_fusion(self, on):
+        """Scheme II real DGEMM: fused reconstruction inside the GEMM kernel, or (default) the separate CRT kernel."""
+        self._check(self._lib.emugemm_set_oz2_fusion(self._h, _int(1 if on else 0)))
+
     def workspace_bytes(self, scheme, elem, m, n, k, pn):
         return int(self._lib.emugemm_workspace_bytes(scheme, elem, m, n, k, pn))
 

@@ -265,12 +265,26 @@ static int oz2_gemm_phase(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_
   g.batch = batch;
   g.m = m; g.n = n; g.kpad = kpad; g.n_moduli = N; g.is3m = is3m; g.RA = RA; g.RB = RB; g.CR = CR; g.cycles = diag;
   g.wave_ctr = diag ? diag + kDiagWaveCtr : nullptr;
-  EMU_TRY(launch_oz2_gemm(h, g));
-  EMU_TRY(mark(h, 2));
   Oz2CrtArgs c;
   c.m = m; c.n = n; c.n_moduli = N; c.CR = CR; c.eA = eA; c.eB = eB; c.tA = tA; c.tB = tB; c.is_complex = is3m; c.out_f32 = out_f32;
   c.alpha[0] = alpha[0]; c.alpha[1] = alpha[1]; c.beta[0] = beta[0]; c.beta[1] = beta[1];
   c.C = C; c.ldc = ldc; c.batch = batch; c.batch_stride_c = batch_stride_c;
+  // Fused reconstruction: real FP64 product, 7 <= N <= 20, and the per-CTA scratch (2 x N x 32 KB for
+  // each of the <= num_sms CTAs) must fit in the region the residue planes would have taken -- true for every problem of
+  // at least two waves of 256 x 256 tiles; smaller ones keep the separate CRT kernel.
+  const int64_t tiles_out = ((m + 255) / 256) * ((n + 255) / 256) * batch;
+  const int64_t ctas = 2 * (tiles_out < h->num_sms / 2 ? tiles_out : h->num_sms / 2);
+  const size_t cr_bytes = static_cast<size_t>(N) * m * n * batch;
+  if (h->oz2_fusion && !is3m && !out_f32 && N >= 7 && static_cast<size_t>(ctas) * 2 * N * 32768 <= cr_bytes) {
+    g.fused = &c;
+    g.scratch_bytes = cr_bytes;
+    EMU_TRY(launch_oz2_gemm(h, g));
+    EMU_TRY(mark(h, 2));
+    EMU_TRY(mark(h, 3));
+    return EMUGEMM_OK;
+  }
+  EMU_TRY(launch_oz2_gemm(h, g));
+  EMU_TRY(mark(h, 2));
   EMU_TRY(launch_oz2_crt(h, c));
   EMU_TRY(mark(h, 3));
   return EMUGEMM_OK;
@@ -421,6 +435,12 @@ int emugemm_set_stream(emugemm_handle_t h, void *s) {
 int emugemm_set_slice_bits(emugemm_handle_t h, int bits) {
   if (!h || (bits != 7 && bits != 8)) return EMUGEMM_ERR_ARG;
   h->slice_bits = bits;
+  return EMUGEMM_OK;
+}
+
+int emugemm_set_oz2_fusion(emugemm_handle_t h, int on) {
+  if (!h || (on & ~1)) return EMUGEMM_ERR_ARG;
+  h->oz2_fusion = on;
   return EMUGEMM_OK;
 }
 

@@ -44,6 +44,8 @@ struct emugemm_ctx {
   int launches = 0;
   int dbg_flags = 0;
   int slice_bits = 7;  // Scheme I digits: 7 = sign-magnitude (R1, default), 8 = balanced base 256 (R23)
+  int oz2_fusion = 0;  // Scheme II real DGEMM: 1 = fused reconstruction when it applies (emugemm_set_oz2_fusion), 0 = separate CRT kernel
+                       // (default: measured 8192^3 N = 16: 8.9 ms fused against 5.3 + 0.6 ms)
   unsigned long long *diag = nullptr;  // device: [0] = GEMM-kernel SM cycles of the last call (inside the workspace)
   unsigned long long *nf_flag = nullptr;  // device word the pre-pass ORs 1 into when an operand holds Inf / NaN (null: off)
   PFN_cuTensorMapEncodeTiled_v12000 encode = nullptr;
@@ -126,6 +128,7 @@ int launch_oz1_gemm(emugemm_ctx *ctx, const Oz1GemmArgs &a);
 int launch_oz1_chunk_reduce(emugemm_ctx *ctx, int64_t m, int64_t n, int n_chunks, const double *part,
                             int out_kind, double alpha, double beta, void *C, int64_t ldc);
 
+struct Oz2CrtArgs;
 struct Oz2GemmArgs {
   int64_t m, n, kpad;
   int n_moduli;
@@ -135,6 +138,10 @@ struct Oz2GemmArgs {
   unsigned long long *cycles;  // as in Oz1GemmArgs
   unsigned long long *wave_ctr = nullptr;  // as in Oz1GemmArgs
   int batch = 1;               // strided batched call: residue planes hold batch * m (n) rows entry-major, CR is [N][batch][m][n]
+  // Fused reconstruction (real product only): non-null = the kernel runs the CRT itself and writes C;
+  // CR is then a scratch of scratch_bytes >= (CTAs launched) * N * 32 KB instead of the [N][m][n] planes.
+  const Oz2CrtArgs *fused = nullptr;
+  size_t scratch_bytes = 0;
 };
 int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &a);
 

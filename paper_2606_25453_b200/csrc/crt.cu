@@ -59,7 +59,7 @@ static long long inv_mod(long long a, long long m) {  // a^-1 mod m (gcd(a, m) =
 }
 
 // Pair moduli, digit width, digit count and all constants for n_moduli = N.  Returns false for an unsupported N.
-static bool crt_constants(int N, CrtConst &c) {
+bool crt_constants_host(int N, CrtConst &c) {
   if (N < 1 || N > kMaxModuli) return false;
   int mod[24];
   oz2_moduli_host(N, mod);
@@ -124,7 +124,7 @@ static bool crt_constants(int N, CrtConst &c) {
 // Python big integers.  digits: [(NP + 1)][J] int64, row q < NP = W_q, row NP = P; pair: [NP][5] = M_q, K1, K2, C0, magic.
 int crt_constants_dump(int N, int *NP, int *J, int *g, long long *digits, unsigned *pair) {
   CrtConst c;
-  if (!crt_constants(N, c)) return -1;
+  if (!crt_constants_host(N, c)) return -1;
   *NP = c.NP; *J = c.J; *g = c.g;
   for (int q = 0; q <= c.NP; ++q)
     for (int j = 0; j < c.J; ++j) {
@@ -298,7 +298,7 @@ static void crt_launch_np(dim3 grid, cudaStream_t st, bool vec, int kind, const 
 int launch_oz2_crt(emugemm_ctx *ctx, const Oz2CrtArgs &a) {
   if (a.m == 0 || a.n == 0) return EMUGEMM_OK;
   CrtConst k;
-  if (!crt_constants(a.n_moduli, k)) return EMUGEMM_ERR_ARG;
+  if (!crt_constants_host(a.n_moduli, k)) return EMUGEMM_ERR_ARG;
   const int kind = a.is_complex ? (a.out_f32 ? 3 : 1) : (a.out_f32 ? 2 : 0);
   const int64_t work = a.m * ((a.n + kCrtVec - 1) / kCrtVec);
   const unsigned gx = static_cast<unsigned>((work + 255) / 256);

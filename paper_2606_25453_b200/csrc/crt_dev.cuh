@@ -45,6 +45,9 @@ struct CrtConst {
   int NP, N, J, g;
 };
 
+// host (crt.cu): pair moduli, digit width, digit count and all constants for n_moduli = N; false for an unsupported N
+bool crt_constants_host(int N, CrtConst &c);
+
 // d = a.lo16 * (signed byte 0 of b) + a.hi16 * (signed byte 1 of b) + c   (a: unsigned halves)
 __device__ __forceinline__ int dp2a_lo_u16_s8(unsigned a, unsigned b, int c) {
   int d;

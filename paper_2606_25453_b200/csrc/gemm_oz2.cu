@@ -17,9 +17,16 @@
 // TMA ring; TMEM holds two 256-column INT32 accumulators per CTA so the
 // mod-epilogue of one item overlaps the MMAs of the next (the paper reuses one
 // accumulator and overlaps only with TMA prefetch).
+//
+// Fused variant (template parameter FNP > 0, real DGEMM only): a work item is an OUTPUT tile
+// and the moduli are the inner loop; the residues of the pair's tile go to a private scratch of 2 x N x 32 KB per CTA
+// (two buffers, alternating by tile; the [N][m][n] planes are never written), and the epilogue warps run the exact FP64
+// CRT of crt_dev.cuh on their own rows of the PREVIOUS tile, 8 columns after every modulus epilogue of the current one,
+// and write C: the reconstruction hides under the tensor-core work of the next tile.  DESIGN.md 5.7 has the measurements.
 #include "common.cuh"
 #include "ptx.cuh"
 #include "gemm_common.cuh"
+#include "crt_dev.cuh"
 
 namespace emu {
 
@@ -85,9 +92,26 @@ __device__ __forceinline__ void store32(int8_t *dst, const unsigned (&w)[8], int
   }
 }
 
-template <int NPROD>  // 1: real (Eq. 6-7); 3: 3M (Eq. 16-18)
+// reconstruction arguments of the fused variant (unused when FNP == 0)
+struct Oz2Fuse {
+  CrtConst k;
+  const int32_t *eA, *eB;
+  int tsum;            // tA + tB
+  double alpha, beta;
+  double *C;
+  int64_t ldc;
+  int64_t batch_stride_c;  // elements between the C matrices of consecutive batch entries
+};
+constexpr int kOz2ScratchPlane = kTileM * kOz2NT;  // 32 KB: one modulus of one CTA's 128 x 256 half tile
+
+// NPROD: 1 real (Eq. 6-7), 3: 3M (Eq. 16-18).  FNP: 0 = residue planes to global memory (CRT in crt.cu); > 0 = fused
+// reconstruction with FNP = ceil(N / 2) modulus pairs (NPROD == 1 only).
+template <int NPROD, int FNP>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(kGemmThreads, 1)
-oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const Oz2Dev a) {
+oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__ CUtensorMap tmB, const Oz2Dev a,
+                const __grid_constant__ Oz2Fuse f) {
+  constexpr bool FUSED = FNP > 0;
+  static_assert(!FUSED || NPROD == 1, "the fused reconstruction covers the real product");
   extern __shared__ uint8_t smem_raw[];
   uint8_t *smem = reinterpret_cast<uint8_t *>((reinterpret_cast<uintptr_t>(smem_raw) + 1023) & ~uintptr_t(1023));
   uint64_t *bars = reinterpret_cast<uint64_t *>(smem + kOz2Stages * kOz2StageBytes);
@@ -98,8 +122,11 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
   const uint32_t cta = cluster_ctarank();  // 0 = leader (issues the MMAs), 1 = peer
   const int cluster_id = blockIdx.x >> 1, num_clusters = gridDim.x >> 1;
   const int tiles_per_mod = a.mt * a.nt_tiles;  // a.mt counts PAIR tiles of 256 rows
-  const int tiles_per_entry = tiles_per_mod * a.n_moduli;
-  const int num_tiles = tiles_per_entry * a.nbatch;  // entry-major: tile = (batch entry, modulus, tile of the modulus)
+  // unfused: tile = (batch entry, modulus, tile of the modulus), NPROD products each; fused: tile = (batch entry, output tile),
+  // the N moduli are the inner loop
+  const int tiles_per_entry = FUSED ? tiles_per_mod : tiles_per_mod * a.n_moduli;
+  const int num_tiles = tiles_per_entry * a.nbatch;
+  const int n_inner = FUSED ? a.n_moduli : NPROD;
 
   if (threadIdx.x == 0) {
     // full[s] (leader's is the one used): 1 arrival (leader's expect_tx) + the bytes of BOTH CTAs' loads;
@@ -131,7 +158,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         // for the same k-block of the same product at the same time, and it comes from DRAM once
         if (a.wave_ctr && wave > 0) grid_wait(a.wave_ctr, static_cast<unsigned long long>(wave) * gridDim.x);
         const int bidx = tile / tiles_per_entry, te = tile - bidx * tiles_per_entry;
-        const int l = te / tiles_per_mod;
+        const int l = FUSED ? 0 : te / tiles_per_mod;
         int mb, nb;
         tile_coords(te - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb, a.group_m);
         const int arow = static_cast<int>(bidx * a.m) + mb * kOz2PairM + static_cast<int>(cta) * kTileM;
@@ -140,8 +167,8 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         // neighbourhood touched last are the first ones asked for again
         const bool rev = a.serp && (((tile - cluster_id) / num_clusters) & 1);
         const int nstage = (a.kblocks + kOz2KPerStage - 1) / kOz2KPerStage;
-        for (int q = 0; q < NPROD; ++q) {
-          const int plane = q * a.n_moduli + l;
+        for (int q = 0; q < n_inner; ++q) {
+          const int plane = FUSED ? q : q * a.n_moduli + l;
           for (int sidx = 0; sidx < nstage; ++sidx) {
             const int kb = (rev ? nstage - 1 - sidx : sidx) * kOz2KPerStage;
             const int nkb = (a.kblocks - kb < kOz2KPerStage) ? a.kblocks - kb : kOz2KPerStage;
@@ -173,7 +200,7 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       const int nstage = (a.kblocks + kOz2KPerStage - 1) / kOz2KPerStage;
       for (int tile = cluster_id; tile < num_tiles; tile += num_clusters) {
         const bool rev = a.serp && (((tile - cluster_id) / num_clusters) & 1);  // the producer's k direction for this tile
-        for (int q = 0; q < NPROD; ++q, ++item) {
+        for (int q = 0; q < n_inner; ++q, ++item) {
           const uint32_t slot = item & 1, tph = (item >> 1) & 1;
           mbar_wait(&tempty[slot], tph ^ 1);
           tc_fence_after();
@@ -212,17 +239,74 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     uint32_t item = 0;
     unsigned t1[NPROD == 3 ? 32 : 1], t2[NPROD == 3 ? 32 : 1];  // T1, T2 of this thread's 128 columns as packed INT8 (3M)
     const uint32_t tempty_leader[2] = {mapa_u32(&tempty[0], 0), mapa_u32(&tempty[1], 0)};
-    for (int tile = cluster_id; tile < num_tiles; tile += num_clusters) {
+    // fused: the reconstruction of the PREVIOUS tile (its residues sit in the other scratch buffer) is spread over the N
+    // modulus epilogues of the current tile, 8 columns per step, so that it never delays the release of an accumulator
+    // by more than one step (a whole-tile burst of ~200k clk after the last modulus stalled the tensor pipe: 5.9 -> 7.9 ms)
+    struct PrevTile { int8_t *scratch; int64_t grow, gcol0; int bidx; bool row_ok; } prev = {nullptr, 0, 0, 0, false};
+    int crt_done = 16;  // 8-column steps of the previous tile already reconstructed (16 = nothing pending)
+    int tile_ord = 0;
+    auto crt_step = [&](const int ch) {
+      if constexpr (FUSED) {
+        constexpr int J = (FNP + 1) / 2;
+        const int64_t gcol = prev.gcol0 + ch * 8;
+        if (!prev.row_ok || gcol >= a.n || EMU_PROBE_FLAG(a.dbg, 0x80000)) return;
+        uint2 w[2 * FNP];
+#pragma unroll
+        for (int l = 0; l < 2 * FNP; ++l) {
+          w[l] = make_uint2(0u, 0u);
+          if ((l < 2 * FNP - 1 || l < a.n_moduli) && !EMU_PROBE_FLAG(a.dbg, 0x100000))
+            w[l] = *reinterpret_cast<const uint2 *>(prev.scratch + static_cast<int64_t>(l) * kOz2ScratchPlane + ch * 8);
+        }
+        const int eAi = __ldg(f.eA + prev.bidx * a.m + prev.grow) - f.tsum - kCrtSC;
+        const int32_t *eBp = f.eB + prev.bidx * a.n;
+        double *crow = f.C + prev.bidx * f.batch_stride_c + prev.grow * f.ldc;
+        const bool vec_c = (f.ldc % 4 == 0) && ((reinterpret_cast<uintptr_t>(f.C) & 31) == 0) && ((f.batch_stride_c & 3) == 0);
+#pragma unroll
+        for (int g = 0; g < 2; ++g) {
+          double acc[4][J], v[4];
+#pragma unroll
+          for (int pq = 0; pq < FNP; ++pq)
+            crt_accumulate_pair<J>(f.k, pq, g == 0 ? w[2 * pq].x : w[2 * pq].y, g == 0 ? w[2 * pq + 1].x : w[2 * pq + 1].y, acc, pq == 0);
+          const int64_t c0 = gcol + 4 * g;
+#pragma unroll
+          for (int e = 0; e < 4; ++e) {
+            const int eb = (c0 + e < a.n) ? __ldg(eBp + c0 + e) : 0;
+            v[e] = crt_scale_pow2(crt_finish<J>(f.k, acc[e]), eAi + eb);
+          }
+          double *o = crow + c0;
+          if (f.beta != 0.0) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+              if (c0 + e < a.n) v[e] = fma(f.alpha, v[e], f.beta * o[e]);
+          } else if (f.alpha != 1.0) {
+#pragma unroll
+            for (int e = 0; e < 4; ++e) v[e] *= f.alpha;
+          }
+          if (vec_c && c0 + 4 <= a.n) {
+            asm volatile("st.global.v4.f64 [%0], {%1,%2,%3,%4};" ::"l"(o), "d"(v[0]), "d"(v[1]), "d"(v[2]), "d"(v[3]) : "memory");
+          } else {
+#pragma unroll
+            for (int e = 0; e < 4; ++e)
+              if (c0 + e < a.n) o[e] = v[e];
+          }
+        }
+      }
+    };
+    for (int tile = cluster_id; tile < num_tiles; tile += num_clusters, ++tile_ord) {
       const int bidx = tile / tiles_per_entry, te = tile - bidx * tiles_per_entry;
-      const int l = te / tiles_per_mod;
+      const int l0 = FUSED ? 0 : te / tiles_per_mod;
       int mb, nb;
-      tile_coords(te - l * tiles_per_mod, a.mt, a.nt_tiles, mb, nb, a.group_m);
-      ModK mk;
-      mk.cvec = a.cvec[l]; mk.c0 = a.c0[l]; mk.magic = a.magic[l]; mk.m = static_cast<unsigned>(a.mod[l]); mk.half = (mk.m + 1) / 2;
+      tile_coords(te - l0 * tiles_per_mod, a.mt, a.nt_tiles, mb, nb, a.group_m);
       const int64_t grow = static_cast<int64_t>(mb) * kOz2PairM + cta * kTileM + row;
       const bool row_ok = grow < a.m;
-#pragma unroll
-      for (int q = 0; q < NPROD; ++q, ++item) {
+      // fused: this thread's 128 residues of modulus q go to [q][row][half * 128 ...] of the CTA's scratch buffer (tile_ord & 1)
+      int8_t *scratch = FUSED ? a.CR + ((static_cast<int64_t>(blockIdx.x) * 2 + (tile_ord & 1)) * a.n_moduli) * kOz2ScratchPlane +
+                                    row * kOz2NT + half * 128
+                              : nullptr;
+      auto drain = [&](const int q) {  // the epilogue of one accumulator: product q (unfused) or modulus q (fused)
+        const int l = FUSED ? q : l0;
+        ModK mk;
+        mk.cvec = a.cvec[l]; mk.c0 = a.c0[l]; mk.magic = a.magic[l]; mk.m = static_cast<unsigned>(a.mod[l]); mk.half = (mk.m + 1) / 2;
         const uint32_t slot = item & 1, tph = (item >> 1) & 1;
         mbar_wait(&tfull[slot], tph);
         tc_fence_after();
@@ -244,8 +328,13 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
               for (int g = 0; g < 8; ++g)
                 w[g] = pack4i(sym_mod_i32(v[4 * g], mk), sym_mod_i32(v[4 * g + 1], mk), sym_mod_i32(v[4 * g + 2], mk),
                               sym_mod_i32(v[4 * g + 3], mk));
-              if (row_ok && gcol < a.n && !EMU_PROBE_FLAG(a.dbg, 4))
+              if constexpr (FUSED) {
+                uint4 *dst = reinterpret_cast<uint4 *>(scratch + static_cast<int64_t>(q) * kOz2ScratchPlane + ch * 32);
+                dst[0] = make_uint4(w[0], w[1], w[2], w[3]);
+                dst[1] = make_uint4(w[4], w[5], w[6], w[7]);
+              } else if (row_ok && gcol < a.n && !EMU_PROBE_FLAG(a.dbg, 4)) {
                 store32(a.CR + ((static_cast<int64_t>(l) * a.nbatch + bidx) * a.m + grow) * a.n + gcol, w, gcol, a.n, vec_ok);
+              }
             } else if (q < 2) {
               // T1 / T2 stay on chip as unsigned residues in [0, m), four per register
 #pragma unroll
@@ -285,7 +374,27 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         tc_fence_before();
         __syncwarp();
         if (lane == 0) mbar_arrive_remote(tempty_leader[slot]);  // the leader's MMA thread waits for both CTAs
+        ++item;
+        if constexpr (FUSED) {  // the previous tile's share of reconstruction steps for this modulus
+          while (crt_done < 16 && crt_done * a.n_moduli < 16 * (q + 1)) crt_step(crt_done++);
+        }
+      };
+      if constexpr (FUSED) {
+#pragma unroll 1
+        for (int q = 0; q < n_inner; ++q) drain(q);
+      } else {
+#pragma unroll
+        for (int q = 0; q < NPROD; ++q) drain(q);
       }
+      if constexpr (FUSED) {
+        while (crt_done < 16) crt_step(crt_done++);  // (only if N > 16 steps could not be placed: never for N <= 20)
+        prev.scratch = scratch; prev.grow = grow; prev.gcol0 = static_cast<int64_t>(nb) * kOz2NT + half * 128; prev.bidx = bidx;
+        prev.row_ok = row_ok;
+        crt_done = 0;
+      }
+    }
+    if constexpr (FUSED) {
+      while (crt_done < 16) crt_step(crt_done++);  // the last tile of this CTA
     }
   }
 
@@ -326,18 +435,42 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
     d.c0[l] = (m - two31) % m;
     d.magic[l] = static_cast<unsigned>(((1ull << 32) + m - 1ull) / m);
   }
-  const int64_t tiles = static_cast<int64_t>(d.mt) * d.nt_tiles * d.n_moduli * batch;
+  const bool fused = g.fused != nullptr;
+  if (fused && g.is3m) return EMUGEMM_ERR_ARG;
+  // work items of the persistent loop: (entry, modulus, tile) or, fused, (entry, output tile) with the moduli inside
+  const int64_t tiles = static_cast<int64_t>(d.mt) * d.nt_tiles * (fused ? 1 : d.n_moduli) * batch;
   if (tiles >= (1LL << 31)) return EMUGEMM_ERR_ARG;
   const int pairs = ctx->num_sms / 2;
   const int grid = 2 * (tiles < pairs ? static_cast<int>(tiles) : pairs);
-  auto kern = g.is3m ? oz2_gemm_kernel<3> : oz2_gemm_kernel<1>;
+  Oz2Fuse fz = {};
+  void (*kern)(CUtensorMap, CUtensorMap, Oz2Dev, Oz2Fuse) = g.is3m ? oz2_gemm_kernel<3, 0> : oz2_gemm_kernel<1, 0>;
+  if (fused) {
+    const Oz2CrtArgs &c = *g.fused;
+    if (!crt_constants_host(g.n_moduli, fz.k) || fz.k.J != (fz.k.NP + 1) / 2) return EMUGEMM_ERR_ARG;
+    fz.eA = c.eA; fz.eB = c.eB; fz.tsum = c.tA + c.tB; fz.alpha = c.alpha[0]; fz.beta = c.beta[0];
+    fz.C = c.C; fz.ldc = c.ldc; fz.batch_stride_c = c.batch_stride_c;
+    switch (fz.k.NP) {  // the BASELINE range N = 12 ... 20 and the FP32-level N = 8 ... 11
+      case 4: kern = oz2_gemm_kernel<1, 4>; break;
+      case 5: kern = oz2_gemm_kernel<1, 5>; break;
+      case 6: kern = oz2_gemm_kernel<1, 6>; break;
+      case 7: kern = oz2_gemm_kernel<1, 7>; break;
+      case 8: kern = oz2_gemm_kernel<1, 8>; break;
+      case 9: kern = oz2_gemm_kernel<1, 9>; break;
+      case 10: kern = oz2_gemm_kernel<1, 10>; break;
+      default: return EMUGEMM_ERR_ARG;
+    }
+    if (static_cast<size_t>(grid) * 2 * g.n_moduli * kOz2ScratchPlane > g.scratch_bytes) return EMUGEMM_ERR_WORKSPACE;  // two buffers per CTA
+  }
   EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kOz2Smem));
   // Wave barrier (gemm_oz1.cu): only when all CTAs are certainly co-resident, there are at least two waves and a tile is
-  // long enough (>= 16 k-blocks per product) to hide the re-alignment
+  // long enough (>= 16 k-blocks per product) to hide the re-alignment.  3M: on (measured); real: off (its DRAM
+  // traffic already sits at the no-drift figure); fused: on (a tile is N products long)
   d.wave_ctr = nullptr;
   d.n_waves = 0;
-  const bool want_sync = g.is3m ? !EMU_PROBE_FLAG(ctx->dbg_flags, 0x10000) : EMU_PROBE_FLAG(ctx->dbg_flags, 0x20000) != 0;
-  if (g.wave_ctr && want_sync && tiles > grid / 2 && d.kblocks >= 16) {
+  // measured (profiles/r2_wave_barrier.md): 3M 8192^3 N = 18 +8 %, N = 14 +15-20 % (DRAM reads 49 -> 31 GB, SM clock 1.2 ->
+  // 1.36-1.49 GHz), 4096^3 neutral, real product -8 % (an item is one modulus, 23 us: the re-alignment is not hidden)
+  const bool want_sync = (g.is3m || fused) ? !EMU_PROBE_FLAG(ctx->dbg_flags, 0x10000) : EMU_PROBE_FLAG(ctx->dbg_flags, 0x20000) != 0;
+  if (g.wave_ctr && want_sync && tiles > grid / 2 && d.kblocks >= (fused ? 16 : 64)) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(grid));
     cfg.blockDim = dim3(kGemmThreads);
@@ -353,7 +486,7 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
       d.n_waves = static_cast<int>((tiles + grid / 2 - 1) / (grid / 2));
     }
   }
-  kern<<<grid, kGemmThreads, kOz2Smem, ctx->stream>>>(tmA, tmB, d);
+  kern<<<grid, kGemmThreads, kOz2Smem, ctx->stream>>>(tmA, tmB, d, fz);
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
   return EMUGEMM_OK;

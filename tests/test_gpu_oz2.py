@@ -289,3 +289,43 @@ def test_dgemm_oz2_extreme_exponents(env):
             assert_within_ulps(got[~tiny], want[~tiny], scale[~tiny], 2, what=f"scales {sa} {sb}")
         # results in the subnormal range: absolute error of two subnormal spacings
         assert (np.abs(got[tiny] - want[tiny]) <= 2 * 2.0 ** -1074).all()
+
+
+# ---- fused reconstruction: the CRT runs inside the per-modulus GEMM kernel ----
+@pytest.mark.parametrize("N,shape", [(12, (256, 256, 256)), (14, (520, 300, 333)), (16, (512, 1024, 384)), (18, (600, 530, 260)),
+                                     (20, (300, 770, 200)), (8, (512, 512, 256)), (15, (770, 512, 140))])
+def test_dgemm_oz2_fused_matches_oracle_and_unfused(env, N, shape):
+    torch, O, h, E = env
+    m, n, k = shape
+    A, B, Cin = G.real_pair(m, n, k, 1.0, 40 + N, with_c=True)
+    Ad, Bd = dev(torch, A), dev(torch, B)
+    out = {}
+    for fused in (True, False):
+        h.set_oz2_fusion(fused)
+        C = torch.full((m, n), float("nan"), dtype=torch.float64, device="cuda")
+        h.dgemm_oz2(Ad, Bd, C, N)
+        C2 = dev(torch, Cin)
+        h.dgemm_oz2(Ad, Bd, C2, N, alpha=-1.5, beta=0.25)
+        out[fused] = (C, C2)
+    h.set_oz2_fusion(False)
+    assert torch.equal(out[True][0], out[False][0]) and torch.equal(out[True][1], out[False][1])  # same arithmetic, same bits
+    _, absAB = O.bf128_dgemm(A, B)
+    assert_within_ulps(out[True][0].cpu().numpy(), O.dgemm_oz2(A, B, N), absAB, 2, what=f"fused oz2 N={N}")
+    assert_within_ulps(out[True][1].cpu().numpy(), O.dgemm_oz2(A, B, N, alpha=-1.5, beta=0.25, Cin=Cin), 1.5 * absAB + 0.25 * np.abs(Cin), 2,
+                       what=f"fused oz2 alpha/beta N={N}")
+
+
+def test_dgemm_oz2_fused_adversarial_and_strided(env):
+    """the fused path on the inputs that broke the round-1 CRT, with a C that has a leading-dimension slack"""
+    torch, O, h, E = env
+    m, n, k, N = 512, 512, 300, 16
+    A, B = _adversarial_pairs(m, n, k)["unit_over_noise"]
+    Cd = torch.full((m, n + 5), 7.0, dtype=torch.float64, device="cuda")
+    h.set_oz2_fusion(True)
+    try:
+        h.dgemm_oz2(dev(torch, A), dev(torch, B), Cd[:, :n], N)
+    finally:
+        h.set_oz2_fusion(False)
+    _, absAB = O.bf128_dgemm(A, B)
+    assert_within_ulps(Cd[:, :n].cpu().numpy(), O.dgemm_oz2(A, B, N), absAB, 2, what="fused adversarial")
+    assert (Cd[:, n:] == 7.0).all()
