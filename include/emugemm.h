@@ -45,7 +45,7 @@ enum emugemm_status {
   EMUGEMM_ERR_ARG = -1,       /* null pointer, negative size, ld too small, p / n_moduli out of range */
   EMUGEMM_ERR_ALIGNMENT = -2, /* A, B, C not 16-byte aligned or workspace not 1024-byte aligned */
   EMUGEMM_ERR_WORKSPACE = -3, /* workspace missing or smaller than emugemm_workspace_bytes() */
-  EMUGEMM_ERR_PRECISION = -4, /* Scheme II: k too large for this n_moduli (bit budget T < 2) */
+  EMUGEMM_ERR_PRECISION = -4, /* Scheme II: k too large for this n_moduli (bit budget T < 2), or k > 131,071 (see Scheme II) */
   EMUGEMM_ERR_DEVICE = -5,    /* no CUDA device or not compute capability 10.x */
   EMUGEMM_ERR_CUDA = -6       /* a CUDA call failed; see emugemm_last_cuda_error() */
 };
@@ -68,8 +68,10 @@ int emugemm_set_slice_bits(emugemm_handle_t h, int bits);
  * INSIDE the per-modulus GEMM kernel -- a work item is an output tile, the moduli are the inner loop, the tile's
  * residues wait in a per-CTA scratch of 2 x N x 32 KB (the [N][m][n] residue planes are never written), and the epilogue
  * warps run the exact FP64 CRT of the previous tile between the modulus epilogues of the current one.  Applies when
- * 7 <= n_moduli and the problem has at least two waves of 256 x 256 tiles (the scratch must fit where the residue planes
- * would have been); otherwise, and with on = 0, the separate CRT kernel runs.  Both paths give bit-identical C.
+ * 7 <= n_moduli and the scratch (CTAs launched x 2 x N x 32 KB, at most 148 x 2 x N x 32 KB) fits in the workspace from
+ * where the residue planes would have started: always for problems of at least two waves of 256 x 256 tiles, else when
+ * the workspace has that much room beyond emugemm_workspace_bytes(); otherwise, and with on = 0, the separate CRT kernel
+ * runs.  Both paths give bit-identical C.
  * DEFAULT: off -- measured on B200 the fused form is slower (8192^3, N = 16: 8.9 ms against 5.3 + 0.6 ms; the eight
  * epilogue warps cannot hide the FP64 reconstruction and the scratch competes with the operand panels for L2,
  * DESIGN.md 5.7): it is kept as the measured answer to "can Scheme II be fully fused on this machine".           */
@@ -139,7 +141,12 @@ int emugemm_cgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, co
  * n_moduli pairwise-coprime moduli <= 256 (256, 255, 253, 251, 247, ... greedy
  * descending); symmetric INT8 residues; one INT8 GEMM per modulus with the
  * mod-reduction fused into its epilogue (Eq. 6-7); CRT (Eq. 8) and inverse
- * scaling in FP64.  Range: 2 <= n_moduli <= 20.                               */
+ * scaling in FP64.  Range: 2 <= n_moduli <= 20.
+ * k <= 131,071: one INT32-safe accumulation range (k 128^2 < 2^31; R7).  Larger k is UNSUPPORTED in Scheme II
+ * (EMUGEMM_ERR_PRECISION): the residues of k-chunks could be added modulo m_l, but no BASELINE configuration needs it
+ * and it is not built; Scheme I chunks k itself.
+ * The FP64 CRT is exact: for every residue vector the reconstructed integer is rounded once (R17), so the
+ * 2-ulp bound of (|A||B|)_ij holds for every finite input, not only for well-scaled ones.                       */
 int emugemm_dgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha,
                       const double *A, int64_t lda, const double *B, int64_t ldb, double beta,
                       double *C, int64_t ldc, int n_moduli);

@@ -133,6 +133,7 @@ class EmuGemm:
     def set_oz2_fusion(self, on):
         """Scheme II real DGEMM: fused reconstruction inside the GEMM kernel, or (default) the separate CRT kernel."""
         self._check(self._lib.emugemm_set_oz2_fusion(self._h, _int(1 if on else 0)))
+        self._fusion = bool(on)
 
     def workspace_bytes(self, scheme, elem, m, n, k, pn):
         return int(self._lib.emugemm_workspace_bytes(scheme, elem, m, n, k, pn))
@@ -154,6 +155,8 @@ class EmuGemm:
 
     def _reserve_for(self, scheme, elem, m, n, k, pn):
         need = self.workspace_bytes(scheme, elem, m, n, k, pn)
+        if scheme == OZ2 and getattr(self, "_fusion", False):
+            need += 160 * 2 * pn * 32768  # room for the per-CTA scratch of the fused reconstruction (include/emugemm.h)
         if self._ws is None or self._ws.numel() - 1024 < need:
             self.reserve(need)
 

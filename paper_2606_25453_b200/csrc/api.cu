@@ -269,15 +269,17 @@ static int oz2_gemm_phase(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_
   c.m = m; c.n = n; c.n_moduli = N; c.CR = CR; c.eA = eA; c.eB = eB; c.tA = tA; c.tB = tB; c.is_complex = is3m; c.out_f32 = out_f32;
   c.alpha[0] = alpha[0]; c.alpha[1] = alpha[1]; c.beta[0] = beta[0]; c.beta[1] = beta[1];
   c.C = C; c.ldc = ldc; c.batch = batch; c.batch_stride_c = batch_stride_c;
-  // Fused reconstruction: real FP64 product, 7 <= N <= 20, and the per-CTA scratch (2 x N x 32 KB for
-  // each of the <= num_sms CTAs) must fit in the region the residue planes would have taken -- true for every problem of
-  // at least two waves of 256 x 256 tiles; smaller ones keep the separate CRT kernel.
+  // Fused reconstruction (opt-in): real FP64 product, 7 <= N <= 20, and the per-CTA scratch (2 x N x
+  // 32 KB for each of the <= num_sms CTAs) must fit in the workspace from where the residue planes would have started --
+  // true for every problem of at least two waves of 256 x 256 tiles, or when the caller's workspace has that much room
+  // beyond emugemm_workspace_bytes(); otherwise the separate CRT kernel runs.
   const int64_t tiles_out = ((m + 255) / 256) * ((n + 255) / 256) * batch;
   const int64_t ctas = 2 * (tiles_out < h->num_sms / 2 ? tiles_out : h->num_sms / 2);
-  const size_t cr_bytes = static_cast<size_t>(N) * m * n * batch;
-  if (h->oz2_fusion && !is3m && !out_f32 && N >= 7 && static_cast<size_t>(ctas) * 2 * N * 32768 <= cr_bytes) {
+  // CR is the last region carved from the workspace by every caller: the scratch may use everything from there on
+  const size_t avail = static_cast<size_t>((static_cast<const uint8_t *>(h->ws) + h->ws_bytes) - reinterpret_cast<const uint8_t *>(CR));
+  if (h->oz2_fusion && !is3m && !out_f32 && N >= 7 && static_cast<size_t>(ctas) * 2 * N * 32768 <= avail) {
     g.fused = &c;
-    g.scratch_bytes = cr_bytes;
+    g.scratch_bytes = avail;
     EMU_TRY(launch_oz2_gemm(h, g));
     EMU_TRY(mark(h, 2));
     EMU_TRY(mark(h, 3));

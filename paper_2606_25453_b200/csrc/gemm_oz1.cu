@@ -401,9 +401,16 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         // at the top of its own k-block, so that its 56-64 KB are not in the way of the next k-block's first A stages
         // (p = 7: 0.884 -> 0.913 per clock, p = 8: 0.941 -> 0.946; with three stages per k-block the two places coincide)
         constexpr bool early_b = !PAIR && Cfg::NPAIR >= 4;
+        // the arrival on the wave barrier is signalled kWaveLead k-blocks before the last load of the tile: the slowest CTA
+        // then releases the others while it still has that much of its tile to go, so the fast ones do not idle at the
+        // barrier, and the drift stays within a few k-blocks (the panels of that window are a few MB of L2)
+        constexpr int kWaveLead = 6;
+        const int lead = EMU_PROBE_FLAG(a.dbg, 0x0F000000) ? 2 * ((EMU_PROBE_FLAG(a.dbg, 0x0F000000) >> 24) - 1) : kWaveLead;  // probe: 0, 2, ... 28
+        const int arrive_it = nkb - 1 - lead > 0 ? nkb - 1 - lead : 0;
         for (int it = 0; it < nkb; ++it) {
           const int kb = rev ? kb1 - 1 - it : kb0 + it;
           const int kb_next = rev ? kb - 1 : kb + 1;
+          if (a.wave_ctr && it == arrive_it) grid_arrive(a.wave_ctr);
           if (!early_b || it == 0) load_b(kb);
 #pragma unroll 1
           for (int j = 0; j < Cfg::NPAIR; ++j) {
@@ -435,7 +442,6 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             if (early_b && j == 2 && it + 1 < nkb) load_b(kb_next);
           }
         }
-        if (a.wave_ctr) grid_arrive(a.wave_ctr);  // all loads of this tile are issued
       }
       if (a.wave_ctr)
         for (; wave < a.n_waves; ++wave) grid_arrive(a.wave_ctr);  // no tile in the last wave(s): the others must not wait for us

@@ -303,7 +303,11 @@ def test_dgemm_oz2_fused_matches_oracle_and_unfused(env, N, shape):
     for fused in (True, False):
         h.set_oz2_fusion(fused)
         C = torch.full((m, n), float("nan"), dtype=torch.float64, device="cuda")
+        h.enable_stage_timing(True)
         h.dgemm_oz2(Ad, Bd, C, N)
+        _, launches = h.stage_ms()
+        h.enable_stage_timing(False)
+        assert launches == (4 if fused else 5), "the fused path must not launch a separate CRT kernel"
         C2 = dev(torch, Cin)
         h.dgemm_oz2(Ad, Bd, C2, N, alpha=-1.5, beta=0.25)
         out[fused] = (C, C2)
