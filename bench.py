@@ -47,6 +47,8 @@ def parse():
     ap.add_argument("--probe-flags", type=lambda x: int(x, 0), default=0,
                     help="A/B experiments only (results may be WRONG): run the PROBES build of the library with these "
                          "emugemm_dbg_set_flags bits (include/emugemm.h), e.g. 0x10000 = no wave barrier")
+    ap.add_argument("--oracle-table", action="store_true",
+                    help="with --impl reference: time the oracle IN FULL on 1024^3 instances of every config family (BASELINE.md 3)")
     ap.add_argument("--fusion", action="store_true", help="Scheme II: fused reconstruction inside the GEMM kernel (default: separate CRT kernel)")
     return ap.parse_args()
 
@@ -195,6 +197,39 @@ def oracle_context(a, w):
     return out
 
 
+def oracle_table():
+    """BASELINE.md 3 / SURVEY 8(d): the oracle in full on config 1 and on 1024^3 instances of configs 2-5 (p / N unchanged),
+    all host threads, plus one thread on 512^3; seconds, emulated GFLOP/s, integer MAC/s.  One JSON line."""
+    import numpy as np
+    import emugemm_inputs as G
+    from oracle import oracle as O
+    nthreads = O.threads()
+    rows = []
+
+    def timed(name, fn, flops, macs):
+        t0 = time.perf_counter(); fn(); dt = time.perf_counter() - t0
+        rows.append({"case": name, "threads": O.threads(), "seconds": round(dt, 3), "emulated_gflops": round(flops / dt / 1e9, 3),
+                     "int_gmac_per_s": round(macs / dt / 1e9, 2)})
+
+    A0, B0 = G.real_pair(256, 256, 256, 0.5, 0)
+    timed("config 1: OZ1 DGEMM 256^3 p=6 (full)", lambda: O.dgemm_oz1(A0, B0, 6), 2.0 * 256 ** 3, 21.0 * 256 ** 3)
+    for s_ in (1024, 512):
+        O.set_threads(nthreads if s_ == 1024 else 1)
+        A, B = G.real_pair(s_, s_, s_, 0.5, 1)
+        for p_ in ((3, 6, 8) if s_ == 1024 else (8,)):
+            timed(f"config 2: OZ1 DGEMM {s_}^3 p={p_}", lambda: O.dgemm_oz1(A, B, p_), 2.0 * s_ ** 3, p_ * (p_ + 1) / 2.0 * s_ ** 3)
+        A, B = G.real_pair(s_, s_, s_, 1.0, 2)
+        for N_ in ((12, 16, 20) if s_ == 1024 else (16,)):
+            timed(f"config 3: OZ2 DGEMM {s_}^3 N={N_}", lambda: O.dgemm_oz2(A, B, N_), 2.0 * s_ ** 3, float(N_) * s_ ** 3)
+        Az, Bz = G.complex_pair(s_, s_, s_, 1.0, 3)
+        for N_ in ((14, 18) if s_ == 1024 else (14,)):
+            timed(f"config 4: OZ2 ZGEMM-3M {s_}^3 N={N_}", lambda: O.zgemm_oz2_3m(Az, Bz, N_), 8.0 * s_ ** 3, 3.0 * N_ * s_ ** 3)
+        Af, Bf = G.real_pair(s_, s_, s_, 1.0, 4, dtype=np.float32)
+        timed(f"config 5: OZ1 SGEMM {s_}^3 p=4", lambda: O.sgemm_oz1(Af, Bf, 4), 2.0 * s_ ** 3, 10.0 * s_ ** 3)
+    O.set_threads(nthreads)
+    print(json.dumps({"impl": "reference", "oracle_table": rows, "cores": nthreads}))
+
+
 def reference_leg(a, w):
     """--impl reference: the oracle on host cores; each step = the same bounded sample of the workload that the main
     arm's `cpu_baseline` uses (calibrated to ~15 s), repeated for `steps` steps or until ~150 s are spent."""
@@ -228,7 +263,10 @@ def main():
 
     if a.impl == "reference":
         if rank == 0:
-            reference_leg(a, w)
+            if a.oracle_table:
+                oracle_table()
+            else:
+                reference_leg(a, w)
         return
 
     import numpy as np

@@ -11,7 +11,7 @@
  *   - Layout: row-major, no transposes.  A is m x k with row stride lda >= k,
  *     B is k x n with ldb >= n, C is m x n with ldc >= n; strides in elements
  *     (complex entry point: in complex elements, storage is (re, im) pairs).
- *   - m, n, k >= 0.  m*n == 0 is a no-op; k == 0 scales C by beta.
+ *   - m, n, k >= 0.  m*n == 0 is a no-op; k == 0 scales C by beta.  m, n < 2^31 - 256, k <= 8,388,480 (65535 * 128).
  *   - All matrix pointers are DEVICE pointers owned by the caller.  A and B are
  *     read-only.  C is read only when beta != 0 (BLAS rule: beta == 0 means C is
  *     not read, NaNs in C do not propagate) and is overwritten.

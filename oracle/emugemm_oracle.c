@@ -717,8 +717,8 @@ int oracle_oz2_crt_limbs(int N, const int32_t *c, uint64_t *mag_limbs) {
 
 /* CRT + inverse scaling: for every (i, j),
  *   X = crt(CR[.][i][j]);  v = X 2^(eA_i + eB_j - tA - tB)  in __float128;
- *   C = round(alpha v + beta_ C_in).   X128 (optional [m][n][2]) receives X as
- *   signed (hi, lo) 64-bit halves of an int128 when |X| < 2^127, for tests. */
+ *   C = round(alpha v + beta_ C_in).   X128 (optional, [m][n][5] uint64) receives X exactly for tests: the sign
+ *   (0, 1 or 2^64 - 1) followed by the four 64-bit limbs of |X| (no truncation: |X| < P/2 < 2^256). */
 void oracle_oz2_crt(int64_t m, int64_t n, int N, const int8_t *CR, const int32_t *eA, const int32_t *eB,
                     int tA, int tB, double alpha, double beta_, double *C, int64_t ldc, int64_t cstride,
                     int64_t *X128) {
@@ -734,10 +734,9 @@ void oracle_oz2_crt(int64_t m, int64_t n, int N, const int8_t *CR, const int32_t
       u256 mag;
       int sg = oz2_crt_one(N, mod, &P, w, c, &mag);
       if (X128) {
-        i128 x = (i128)(((u128)mag.w[1] << 64) | mag.w[0]);
-        if (sg < 0) x = -x;
-        X128[2 * (i * n + j)] = (int64_t)(x >> 64);
-        X128[2 * (i * n + j) + 1] = (int64_t)(uint64_t)x;
+        int64_t *xo = X128 + 5 * (i * n + j);
+        xo[0] = sg;
+        for (int q = 0; q < 4; ++q) xo[1 + q] = (int64_t)mag.w[q];
       }
       __float128 v = scalbnq(u256_to_q(&mag), eA[i] + eB[j] - tA - tB);
       if (sg < 0) v = -v;

@@ -333,11 +333,12 @@ def oz2_crt(CR, eA, eB, tA, tB, alpha=1.0, beta=0.0, Cin=None, want_X=False):
     out = np.zeros((m, n), np.float64) if Cin is None else _f64(Cin).copy()
     eA = np.ascontiguousarray(eA, np.int32)
     eB = np.ascontiguousarray(eB, np.int32)
-    X = np.empty((m, n, 2), np.int64) if want_X else None
+    X = np.empty((m, n, 5), np.int64) if want_X else None
     _lib.oracle_oz2_crt(_i64(m), _i64(n), C.c_int(N), _ptr(CR), _ptr(eA), _ptr(eB), C.c_int(tA), C.c_int(tB),
                         _dbl(alpha), _dbl(beta), _ptr(out), _i64(n), _i64(1), _ptr(X) if want_X else None)
     if want_X:
-        Xi = [[(int(X[i, j, 0]) << 64) + (int(X[i, j, 1]) & ((1 << 64) - 1)) for j in range(n)] for i in range(m)]
+        Xu = X.view(np.uint64)
+        Xi = [[int(X[i, j, 0]) * _limbs_to_int(Xu[i, j, 1:5]) for j in range(n)] for i in range(m)]
         return out, Xi
     return out
 

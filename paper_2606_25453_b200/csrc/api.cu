@@ -117,6 +117,12 @@ static int mark(emugemm_ctx *h, int i) {
   return EMUGEMM_OK;
 }
 
+// degenerate calls (m n == 0) launch nothing: the stage events are still recorded so that emugemm_stage_ms stays valid
+static int mark_all(emugemm_ctx *h) {
+  for (int i = 0; i < 4; ++i) EMU_TRY(mark(h, i));
+  return EMUGEMM_OK;
+}
+
 static int check_gemm_args(emugemm_ctx *h, int ta, int tb, int64_t m, int64_t n, int64_t k, const void *A, int64_t lda,
                            const void *B, int64_t ldb, const void *C, int64_t ldc) {
   if (!h) return EMUGEMM_ERR_ARG;
@@ -128,6 +134,9 @@ static int check_gemm_args(emugemm_ctx *h, int ta, int tb, int64_t m, int64_t n,
   if ((reinterpret_cast<uintptr_t>(A) | reinterpret_cast<uintptr_t>(B) | reinterpret_cast<uintptr_t>(C)) & 15)
     return EMUGEMM_ERR_ALIGNMENT;
   if (k >= (1LL << 31) - 256 || m >= (1LL << 31) - 256 || n >= (1LL << 31) - 256) return EMUGEMM_ERR_ARG;
+  // the k-strided (column) pre-pass puts k / 128 in grid.y (<= 65535): a clean argument error instead of a launch failure
+  // after part of the call has been enqueued; 8,388,480 is far beyond any workspace a B200 can hold anyway
+  if (k > 65535LL * kBlockK) return EMUGEMM_ERR_ARG;
   return EMUGEMM_OK;
 }
 
@@ -163,7 +172,7 @@ static int run_oz1(emugemm_ctx *h, int ta, int tb, int elem, int64_t m, int64_t 
   EMU_TRY(check_gemm_args(h, ta, tb, m, n, k, A, lda, B, ldb, dump ? static_cast<const void *>(dump) : C, dump ? n : ldc));
   if (p < 1 || p > (elem == kF32 ? 4 : 8)) return EMUGEMM_ERR_ARG;
   h->launches = 0;
-  if (m == 0 || n == 0) return EMUGEMM_OK;
+  if (m == 0 || n == 0) return mark_all(h);
   EMU_TRY(mark(h, 0));
   if (k == 0) {
     if (!dump) EMU_TRY(scale_c(h, m, n, beta, 0.0, C, ldc, elem));
@@ -211,7 +220,7 @@ static int run_oz1_batched(emugemm_ctx *h, int elem, int64_t batch, int64_t m, i
   EMU_TRY(check_gemm_args(h, 0, 0, m, n, k, A, lda, B, ldb, C, ldc));
   if (p < 1 || p > (elem == kF32 ? 4 : 8)) return EMUGEMM_ERR_ARG;
   h->launches = 0;
-  if (batch == 0 || m == 0 || n == 0) return EMUGEMM_OK;
+  if (batch == 0 || m == 0 || n == 0) return mark_all(h);
   const int64_t es = (elem == kF32) ? 4 : 8;
   if (batch > 1) {
     if (((strideA * es) | (strideB * es) | (strideC * es)) & 15) return EMUGEMM_ERR_ALIGNMENT;
@@ -298,7 +307,7 @@ static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t 
   EMU_TRY(check_gemm_args(h, ta, tb, m, n, k, A, lda, B, ldb, C, ldc));
   if (N < 2 || N > kMaxModuli) return EMUGEMM_ERR_ARG;
   h->launches = 0;
-  if (m == 0 || n == 0) return EMUGEMM_OK;
+  if (m == 0 || n == 0) return mark_all(h);
   const int elem = is3m ? (f32 ? kC64 : kZ128) : (f32 ? kF32 : kF64);
   EMU_TRY(mark(h, 0));
   if (k == 0) {
@@ -342,7 +351,7 @@ static int run_oz2_batched(emugemm_ctx *h, int is3m, int f32, int64_t batch, int
   EMU_TRY(check_gemm_args(h, 0, 0, m, n, k, A, lda, B, ldb, C, ldc));
   if (N < 2 || N > kMaxModuli) return EMUGEMM_ERR_ARG;
   h->launches = 0;
-  if (batch == 0 || m == 0 || n == 0) return EMUGEMM_OK;
+  if (batch == 0 || m == 0 || n == 0) return mark_all(h);
   if (is3m && f32) return EMUGEMM_ERR_ARG;
   const int elem = is3m ? kZ128 : (f32 ? kF32 : kF64);
   const int64_t es = is3m ? 16 : (f32 ? 4 : 8);
@@ -508,7 +517,7 @@ static int run_oz1_4m(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k,
   EMU_TRY(check_gemm_args(h, 0, 0, m, n, k, A, lda, B, ldb, C, ldc));
   if (p < 1 || p > (elem == kC64 ? 4 : 8)) return EMUGEMM_ERR_ARG;
   h->launches = 0;
-  if (m == 0 || n == 0) return EMUGEMM_OK;
+  if (m == 0 || n == 0) return mark_all(h);
   EMU_TRY(mark(h, 0));
   if (k == 0) {
     EMU_TRY(scale_c(h, m, n, beta[0], beta[1], C, ldc, elem));

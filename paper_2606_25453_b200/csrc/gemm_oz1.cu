@@ -252,10 +252,14 @@ struct Oz1Epi {
             acc = sum;
           }
         }
-        // power-of-two scaling 2^E, E = eA_i + eB_j - 7 (p+1), split so that both factors are normal doubles
-        // for every |E| <= 2044 (branch-free; covers subnormal inputs and results)
+        // power-of-two scaling 2^E, E = eA_i + eB_j - 7 (p+1), as two factors: the first is clamped so that acc 2^h1
+        // (|acc| an integer below 2^83, or 0) stays a normal number, the second (clamped to the exponent range) takes the
+        // result to zero / subnormal / infinity when it must: one rounding for every finite input (operands
+        // near DBL_MIN made E >> 1 fall below -1022 and the exponent field wrap)
         const int E = eArow + eb[c];
-        const double d1 = pow2d(E >> 1), d2 = pow2d(E - (E >> 1));
+        const int h1 = max(min(E, 930), -1000);
+        const int h2 = max(min(E - h1, 1023), -1022);
+        const double d1 = pow2d(h1), d2 = pow2d(h2);
         r[c] = acc * d1 * d2;
         if constexpr (OUT == 3) rlo[c] = lo * d1 * d2;
       }
@@ -360,8 +364,9 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
     if (lane == 0) {
       int sa = 0, sb = 0, nloada = 0, nloadb = 0;
       uint32_t pa = 0, pb = 0;
-      // L2 eviction hints were measured and dropped: EVICT_LAST on A changes nothing (15.1 vs 15.2 GB DRAM reads per
-      // 8192^3 p = 8 launch), EVICT_FIRST on B raises them to 21.9 GB
+      // L2 eviction hints were measured and dropped twice: without the wave barrier EVICT_LAST on A changes nothing (15.1 vs
+      // 15.2 GB) and EVICT_FIRST on B raises the DRAM reads to 21.9 GB; with the barrier A EVICT_LAST / B EVICT_FIRST /
+      // B EVICT_LAST all time within noise of the plain policy (11.98-12.24 against 11.88-12.00 ms at 8192^3 p = 8)
       constexpr uint64_t polA = kEvictNormal, polB = kEvictNormal;
       int wave = 0;
       for (int item = work_id; item < num_items; item += num_workers, ++wave) {
@@ -642,7 +647,7 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   cfg.blockDim = dim3(kGemmThreads);
   cfg.dynamicSmemBytes = Cfg::kSmemBytes;
   cfg.stream = ctx->stream;
-  cudaLaunchAttribute attr[1];
+  cudaLaunchAttribute attr[2];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = CL2 ? 2 : 1;
   attr[0].val.clusterDim.y = 1;
@@ -664,7 +669,22 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
       d.n_waves = static_cast<int>((tiles + workers_used - 1) / workers_used);
     }
   }
-  EMU_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d));
+  if (d.wave_ctr) {
+    // the barrier needs all CTAs on the machine at once: a cooperative launch is scheduled as a gang or not at all, so two
+    // handles launching on two streams can never hold each other's SMs while waiting at their barriers
+    attr[1].id = cudaLaunchAttributeCooperative;
+    attr[1].val.cooperative = 1;
+    cfg.numAttrs = 2;
+    if (cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d) != cudaSuccess) {
+      (void)cudaGetLastError();  // not launchable as a gang (e.g. SMs reserved by another context): run without the barrier
+      d.wave_ctr = nullptr;
+      d.n_waves = 0;
+      cfg.numAttrs = 1;
+      EMU_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d));
+    }
+  } else {
+    EMU_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d));
+  }
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
   return EMUGEMM_OK;

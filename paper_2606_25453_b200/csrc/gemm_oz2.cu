@@ -167,11 +167,15 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
         // neighbourhood touched last are the first ones asked for again
         const bool rev = a.serp && (((tile - cluster_id) / num_clusters) & 1);
         const int nstage = (a.kblocks + kOz2KPerStage - 1) / kOz2KPerStage;
+        // the arrival on the wave barrier is signalled a few stages before the last load of the tile (see gemm_oz1.cu)
+        constexpr int kWaveLead = 6;
+        const int arrive_sidx = nstage - 1 - kWaveLead > 0 ? nstage - 1 - kWaveLead : 0;
         for (int q = 0; q < n_inner; ++q) {
           const int plane = FUSED ? q : q * a.n_moduli + l;
           for (int sidx = 0; sidx < nstage; ++sidx) {
             const int kb = (rev ? nstage - 1 - sidx : sidx) * kOz2KPerStage;
             const int nkb = (a.kblocks - kb < kOz2KPerStage) ? a.kblocks - kb : kOz2KPerStage;
+            if (a.wave_ctr && q == n_inner - 1 && sidx == arrive_sidx) grid_arrive(a.wave_ctr);
             mbar_wait(&empty[st], ph ^ 1);
             const uint32_t full_leader = mapa_u32(&full[st], 0);
             if (cta == 0) mbar_arrive_expect_tx(&full[st], 2 * nkb * kOz2KbBytes);
@@ -183,7 +187,6 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             if (++st == kOz2Stages) { st = 0; ph ^= 1; }
           }
         }
-        if (a.wave_ctr) grid_arrive(a.wave_ctr);
       }
       if (a.wave_ctr)
         for (; wave < a.n_waves; ++wave) grid_arrive(a.wave_ctr);
@@ -469,7 +472,10 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
   d.n_waves = 0;
   // measured (profiles/r2_wave_barrier.md): 3M 8192^3 N = 18 +8 %, N = 14 +15-20 % (DRAM reads 49 -> 31 GB, SM clock 1.2 ->
   // 1.36-1.49 GHz), 4096^3 neutral, real product -8 % (an item is one modulus, 23 us: the re-alignment is not hidden)
-  const bool want_sync = (g.is3m || fused) ? !EMU_PROBE_FLAG(ctx->dbg_flags, 0x10000) : EMU_PROBE_FLAG(ctx->dbg_flags, 0x20000) != 0;
+  // real product: on from k = 16,384 (16384^3 N = 15: 52.2 -> 44.0 ms, SM clock 1.09 -> 1.31 GHz, 0.953 -> 0.943 per clock);
+  // probes build: 0x20000 forces it on for shorter k, 0x10000 switches it off everywhere
+  const bool want_sync = !EMU_PROBE_FLAG(ctx->dbg_flags, 0x10000) &&
+                         (g.is3m || fused || d.kblocks >= 128 || EMU_PROBE_FLAG(ctx->dbg_flags, 0x20000));
   if (g.wave_ctr && want_sync && tiles > grid / 2 && d.kblocks >= (fused ? 16 : 64)) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(grid));
@@ -486,7 +492,29 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
       d.n_waves = static_cast<int>((tiles + grid / 2 - 1) / (grid / 2));
     }
   }
-  kern<<<grid, kGemmThreads, kOz2Smem, ctx->stream>>>(tmA, tmB, d, fz);
+  bool launched = false;
+  if (d.wave_ctr) {  // gang-scheduled (cooperative) launch: see gemm_oz1.cu
+    cudaLaunchConfig_t cfg = {};
+    cfg.gridDim = dim3(static_cast<unsigned>(grid));
+    cfg.blockDim = dim3(kGemmThreads);
+    cfg.dynamicSmemBytes = kOz2Smem;
+    cfg.stream = ctx->stream;
+    cudaLaunchAttribute attr[2];
+    attr[0].id = cudaLaunchAttributeClusterDimension;
+    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
+    attr[1].id = cudaLaunchAttributeCooperative;
+    attr[1].val.cooperative = 1;
+    cfg.attrs = attr;
+    cfg.numAttrs = 2;
+    if (cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d, fz) == cudaSuccess) {
+      launched = true;
+    } else {
+      (void)cudaGetLastError();
+      d.wave_ctr = nullptr;
+      d.n_waves = 0;
+    }
+  }
+  if (!launched) kern<<<grid, kGemmThreads, kOz2Smem, ctx->stream>>>(tmA, tmB, d, fz);
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
   return EMUGEMM_OK;

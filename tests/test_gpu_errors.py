@@ -119,3 +119,30 @@ def test_nonfinite_flag(env):
     torch.cuda.synchronize()  # no fault: the device is still usable
     h.dgemm_oz1(A, B, C, 4)
     assert torch.isfinite(C).all()
+
+
+def test_two_handles_on_two_streams_with_wave_barrier(env):
+    """The fused kernels that use the grid-wide wave barrier are launched as a gang (cooperative launch): two handles
+    issuing such kernels on two streams at once must complete (no CTA may hold an SM while its own kernel waits for CTAs
+    that cannot be scheduled) and give the results of the serial calls."""
+    torch, E, h = env
+    m, n, k, p = 4096, 4096, 8192, 8   # 64 KB of slices per operand row: the barrier is on
+    A = torch.rand((m, k), dtype=torch.float64, device="cuda") - 0.5
+    B = torch.rand((k, n), dtype=torch.float64, device="cuda") - 0.5
+    ref = torch.empty((m, n), dtype=torch.float64, device="cuda")
+    h.dgemm_oz1(A, B, ref, p)
+    torch.cuda.synchronize()
+    s1, s2 = torch.cuda.Stream(), torch.cuda.Stream()
+    h1, h2 = E.EmuGemm(), E.EmuGemm()
+    h1.set_stream(s1); h2.set_stream(s2)
+    C1 = torch.empty_like(ref); C2 = torch.empty_like(ref)
+    try:
+        for _ in range(3):
+            with torch.cuda.stream(s1):
+                h1.dgemm_oz1(A, B, C1, p)
+            with torch.cuda.stream(s2):
+                h2.dgemm_oz1(A, B, C2, p)
+        torch.cuda.synchronize()
+        assert torch.equal(C1, ref) and torch.equal(C2, ref)
+    finally:
+        h1.close(); h2.close()

@@ -179,3 +179,24 @@ def test_degenerate_sizes(env):
     Cz = torch.ones((130, 130), dtype=torch.float64, device="cuda")
     h.dgemm_oz1(Z, Z, Cz, 5)  # all-zero operands
     assert (Cz == 0).all()
+
+
+def test_dgemm_oz1_extreme_exponents(env):
+    """operands near DBL_MIN / DBL_MAX: 2^(eA_i + eB_j - 7(p+1)) must flush to zero / subnormals / infinity
+    correctly instead of wrapping the exponent field."""
+    torch, O, h = env
+    m, n, k, p = 70, 66, 130, 6
+    A, B = G.real_pair(m, n, k, 1.0, 21)
+    for sa, sb in ((2.0 ** -1000, 2.0 ** -1000), (2.0 ** -1020, 2.0 ** -40), (2.0 ** 500, 2.0 ** 500), (2.0 ** -600, 2.0 ** -440),
+                   (2.0 ** -1021, 2.0 ** 0)):
+        As, Bs = A * sa, B * sb
+        C = torch.full((m, n), float("nan"), dtype=torch.float64, device="cuda")
+        h.dgemm_oz1(dev(torch, As), dev(torch, Bs), C, p)
+        want = O.dgemm_oz1(As, Bs, p)
+        got = C.cpu().numpy()
+        with np.errstate(over="ignore", under="ignore"):
+            scale = np.abs(As) @ np.abs(Bs)
+        tiny = scale < 2.0 ** -1021
+        if (~tiny).any():
+            assert_within_ulps(got[~tiny], want[~tiny], scale[~tiny], 2, what=f"scales {sa} {sb}")
+        assert (np.abs(got[tiny] - want[tiny]) <= 2 * 2.0 ** -1074).all()   # subnormal range: two subnormal spacings

@@ -254,3 +254,18 @@ def test_sgemm_oz2_matches_dgemm_oz2_rounded_once():
     C32 = O.sgemm_oz2(A, B, 9)
     C64 = O.dgemm_oz2(A.astype(np.float64), B.astype(np.float64), 9)
     assert (np.abs(C32.astype(np.float64) - C64) <= np.spacing(np.abs(C64).astype(np.float32)).astype(np.float64)).all()
+
+
+def test_crt_X_hook_is_exact_beyond_128_bits():
+    """The test hook that returns the reconstructed integer must not truncate: |X| up to P/4 ~ 2^154 at N = 20."""
+    N = 20
+    mods = [int(x) for x in O.oz2_moduli(N)]
+    P = O.oz2_P(N)
+    Xs = [P // 4 - 1, -(P // 4) + 3, 12345, -1, 0, 2 ** 140 + 7]
+    CR = np.empty((N, 2, 3), np.int8)
+    for l, m in enumerate(mods):
+        r = np.array([x % m for x in Xs])
+        CR[l] = np.where(r >= (m + 1) // 2, r - m, r).reshape(2, 3)
+    out, Xi = O.oz2_crt(CR, np.zeros(2, np.int32), np.zeros(3, np.int32), 0, 0, want_X=True)
+    assert sum(Xi, []) == Xs
+    assert out.ravel().tolist() == [float(x) for x in Xs] or np.allclose(out.ravel(), [float(x) for x in Xs], rtol=2e-16, atol=0)
