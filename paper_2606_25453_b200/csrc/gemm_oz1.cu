@@ -369,11 +369,12 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       // B EVICT_LAST all time within noise of the plain policy (11.98-12.24 against 11.88-12.00 ms at 8192^3 p = 8)
       constexpr uint64_t polA = kEvictNormal, polB = kEvictNormal;
       int wave = 0;
+      bool wave_off = false;  // a barrier wait ran into its bound: stop waiting (keep arriving) for the rest of the launch
       for (int item = work_id; item < num_items; item += num_workers, ++wave) {
         // static round-robin keeps the tiles of a wave adjacent, but CTAs drift apart by whole tiles over a launch (the
         // per-SM speed differs by a few per cent) and then every CTA streams its own copy of the panels from DRAM
         // (13.7 GB instead of ~7 GB per 8192^3 p = 8 launch, ncu): re-align the producers at every tile
-        if (a.wave_ctr && wave > 0) grid_wait(a.wave_ctr, static_cast<unsigned long long>(wave) * gridDim.x);
+        if (a.wave_ctr && wave > 0 && !wave_off) wave_off = !grid_wait(a.wave_ctr, static_cast<unsigned long long>(wave) * gridDim.x);
         const int bidx = item / per_entry, rem = item - bidx * per_entry;
         const int chunk = rem / num_tiles, tile = rem - chunk * num_tiles;
         const int kb0 = a.kb0 + chunk * a.chunk_kb, kb1 = (kb0 + a.chunk_kb < a.kb1) ? kb0 + a.chunk_kb : a.kb1;
@@ -647,7 +648,7 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   cfg.blockDim = dim3(kGemmThreads);
   cfg.dynamicSmemBytes = Cfg::kSmemBytes;
   cfg.stream = ctx->stream;
-  cudaLaunchAttribute attr[2];
+  cudaLaunchAttribute attr[1];
   attr[0].id = cudaLaunchAttributeClusterDimension;
   attr[0].val.clusterDim.x = CL2 ? 2 : 1;
   attr[0].val.clusterDim.y = 1;
@@ -669,22 +670,9 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
       d.n_waves = static_cast<int>((tiles + workers_used - 1) / workers_used);
     }
   }
-  if (d.wave_ctr) {
-    // the barrier needs all CTAs on the machine at once: a cooperative launch is scheduled as a gang or not at all, so two
-    // handles launching on two streams can never hold each other's SMs while waiting at their barriers
-    attr[1].id = cudaLaunchAttributeCooperative;
-    attr[1].val.cooperative = 1;
-    cfg.numAttrs = 2;
-    if (cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d) != cudaSuccess) {
-      (void)cudaGetLastError();  // not launchable as a gang (e.g. SMs reserved by another context): run without the barrier
-      d.wave_ctr = nullptr;
-      d.n_waves = 0;
-      cfg.numAttrs = 1;
-      EMU_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d));
-    }
-  } else {
-    EMU_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d));
-  }
+  // plain launch: the barrier's wait is bounded and gives up (ptx.cuh), so CTAs that are not co-resident after all (a
+  // second handle launching on another stream, a profiler) cost time, never progress
+  EMU_CUDA(ctx, cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d));
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
   return EMUGEMM_OK;

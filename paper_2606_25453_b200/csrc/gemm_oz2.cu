@@ -153,10 +153,11 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       int st = 0;
       uint32_t ph = 0;
       int wave = 0;
+      bool wave_off = false;  // a barrier wait ran into its bound: no more waiting in this launch (arrivals continue)
       for (int tile = cluster_id; tile < num_tiles; tile += num_clusters, ++wave) {
         // re-align the producers of all CTAs at every tile (see gemm_oz1.cu): the pairs that share an A or a B panel then ask
         // for the same k-block of the same product at the same time, and it comes from DRAM once
-        if (a.wave_ctr && wave > 0) grid_wait(a.wave_ctr, static_cast<unsigned long long>(wave) * gridDim.x);
+        if (a.wave_ctr && wave > 0 && !wave_off) wave_off = !grid_wait(a.wave_ctr, static_cast<unsigned long long>(wave) * gridDim.x);
         const int bidx = tile / tiles_per_entry, te = tile - bidx * tiles_per_entry;
         const int l = FUSED ? 0 : te / tiles_per_mod;
         int mb, nb;
@@ -465,17 +466,16 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
     if (static_cast<size_t>(grid) * 2 * g.n_moduli * kOz2ScratchPlane > g.scratch_bytes) return EMUGEMM_ERR_WORKSPACE;  // two buffers per CTA
   }
   EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, kOz2Smem));
-  // Wave barrier (gemm_oz1.cu): only when all CTAs are certainly co-resident, there are at least two waves and a tile is
-  // long enough (>= 16 k-blocks per product) to hide the re-alignment.  3M: on (measured); real: off (its DRAM
-  // traffic already sits at the no-drift figure); fused: on (a tile is N products long)
+  // Wave barrier (gemm_oz1.cu): only when all CTAs are co-resident by the occupancy query, there are at least two waves
+  // and the k-loop is long enough (>= 64 k-blocks per product, >= 16 for the fused variant whose tile is N products long)
+  // for the early arrival (kWaveLead stages before the item's last load) to hide the re-alignment.
+  // Measured A/B (profiles/r2_wave_barrier.md), barrier on against off: 3M 8192^3 N = 18 19.6 / 20.9 ms, N = 14 14.8 / 16.3
+  // (DRAM reads 50.5 -> 31.3 GB), real 8192^3 N = 16 5.76 / 6.12 ms, real 16384^3 N = 15 43.9 / 49.9 ms; 4096^3 neutral.
+  // With the arrival at the END of the item the real product lost 8 % (an item is one modulus, 23 us); the early arrival
+  // turned that into a gain.  Probes build: 0x10000 switches the barrier off.
   d.wave_ctr = nullptr;
   d.n_waves = 0;
-  // measured (profiles/r2_wave_barrier.md): 3M 8192^3 N = 18 +8 %, N = 14 +15-20 % (DRAM reads 49 -> 31 GB, SM clock 1.2 ->
-  // 1.36-1.49 GHz), 4096^3 neutral, real product -8 % (an item is one modulus, 23 us: the re-alignment is not hidden)
-  // real product: on from k = 16,384 (16384^3 N = 15: 52.2 -> 44.0 ms, SM clock 1.09 -> 1.31 GHz, 0.953 -> 0.943 per clock);
-  // probes build: 0x20000 forces it on for shorter k, 0x10000 switches it off everywhere
-  const bool want_sync = !EMU_PROBE_FLAG(ctx->dbg_flags, 0x10000) &&
-                         (g.is3m || fused || d.kblocks >= 128 || EMU_PROBE_FLAG(ctx->dbg_flags, 0x20000));
+  const bool want_sync = !EMU_PROBE_FLAG(ctx->dbg_flags, 0x10000);
   if (g.wave_ctr && want_sync && tiles > grid / 2 && d.kblocks >= (fused ? 16 : 64)) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(grid));
@@ -492,29 +492,8 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
       d.n_waves = static_cast<int>((tiles + grid / 2 - 1) / (grid / 2));
     }
   }
-  bool launched = false;
-  if (d.wave_ctr) {  // gang-scheduled (cooperative) launch: see gemm_oz1.cu
-    cudaLaunchConfig_t cfg = {};
-    cfg.gridDim = dim3(static_cast<unsigned>(grid));
-    cfg.blockDim = dim3(kGemmThreads);
-    cfg.dynamicSmemBytes = kOz2Smem;
-    cfg.stream = ctx->stream;
-    cudaLaunchAttribute attr[2];
-    attr[0].id = cudaLaunchAttributeClusterDimension;
-    attr[0].val.clusterDim.x = 2; attr[0].val.clusterDim.y = 1; attr[0].val.clusterDim.z = 1;
-    attr[1].id = cudaLaunchAttributeCooperative;
-    attr[1].val.cooperative = 1;
-    cfg.attrs = attr;
-    cfg.numAttrs = 2;
-    if (cudaLaunchKernelEx(&cfg, kern, tmA, tmB, d, fz) == cudaSuccess) {
-      launched = true;
-    } else {
-      (void)cudaGetLastError();
-      d.wave_ctr = nullptr;
-      d.n_waves = 0;
-    }
-  }
-  if (!launched) kern<<<grid, kGemmThreads, kOz2Smem, ctx->stream>>>(tmA, tmB, d, fz);
+  // plain launch: a barrier wait that runs into its bound gives up (ptx.cuh), so co-residency is an optimisation only
+  kern<<<grid, kGemmThreads, kOz2Smem, ctx->stream>>>(tmA, tmB, d, fz);
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
   return EMUGEMM_OK;

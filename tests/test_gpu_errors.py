@@ -122,9 +122,9 @@ def test_nonfinite_flag(env):
 
 
 def test_two_handles_on_two_streams_with_wave_barrier(env):
-    """The fused kernels that use the grid-wide wave barrier are launched as a gang (cooperative launch): two handles
-    issuing such kernels on two streams at once must complete (no CTA may hold an SM while its own kernel waits for CTAs
-    that cannot be scheduled) and give the results of the serial calls."""
+    """The grid-wide wave barrier of the fused kernels is an optimisation with a bounded wait that gives up
+    (csrc/ptx.cuh): two handles issuing such kernels on two streams at once -- their CTAs are then NOT all co-resident --
+    must complete and give the results of the serial calls."""
     torch, E, h = env
     m, n, k, p = 4096, 4096, 8192, 8   # 64 KB of slices per operand row: the barrier is on
     A = torch.rand((m, k), dtype=torch.float64, device="cuda") - 0.5
