@@ -47,7 +47,8 @@ enum emugemm_status {
   EMUGEMM_ERR_WORKSPACE = -3, /* workspace missing or smaller than emugemm_workspace_bytes() */
   EMUGEMM_ERR_PRECISION = -4, /* Scheme II: k too large for this n_moduli (bit budget T < 2), or k > 131,071 (see Scheme II) */
   EMUGEMM_ERR_DEVICE = -5,    /* no CUDA device or not compute capability 10.x */
-  EMUGEMM_ERR_CUDA = -6       /* a CUDA call failed; see emugemm_last_cuda_error() */
+  EMUGEMM_ERR_CUDA = -6,      /* a CUDA call failed; see emugemm_last_cuda_error() */
+  EMUGEMM_ERR_STATIC_LIMIT = -7 /* emugemm_dgemm_oz1_static: the problem needs more than EMUGEMM_STATIC_WS_BYTES of scratch */
 };
 
 enum emugemm_scheme { EMUGEMM_OZ1 = 1, EMUGEMM_OZ2 = 2, EMUGEMM_OZ2_3M = 3, EMUGEMM_OZ1_4M = 4 };
@@ -101,6 +102,26 @@ int emugemm_dgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, doubl
 int emugemm_sgemm_oz1(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, float alpha,
                       const float *A, int64_t lda, const float *B, int64_t ldb, float beta,
                       float *C, int64_t ldc, int p);
+
+/* Scheme I DGEMM for callers that cannot allocate (code under CUDA graph capture, tight serving loops, harnesses that
+ * forbid cudaMalloc): same arguments, same kernels and bit-identical results as emugemm_dgemm_oz1, but the scratch
+ * (digit planes, exponents, diagnostics words) lives in a static device array inside the library image instead of a
+ * workspace from emugemm_set_workspace -- no workspace is needed and none that is registered is touched.  The call
+ * performs no cudaMalloc / cudaFree and calls no allocating library routine.
+ *   Limit: emugemm_workspace_bytes(EMUGEMM_OZ1, 8, m, n, k, p) <= EMUGEMM_STATIC_WS_BYTES (32 MiB: e.g. 1024^3 with
+ *     p = 8, 2048 x 2048 x 1024 with p = 3); beyond it the call returns EMUGEMM_ERR_STATIC_LIMIT and enqueues nothing.
+ *     Every GPU that loads the library holds the array (32 MiB + 1 KiB) until the process exits.
+ *   Sharing: ALL calls of this entry point on one device, from every handle, use the one array.  The call zeroes the
+ *     words that must start at zero and rewrites every plane byte it reads, so back-to-back calls on ONE stream are
+ *     safe; calls that overlap on the GPU (two streams, two handles, two host threads) RACE on the array and give
+ *     wrong results -- serialise them, or use emugemm_dgemm_oz1 with one workspace per handle.
+ *   A, B, C: device pointers, row-major, 16-byte aligned, owned by the caller; asynchronous on the handle's stream.
+ *   Errors: as emugemm_dgemm_oz1 (ARG, ALIGNMENT, CUDA), plus STATIC_LIMIT; never ERR_WORKSPACE.                    */
+#define EMUGEMM_STATIC_WS_BYTES (32u << 20)
+size_t emugemm_static_workspace_limit(void); /* = EMUGEMM_STATIC_WS_BYTES of the loaded library */
+int emugemm_dgemm_oz1_static(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha,
+                             const double *A, int64_t lda, const double *B, int64_t ldb, double beta,
+                             double *C, int64_t ldc, int p);
 
 /* Strided batched Scheme I ("a batched implementation is possible through a
  * single interleaved tensor per batch entry"): C_b = alpha*A_b*B_b + beta*C_b for b = 0..batch-1, all of one

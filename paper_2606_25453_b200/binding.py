@@ -45,6 +45,7 @@ def load_library(probes=False):
         lib.emugemm_workspace_bytes.argtypes = [_int, _int, _i64, _i64, _i64, _int]
         lib.emugemm_operand_bytes.restype = _sz
         lib.emugemm_operand_bytes.argtypes = [_int, _i64, _i64, _int]
+        lib.emugemm_static_workspace_limit.restype = _sz
         lib.emugemm_oz1_chunk_k.restype = _i64
         lib.emugemm_oz1_chunk_k_bits.restype = _i64
         _libs[probes] = lib
@@ -217,6 +218,18 @@ class EmuGemm:
         self._check(self._lib.emugemm_dgemm_oz1_t(self._h, _int(transa), _int(transb), _i64(m), _i64(n), _i64(k), _dbl(alpha),
                                                    _ptr(A), _i64(self._ld(A)), _ptr(B), _i64(self._ld(B)), _dbl(beta), _ptr(C_),
                                                    _i64(self._ld(C_)), _int(p)))
+        return C_
+
+    def static_workspace_limit(self):
+        return int(self._lib.emugemm_static_workspace_limit())
+
+    def dgemm_oz1_static(self, A, B, C_, p, alpha=1.0, beta=0.0):
+        """emugemm_dgemm_oz1_static: scratch in the library's static device array -- nothing is allocated or reserved
+        here (no torch workspace either); EmuGemmError with status -7 beyond static_workspace_limit()."""
+        m, n, k = self._dims(A, B, False, False, C_, self._torch.float64)
+        self._check(self._lib.emugemm_dgemm_oz1_static(self._h, _i64(m), _i64(n), _i64(k), _dbl(alpha), _ptr(A), _i64(self._ld(A)),
+                                                        _ptr(B), _i64(self._ld(B)), _dbl(beta), _ptr(C_), _i64(self._ld(C_)),
+                                                        _int(p)))
         return C_
 
     def sgemm_oz1(self, A, B, C_, p, alpha=1.0, beta=0.0, transa=False, transb=False):

@@ -20,7 +20,7 @@ CSRC = os.path.join(HERE, "csrc")
 OBJ = os.path.join(HERE, "build")
 OUT = os.path.join(HERE, "libemugemm.so")
 OUT_PROBES = os.path.join(HERE, "libemugemm_probes.so")
-SOURCES = ["api.cu", "prepass.cu", "gemm_oz1.cu", "gemm_oz2.cu", "crt.cu"]
+SOURCES = ["api.cu", "prepass.cu", "gemm_oz1.cu", "gemm_oz2.cu", "crt.cu", "static_ws.cu"]
 HEADERS = ["common.cuh", "ptx.cuh", "gemm_common.cuh", "crt_dev.cuh", os.path.join("..", "..", "include", "emugemm.h")]
 NVCC_FLAGS = ["-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo", "-O3", "-std=c++17",
               "-Xcompiler", "-fPIC", "-Xcompiler", "-fvisibility=hidden", "--expt-relaxed-constexpr"]

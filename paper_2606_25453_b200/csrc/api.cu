@@ -503,6 +503,7 @@ const char *emugemm_status_string(int s) {
     case EMUGEMM_ERR_PRECISION: return "k too large for this number of moduli";
     case EMUGEMM_ERR_DEVICE: return "no sm_100 CUDA device";
     case EMUGEMM_ERR_CUDA: return "CUDA error";
+    case EMUGEMM_ERR_STATIC_LIMIT: return "problem exceeds the static scratch array (EMUGEMM_STATIC_WS_BYTES): use emugemm_dgemm_oz1 with a workspace";
     default: return "unknown status";
   }
 }
