@@ -367,7 +367,9 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
       // L2 eviction hints were measured and dropped twice: without the wave barrier EVICT_LAST on A changes nothing (15.1 vs
       // 15.2 GB) and EVICT_FIRST on B raises the DRAM reads to 21.9 GB; with the barrier A EVICT_LAST / B EVICT_FIRST /
       // B EVICT_LAST all time within noise of the plain policy (11.98-12.24 against 11.88-12.00 ms at 8192^3 p = 8)
-      constexpr uint64_t polA = kEvictNormal, polB = kEvictNormal;
+      // (probes build: 0x200000 = A EVICT_LAST, 0x400000 = B EVICT_FIRST, 0x800000 = B EVICT_LAST, for the DRAM-byte captures)
+      const uint64_t polA = EMU_PROBE_FLAG(a.dbg, 0x200000) ? kEvictLast : kEvictNormal;
+      const uint64_t polB = EMU_PROBE_FLAG(a.dbg, 0x400000) ? kEvictFirst : EMU_PROBE_FLAG(a.dbg, 0x800000) ? kEvictLast : kEvictNormal;
       int wave = 0;
       bool wave_off = false;  // a barrier wait ran into its bound: stop waiting (keep arriving) for the rest of the launch
       for (int item = work_id; item < num_items; item += num_workers, ++wave) {

@@ -469,13 +469,17 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
   // Wave barrier (gemm_oz1.cu): only when all CTAs are co-resident by the occupancy query, there are at least two waves
   // and the k-loop is long enough (>= 64 k-blocks per product, >= 16 for the fused variant whose tile is N products long)
   // for the early arrival (kWaveLead stages before the item's last load) to hide the re-alignment.
-  // Measured A/B (profiles/r2_wave_barrier.md), barrier on against off: 3M 8192^3 N = 18 19.6 / 20.9 ms, N = 14 14.8 / 16.3
-  // (DRAM reads 50.5 -> 31.3 GB), real 8192^3 N = 16 5.76 / 6.12 ms, real 16384^3 N = 15 43.9 / 49.9 ms; 4096^3 neutral.
-  // With the arrival at the END of the item the real product lost 8 % (an item is one modulus, 23 us); the early arrival
-  // turned that into a gain.  Probes build: 0x10000 switches the barrier off.
+  // Measured A/B on two boxes (profiles/r2_wave_barrier.md), barrier on / off:
+  //   3M 8192^3 N = 18    19.6 / 20.9 and 19.8 / 21.2 ms (DRAM reads 50.5 -> 31.3 GB)          -> on
+  //   3M 8192^3 N = 14    14.8 / 16.3 and 15.7 / 14.9 ms (within the box-to-box spread)         -> on (same rule as N = 18)
+  //   real 16384^3 N = 15 43.9 / 49.9 and 45.9 / 50.5 ms (a modulus' planes, 2 x 268 MB, exceed the L2) -> on from k = 16,384
+  //   real 8192^3 N = 16  5.76 / 6.12 and 5.86 / 5.74 ms: a modulus' planes (2 x 67 MB) fit the L2, the DRAM reads do not
+  //                       change (5.57 / 5.53 GB) and the barrier costs 2.7 % per clock (an item is one modulus, 23 us) -> off
+  // Probes build: 0x20000 forces it on for the real product at shorter k, 0x10000 switches it off everywhere.
   d.wave_ctr = nullptr;
   d.n_waves = 0;
-  const bool want_sync = !EMU_PROBE_FLAG(ctx->dbg_flags, 0x10000);
+  const bool want_sync = !EMU_PROBE_FLAG(ctx->dbg_flags, 0x10000) &&
+                         (g.is3m || fused || d.kblocks >= 128 || EMU_PROBE_FLAG(ctx->dbg_flags, 0x20000));
   if (g.wave_ctr && want_sync && tiles > grid / 2 && d.kblocks >= (fused ? 16 : 64)) {
     cudaLaunchConfig_t cfg = {};
     cfg.gridDim = dim3(static_cast<unsigned>(grid));
