@@ -1,4 +1,7 @@
 """Helpers for the -m gpu parity tests: tolerance of north_star (2 ulp of (|A||B|)_ij) and handles."""
+import json
+import os
+
 import numpy as np
 
 
@@ -21,4 +24,10 @@ def assert_within_ulps(got, want, scale, n_ulp=2, bits=52, what=""):
         idx = np.unravel_index(np.argmax(err / np.maximum(tol, 1e-300)), err.shape)
         raise AssertionError(f"{what}: {bad.sum()} / {bad.size} elements beyond {n_ulp} ulp; worst at {idx}: "
                              f"got {got[idx]!r} want {want[idx]!r} err {err[idx]:.3e} tol {tol[idx]:.3e}")
-    return float((err / np.maximum(ulp_of(scale, bits), 1e-300)).max())
+    worst = float((err / np.maximum(ulp_of(scale, bits), 1e-300)).max()) if err.size else 0.0
+    log = os.environ.get("EMUGEMM_PARITY_LOG")  # optional record of the measured errors (BASELINE.md section 4's last column)
+    if log:
+        with open(log, "a") as f:
+            f.write(json.dumps({"test": os.environ.get("PYTEST_CURRENT_TEST", "").split(" ")[0], "what": what,
+                                "elements": int(err.size), "max_err_ulps": worst, "tolerance_ulps": n_ulp, "bits": bits}) + "\n")
+    return worst
