@@ -59,6 +59,32 @@ static int oz1_chunks(int p, int bits, int64_t kpad, int64_t chunk_override, int
   return n;
 }
 
+// Chunk count of a one-shot / operand-handle Scheme I product: the overflow-safe minimum, or -- when k needs several
+// chunks anyway and the output has so few tiles that whole waves of the persistent kernel would run partly empty -- up
+// to twice as many, shorter chunks, chosen to minimise (waves of work items) x (chunk length + the per-item epilogue,
+// ~250 columns' worth of MMA time).  1024 x 1024 x 65536 at p = 7: 64 cluster tiles x 4 chunks = 256 items on 74 workers
+// = 4 waves of 16,384 columns; with 8 chunks 512 items = 7 waves of 8,192: 12 % less.  The partials are exact
+// double-doubles, so the chunk count does not change the result (tests/test_gpu_full_size.py, k = 65,536).
+static constexpr int64_t kChunkItemOverheadK = 256;
+static bool oz1_chunks_may_balance(int nmin, int64_t tiles) { return nmin >= 2 && tiles * nmin < 8 * 128; }
+static int oz1_chunks_balanced(int p, int bits, int64_t kpad, int64_t m, int64_t n, int num_sms, int64_t *chunk_len) {
+  int64_t clen;
+  const int nmin = oz1_chunks(p, bits, kpad, 0, &clen);
+  *chunk_len = clen;
+  const int64_t tiles = oz1_cluster_tiles_host(p, m, n), workers = num_sms / 2;
+  if (!oz1_chunks_may_balance(nmin, tiles) || workers < 1 || tiles * nmin >= 8 * workers) return nmin;
+  int best = nmin;
+  int64_t best_cost = -1;
+  for (int c = nmin; c <= 2 * nmin; ++c) {
+    const int64_t len = round_up((kpad + c - 1) / c, kBlockK);
+    const int nc = static_cast<int>((kpad + len - 1) / len);  // chunks actually needed at this length
+    const int64_t waves = (tiles * nc + workers - 1) / workers;
+    const int64_t cost = waves * (len + kChunkItemOverheadK);
+    if (best_cost < 0 || cost < best_cost) { best_cost = cost; best = nc; *chunk_len = len; }
+  }
+  return best;
+}
+
 static size_t ws_common(int64_t m, int64_t n) {
   return 1024 /*diagnostics*/ + granule(8 * m) + granule(8 * n) + granule(4 * m) + granule(4 * n);
 }
@@ -183,7 +209,9 @@ static int run_oz1(emugemm_ctx *h, int ta, int tb, int elem, int64_t m, int64_t 
   const int64_t kpad = round_up(k, kBlockK);
   int64_t clen;
   const int bits = h->slice_bits;
-  const int nch = oz1_chunks(p, bits, kpad, chunk_override, &clen);
+  // the dump hook and an explicit chunk length keep the plain split; product calls may take more, shorter chunks
+  const int nch = (dump || chunk_override > 0) ? oz1_chunks(p, bits, kpad, chunk_override, &clen)
+                                               : oz1_chunks_balanced(p, bits, kpad, m, n, h->num_sms, &clen);
   if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
   Carver cv(h->ws, h->ws_bytes);
   auto *diag = cv.take<unsigned long long>(1);
@@ -474,7 +502,8 @@ size_t emugemm_workspace_bytes(int scheme, int elem, int64_t m, int64_t n, int64
     if (pn > 8 || (elem != 4 && elem != 8)) return 0;
     total += granule(static_cast<size_t>(pn) * m * kpad) + granule(static_cast<size_t>(pn) * n * kpad);
     int64_t clen;
-    const int nch = oz1_chunks(pn, 8, kpad, 0, &clen);  // the 8-bit mode has the shorter chunks: size for it
+    int nch = oz1_chunks(pn, 8, kpad, 0, &clen);  // the 8-bit mode has the shorter chunks: size for it
+    if (oz1_chunks_may_balance(nch, oz1_cluster_tiles_host(pn, m, n))) nch *= 2;  // room for the balanced split (few tiles: small)
     if (nch > 1) total += granule(static_cast<size_t>(nch) * m * n * 16);
   } else if (scheme == EMUGEMM_OZ1_4M) {
     if (pn > 8 || elem != 16) return 0;
@@ -726,7 +755,7 @@ int emugemm_gemm_pre(emugemm_handle_t h, const emugemm_operand_t *A, const emuge
   EMU_TRY(mark(h, 1));
   if (scheme == EMUGEMM_OZ1) {
     int64_t clen;
-    const int nch = oz1_chunks(pn, A->slice_bits, kpad, 0, &clen);
+    const int nch = oz1_chunks_balanced(pn, A->slice_bits, kpad, m, n, h->num_sms, &clen);  // as the one-shot call
     double *part = nch > 1 ? cv.take<double>(static_cast<size_t>(nch) * m * n * 2) : nullptr;
     if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
     h->diag = diag;

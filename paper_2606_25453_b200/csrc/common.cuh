@@ -171,5 +171,8 @@ int launch_i8_probe(emugemm_ctx *ctx, int n_ops, const int *ops, int iters, floa
 int oz2_moduli_host(int n, int *mod);                  // greedy coprime list, descending from 256
 int oz2_budget_host(int n, int64_t k, int is3m, int *tA, int *tB);
 int64_t oz1_chunk_k_host(int p, int slice_bits = 7);
+// Work items (cluster tiles) of one k-chunk of the fused Scheme I kernel for an m x n output with p slices; the
+// kernel runs num_sms / 2 workers (CTA pairs) for every p (gemm_oz1.cu)
+int64_t oz1_cluster_tiles_host(int p, int64_t m, int64_t n);
 
 }  // namespace emu

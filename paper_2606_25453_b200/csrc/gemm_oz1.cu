@@ -713,6 +713,18 @@ int64_t oz1_chunk_k_host(int p, int slice_bits) {
   return bound / kBlockK * kBlockK;
 }
 
+int64_t oz1_cluster_tiles_host(int p, int64_t m, int64_t n) {
+  auto cdiv = [](int64_t a, int64_t b) { return (a + b - 1) / b; };
+  switch (p) {  // the NT table of Oz1Cfg; p <= 3: 256-row pair tiles, p >= 4: two N-adjacent 128-row tiles per cluster
+    case 1: case 2: return cdiv(m, 2 * kTileM) * cdiv(n, Oz1Cfg<2, true>::NT);
+    case 3: return cdiv(m, 2 * kTileM) * cdiv(n, Oz1Cfg<3, true>::NT);
+    case 4: return cdiv(m, kTileM) * cdiv(cdiv(n, Oz1Cfg<4>::NT), 2);
+    case 5: return cdiv(m, kTileM) * cdiv(cdiv(n, Oz1Cfg<5>::NT), 2);
+    case 6: return cdiv(m, kTileM) * cdiv(cdiv(n, Oz1Cfg<6>::NT), 2);
+    default: return cdiv(m, kTileM) * cdiv(cdiv(n, Oz1Cfg<8>::NT), 2);  // p = 7, 8: NT = 64
+  }
+}
+
 // ---- k-chunk reduction: C = alpha * sum_c (hi_c + lo_c) + beta C, double-double sum ----
 __global__ void __launch_bounds__(256) oz1_chunk_reduce_kernel(int64_t m, int64_t n, int n_chunks,
                                                                const double *__restrict__ part, int out_kind,
