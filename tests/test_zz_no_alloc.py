@@ -99,3 +99,32 @@ def test_static_entry_rejects_sizes_beyond_the_array(env):
     with pytest.raises(E.EmuGemmError) as ei:
         h.dgemm_oz1_static(A, B, C, 9)
     assert ei.value.status == -1
+
+
+def test_static_entry_under_cuda_graph_capture(env):
+    """The use case the entry point exists for: the call is captured into a CUDA graph in GLOBAL capture-error mode (a
+    cudaMalloc / cudaFree or any other capture-unsafe call during the capture would fail it) and replayed twice."""
+    torch, E, _ = env
+    h = E.EmuGemm()
+    try:
+        m, n, k, p = 512, 384, 1000, 8
+        A, B = _operands(torch, m, n, k, seed=5)
+        want = torch.empty((m, n), dtype=torch.float64, device="cuda")
+        E.EmuGemm().dgemm_oz1(A, B, want, p)
+        C = torch.empty_like(want)
+        h.dgemm_oz1_static(A, B, C, p)     # outside the capture: module load and the per-device symbol-address set-up
+        torch.cuda.synchronize()
+        s = torch.cuda.Stream()
+        g = torch.cuda.CUDAGraph()
+        with torch.cuda.stream(s):
+            h.set_stream(s)
+            with torch.cuda.graph(g, stream=s, capture_error_mode="global"):
+                h.dgemm_oz1_static(A, B, C, p)
+        for _ in range(2):
+            C.zero_()
+            torch.cuda.synchronize()
+            g.replay()
+            torch.cuda.synchronize()
+            assert torch.equal(C, want)
+    finally:
+        h.close()
