@@ -45,7 +45,7 @@ enum emugemm_status {
   EMUGEMM_ERR_ARG = -1,       /* null pointer, negative size, ld too small, p / n_moduli out of range */
   EMUGEMM_ERR_ALIGNMENT = -2, /* A, B, C not 16-byte aligned or workspace not 1024-byte aligned */
   EMUGEMM_ERR_WORKSPACE = -3, /* workspace missing or smaller than emugemm_workspace_bytes() */
-  EMUGEMM_ERR_PRECISION = -4, /* Scheme II: k too large for this n_moduli (bit budget T < 2), or k > 131,071 (see Scheme II) */
+  EMUGEMM_ERR_PRECISION = -4, /* Scheme II: k too large for this n_moduli (bit budget T < 2) */
   EMUGEMM_ERR_DEVICE = -5,    /* no CUDA device or not compute capability 10.x */
   EMUGEMM_ERR_CUDA = -6,      /* a CUDA call failed; see emugemm_last_cuda_error() */
   EMUGEMM_ERR_STATIC_LIMIT = -7 /* emugemm_dgemm_oz1_static: the problem needs more than EMUGEMM_STATIC_WS_BYTES of scratch */
@@ -163,9 +163,11 @@ int emugemm_cgemm_oz2_3m(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, co
  * descending); symmetric INT8 residues; one INT8 GEMM per modulus with the
  * mod-reduction fused into its epilogue (Eq. 6-7); CRT (Eq. 8) and inverse
  * scaling in FP64.  Range: 2 <= n_moduli <= 20.
- * k <= 131,071: one INT32-safe accumulation range (k 128^2 < 2^31; R7).  Larger k is UNSUPPORTED in Scheme II
- * (EMUGEMM_ERR_PRECISION): the residues of k-chunks could be added modulo m_l, but no BASELINE configuration needs it
- * and it is not built; Scheme I chunks k itself.
+ * k: one launch covers one INT32-safe accumulation range (k 128^2 < 2^31, i.e. k <= 130,944 padded columns; R7).
+ * A longer k is cut into equal chunks of at most that length: one GEMM launch per chunk, the output residues of the chunks
+ * are added modulo m_l (the residues of a sum are the sums of the residues) and ONE reconstruction follows; the
+ * workspace then holds a second set of output residue planes (emugemm_workspace_bytes accounts for it).  The bit budget
+ * T (emugemm_oz2_budget) is taken for the whole k.  The strided batched entry points run such entries one by one.
  * The FP64 CRT is exact: for every residue vector the reconstructed integer is rounded once (R17), so the
  * 2-ulp bound of (|A||B|)_ij holds for every finite input, not only for well-scaled ones.                       */
 int emugemm_dgemm_oz2(emugemm_handle_t h, int64_t m, int64_t n, int64_t k, double alpha,

@@ -293,6 +293,13 @@ static int run_oz1_batched(emugemm_ctx *h, int elem, int64_t batch, int64_t m, i
                         strideC * es);
 }
 
+// Output residue planes of a Scheme II call: [parts_out][N][m][n] INT8; a k beyond one INT32-safe range (kOz2MaxChunkK) is cut
+// into chunks whose output residues are added modulo m_l, which takes a second buffer of the same size right behind the first
+static size_t oz2_cr_elems(int parts_out, int N, int64_t m, int64_t n, int64_t kpad) {
+  const size_t one = granule(static_cast<size_t>(parts_out) * N * m * n);
+  return kpad > kOz2MaxChunkK ? 2 * one : one;
+}
+
 // Per-modulus GEMMs with fused reduction + CRT from residue planes (one-shot calls and pre-decomposed operands).
 static int oz2_gemm_phase(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_t kpad, int N, const int8_t *RA,
                           const int8_t *RB, int8_t *CR, const int32_t *eA, const int32_t *eB, int tA, int tB,
@@ -314,7 +321,7 @@ static int oz2_gemm_phase(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_
   const int64_t ctas = 2 * (tiles_out < h->num_sms / 2 ? tiles_out : h->num_sms / 2);
   // CR is the last region carved from the workspace by every caller: the scratch may use everything from there on
   const size_t avail = static_cast<size_t>((static_cast<const uint8_t *>(h->ws) + h->ws_bytes) - reinterpret_cast<const uint8_t *>(CR));
-  if (h->oz2_fusion && !is3m && !out_f32 && N >= 7 && static_cast<size_t>(ctas) * 2 * N * 32768 <= avail) {
+  if (h->oz2_fusion && !is3m && !out_f32 && N >= 7 && kpad <= kOz2MaxChunkK && static_cast<size_t>(ctas) * 2 * N * 32768 <= avail) {
     g.fused = &c;
     g.scratch_bytes = avail;
     EMU_TRY(launch_oz2_gemm(h, g));
@@ -322,7 +329,25 @@ static int oz2_gemm_phase(emugemm_ctx *h, int is3m, int64_t m, int64_t n, int64_
     EMU_TRY(mark(h, 3));
     return EMUGEMM_OK;
   }
-  EMU_TRY(launch_oz2_gemm(h, g));
+  if (kpad > kOz2MaxChunkK) {
+    // k-chunks of at most kOz2MaxChunkK columns (equalised): chunk 0 writes CR, every later chunk writes the second buffer
+    // and is added modulo m_l (the residues of a sum are the sums of the residues)
+    if (batch != 1) return EMUGEMM_ERR_ARG;  // the batched entry points run such entries one by one
+    const int parts_out = is3m ? 2 : 1;
+    const int nch = static_cast<int>((kpad + kOz2MaxChunkK - 1) / kOz2MaxChunkK);
+    const int64_t clen = round_up((kpad + nch - 1) / nch, kBlockK);
+    int8_t *CRtmp = CR + granule(static_cast<size_t>(parts_out) * N * m * n);
+    for (int64_t k0 = 0; k0 < kpad; k0 += clen) {
+      g.k0 = k0;
+      g.k1 = k0 + clen < kpad ? k0 + clen : kpad;
+      g.CR = k0 == 0 ? CR : CRtmp;
+      if (k0 > 0 && g.wave_ctr) EMU_CUDA(h, cudaMemsetAsync(g.wave_ctr, 0, sizeof(unsigned long long), h->stream));
+      EMU_TRY(launch_oz2_gemm(h, g));
+      if (k0 > 0) EMU_TRY(launch_oz2_residue_add(h, CR, CRtmp, N, parts_out * N, m * n));
+    }
+  } else {
+    EMU_TRY(launch_oz2_gemm(h, g));
+  }
   EMU_TRY(mark(h, 2));
   EMU_TRY(launch_oz2_crt(h, c));
   EMU_TRY(mark(h, 3));
@@ -345,8 +370,7 @@ static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t 
   }
   int tA, tB;
   if (oz2_budget_host(N, k, is3m, &tA, &tB) < 2) return EMUGEMM_ERR_PRECISION;
-  if (k > 131071) return EMUGEMM_ERR_PRECISION;  // INT32 accumulation bound k * 128^2 < 2^31 (R7)
-  const int64_t kpad = round_up(k, kBlockK);
+  const int64_t kpad = round_up(k, kBlockK);  // k beyond one INT32-safe range (R7) is chunked inside oz2_gemm_phase
   const int parts_in = is3m ? 3 : 1, parts_out = is3m ? 2 : 1;
   if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
   Carver cv(h->ws, h->ws_bytes);
@@ -357,7 +381,7 @@ static int run_oz2(emugemm_ctx *h, int ta, int tb, int is3m, int64_t m, int64_t 
   auto *eB = cv.take<int32_t>(n);
   auto *RA = cv.take<int8_t>(static_cast<size_t>(parts_in) * N * m * kpad);
   auto *RB = cv.take<int8_t>(static_cast<size_t>(parts_in) * N * n * kpad);
-  auto *CR = cv.take<int8_t>(static_cast<size_t>(parts_out) * N * m * n);
+  auto *CR = cv.take<int8_t>(oz2_cr_elems(parts_out, N, m, n, kpad));
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   h->diag = diag;
   h->nf_flag = diag + kDiagNonFinite;
@@ -389,7 +413,7 @@ static int run_oz2_batched(emugemm_ctx *h, int is3m, int f32, int64_t batch, int
     if (strideC < (m - 1) * ldc + n) return EMUGEMM_ERR_ARG;
     if (batch > 65535 || batch * m >= (1LL << 31) - 256 || batch * n >= (1LL << 31) - 256) return EMUGEMM_ERR_ARG;
   }
-  if (batch == 1 || k == 0) {
+  if (batch == 1 || k == 0 || round_up(k, kBlockK) > kOz2MaxChunkK) {  // k-chunked entries run one by one
     int launches = 0;
     for (int64_t b = 0; b < batch; ++b) {
       EMU_TRY(run_oz2(h, 0, 0, is3m, m, n, k, al, static_cast<const char *>(A) + b * strideA * es, lda,
@@ -402,7 +426,6 @@ static int run_oz2_batched(emugemm_ctx *h, int is3m, int f32, int64_t batch, int
   }
   int tA, tB;
   if (oz2_budget_host(N, k, is3m, &tA, &tB) < 2) return EMUGEMM_ERR_PRECISION;
-  if (k > 131071) return EMUGEMM_ERR_PRECISION;
   EMU_TRY(mark(h, 0));
   const int64_t kpad = round_up(k, kBlockK);
   if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
@@ -516,7 +539,7 @@ size_t emugemm_workspace_bytes(int scheme, int elem, int64_t m, int64_t n, int64
   } else if (scheme == EMUGEMM_OZ2 || scheme == EMUGEMM_OZ2_3M) {
     if (pn > kMaxModuli) return 0;
     const size_t pi = scheme == EMUGEMM_OZ2_3M ? 3 : 1, po = scheme == EMUGEMM_OZ2_3M ? 2 : 1;
-    total += granule(pi * pn * m * kpad) + granule(pi * pn * n * kpad) + granule(po * pn * m * n);
+    total += granule(pi * pn * m * kpad) + granule(pi * pn * n * kpad) + oz2_cr_elems(static_cast<int>(po), pn, m, n, kpad);
   } else {
     return 0;
   }
@@ -711,7 +734,7 @@ int emugemm_decompose(emugemm_handle_t h, int scheme, int role, int trans, int e
   int t_bits = 0;
   if (!oz1) {
     int tA, tB;
-    if (oz2_budget_host(pn, k, z3m, &tA, &tB) < 2 || k > 131071) return EMUGEMM_ERR_PRECISION;
+    if (oz2_budget_host(pn, k, z3m, &tA, &tB) < 2) return EMUGEMM_ERR_PRECISION;
     t_bits = role == 0 ? tA : tB;
   }
   const int64_t kpad = round_up(k, kBlockK);
@@ -765,7 +788,7 @@ int emugemm_gemm_pre(emugemm_handle_t h, const emugemm_operand_t *A, const emuge
                           clen, part, diag);
   }
   const int is3m = scheme == EMUGEMM_OZ2_3M;
-  auto *CR = cv.take<int8_t>(static_cast<size_t>(is3m ? 2 : 1) * pn * m * n);
+  auto *CR = cv.take<int8_t>(oz2_cr_elems(is3m ? 2 : 1, pn, m, n, kpad));
   if (!cv.ok) return EMUGEMM_ERR_WORKSPACE;
   h->diag = diag;
   h->nf_flag = diag + kDiagNonFinite;

@@ -138,12 +138,18 @@ struct Oz2GemmArgs {
   unsigned long long *cycles;  // as in Oz1GemmArgs
   unsigned long long *wave_ctr = nullptr;  // as in Oz1GemmArgs
   int batch = 1;               // strided batched call: residue planes hold batch * m (n) rows entry-major, CR is [N][batch][m][n]
+  int64_t k0 = 0, k1 = 0;      // k range [k0, k1) of this launch (multiples of kBlockK); k1 == 0: the whole kpad
   // Fused reconstruction (real product only): non-null = the kernel runs the CRT itself and writes C;
   // CR is then a scratch of scratch_bytes >= (CTAs launched) * N * 32 KB instead of the [N][m][n] planes.
   const Oz2CrtArgs *fused = nullptr;
   size_t scratch_bytes = 0;
 };
 int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &a);
+// Longest k one launch may cover: INT32 accumulators of symmetric INT8 residues, k 128^2 < 2^31 (R7), in k-blocks
+constexpr int64_t kOz2MaxChunkK = (131071 / kBlockK) * kBlockK;  // 130,944
+// CR[plane][i] = sym((CR[plane][i] + T[plane][i]) mod m_(plane mod N)) for `planes` planes of `plane_elems` residues each:
+// adds the output residues of one more k-chunk (Scheme II k-chunking: residues of chunks add modulo m_l)
+int launch_oz2_residue_add(emugemm_ctx *ctx, int8_t *CR, const int8_t *T, int n_moduli, int planes, int64_t plane_elems);
 
 struct Oz2CrtArgs {
   int64_t m, n;

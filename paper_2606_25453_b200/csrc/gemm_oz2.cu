@@ -41,7 +41,8 @@ constexpr int kOz2Smem = kOz2Stages * kOz2StageBytes + 1024 + 256;
 
 struct Oz2Dev {
   int64_t m, n;
-  int kblocks;
+  int kblocks;  // k-blocks of this launch, starting at k-block kb0 of the planes
+  int kb0;
   int mt, nt_tiles, n_moduli;
   int nbatch;  // strided batched call: entry b uses plane rows [b m, (b+1) m) / [b n, (b+1) n) and CR[l][b]
   int8_t *CR;
@@ -182,8 +183,8 @@ oz2_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
             if (cta == 0) mbar_arrive_expect_tx(&full[st], 2 * nkb * kOz2KbBytes);
             for (int i = 0; i < nkb; ++i) {
               uint8_t *dst = smem + st * kOz2StageBytes + i * kOz2KbBytes;
-              tma_load_3d_cg2(dst, &tmA, full_leader, (kb + i) * kBlockK, arow, plane);
-              tma_load_3d_cg2(dst + kAStageBytes, &tmB, full_leader, (kb + i) * kBlockK, brow, plane);
+              tma_load_3d_cg2(dst, &tmA, full_leader, (a.kb0 + kb + i) * kBlockK, arow, plane);
+              tma_load_3d_cg2(dst + kAStageBytes, &tmB, full_leader, (a.kb0 + kb + i) * kBlockK, brow, plane);
             }
             if (++st == kOz2Stages) { st = 0; ph ^= 1; }
           }
@@ -417,7 +418,10 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
   EMU_TRY(encode_planes_tmap(ctx, &tmB, g.RB, g.kpad, g.n * batch, static_cast<int64_t>(parts) * g.n_moduli, kOz2NT / 2, 1));
   Oz2Dev d;
   d.m = g.m; d.n = g.n;
-  d.kblocks = static_cast<int>(g.kpad / kBlockK);
+  const int64_t k0 = g.k1 > 0 ? g.k0 : 0, k1 = g.k1 > 0 ? g.k1 : g.kpad;
+  if (k0 < 0 || k1 > g.kpad || k0 >= k1 || (k0 % kBlockK) || (k1 % kBlockK) || k1 - k0 > kOz2MaxChunkK) return EMUGEMM_ERR_ARG;
+  d.kb0 = static_cast<int>(k0 / kBlockK);
+  d.kblocks = static_cast<int>((k1 - k0) / kBlockK);
   d.mt = static_cast<int>((g.m + kOz2PairM - 1) / kOz2PairM);  // pair tiles
   d.nt_tiles = static_cast<int>((g.n + kOz2NT - 1) / kOz2NT);
   d.n_moduli = g.n_moduli;
@@ -498,6 +502,39 @@ int launch_oz2_gemm(emugemm_ctx *ctx, const Oz2GemmArgs &g) {
   }
   // plain launch: a barrier wait that runs into its bound gives up (ptx.cuh), so co-residency is an optimisation only
   kern<<<grid, kGemmThreads, kOz2Smem, ctx->stream>>>(tmA, tmB, d, fz);
+  ctx->launches++;
+  EMU_CUDA(ctx, cudaGetLastError());
+  return EMUGEMM_OK;
+}
+
+// ---- Scheme II k-chunking: output residues of k-chunks add modulo m_l ---------------------------------------
+struct Oz2AddMod {
+  int mod[kMaxModuli];
+};
+__global__ void __launch_bounds__(256) oz2_residue_add_kernel(int8_t *__restrict__ CR, const int8_t *__restrict__ T, int n_moduli,
+                                                              int64_t plane_elems, const __grid_constant__ Oz2AddMod mk) {
+  const int plane = blockIdx.y;
+  const int m = mk.mod[plane % n_moduli], half = (m + 1) / 2;
+  int8_t *c = CR + static_cast<int64_t>(plane) * plane_elems;
+  const int8_t *t = T + static_cast<int64_t>(plane) * plane_elems;
+  for (int64_t i = static_cast<int64_t>(blockIdx.x) * 256 + threadIdx.x; i < plane_elems; i += static_cast<int64_t>(gridDim.x) * 256) {
+    int s = static_cast<int>(c[i]) + static_cast<int>(t[i]);  // both symmetric residues: |s| <= m
+    s += (s < 0) ? m : 0;                                     // [0, m]
+    s -= (s >= m) ? m : 0;                                    // [0, m)
+    s -= (s >= half) ? m : 0;                                 // [ceil(m/2) - m, ceil(m/2) - 1]  (R11, R13)
+    c[i] = static_cast<int8_t>(s);
+  }
+}
+
+int launch_oz2_residue_add(emugemm_ctx *ctx, int8_t *CR, const int8_t *T, int n_moduli, int planes, int64_t plane_elems) {
+  if (planes <= 0 || plane_elems <= 0) return EMUGEMM_OK;
+  Oz2AddMod mk;
+  int mod[24];
+  oz2_moduli_host(n_moduli, mod);
+  for (int l = 0; l < kMaxModuli; ++l) mk.mod[l] = l < n_moduli ? mod[l] : 256;
+  int64_t gx = (plane_elems + 255) / 256;
+  if (gx > 4096) gx = 4096;
+  oz2_residue_add_kernel<<<dim3(static_cast<unsigned>(gx), static_cast<unsigned>(planes)), 256, 0, ctx->stream>>>(CR, T, n_moduli, plane_elems, mk);
   ctx->launches++;
   EMU_CUDA(ctx, cudaGetLastError());
   return EMUGEMM_OK;

@@ -333,3 +333,39 @@ def test_dgemm_oz2_fused_adversarial_and_strided(env):
     _, absAB = O.bf128_dgemm(A, B)
     assert_within_ulps(Cd[:, :n].cpu().numpy(), O.dgemm_oz2(A, B, N), absAB, 2, what="fused adversarial")
     assert (Cd[:, n:] == 7.0).all()
+
+
+# ---- k beyond one INT32-safe range (k 128^2 < 2^31): one GEMM launch per k-chunk, output residues added modulo m_l ----------
+@pytest.mark.parametrize("N,shape", [(12, (48, 40, 133000)), (16, (130, 70, 131072)), (20, (33, 17, 270001))])
+def test_dgemm_oz2_k_chunked(env, N, shape):
+    """k > 130,944: 2 chunks (133,000; 131,072 = one k-block over the limit) and 3 chunks (270,001, ragged), against the
+    oracle, whose per-modulus products accumulate in int64 over the whole k."""
+    torch, O, h, E = env
+    m, n, k = shape
+    A, B = G.real_pair(m, n, k, 1.0, 12)
+    C = torch.full((m, n), float("nan"), dtype=torch.float64, device="cuda")
+    h.dgemm_oz2(dev(torch, A), dev(torch, B), C, N, alpha=1.5)
+    absAB = np.abs(A) @ np.abs(B)
+    assert_within_ulps(C.cpu().numpy(), O.dgemm_oz2(A, B, N, alpha=1.5), 1.5 * absAB, 2, what=f"oz2 k={k} N={N}")
+
+
+def test_zgemm_oz2_3m_k_chunked_and_operand_handles(env):
+    torch, O, h, E = env
+    m, n, k, N = 40, 24, 131500, 14
+    A, B = G.complex_pair(m, n, k, 1.0, 13)
+    C = torch.zeros((m, n), dtype=torch.complex128, device="cuda")
+    h.zgemm_oz2_3m(dev(torch, A), dev(torch, B), C, N)
+    want = O.zgemm_oz2_3m(A, B, N)
+    absZ = (np.abs(A.real) + np.abs(A.imag)) @ (np.abs(B.real) + np.abs(B.imag))
+    got = C.cpu().numpy()
+    assert_within_ulps(got.real, want.real, absZ, 2, what="3M chunked re")
+    assert_within_ulps(got.imag, want.imag, absZ, 2, what="3M chunked im")
+    # pre-decomposed operands take the same chunked path and give the same bits
+    Ar, Br = G.real_pair(m, n, k, 1.0, 14)
+    C1 = torch.empty((m, n), dtype=torch.float64, device="cuda")
+    C2 = torch.empty_like(C1)
+    h.dgemm_oz2(dev(torch, Ar), dev(torch, Br), C1, 15)
+    opA = h.decompose(E.OZ2, 0, dev(torch, Ar), 15)
+    opB = h.decompose(E.OZ2, 1, dev(torch, Br), 15)
+    h.gemm_pre(opA, opB, C2)
+    assert torch.equal(C1, C2)
