@@ -525,8 +525,15 @@ size_t emugemm_workspace_bytes(int scheme, int elem, int64_t m, int64_t n, int64
     if (pn > 8 || (elem != 4 && elem != 8)) return 0;
     total += granule(static_cast<size_t>(pn) * m * kpad) + granule(static_cast<size_t>(pn) * n * kpad);
     int64_t clen;
-    int nch = oz1_chunks(pn, 8, kpad, 0, &clen);  // the 8-bit mode has the shorter chunks: size for it
-    if (oz1_chunks_may_balance(nch, oz1_cluster_tiles_host(pn, m, n))) nch *= 2;  // room for the balanced split (few tiles: small)
+    // upper bound of the chunk count over both digit modes (the 8-bit mode has the shorter chunks), with room for the
+    // balanced split where it may apply (few tiles: the partials are small)
+    const int64_t tiles = oz1_cluster_tiles_host(pn, m, n);
+    int nch = 1;
+    for (int bits = 7; bits <= 8; ++bits) {
+      const int nb = oz1_chunks(pn, bits, kpad, 0, &clen);
+      const int ub = oz1_chunks_may_balance(nb, tiles) ? 2 * nb : nb;
+      if (ub > nch) nch = ub;
+    }
     if (nch > 1) total += granule(static_cast<size_t>(nch) * m * n * 16);
   } else if (scheme == EMUGEMM_OZ1_4M) {
     if (pn > 8 || elem != 16) return 0;

@@ -200,3 +200,27 @@ def test_dgemm_oz1_extreme_exponents(env):
         if (~tiny).any():
             assert_within_ulps(got[~tiny], want[~tiny], scale[~tiny], 2, what=f"scales {sa} {sb}")
         assert (np.abs(got[tiny] - want[tiny]) <= 2 * 2.0 ** -1074).all()   # subnormal range: two subnormal spacings
+
+
+@pytest.mark.parametrize("bits", [7, 8])
+@pytest.mark.parametrize("p,shape", [(8, (40, 24, 34000)), (7, (130, 70, 39000)), (3, (64, 48, 90000)), (8, (256, 200, 17000))])
+def test_dgemm_oz1_balanced_chunks_fit_the_declared_workspace(env, bits, p, shape):
+    """Long k on few tiles: the chunk count is balanced against the worker count (api.cu oz1_chunks_balanced, up to twice
+    the overflow-safe minimum).  A FRESH handle reserves exactly emugemm_workspace_bytes(), so the call fails with
+    EMUGEMM_ERR_WORKSPACE if the declared size does not cover the chunk count the call picks in either digit mode; the
+    result must not depend on the split (exact double-double partials)."""
+    torch, O, _ = env
+    import paper_2606_25453_b200 as E
+    m, n, k = shape
+    A, B = G.real_pair(m, n, k, 1.0, 21)
+    h = E.EmuGemm()
+    try:
+        h.set_slice_bits(bits)
+        O.set_slice_bits(bits)
+        C = torch.zeros((m, n), dtype=torch.float64, device="cuda")
+        h.dgemm_oz1(dev(torch, A), dev(torch, B), C, p)
+        want = O.dgemm_oz1(A, B, p)
+    finally:
+        O.set_slice_bits(7)
+        h.close()
+    assert_within_ulps(C.cpu().numpy(), want, np.abs(A) @ np.abs(B), 2, what=f"balanced chunks p={p} bits={bits}")
