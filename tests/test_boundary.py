@@ -59,3 +59,25 @@ def test_workspace_bytes_monotone():
     d = lib.emugemm_workspace_bytes(3, 16, 1024, 1024, 1024, 16)
     assert 0 < a < b and c > 0 and d > c
     assert lib.emugemm_workspace_bytes(1, 8, 1024, 1024, 1024, 9) == 0
+
+
+def test_static_limit_and_chunked_workspace_sizes():
+    """Host-only sizing rules: the static-array limit of emugemm_dgemm_oz1_static, the room for balanced Scheme I
+    k-chunks (few tiles, long k) and the second output-residue buffer of a k-chunked Scheme II call."""
+    lib = E.load_library()
+    lib.emugemm_static_workspace_limit.restype = ctypes.c_size_t
+    assert lib.emugemm_static_workspace_limit() == 32 << 20
+    assert lib.emugemm_workspace_bytes(1, 8, 1024, 1024, 1024, 8) <= 32 << 20 < lib.emugemm_workspace_bytes(1, 8, 1024, 1024, 2176, 8)
+    planes = 2 * 7 * 1024 * 65536
+    # 1024 x 1024 x 65536, p = 7: both digit modes need 4 overflow-safe chunks (18,944 / 18,688 columns), balanced up to 8
+    # partial buffers of 16 MB
+    ws = lib.emugemm_workspace_bytes(1, 8, 1024, 1024, 65536, 7)
+    assert planes + 8 * 1024 * 1024 * 16 <= ws <= planes + 8 * 1024 * 1024 * 16 + (1 << 20)
+    # many tiles: no balancing, the partials stay at the minimum count (p = 8, 8-bit mode: ceil(65536 / 16256) = 5)
+    ws_big = lib.emugemm_workspace_bytes(1, 8, 8192, 8192, 65536, 8)
+    assert ws_big <= 2 * 8 * 8192 * 65536 + 5 * 8192 * 8192 * 16 + (1 << 20)
+    # Scheme II: one set of output residue planes up to k = 130,944, two beyond
+    one = lib.emugemm_workspace_bytes(2, 8, 256, 256, 130944, 16) - 2 * 16 * 256 * 130944
+    two = lib.emugemm_workspace_bytes(2, 8, 256, 256, 131072, 16) - 2 * 16 * 256 * 131072
+    assert 16 * 256 * 256 <= one < 16 * 256 * 256 + (1 << 16)
+    assert 2 * 16 * 256 * 256 <= two < 2 * 16 * 256 * 256 + (1 << 16)
