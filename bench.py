@@ -424,9 +424,13 @@ def main():
                "d2h_bytes_per_step": int(hC.numel() * hC.element_size())}
         del bufA, bufB, bufC, hC2
 
+    # every collective is done: all ranks leave the process group together (rank 0 goes on alone with the probe leg and the
+    # CPU oracle, which take tens of seconds; the other ranks must not sit in a half-torn-down group meanwhile)
+    if dist is not None:
+        barrier()
+        dist.destroy_process_group()
+        dist = None
     if rank != 0:
-        if dist is not None:
-            dist.destroy_process_group()
         return
 
     # ---- roofline of the dominant kernel (the fused tensor-core GEMM), measured live ----
