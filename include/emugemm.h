@@ -351,8 +351,13 @@ int emugemm_dbg_oz1_issue_probe(emugemm_handle_t h, int p, int use_collector, in
  * the one-CTA N-concatenated kernel instead of the CTA-pair kernel, bit 4 = Scheme I
  * with p >= 4 runs without the 2-CTA multicast of A (A/B timing), bit 5 = the Scheme I
  * row pre-pass runs its two-phase form (row re-read) instead of the register-resident
- * single-read kernel.
- * Used to attribute tensor-pipe idle time.                        */
+ * single-read kernel; 0x40 = every CTA loads tile (0, 0) (no DRAM traffic, same L2 -> SM traffic), 0x80 = no serpentine k,
+ * 0xFF00 = rasterisation group override, 0x10000 = wave barrier off, 0x20000 / 0x40000 = wave barrier forced on
+ * (Scheme II real / Scheme I), 0x80000 / 0x100000 = fused Scheme II without the CRT arithmetic / the scratch loads,
+ * 0x200000 / 0x400000 / 0x800000 = L2 eviction hints A EVICT_LAST / B EVICT_FIRST / B EVICT_LAST (results stay right),
+ * 0x0F000000 = wave-barrier lead 2 (v - 1) k-blocks, 0x20000000 = set the device's persisting-L2 carve-out to its maximum
+ * (device-wide and sticky: probe processes only).
+ * Used to attribute tensor-pipe idle time and DRAM traffic (profiles/r2_wave_barrier.md).                  */
 int emugemm_dbg_set_flags(emugemm_handle_t h, int flags);
 
 #endif /* EMUGEMM_PROBES */

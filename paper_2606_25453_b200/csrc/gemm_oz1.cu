@@ -645,6 +645,19 @@ static int launch_pp(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
   }
   if (g.out_kind == 1 && P > 4) return EMUGEMM_ERR_ARG;
   EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, Cfg::kSmemBytes));
+#ifdef EMUGEMM_PROBES
+  // probe 0x20000000: give the L2 a persisting carve-out (with 0x200000 = A EVICT_LAST) -- does the hint need one?
+  if (ctx->dbg_flags & 0x20000000) {
+    int maxp = 0, dev = 0;
+    cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&maxp, cudaDevAttrMaxPersistingL2CacheSize, dev);
+    size_t want = static_cast<size_t>(80) << 20;
+    if (want > static_cast<size_t>(maxp)) want = static_cast<size_t>(maxp);
+    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, want);
+    static bool said = false;
+    if (!said) { printf("emugemm probe: persisting L2 max %d bytes, set %zu\n", maxp, want); said = true; }
+  }
+#endif
   cudaLaunchConfig_t cfg = {};
   cfg.gridDim = dim3(static_cast<unsigned>(grid));
   cfg.blockDim = dim3(kGemmThreads);
