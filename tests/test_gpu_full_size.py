@@ -196,3 +196,63 @@ def test_output_residues_3m_4096(env):
     del out
     want = O.oz2_modprod_3m(np.ascontiguousarray(RA3[:, :, rows]), np.ascontiguousarray(RB3[:, :, cols]))
     assert np.array_equal(got, want)
+
+
+# ---- SURVEY 8(f) features at the sizes bench.py's `detail` legs run them ----------------------------------------
+def test_8bit_digits_p7_8192(env):
+    """R23: balanced base-256 digits, p = 7 at 8192^3 (bench detail f1), sampled against the oracle's 8-bit mode."""
+    torch, O, _ = env
+    import paper_2606_25453_b200 as E
+    size, p = 8192, 7
+    A, B = G.real_pair(size, size, size, 0.5, 1)
+    h = E.EmuGemm()
+    try:
+        h.set_slice_bits(8)
+        O.set_slice_bits(8)
+        C = torch.full((size, size), float("nan"), dtype=torch.float64, device="cuda")
+        h.dgemm_oz1(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, p)
+        rows, cols = _samples(size, size, 23)
+        got = C[torch.from_numpy(rows).cuda()][:, torch.from_numpy(cols).cuda()].cpu().numpy()
+        want = O.oz1_sampled(A, B, p, rows, cols)
+    finally:
+        O.set_slice_bits(7)
+        h.close()
+    assert_within_ulps(got, want, _abs_ab(A, B, rows, cols), 2, what="8-bit digits p=7 8192")
+    assert torch.isfinite(C).all()
+
+
+def test_strided_batched_64x512_p8(env):
+    """64 products of 512^3 through ONE fused launch (bench detail f2); every entry sampled."""
+    torch, O, h = env
+    batch, s, p = 64, 512, 8
+    rng = np.random.default_rng(31)
+    A = (rng.random((batch, s, s)) - 0.5) * np.exp(0.5 * rng.standard_normal((batch, s, s)))
+    B = (rng.random((batch, s, s)) - 0.5) * np.exp(0.5 * rng.standard_normal((batch, s, s)))
+    C = torch.full((batch, s, s), float("nan"), dtype=torch.float64, device="cuda")
+    h.dgemm_oz1_strided_batched(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, p)
+    rows, cols = _samples(s, s, 29, count=8)
+    Cs = C[:, torch.from_numpy(rows).cuda()][:, :, torch.from_numpy(cols).cuda()].cpu().numpy()
+    for b in range(batch):
+        want = O.oz1_sampled(A[b], B[b], p, rows, cols)
+        assert_within_ulps(Cs[b], want, _abs_ab(A[b], B[b], rows, cols), 2, what=f"batched entry {b}")
+    assert torch.isfinite(C).all()
+
+
+def test_zgemm_4m_2048_p8(env):
+    """Scheme I complex by 4M at 2048^3, p = 8: sampled against the oracle's real products of the embedding
+    (re = Re A Re B - Im A Im B as ONE sliced product of [Re A, -Im A] [Re B; Im B], likewise im: oracle_zgemm_oz1_4m's definition)."""
+    torch, O, h = env
+    size, p = 2048, 8
+    A, B = G.complex_pair(size, size, size, 1.0, 3)
+    C = torch.zeros((size, size), dtype=torch.complex128, device="cuda")
+    h.zgemm_oz1_4m(torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda(), C, p)
+    rows, cols = _samples(size, size, 37, count=12)
+    got = C[torch.from_numpy(rows).cuda()][:, torch.from_numpy(cols).cuda()].cpu().numpy()
+    # the real embedding (DESIGN.md 1): A' = [[Re A, -Im A], [Im A, Re A]] (2m x 2k), B' = [[Re B], [Im B]] (2k x n)
+    Ae = np.block([[A.real, -A.imag], [A.imag, A.real]])
+    Be = np.vstack([B.real, B.imag])
+    want_re = O.oz1_sampled(Ae, Be, p, rows, cols)
+    want_im = O.oz1_sampled(Ae, Be, p, rows + size, cols)
+    scale = (np.abs(A.real[rows]) + np.abs(A.imag[rows])) @ (np.abs(B.real[:, cols]) + np.abs(B.imag[:, cols]))
+    assert_within_ulps(got.real, want_re, scale, 2, what="4M re")
+    assert_within_ulps(got.imag, want_im, scale, 2, what="4M im")
