@@ -49,6 +49,9 @@ def parse():
                          "emugemm_dbg_set_flags bits (include/emugemm.h), e.g. 0x10000 = no wave barrier")
     ap.add_argument("--oracle-table", action="store_true",
                     help="with --impl reference: time the oracle IN FULL on 1024^3 instances of every config family (BASELINE.md 3)")
+    ap.add_argument("--inputs", default="eq19", choices=["eq19", "nonneg", "a_nonneg", "ones"],
+                    help="eq19 (default): the paper's signed distribution; nonneg: |A|, |B| of the same draw; a_nonneg: |A|, B; ones: all ones -- "
+                         "power experiments only (operand sign bits cost clock under the power cap, profiles/r2_operand_sign_power.md)")
     ap.add_argument("--fusion", action="store_true", help="Scheme II: fused reconstruction inside the GEMM kernel (default: separate CRT kernel)")
     return ap.parse_args()
 
@@ -85,6 +88,12 @@ def make_inputs(a, w, seed_offset=0):
     else:
         A, B = G.real_pair(w["m"], w["n"], w["k"], w["phi"], w["seed"] + seed_offset,
                            dtype=np.float32 if a.scheme == "oz1s" else np.float64)
+    if a.inputs == "nonneg":   # same magnitudes, no sign bits (complex: both parts)
+        A, B = (np.abs(A.real) + 1j * np.abs(A.imag), np.abs(B.real) + 1j * np.abs(B.imag)) if a.scheme == "oz2z" else (np.abs(A), np.abs(B))
+    elif a.inputs == "a_nonneg" and a.scheme != "oz2z":
+        A = np.abs(A)
+    elif a.inputs == "ones":
+        A, B = np.ones_like(A), np.ones_like(B)
     return A, B
 
 
@@ -538,7 +547,7 @@ def main():
             "value_at_median": w["flops"] / (ms_median * 1e-3) / 1e12,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "int8", "data": "synthetic",
-            "config": {"workload": w["name"], "phi": w["phi"], "seed": w["seed"], "alpha": 1, "beta": 0, "slice_bits": a.slice_bits, "probe_flags": hex(a.probe_flags), "oz2_fusion": bool(a.fusion),
+            "config": {"workload": w["name"] + ("" if a.inputs == "eq19" else f" [inputs: {a.inputs}]"), "phi": w["phi"], "seed": w["seed"], "alpha": 1, "beta": 0, "slice_bits": a.slice_bits, "probe_flags": hex(a.probe_flags), "oz2_fusion": bool(a.fusion), "inputs": a.inputs,
                        "l2": "inputs (A, B, slices > 1 GB) exceed the 126 MB L2, no flush needed",
                        "parallelism": f"{world} independent problems" if world > 1 else "1 GPU"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "detail": detail}

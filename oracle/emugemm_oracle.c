@@ -50,7 +50,10 @@
  * unsigned remaining slices; the balanced form keeps one signedness).  Two guard bits: x = a 2^-(e+2) in
  * (-1/4, 1/4) so that X + sum_j 128 256^j stays inside [0, 256^p). */
 static int g_slice_bits = 7;
-void oracle_set_slice_bits(int bits) { g_slice_bits = (bits == 8) ? 8 : 7; }
+/* 7: sign-magnitude 7-bit digits (R1, default); 8: balanced base-256 digits (R23); 0x107: two's-complement 7-bit
+ * digits -- signed leading slice, non-negative remaining slices (R24; the slice form of PAPER.md:345 at beta = 7) */
+#define ORACLE_DIGITS_TWOS 0x107
+void oracle_set_slice_bits(int bits) { g_slice_bits = (bits == 8) ? 8 : (bits == ORACLE_DIGITS_TWOS) ? ORACLE_DIGITS_TWOS : 7; }
 int oracle_get_slice_bits(void) { return g_slice_bits; }
 #define ORACLE_MAX_MODULI 24
 
@@ -152,8 +155,26 @@ static void slice_one_balanced(double a, int e, int p, int8_t *digits /* [p] */)
   for (int t = 0; t < p; ++t) digits[t] = (int8_t)((int)((Y >> (8 * (p - 1 - t))) & 255u) - 128);
 }
 
+/* R24 ("a signed leading slice with unsigned remaining slices", here with beta = 7 so that every slice is
+ * an INT8 value): the SAME integer as R1, X = trunc(a 2^(beta p - e)) toward zero, |X| < 2^(beta p), written in two's
+ * complement: d_0 = floor(X / 2^(beta (p-1))) in [-128, 127], d_t = floor(X / 2^(beta (p-1-t))) mod 2^beta in [0, 127]
+ * for t >= 1, so that sum_t d_t 2^(beta (p-1-t)) == X exactly. */
+static void slice_one_twos(double a, int e, int p, int8_t *digits /* [p] */) {
+  __float128 sc = scalbnq((__float128)a, ORACLE_BETA * p - e);
+  int64_t X = (int64_t)truncq(sc); /* |X| < 2^56 */
+  for (int t = 0; t < p; ++t) {
+    const int sh = ORACLE_BETA * (p - 1 - t);
+    /* floor division by a power of two of a possibly negative X, written out (no reliance on >> of negatives) */
+    int64_t q = X / ((int64_t)1 << sh);
+    if (X % ((int64_t)1 << sh) < 0) q -= 1;
+    if (t == 0) digits[t] = (int8_t)q;                      /* in [-128, 127] */
+    else digits[t] = (int8_t)(((q % 128) + 128) % 128);     /* in [0, 127] */
+  }
+}
+
 static void slice_one(double a, int e, int p, int8_t *digits /* [p] */) {
   if (g_slice_bits == 8) { slice_one_balanced(a, e, p, digits); return; }
+  if (g_slice_bits == ORACLE_DIGITS_TWOS) { slice_one_twos(a, e, p, digits); return; }
   /* |a| * 2^(beta p - e): a power-of-two scaling, exact in __float128. */
   __float128 sc = scalbnq(fabsq((__float128)a), ORACLE_BETA * p - e);
   uint64_t X = (uint64_t)truncq(sc); /* X < 2^(beta p) <= 2^56 */

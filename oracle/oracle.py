@@ -35,8 +35,12 @@ def set_threads(t):
 
 
 # ---------------------------------------------------------------- exponents
+DIGITS_TWOS = 0x107
+
+
 def set_slice_bits(bits):
-    """7 (default, R1): sign-magnitude 7-bit digits; 8: balanced signed base-256 digits (R23)."""
+    """7 (default, R1): sign-magnitude 7-bit digits; 8: balanced signed base-256 digits (R23); DIGITS_TWOS (0x107, R24):
+    two's-complement 7-bit digits, signed leading slice and non-negative remaining slices (PAPER.md:345 at beta = 7)."""
     _lib.oracle_set_slice_bits(C.c_int(bits))
 
 

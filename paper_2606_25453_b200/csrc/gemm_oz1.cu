@@ -66,7 +66,8 @@ struct Oz1Cfg {
 // MMAs of slice t for one 128-byte k-block: A_t x [B_0 | ... | B_{P-1-t}] -> TMEM columns [t NT, P NT), split at 256
 // columns, four k32 sub-blocks.  `accumulate` = false only for the very first MMAs of a tile (t = 0, ks = 0).
 template <int P, bool COLL>
-__device__ __forceinline__ void oz1_issue_slice(int t, uint32_t tmem_base, uint32_t a_base, uint32_t b_base, bool accumulate) {
+__device__ __forceinline__ void oz1_issue_slice(int t, uint32_t tmem_base, uint32_t a_base, uint32_t b_base, bool accumulate,
+                                                uint32_t imask = ~0u /* probes: clears the operand signedness bits */) {
   constexpr int NT = Oz1Cfg<P>::NT;
   // (P - t) NT columns: one MMA if <= 256, else two of near-equal width (multiples of 16).  An even split keeps
   // both above the ~112-column width below which an MMA is bound by its fixed cost (256 + 32 at p = 5, t = 2 would
@@ -82,16 +83,16 @@ __device__ __forceinline__ void oz1_issue_slice(int t, uint32_t tmem_base, uint3
     const uint32_t d = tmem_base + t * NT;
     const uint64_t bdesc0 = sdesc_from_lo(b_lo + ((ks * 32) >> 4));
     if (n1 == 0) {
-      umma_i8<0>(d, adesc, bdesc0, make_idesc_i8(kTileM, n0), acc);
+      umma_i8<0>(d, adesc, bdesc0, make_idesc_i8(kTileM, n0) & imask, acc);
     } else {
       // the two MMAs share A_t: the first keeps it in the collector, the second drops it
       const uint64_t bdesc1 = sdesc_from_lo(b_lo + ((n0 * kBlockK + ks * 32) >> 4));
       if (COLL) {
-        umma_i8<1>(d, adesc, bdesc0, make_idesc_i8(kTileM, n0), acc);
-        umma_i8<3>(d + n0, adesc, bdesc1, make_idesc_i8(kTileM, n1), acc);
+        umma_i8<1>(d, adesc, bdesc0, make_idesc_i8(kTileM, n0) & imask, acc);
+        umma_i8<3>(d + n0, adesc, bdesc1, make_idesc_i8(kTileM, n1) & imask, acc);
       } else {
-        umma_i8<0>(d, adesc, bdesc0, make_idesc_i8(kTileM, n0), acc);
-        umma_i8<0>(d + n0, adesc, bdesc1, make_idesc_i8(kTileM, n1), acc);
+        umma_i8<0>(d, adesc, bdesc0, make_idesc_i8(kTileM, n0) & imask, acc);
+        umma_i8<0>(d + n0, adesc, bdesc1, make_idesc_i8(kTileM, n1) & imask, acc);
       }
     }
   }
@@ -489,8 +490,11 @@ oz1_gemm_kernel(const __grid_constant__ CUtensorMap tmA, const __grid_constant__
               if (hi != lo) oz1_issue_slice_pair<P>(hi, tmem_base, a_base + kAStageBytes, b_base, true);
               umma_commit_cg2(&aempty[sa_cur], 3);  // both CTAs' stages reusable once these MMAs have read them
             } else {
-              oz1_issue_slice<P, kUseCollector>(lo, tmem_base, a_base, b_base, kb != kb0 || lo != 0);
-              if (hi != lo) oz1_issue_slice<P, kUseCollector>(hi, tmem_base, a_base + kAStageBytes, b_base, true);
+              // probes build, 0x40000000: the MMAs treat both operands as UNSIGNED bytes (results wrong): all products
+              // non-negative, same bytes -- what operand / accumulator signs cost in clock under the power cap
+              const uint32_t imask = EMU_PROBE_FLAG(a.dbg, 0x40000000) ? ~((1u << 7) | (1u << 10)) : ~0u;
+              oz1_issue_slice<P, kUseCollector>(lo, tmem_base, a_base, b_base, kb != kb0 || lo != 0, imask);
+              if (hi != lo) oz1_issue_slice<P, kUseCollector>(hi, tmem_base, a_base + kAStageBytes, b_base, true, imask);
               if constexpr (MC) umma_commit_mc(&aempty[sa_cur], 3);  // both CTAs must be done before either refills
               else umma_commit(&aempty[sa_cur]);                     // stage reusable once these MMAs have read it
             }
