@@ -40,6 +40,8 @@ def parse():
     ap.add_argument("--p", type=int, default=0, help="slices (oz1) or moduli (oz2); default 8 / 16")
     ap.add_argument("--phi", type=float, default=-1.0)
     ap.add_argument("--slice-bits", type=int, default=7, choices=[7, 8], help="Scheme I digit width (8: balanced base 256, DESIGN.md R23)")
+    ap.add_argument("--slice-form", type=int, default=0, choices=[0, 1],
+                    help="7-bit Scheme I digits: 0 = sign-magnitude (R1, default), 1 = two's-complement fields (R24, PAPER.md:345)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-probe", action="store_true")
@@ -306,6 +308,8 @@ def main():
     stream = torch.cuda.current_stream()
     h.set_stream(stream)
     h.set_slice_bits(a.slice_bits)
+    if a.slice_form:
+        h.set_slice_form(a.slice_form)
     if a.probe_flags:
         h.dbg_set_flags(a.probe_flags)
     if a.fusion:
@@ -547,7 +551,7 @@ def main():
             "value_at_median": w["flops"] / (ms_median * 1e-3) / 1e12,
             "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
             "dtype": "int8", "data": "synthetic",
-            "config": {"workload": w["name"] + ("" if a.inputs == "eq19" else f" [inputs: {a.inputs}]"), "phi": w["phi"], "seed": w["seed"], "alpha": 1, "beta": 0, "slice_bits": a.slice_bits, "probe_flags": hex(a.probe_flags), "oz2_fusion": bool(a.fusion), "inputs": a.inputs,
+            "config": {"workload": w["name"] + ("" if a.inputs == "eq19" else f" [inputs: {a.inputs}]"), "phi": w["phi"], "seed": w["seed"], "alpha": 1, "beta": 0, "slice_bits": a.slice_bits, "slice_form": a.slice_form, "probe_flags": hex(a.probe_flags), "oz2_fusion": bool(a.fusion), "inputs": a.inputs,
                        "l2": "inputs (A, B, slices > 1 GB) exceed the 126 MB L2, no flush needed",
                        "parallelism": f"{world} independent problems" if world > 1 else "1 GPU"},
             "clocks": clocks, "e2e": e2e, "gpu_launches": launches, "roofline": roof, "detail": detail}

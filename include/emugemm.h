@@ -64,6 +64,16 @@ int emugemm_set_workspace(emugemm_handle_t h, void *dev_ptr, size_t bytes);
  * column exponent -- 8p - 2 bits per operand, so p = 7 reaches the accuracy of p = 8 at 7 bits
  * with 28 instead of 36 slice products.  Applies to dgemm_oz1, sgemm_oz1 and the Scheme I hooks. */
 int emugemm_set_slice_bits(emugemm_handle_t h, int bits);
+/* Digit FORM of the 7-bit Scheme I slices of this handle (real calls: emugemm_{d,s}gemm_oz1[_t|_strided_batched], operand
+ * handles; the 4M complex calls return EMUGEMM_ERR_ARG in form 1).
+ *   0 (default; R1): sign-magnitude digits, d_t = sign(x) * (7-bit field of |X|), all in [-127, 127].
+ *   1 (R24; "a signed leading slice with unsigned remaining slices", at beta = 7 so that every slice is
+ *     an INT8 value): the two's-complement fields of the SAME integer X = trunc(x 2^(7p)): d_0 in [-128, 127], d_t in [0, 127]
+ *     for t >= 1.  Same accuracy class, same kernels, same weights; the results differ from form 0 only through the dropped
+ *     slice pairs (t + u >= p).  Seven of eight slices carry no sign bits, which the tensor pipe rewards with a higher clock
+ *     under the power cap (profiles/r2_operand_sign_power.md).  Overflow-safe chunk: emugemm_oz1_chunk_k_bits(p, 0x107).
+ * Call after emugemm_set_slice_bits (which resets the form to 0); form 1 needs 7-bit digits (else EMUGEMM_ERR_ARG).          */
+int emugemm_set_slice_form(emugemm_handle_t h, int form);
 /* Scheme II real FP64 product (emugemm_dgemm_oz2 and its _t / strided-batched / pre-decomposed forms), SURVEY 8(f) item 4
  * (the paper keeps the CRT separate and pays the residue workspace): on = 1 runs the reconstruction
  * INSIDE the per-modulus GEMM kernel -- a work item is an output tile, the moduli are the inner loop, the tile's

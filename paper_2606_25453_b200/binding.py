@@ -131,6 +131,11 @@ class EmuGemm:
         self._check(self._lib.emugemm_set_slice_bits(self._h, _int(bits)))
         self.slice_bits = bits
 
+    def set_slice_form(self, form):
+        """7-bit Scheme I digits: 0 = sign-magnitude (default, R1), 1 = two's-complement fields (R24; include/emugemm.h)."""
+        self._check(self._lib.emugemm_set_slice_form(self._h, _int(form)))
+        self.slice_bits = 0x107 if form else 7
+
     def set_oz2_fusion(self, on):
         """Scheme II real DGEMM: fused reconstruction inside the GEMM kernel, or (default) the separate CRT kernel."""
         self._check(self._lib.emugemm_set_oz2_fusion(self._h, _int(1 if on else 0)))

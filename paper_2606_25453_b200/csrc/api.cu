@@ -500,6 +500,13 @@ int emugemm_set_slice_bits(emugemm_handle_t h, int bits) {
   return EMUGEMM_OK;
 }
 
+int emugemm_set_slice_form(emugemm_handle_t h, int form) {
+  if (!h || (form & ~1)) return EMUGEMM_ERR_ARG;
+  if (form && (h->slice_bits & 0xFF) != 7) return EMUGEMM_ERR_ARG;  // the two's-complement form exists for 7-bit digits
+  h->slice_bits = form ? kDigitsTwos : (h->slice_bits & 0xFF);
+  return EMUGEMM_OK;
+}
+
 int emugemm_set_oz2_fusion(emugemm_handle_t h, int on) {
   if (!h || (on & ~1)) return EMUGEMM_ERR_ARG;
   h->oz2_fusion = on;
@@ -586,6 +593,7 @@ static int run_oz1_4m(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k,
   }
   const int64_t kpad = round_up(k, kBlockK), kk = 2 * kpad, mm = 2 * m;
   const int bits = h->slice_bits;
+  if (bits == kDigitsTwos) return EMUGEMM_ERR_ARG;  // the two's-complement digit form (R24) covers the real Scheme I calls
   int64_t clen;
   const int nch = oz1_chunks(p, bits, kk, 0, &clen);
   if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
@@ -937,7 +945,7 @@ int emugemm_dbg_crt_constants(int n_moduli, int *n_pairs, int *n_digits, int *di
 
 int64_t emugemm_oz1_chunk_k(int p) { return (p >= 1 && p <= 8) ? oz1_chunk_k_host(p, 7) : 0; }
 int64_t emugemm_oz1_chunk_k_bits(int p, int slice_bits) {
-  return (p >= 1 && p <= 8 && (slice_bits == 7 || slice_bits == 8)) ? oz1_chunk_k_host(p, slice_bits) : 0;
+  return (p >= 1 && p <= 8 && (slice_bits == 7 || slice_bits == 8 || slice_bits == kDigitsTwos)) ? oz1_chunk_k_host(p, slice_bits) : 0;
 }
 
 #ifdef EMUGEMM_PROBES

@@ -13,6 +13,9 @@ namespace emu {
 
 constexpr int kBeta = 7;          // bits per signed slice (R1)
 constexpr int kMaxModuli = 20;    // API range of n_moduli
+// Scheme I digit formats as carried in slice_bits: 7 = sign-magnitude (R1), 8 = balanced base 256 (R23), kDigitsTwos = 7-bit
+// two's-complement fields (R24): low byte = bits per slice, bit 8 = the form
+constexpr int kDigitsTwos = 0x107;
 constexpr int kTileM = 128;       // rows per CTA tile == tcgen05.mma M (PAPER.md:43 t_M = 128 on Blackwell)
 constexpr int kBlockK = 128;      // bytes of k per pipeline block (one 128B swizzle row, 4 MMAs of K = 32)
 // diagnostics words at the head of the workspace (zeroed per call): [0] SM cycles of the fused GEMM kernel (CTA 0),
@@ -43,7 +46,7 @@ struct emugemm_ctx {
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   int launches = 0;
   int dbg_flags = 0;
-  int slice_bits = 7;  // Scheme I digits: 7 = sign-magnitude (R1, default), 8 = balanced base 256 (R23)
+  int slice_bits = 7;  // Scheme I digits: 7 = sign-magnitude (R1, default), 8 = balanced base 256 (R23), kDigitsTwos (R24)
   int oz2_fusion = 0;  // Scheme II real DGEMM: 1 = fused reconstruction when it applies (emugemm_set_oz2_fusion), 0 = separate CRT kernel
                        // (default: measured 8192^3 N = 16: 8.9 ms fused against 5.3 + 0.6 ms)
   unsigned long long *diag = nullptr;  // device: [0] = GEMM-kernel SM cycles of the last call (inside the workspace)

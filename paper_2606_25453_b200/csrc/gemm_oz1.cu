@@ -185,7 +185,7 @@ struct Oz1Epi {
   }
   __device__ __forceinline__ void init(const Oz1Dev &a) {
     set_item(a);
-    const int bits = a.slice_bits;
+    const int bits = a.slice_bits & 0xFF;  // kDigitsTwos: 7-bit weights like R1
     w1 = 1 << bits;
     w2 = 1 << (2 * bits);
 #pragma unroll
@@ -725,6 +725,12 @@ int launch_oz1_gemm(emugemm_ctx *ctx, const Oz1GemmArgs &g) {
 // Overflow-safe k-chunk (R7): the fullest accumulator C_{p-1} sums p products of k_c
 // terms each bounded by 127^2, so p k_c 127^2 <= 2^31 - 1; rounded down to a multiple of 128.
 int64_t oz1_chunk_k_host(int p, int slice_bits) {
+  if (slice_bits == kDigitsTwos) {
+    // R24: leading digit in [-128, 127], the others in [0, 127]; the fullest accumulator C_(p-1) sums the pairs (0, p-1),
+    // (p-1, 0) with |d d'| <= 128 * 127 and p - 2 pairs <= 127^2 (p = 1: one pair <= 128^2)
+    const int64_t per_k = p == 1 ? 128 * 128 : 2 * 128 * 127 + static_cast<int64_t>(p - 2) * 127 * 127;
+    return (2147483647LL / per_k) / kBlockK * kBlockK;
+  }
   const int64_t dmax = (slice_bits == 8) ? 128 : 127;  // largest digit magnitude
   const int64_t bound = 2147483647LL / (static_cast<int64_t>(p) * dmax * dmax);
   return bound / kBlockK * kBlockK;

@@ -268,6 +268,33 @@ __device__ __forceinline__ void emit_oz1_b8(const Prep (&q)[4], Sink sink) {
   }
 }
 
+// Two's-complement 7-bit digits (R24; PAPER.md:345 at beta = 7): X = +-|X| (|X| < 2^(7P)) as a 64-bit two's-complement integer;
+// digit 0 = the low BYTE of X >> 7 (P - 1) (in [-128, 127]), digit t >= 1 = the 7-bit field (X >> 7 (P - 1 - t)) & 127 in [0, 127]:
+// per plane one funnel shift per element, three byte permutes, one AND; no sign fix-up.  Every slice but the leading one is
+// sign-free, which is what the tensor pipe's power likes (profiles/r2_operand_sign_power.md).
+template <int P, typename Sink>
+__device__ __forceinline__ void emit_oz1_tc(const Prep (&q)[4], Sink sink) {
+  unsigned int lo[4], hi[4];
+#pragma unroll
+  for (int i = 0; i < 4; ++i) {
+    const long long mag = static_cast<long long>((static_cast<unsigned long long>(q[i].w1) << 32) | q[i].w0);
+    const unsigned long long Y = static_cast<unsigned long long>(q[i].neg ? -mag : mag);
+    lo[i] = static_cast<unsigned int>(Y);
+    hi[i] = static_cast<unsigned int>(Y >> 32);
+  }
+#pragma unroll
+  for (int t = 0; t < P; ++t) {
+    const int sh = kBeta * (P - 1 - t);  // compile-time after unrolling
+    unsigned int b[4];
+#pragma unroll
+    for (int i = 0; i < 4; ++i)  // low byte of the arithmetic shift: for sh >= 32 the bits above come from hi's sign extension
+      b[i] = (sh == 0) ? lo[i] : (sh < 32) ? __funnelshift_r(lo[i], hi[i], sh) : (sh == 32) ? hi[i]
+                                           : static_cast<unsigned int>(static_cast<int>(hi[i]) >> (sh - 32));
+    const unsigned int w = __byte_perm(__byte_perm(b[0], b[1], 0x0040), __byte_perm(b[2], b[3], 0x0040), 0x5410);
+    sink(t, t == 0 ? w : (w & 0x7F7F7F7Fu));
+  }
+}
+
 // Sign-magnitude 7-bit digits (R1) of four elements, one packed word per plane.  Per plane: one funnel shift per
 // element brings digit t to byte 0, three byte permutes gather the four bytes, one AND keeps 7 bits, and the signs
 // are applied to the whole word at once: for a byte d in [0, 127] of a negative element
@@ -417,7 +444,8 @@ __device__ __forceinline__ void emit_quad(const T (&v)[4][W], int e_row, int par
 #pragma unroll
   for (int i = 0; i < 4; ++i) a[i] = prepare<T, NW>(v[i][0], e_row, scale_bits);
   if constexpr (MODE == 0) {
-    if constexpr (PARAM >= 16) emit_oz1_b8<PARAM - 16>(a, sink);  // PARAM = 16 + p: balanced 8-bit digits
+    if constexpr (PARAM >= 32) emit_oz1_tc<PARAM - 32>(a, sink);       // PARAM = 32 + p: two's-complement 7-bit digits (R24)
+    else if constexpr (PARAM >= 16) emit_oz1_b8<PARAM - 16>(a, sink);  // PARAM = 16 + p: balanced 8-bit digits
     else emit_oz1<PARAM>(a, sink);
   } else if constexpr (W == 1) {
     PrepS u[4];
@@ -682,6 +710,8 @@ static int launch_planes(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, 
 template <typename T, int P>
 static int slice_p(emugemm_ctx *ctx, int by_cols, int64_t rows, int64_t k, int64_t kpad, const void *X, int64_t ldx,
                    unsigned long long *maxbits, int32_t *e, int slice_bits, int8_t *out, int batch, int64_t xstride) {
+  if (slice_bits == kDigitsTwos)  // the same X as R1, two's-complement fields
+    return launch_planes<T, 1, 0, 32 + P>(ctx, sizeof(T) == 8 ? kF64 : kF32, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, kBeta * P, P, out, batch, xstride);
   if (slice_bits == 8)  // |X| = trunc(|x| 2^(8p - 2 - e)): two guard bits
     return launch_planes<T, 1, 0, 16 + P>(ctx, sizeof(T) == 8 ? kF64 : kF32, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, 8 * P - 2, P, out, batch, xstride);
   return launch_planes<T, 1, 0, P>(ctx, sizeof(T) == 8 ? kF64 : kF32, by_cols, rows, k, kpad, X, ldx, maxbits, e, P, kBeta * P, P, out, batch, xstride);
