@@ -41,7 +41,7 @@ def parse():
     ap.add_argument("--phi", type=float, default=-1.0)
     ap.add_argument("--slice-bits", type=int, default=7, choices=[7, 8], help="Scheme I digit width (8: balanced base 256, DESIGN.md R23)")
     ap.add_argument("--slice-form", type=int, default=0, choices=[0, 1],
-                    help="7-bit Scheme I digits: 0 = sign-magnitude (R1, default), 1 = two's-complement fields (R24, PAPER.md:345)")
+                    help="7-bit Scheme I digits: 0 = two's-complement fields (R24, PAPER.md:345; default), 1 = sign-magnitude (R1, round 1's default)")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--no-cpu", action="store_true")
     ap.add_argument("--no-probe", action="store_true")

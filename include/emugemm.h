@@ -58,21 +58,23 @@ int emugemm_create(emugemm_handle_t *h);  /* host-only state; checks the device 
 int emugemm_destroy(emugemm_handle_t h);
 int emugemm_set_stream(emugemm_handle_t h, void *cuda_stream /* cudaStream_t */);
 int emugemm_set_workspace(emugemm_handle_t h, void *dev_ptr, size_t bytes);
-/* Scheme I digit format of this handle.  7 (default; R1): sign-magnitude digits of
- * 7 bits, |d| <= 127.  8 (R23; "slices of beta <= 8
+/* Scheme I digit format of this handle.  7 (default): digits of 7 bits in the form emugemm_set_slice_form
+ * selects (two's-complement fields by default).  8 (R23; "slices of beta <= 8
  * bits"): balanced signed base-256 digits, d in [-128, 127], two guard bits under the row /
  * column exponent -- 8p - 2 bits per operand, so p = 7 reaches the accuracy of p = 8 at 7 bits
  * with 28 instead of 36 slice products.  Applies to dgemm_oz1, sgemm_oz1 and the Scheme I hooks. */
 int emugemm_set_slice_bits(emugemm_handle_t h, int bits);
-/* Digit FORM of the 7-bit Scheme I slices of this handle (real calls: emugemm_{d,s}gemm_oz1[_t|_strided_batched], operand
- * handles; the 4M complex calls return EMUGEMM_ERR_ARG in form 1).
- *   0 (default; R1): sign-magnitude digits, d_t = sign(x) * (7-bit field of |X|), all in [-127, 127].
- *   1 (R24; "a signed leading slice with unsigned remaining slices", at beta = 7 so that every slice is
- *     an INT8 value): the two's-complement fields of the SAME integer X = trunc(x 2^(7p)): d_0 in [-128, 127], d_t in [0, 127]
- *     for t >= 1.  Same accuracy class, same kernels, same weights; the results differ from form 0 only through the dropped
- *     slice pairs (t + u >= p).  Seven of eight slices carry no sign bits, which the tensor pipe rewards with a higher clock
- *     under the power cap (profiles/r2_operand_sign_power.md).  Overflow-safe chunk: emugemm_oz1_chunk_k_bits(p, 0x107).
- * Call after emugemm_set_slice_bits (which resets the form to 0); form 1 needs 7-bit digits (else EMUGEMM_ERR_ARG).          */
+/* Digit FORM of the 7-bit Scheme I slices of this handle (all Scheme I calls, operand handles included).
+ *   0 (default; R24; "a signed leading slice with unsigned remaining slices", here at beta = 7 so that
+ *     every slice is an INT8 value): the two's-complement fields of X = trunc(x 2^(7p)): d_0 in [-128, 127], d_t in [0, 127]
+ *     for t >= 1.  Seven of eight slices carry no sign bits, which the tensor pipe rewards with a higher clock under the
+ *     power cap (profiles/r2_operand_sign_power.md: 8192^3 p = 8 74.5 -> 76.9 % of the nominal INT8 peak).
+ *   1 (EMUGEMM_DIGITS_SIGN_MAGNITUDE; R1, the default of round 1): d_t = sign(x) * (7-bit field of |X|), all in
+ *     [-127, 127].  The SAME integer X, same kernels, same weights; the results of the two forms differ only through the dropped
+ *     slice pairs (t + u >= p).
+ * Call after emugemm_set_slice_bits (which selects form 0); with 8-bit digits form 1 is EMUGEMM_ERR_ARG.
+ * Overflow-safe chunk of a form: emugemm_oz1_chunk_k_bits(p, 7 | 8 | EMUGEMM_DIGITS_SIGN_MAGNITUDE).                          */
+#define EMUGEMM_DIGITS_SIGN_MAGNITUDE 0x207
 int emugemm_set_slice_form(emugemm_handle_t h, int form);
 /* Scheme II real FP64 product (emugemm_dgemm_oz2 and its _t / strided-batched / pre-decomposed forms), SURVEY 8(f) item 4
  * (the paper keeps the CRT separate and pays the residue workspace): on = 1 runs the reconstruction
@@ -327,8 +329,8 @@ int emugemm_oz2_budget(int n_moduli, int64_t k, int is3m, int *tA, int *tB);
  * m2, K2 the other way round; C0 a multiple of M_q >= 2^24).  Caller arrays (HOST): digits >= 11 * 5 int64, pair >=
  * 10 * 5 uint32.  Returns 0, or EMUGEMM_ERR_ARG.                                                                  */
 int emugemm_dbg_crt_constants(int n_moduli, int *n_pairs, int *n_digits, int *digit_bits, long long *digits, unsigned *pair);
-int64_t emugemm_oz1_chunk_k(int p);                       /* 7-bit digits */
-int64_t emugemm_oz1_chunk_k_bits(int p, int slice_bits);   /* p k_c dmax^2 <= 2^31 - 1, dmax = 127 / 128 */
+int64_t emugemm_oz1_chunk_k(int p);                       /* 7-bit digits, default form */
+int64_t emugemm_oz1_chunk_k_bits(int p, int code);   /* code 7 (default form) | 8 | EMUGEMM_DIGITS_SIGN_MAGNITUDE: the fullest accumulator stays below 2^31 */
 /* ---- PROBES build only (libemugemm_probes.so, compiled with -DEMUGEMM_PROBES; bench.py loads it for its probe leg).
  * The shipped libemugemm.so exports none of the three calls below and carries no experiment switch in its kernels. */
 #ifdef EMUGEMM_PROBES

@@ -42,19 +42,23 @@
 #include <omp.h>
 #endif
 
-#define ORACLE_BETA 7 /* R1: beta = 7, all slices signed ("signed-slice method supports beta <= 7") */
+#define ORACLE_BETA 7 /* beta = 7: every slice is a signed INT8 value ("signed-slice method supports beta <= 7") */
 
-/* Slice-digit mode (R23).  7 (default, R1): sign-magnitude 7-bit digits.
- * 8: balanced signed base-256 digits, d_t in [-128, 127], all-signed INT8 like R1 but 8 bits per slice
- * ("slices of beta <= 8 bits", PAPER.md:345 the paper's code reaches beta = 8 with a signed leading and
- * unsigned remaining slices; the balanced form keeps one signedness).  Two guard bits: x = a 2^-(e+2) in
- * (-1/4, 1/4) so that X + sum_j 128 256^j stays inside [0, 256^p). */
-static int g_slice_bits = 7;
-/* 7: sign-magnitude 7-bit digits (R1, default); 8: balanced base-256 digits (R23); 0x107: two's-complement 7-bit
- * digits -- signed leading slice, non-negative remaining slices (R24; the slice form of PAPER.md:345 at beta = 7) */
+/* Slice-digit mode of Scheme I (R24 / R1 / R23).  The caller selects it with one code:
+ *   7      (default; R24): 7-bit two's-complement digits -- a signed leading slice d_0 in [-128, 127] and non-negative
+ *          remaining slices d_t in [0, 127], the slice form the paper's own implementation uses ("a signed
+ *          leading slice with unsigned remaining slices"), here at beta = 7 so that every slice is an INT8 value
+ *          ("signed-slice method supports beta <= 7").
+ *   0x207  (R1): 7-bit sign-magnitude digits d_t = sign(x) * field_t(|X|) in [-127, 127], the reading of round 1; the SAME
+ *          integer X = trunc(x 2^(7p)) as the default form, spelled with other digits.
+ *   8      (R23): balanced signed base-256 digits, d_t in [-128, 127], two guard bits: x = a 2^-(e+2)
+ *          in (-1/4, 1/4) so that X + sum_j 128 256^j stays inside [0, 256^p).
+ * Internally g_slice_bits holds 0x107 (two's complement), 7 (sign-magnitude) or 8. */
 #define ORACLE_DIGITS_TWOS 0x107
-void oracle_set_slice_bits(int bits) { g_slice_bits = (bits == 8) ? 8 : (bits == ORACLE_DIGITS_TWOS) ? ORACLE_DIGITS_TWOS : 7; }
-int oracle_get_slice_bits(void) { return g_slice_bits; }
+#define ORACLE_DIGITS_SIGNMAG_CODE 0x207
+static int g_slice_bits = ORACLE_DIGITS_TWOS;
+void oracle_set_slice_bits(int code) { g_slice_bits = (code == 8) ? 8 : (code == ORACLE_DIGITS_SIGNMAG_CODE) ? 7 : ORACLE_DIGITS_TWOS; }
+int oracle_get_slice_bits(void) { return g_slice_bits == 8 ? 8 : g_slice_bits == 7 ? ORACLE_DIGITS_SIGNMAG_CODE : 7; }
 #define ORACLE_MAX_MODULI 24
 
 typedef __int128 i128;

@@ -35,13 +35,14 @@ def set_threads(t):
 
 
 # ---------------------------------------------------------------- exponents
-DIGITS_TWOS = 0x107
+DIGITS_SIGNMAG = 0x207
 
 
-def set_slice_bits(bits):
-    """7 (default, R1): sign-magnitude 7-bit digits; 8: balanced signed base-256 digits (R23); DIGITS_TWOS (0x107, R24):
-    two's-complement 7-bit digits, signed leading slice and non-negative remaining slices (PAPER.md:345 at beta = 7)."""
-    _lib.oracle_set_slice_bits(C.c_int(bits))
+def set_slice_bits(code):
+    """Scheme I digit mode: 7 (default, R24) = 7-bit two's-complement digits, signed leading slice and non-negative
+    remaining slices (PAPER.md:345 at beta = 7); DIGITS_SIGNMAG (0x207, R1) = 7-bit sign-magnitude digits; 8 (R23) =
+    balanced signed base-256 digits."""
+    _lib.oracle_set_slice_bits(C.c_int(code))
 
 
 def get_slice_bits():

@@ -12,6 +12,7 @@ PROBES_LIB_PATH = os.path.join(os.path.dirname(os.path.abspath(__file__)), "libe
 _HEADER = os.path.join(os.path.dirname(os.path.dirname(os.path.abspath(__file__))), "include", "emugemm.h")
 
 OZ1, OZ2, OZ2_3M, OZ1_4M = 1, 2, 3, 4
+DIGITS_SIGN_MAGNITUDE = 0x207   # EMUGEMM_DIGITS_SIGN_MAGNITUDE: code of the sign-magnitude digit form for oz1_chunk_k
 _i64, _int, _dbl, _flt, _vp, _sz = C.c_int64, C.c_int, C.c_double, C.c_float, C.c_void_p, C.c_size_t
 
 
@@ -127,14 +128,15 @@ class EmuGemm:
         self._stream = stream
 
     def set_slice_bits(self, bits):
-        """Scheme I digits: 7 = sign-magnitude (default), 8 = balanced base 256 (see include/emugemm.h)."""
+        """Scheme I digits: 7 (default, form per set_slice_form) or 8 = balanced base 256 (see include/emugemm.h)."""
         self._check(self._lib.emugemm_set_slice_bits(self._h, _int(bits)))
         self.slice_bits = bits
 
     def set_slice_form(self, form):
-        """7-bit Scheme I digits: 0 = sign-magnitude (default, R1), 1 = two's-complement fields (R24; include/emugemm.h)."""
+        """7-bit Scheme I digits: 0 = two's-complement fields (default, R24), 1 = sign-magnitude (R1; include/emugemm.h)."""
         self._check(self._lib.emugemm_set_slice_form(self._h, _int(form)))
-        self.slice_bits = 0x107 if form else 7
+        if self.slice_bits != 8:
+            self.slice_bits = DIGITS_SIGN_MAGNITUDE if form else 7
 
     def set_oz2_fusion(self, on):
         """Scheme II real DGEMM: fused reconstruction inside the GEMM kernel, or (default) the separate CRT kernel."""

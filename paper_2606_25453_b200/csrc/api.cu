@@ -494,16 +494,18 @@ int emugemm_set_stream(emugemm_handle_t h, void *s) {
   return EMUGEMM_OK;
 }
 
+// handle state: 7-bit digits are two's-complement fields (kDigitsTwos, R24) unless the sign-magnitude form (internal code 7,
+// R1) was selected; 8 = balanced base 256 (R23)
 int emugemm_set_slice_bits(emugemm_handle_t h, int bits) {
   if (!h || (bits != 7 && bits != 8)) return EMUGEMM_ERR_ARG;
-  h->slice_bits = bits;
+  h->slice_bits = bits == 7 ? kDigitsTwos : 8;
   return EMUGEMM_OK;
 }
 
 int emugemm_set_slice_form(emugemm_handle_t h, int form) {
   if (!h || (form & ~1)) return EMUGEMM_ERR_ARG;
-  if (form && (h->slice_bits & 0xFF) != 7) return EMUGEMM_ERR_ARG;  // the two's-complement form exists for 7-bit digits
-  h->slice_bits = form ? kDigitsTwos : (h->slice_bits & 0xFF);
+  if ((h->slice_bits & 0xFF) != 7) return form ? EMUGEMM_ERR_ARG : EMUGEMM_OK;  // the forms exist for 7-bit digits
+  h->slice_bits = form ? 7 : kDigitsTwos;
   return EMUGEMM_OK;
 }
 
@@ -593,7 +595,6 @@ static int run_oz1_4m(emugemm_ctx *h, int elem, int64_t m, int64_t n, int64_t k,
   }
   const int64_t kpad = round_up(k, kBlockK), kk = 2 * kpad, mm = 2 * m;
   const int bits = h->slice_bits;
-  if (bits == kDigitsTwos) return EMUGEMM_ERR_ARG;  // the two's-complement digit form (R24) covers the real Scheme I calls
   int64_t clen;
   const int nch = oz1_chunks(p, bits, kk, 0, &clen);
   if (!h->ws || (reinterpret_cast<uintptr_t>(h->ws) & 1023)) return h->ws ? EMUGEMM_ERR_ALIGNMENT : EMUGEMM_ERR_WORKSPACE;
@@ -943,9 +944,10 @@ int emugemm_dbg_crt_constants(int n_moduli, int *n_pairs, int *n_digits, int *di
   return crt_constants_dump(n_moduli, n_pairs, n_digits, digit_bits, digits, pair) ? EMUGEMM_ERR_ARG : EMUGEMM_OK;
 }
 
-int64_t emugemm_oz1_chunk_k(int p) { return (p >= 1 && p <= 8) ? oz1_chunk_k_host(p, 7) : 0; }
-int64_t emugemm_oz1_chunk_k_bits(int p, int slice_bits) {
-  return (p >= 1 && p <= 8 && (slice_bits == 7 || slice_bits == 8 || slice_bits == kDigitsTwos)) ? oz1_chunk_k_host(p, slice_bits) : 0;
+int64_t emugemm_oz1_chunk_k(int p) { return (p >= 1 && p <= 8) ? oz1_chunk_k_host(p, kDigitsTwos) : 0; }  // default digit form
+int64_t emugemm_oz1_chunk_k_bits(int p, int code) {  // public codes: 7 (default form), 8, EMUGEMM_DIGITS_SIGN_MAGNITUDE
+  const int internal = code == 7 ? kDigitsTwos : code == 8 ? 8 : code == EMUGEMM_DIGITS_SIGN_MAGNITUDE ? 7 : 0;
+  return (p >= 1 && p <= 8 && internal) ? oz1_chunk_k_host(p, internal) : 0;
 }
 
 #ifdef EMUGEMM_PROBES

@@ -46,7 +46,7 @@ struct emugemm_ctx {
   cudaEvent_t ev[4] = {nullptr, nullptr, nullptr, nullptr};
   int launches = 0;
   int dbg_flags = 0;
-  int slice_bits = 7;  // Scheme I digits: 7 = sign-magnitude (R1, default), 8 = balanced base 256 (R23), kDigitsTwos (R24)
+  int slice_bits = emu::kDigitsTwos;  // Scheme I digits: kDigitsTwos = 7-bit two's-complement fields (R24, default), 7 = 7-bit sign-magnitude (R1), 8 = balanced base 256 (R23)
   int oz2_fusion = 0;  // Scheme II real DGEMM: 1 = fused reconstruction when it applies (emugemm_set_oz2_fusion), 0 = separate CRT kernel
                        // (default: measured 8192^3 N = 16: 8.9 ms fused against 5.3 + 0.6 ms)
   unsigned long long *diag = nullptr;  // device: [0] = GEMM-kernel SM cycles of the last call (inside the workspace)
@@ -179,7 +179,7 @@ int launch_i8_probe(emugemm_ctx *ctx, int n_ops, const int *ops, int iters, floa
 // host helpers shared by api.cu and the drivers
 int oz2_moduli_host(int n, int *mod);                  // greedy coprime list, descending from 256
 int oz2_budget_host(int n, int64_t k, int is3m, int *tA, int *tB);
-int64_t oz1_chunk_k_host(int p, int slice_bits = 7);
+int64_t oz1_chunk_k_host(int p, int slice_bits = kDigitsTwos);
 // Work items (cluster tiles) of one k-chunk of the fused Scheme I kernel for an m x n output with p slices; the
 // kernel runs num_sms / 2 workers (CTA pairs) for every p (gemm_oz1.cu)
 int64_t oz1_cluster_tiles_host(int p, int64_t m, int64_t n);

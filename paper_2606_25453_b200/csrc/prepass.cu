@@ -766,7 +766,8 @@ int launch_oz2_residues(emugemm_ctx *ctx, int elem, int by_cols, int64_t rows, i
 // Embedded k index: [0, kpad) = first half, [kpad, 2 kpad) = second half (each half zero-padded to kpad).
 template <int PARAM, typename Sink>
 __device__ __forceinline__ void emit_oz1_any(const Prep (&q)[4], Sink sink) {
-  if constexpr (PARAM >= 16) emit_oz1_b8<PARAM - 16>(q, sink);
+  if constexpr (PARAM >= 32) emit_oz1_tc<PARAM - 32>(q, sink);
+  else if constexpr (PARAM >= 16) emit_oz1_b8<PARAM - 16>(q, sink);
   else emit_oz1<PARAM>(q, sink);
 }
 
@@ -864,12 +865,17 @@ static int slice4m_p(emugemm_ctx *ctx, int is_b, int64_t rows, int64_t k, int64_
   const int scale_bits = slice_bits == 8 ? 8 * P - 2 : kBeta * P;
   if (!is_b) {
     if (slice_bits == 8) oz1_4m_rows_kernel<T, 16 + P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out, ctx->nf_flag);
+    else if (slice_bits == kDigitsTwos) oz1_4m_rows_kernel<T, 32 + P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out, ctx->nf_flag);
     else oz1_4m_rows_kernel<T, P><<<static_cast<unsigned>(rows), 256, 0, st>>>(x, ldx, rows, k, kpad, e, scale_bits, out, ctx->nf_flag);
   } else {
     const size_t smem = static_cast<size_t>(2 * P) * 32 * 33 * 4;
     const dim3 grid(static_cast<unsigned>((rows + 31) / 32), static_cast<unsigned>(kpad / 128));
     if (slice_bits == 8) {
       auto kern = oz1_4m_cols_kernel<T, 16 + P>;
+      EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 32 * 33 * 4));
+      kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, scale_bits, P, out, ctx->nf_flag);
+    } else if (slice_bits == kDigitsTwos) {
+      auto kern = oz1_4m_cols_kernel<T, 32 + P>;
       EMU_CUDA(ctx, cudaFuncSetAttribute(kern, cudaFuncAttributeMaxDynamicSharedMemorySize, 16 * 32 * 33 * 4));
       kern<<<grid, 256, smem, st>>>(x, ldx, rows, k, kpad, maxbits, e, scale_bits, P, out, ctx->nf_flag);
     } else {

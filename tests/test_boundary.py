@@ -34,10 +34,16 @@ def test_host_helpers_match_oracle():
         for k in (1, 4096, 8192, 65536):
             assert E.oz2_budget(N, k) == O.oz2_budget(N, k)
             assert E.oz2_budget(N, k, True) == O.oz2_budget(N, k, True)
-    # overflow-safe chunk (R7): p k_c 127^2 <= 2^31 - 1, multiple of 128
+    # overflow-safe chunk (R7), a multiple of 128.  Sign-magnitude digits (R1): p k_c 127^2 <= 2^31 - 1.  Default two's-complement
+    # digits (R24): the leading digit reaches -128, the fullest accumulator sums 2 pairs <= 128 * 127 and p - 2 pairs <= 127^2.
     for p in range(1, 9):
-        ck = E.oz1_chunk_k(p)
+        ck = E.oz1_chunk_k(p, E.DIGITS_SIGN_MAGNITUDE)
         assert ck % 128 == 0 and p * ck * 127 * 127 <= 2 ** 31 - 1 < p * (ck + 128) * 127 * 127
+        per_k = 128 * 128 if p == 1 else 2 * 128 * 127 + (p - 2) * 127 * 127
+        ck = E.oz1_chunk_k(p)
+        assert ck % 128 == 0 and ck * per_k <= 2 ** 31 - 1 < (ck + 128) * per_k
+        ck8 = E.oz1_chunk_k(p, 8)
+        assert ck8 % 128 == 0 and p * ck8 * 128 * 128 <= 2 ** 31 - 1 < p * (ck8 + 128) * 128 * 128
 
 
 def test_no_cpu_fallback_without_gpu():

@@ -1,5 +1,5 @@
-"""-m gpu parity tests, Scheme I with two's-complement 7-bit digits (emugemm_set_slice_form(h, 1); R24,
-PAPER.md:345): digits and INT32 accumulators bit-exact against the oracle's R24 mode, final FP64 / FP32 within 2 ulp of
+"""-m gpu parity tests, Scheme I with the DEFAULT two's-complement 7-bit digits (R24; form 0 of
+emugemm_set_slice_form) and the switch to the sign-magnitude form (R1): digits and INT32 accumulators bit-exact against the oracle's R24 mode, final FP64 / FP32 within 2 ulp of
 (|A||B|)_ij, the k-chunk bound of the form, batched and operand-handle calls, one full-size point."""
 import numpy as np
 import pytest
@@ -16,8 +16,9 @@ def env():
     from oracle import oracle as O
     import paper_2606_25453_b200 as E
     h = E.EmuGemm()
-    h.set_slice_form(1)
-    O.set_slice_bits(O.DIGITS_TWOS)
+    h.set_slice_bits(7)
+    h.set_slice_form(0)          # the defaults, spelled out
+    O.set_slice_bits(7)
     yield torch, O, h, E
     O.set_slice_bits(7)
     h.close()
@@ -108,9 +109,9 @@ def test_chunk_bound_and_k_chunked(env):
     torch, O, h, E = env
     for p in range(1, 9):
         per_k = 128 * 128 if p == 1 else 2 * 128 * 127 + (p - 2) * 127 * 127
-        ck = E.oz1_chunk_k(p, 0x107)
+        ck = E.oz1_chunk_k(p)
         assert ck % 128 == 0 and ck * per_k <= 2 ** 31 - 1 < (ck + 128) * per_k
-    assert E.oz1_chunk_k(8, 0x107) == 16512
+    assert E.oz1_chunk_k(8) == 16512 and E.oz1_chunk_k(8, E.DIGITS_SIGN_MAGNITUDE) == 16640
     m, n, k, p = 64, 48, 17000, 8
     A, B = G.real_pair(m, n, k, 1.0, 4)
     C = torch.zeros((m, n), dtype=torch.float64, device="cuda")
@@ -142,6 +143,7 @@ def test_batched_and_operand_handles(env):
     assert torch.equal(C2, C[0])
     # an operand decomposed in the other digit form must be refused, not silently mixed
     h0 = E.EmuGemm()
+    h0.set_slice_form(1)
     try:
         opB0 = h0.decompose(E.OZ1, 1, dev(torch, B[0]), p)
         with pytest.raises(E.EmuGemmError):
@@ -150,23 +152,38 @@ def test_batched_and_operand_handles(env):
         h0.close()
 
 
-def test_form_switching_and_4m_refused(env):
+def test_form_switching_sign_magnitude_and_4m(env):
+    """Form 1 = sign-magnitude digits (R1): bit-exact digits and 2-ulp parity against the oracle's R1 mode on the same handle type;
+    8-bit digits have no forms; the 4M complex call runs in both 7-bit forms."""
     torch, O, h, E = env
     h2 = E.EmuGemm()
     try:
         h2.set_slice_bits(8)
         with pytest.raises(E.EmuGemmError):
-            h2.set_slice_form(1)            # the form exists for 7-bit digits only
+            h2.set_slice_form(1)            # the forms exist for 7-bit digits only
         h2.set_slice_bits(7)
         h2.set_slice_form(1)
-        A, B = G.complex_pair(40, 24, 100, 1.0, 3)
-        C = torch.zeros((40, 24), dtype=torch.complex128, device="cuda")
-        with pytest.raises(E.EmuGemmError):
-            h2.zgemm_oz1_4m(dev(torch, A), dev(torch, B), C, 4)
-        h2.set_slice_form(0)
-        h2.zgemm_oz1_4m(dev(torch, A), dev(torch, B), C, 4)
-        assert torch.isfinite(C.real).all()
+        O.set_slice_bits(O.DIGITS_SIGNMAG)
+        A, B = G.real_pair(130, 70, 333, 2.0, 5)
+        A[1, :] = -np.abs(A[1, :])
+        SA, eA = h2.dbg_oz1_slices(dev(torch, A), False, 6)
+        SAh = SA.cpu().numpy()
+        assert np.array_equal(SAh, O.oz1_slices_rows(A, O.row_exponents(A), 6)) and SAh.min() >= -127 and SAh[1:].min() < 0
+        C = torch.empty((130, 70), dtype=torch.float64, device="cuda")
+        h2.dgemm_oz1(dev(torch, A), dev(torch, B), C, 6)
+        assert_within_ulps(C.cpu().numpy(), O.dgemm_oz1(A, B, 6), np.abs(A) @ np.abs(B), 2, what="sign-magnitude form")
+        Az, Bz = G.complex_pair(40, 24, 100, 1.0, 3)
+        absZ = (np.abs(Az.real) + np.abs(Az.imag)) @ (np.abs(Bz.real) + np.abs(Bz.imag))
+        for form, code in ((1, O.DIGITS_SIGNMAG), (0, 7)):
+            h2.set_slice_form(form)
+            O.set_slice_bits(code)
+            Cz = torch.zeros((40, 24), dtype=torch.complex128, device="cuda")
+            h2.zgemm_oz1_4m(dev(torch, Az), dev(torch, Bz), Cz, 4)
+            want = O.zgemm_oz1_4m(Az, Bz, 4)
+            assert_within_ulps(Cz.cpu().numpy().real, want.real, absZ, 2, what=f"4M re form {form}")
+            assert_within_ulps(Cz.cpu().numpy().imag, want.imag, absZ, 2, what=f"4M im form {form}")
     finally:
+        O.set_slice_bits(7)
         h2.close()
 
 

@@ -15,6 +15,16 @@ from exact_helpers import BETA, max_exp, trunc_scaled, read_golden
 GOLD = read_golden(os.path.join(os.path.dirname(__file__), "golden", "paper_values.txt"))
 
 
+@pytest.fixture(autouse=True, params=["twos", "signmag"])
+def digit_form(request):
+    """Every pin below runs in both 7-bit digit forms: the default two's-complement digits (R24) and the
+    sign-magnitude digits (R1).  Both spell the same integer X = trunc(x 2^(7p)), so the invariants are shared; the two
+    pins that describe the digits themselves branch on the form."""
+    O.set_slice_bits(7 if request.param == "twos" else O.DIGITS_SIGNMAG)
+    yield request.param
+    O.set_slice_bits(7)
+
+
 def test_paper_constants():
     # PAPER.md:88 p(p+1)/2 products; PAPER.md:76 signed slices => beta <= 7
     assert int(GOLD["oz1_product_count_p6"][0]) == 6 * 7 // 2
@@ -34,14 +44,18 @@ def test_exponents_match_frexp_definition():
 
 
 @pytest.mark.parametrize("p", [1, 2, 3, 6, 8])
-def test_slices_resum_to_truncated_input(p):
+def test_slices_resum_to_truncated_input(p, digit_form):
     """Invariant: sum_t A'_t 2^(beta(p-1-t)) == sign * trunc(|x| 2^(beta p)), x = a 2^-eA (exact ints)."""
     A, B = G.real_pair(6, 5, 40, 2.0, 5)
     A[0, 0] = 0.0
     A[1, 1] = -A[1].max() * 3  # the row maximum itself, negative
     eA, eB = O.row_exponents(A), O.col_exponents(B)
     SA, SB = O.oz1_slices_rows(A, eA, p), O.oz1_slices_cols(B, eB, p)
-    assert SA.min() >= -127 and SA.max() <= 127 and SB.min() >= -127 and SB.max() <= 127
+    if digit_form == "signmag":
+        assert SA.min() >= -127 and SA.max() <= 127 and SB.min() >= -127 and SB.max() <= 127
+    else:   # signed leading slice, non-negative remaining slices
+        assert SA[0].min() >= -128 and SA[0].max() <= 127 and SB[0].min() >= -128 and SB[0].max() <= 127
+        assert p == 1 or (SA[1:].min() >= 0 and SA[1:].max() <= 127 and SB[1:].min() >= 0 and SB[1:].max() <= 127)
     for i in range(A.shape[0]):
         for h in range(A.shape[1]):
             want = trunc_scaled(A[i, h], BETA * p - int(eA[i]))
@@ -55,20 +69,40 @@ def test_slices_resum_to_truncated_input(p):
             assert got == want
 
 
-def test_slices_match_fp64_digit_recurrence():
-    """Second derivation: d = trunc(r 2^beta); r = r 2^beta - d in FP64 (exact: power-of-two
-    scalings and subtraction of the integer part only)."""
+def test_slices_match_fp64_digit_recurrence(digit_form):
+    """Second derivation: d = trunc(r 2^beta); r = r 2^beta - d in FP64 (exact: power-of-two scalings and subtraction of
+    the integer part only) gives the 7-bit fields of |X|: the sign-magnitude digits are sign * field; the two's-complement
+    digits are the fields of X = sign * |X| -- for a negative element the fields of 2^(7p + 1) - |X| (borrow propagation from
+    the lowest non-zero field), the leading one read as a signed byte."""
     p = 7
     A, _ = G.real_pair(16, 4, 64, 1.0, 9)
+    A[2, 3] = -A[2, 3] if A[2, 3] > 0 else A[2, 3]
     eA = O.row_exponents(A)
     SA = O.oz1_slices_rows(A, eA, p)
     r = np.abs(A) * np.exp2(-eA.astype(np.float64))[:, None]
     sgn = np.where(A < 0, -1, 1)
+    fields = []
     for t in range(p):
         r = r * 2.0 ** BETA
         d = np.floor(r)
         r = r - d
-        assert np.array_equal((sgn * d).astype(np.int8), SA[t])
+        fields.append(d.astype(np.int64))
+    if digit_form == "signmag":
+        for t in range(p):
+            assert np.array_equal((sgn * fields[t]).astype(np.int8), SA[t])
+        return
+    # negate field-wise with borrow, from the least significant field up: -|X| = sum_t d_t 128^(p-1-t), d_t in [0, 127] (t > 0)
+    want = [f.copy() for f in fields]
+    neg = A < 0
+    borrow = np.zeros_like(fields[0])
+    for t in range(p - 1, -1, -1):
+        v = -fields[t] - borrow                      # in [-128, 0]
+        if t > 0:
+            borrow = (v < 0).astype(np.int64)
+            v = v + 128 * borrow                     # in [0, 127]
+        want[t] = np.where(neg, v, fields[t])
+    for t in range(p):
+        assert np.array_equal(want[t].astype(np.int8), SA[t]), t
 
 
 def test_row_scaling_changes_only_exponent():
@@ -89,10 +123,10 @@ def test_accumulators_are_textbook_integer_matmul():
     for s in range(p):
         ref = sum(SA[t].astype(np.int64) @ SB[s - t].astype(np.int64).T for t in range(s + 1))
         assert np.array_equal(CS[s], ref)
-        assert np.abs(CS[s]).max() <= (s + 1) * A.shape[1] * 127 * 127
+        assert np.abs(CS[s]).max() <= (s + 1) * A.shape[1] * 128 * 128   # |digit| <= 127 (sign-magnitude) / 128 (leading two's-complement digit)
 
 
-def test_shift_reduce_closed_form_fractions():
+def test_shift_reduce_closed_form_fractions(digit_form):
     """C == product of the truncated operands minus the dropped pairs (t+u >= p), exactly, then
     one rounding; checked with Fractions on a tiny input, with alpha and beta."""
     p = 4
@@ -106,9 +140,14 @@ def test_shift_reduce_closed_form_fractions():
             for h in range(9):
                 XA = trunc_scaled(A[i, h], BETA * p - int(eA[i]))
                 XB = trunc_scaled(B[h, j], BETA * p - int(eB[j]))
-                da = [(abs(XA) >> (BETA * (p - 1 - t))) & 127 for t in range(p)]
-                db = [(abs(XB) >> (BETA * (p - 1 - t))) & 127 for t in range(p)]
-                sg = (-1 if XA < 0 else 1) * (-1 if XB < 0 else 1)
+                if digit_form == "signmag":   # digits = sign * 7-bit fields of |X|
+                    da = [(abs(XA) >> (BETA * (p - 1 - t))) & 127 for t in range(p)]
+                    db = [(abs(XB) >> (BETA * (p - 1 - t))) & 127 for t in range(p)]
+                    sg = (-1 if XA < 0 else 1) * (-1 if XB < 0 else 1)
+                else:                         # two's-complement fields of X itself (Python's >> floors): signed leading digit
+                    da = [(XA >> (BETA * (p - 1 - t))) & 127 if t else XA >> (BETA * (p - 1)) for t in range(p)]
+                    db = [(XB >> (BETA * (p - 1 - t))) & 127 if t else XB >> (BETA * (p - 1)) for t in range(p)]
+                    sg = 1
                 for t in range(p):
                     for u in range(p):
                         if t + u < p:  # kept pairs only (Eq. 2)

@@ -59,7 +59,7 @@ def test_four_products_equal_the_real_embedding():
     product on the embedding A' = [[Re A, -Im A], [Im A, Re A]], B' = [[Re B], [Im B]] (the form the CUDA path uses),
     bit for bit: rows i and m + i of A' share the exponent of row i of A, the digits of -Im A are the negated digits."""
     try:
-        for bits, p, seed in ((7, 3, 5), (7, 6, 6), (7, 8, 7), (8, 4, 8), (8, 7, 9)):
+        for bits, p, seed in ((7, 3, 5), (7, 6, 6), (7, 8, 7), (8, 4, 8), (8, 7, 9), (O.DIGITS_SIGNMAG, 3, 5), (O.DIGITS_SIGNMAG, 8, 7)):
             O.set_slice_bits(bits)
             A, B = G.complex_pair(21, 17, 50, 1.0, seed)
             m = A.shape[0]

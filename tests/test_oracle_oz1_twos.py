@@ -1,4 +1,4 @@
-"""not-gpu: oracle pins for the two's-complement digit form of Scheme I (R24; "a signed leading
+"""not-gpu: oracle pins for the DEFAULT digit form of Scheme I, two's-complement 7-bit digits (R24; "a signed leading
 slice with unsigned remaining slices", here at beta = 7 so that every slice is an INT8 value).
 
 What is fixed by the mathematics: the digits are the two's-complement fields of the SAME integer X = trunc(x 2^(7p))
@@ -17,7 +17,7 @@ from oracle import oracle as O
 
 @pytest.fixture()
 def twos():
-    O.set_slice_bits(O.DIGITS_TWOS)
+    O.set_slice_bits(7)      # the default form (R24)
     yield
     O.set_slice_bits(7)
 
@@ -39,9 +39,9 @@ def test_digits_are_the_twos_complement_fields_of_the_same_integer(twos, p):
     A[4, 7] = -2.0 ** -60 * np.abs(A[4]).max()       # a tiny negative value: X = 0 or -0 -> digits all zero (trunc toward zero)
     eA = O.row_exponents(A)
     S = O.oz1_slices_rows(A, eA, p).astype(np.int64)          # [p][m][k]
-    O.set_slice_bits(7)
+    O.set_slice_bits(O.DIGITS_SIGNMAG)
     S1 = O.oz1_slices_rows(A, eA, p).astype(np.int64)
-    O.set_slice_bits(O.DIGITS_TWOS)
+    O.set_slice_bits(7)
     assert S[0].min() >= -128 and S[0].max() <= 127
     if p > 1:
         assert S[1:].min() >= 0 and S[1:].max() <= 127           # every slice but the leading one is sign-free
@@ -76,9 +76,9 @@ def test_small_integer_operands_are_exact_in_both_forms(twos):
         S = O.oz1_slices_rows(A, O.row_exponents(A), p)
         assert (S[1:] == 0).all()
         assert np.array_equal(O.dgemm_oz1(A, B, p), want), p
-        O.set_slice_bits(7)
+        O.set_slice_bits(O.DIGITS_SIGNMAG)
         r1 = O.dgemm_oz1(A, B, p)
-        O.set_slice_bits(O.DIGITS_TWOS)
+        O.set_slice_bits(7)
         assert np.array_equal(r1, want)
 
 
@@ -93,9 +93,9 @@ def test_error_bound_against_the_exact_product(twos, p):
     scale = np.exp2(eA.astype(np.float64))[:, None] * np.exp2(eB.astype(np.float64))[None, :]
     bound = (200 * (p + 1) * 2.0 ** (-7 * p + 2) + 2.0 ** -52) * scale
     assert (np.abs(got - exact) <= bound).all()
-    O.set_slice_bits(7)
+    O.set_slice_bits(O.DIGITS_SIGNMAG)
     r1 = O.dgemm_oz1(A, B, p)
-    O.set_slice_bits(O.DIGITS_TWOS)
+    O.set_slice_bits(7)
     assert (np.abs(got - r1) <= 2 * bound).all()     # the two digit forms differ only by their dropped pairs
     if p == 8:
         assert np.abs(got - exact).max() <= 4 * np.abs(exact).max() * 2.0 ** -45
