@@ -24,8 +24,8 @@ HOT = [
     ("Scheme II GEMM with fused reconstruction, N = 15 / 16", r"oz2_gemm_kernel<1, 8>"),
     ("exact FP64 CRT, N = 15 / 16, real", r"crt_kernel<8, 0>"),
     ("exact FP64 CRT, N = 17 / 18, complex", r"crt_kernel<9, 1>"),
-    ("Scheme I row pre-pass, p = 8 (register-resident row)", r"planes_rows_reg_kernel<double, 1, 0, 8, 256>"),
-    ("Scheme I column pre-pass, p = 8", r"planes_cols_kernel<double, 1, 0, 8, 128>"),
+    ("Scheme I row pre-pass, p = 8, default two's-complement digits (register-resident row)", r"planes_rows_reg_kernel<double, 1, 0, 40, 256>"),
+    ("Scheme I column pre-pass, p = 8, default two's-complement digits", r"planes_cols_kernel<double, 1, 0, 40, 128>"),
     ("Scheme II row pre-pass (residues, 2 words)", r"planes_rows_kernel<double, 1, 1, 2>"),
     ("Scheme II column pre-pass (residues, 2 words)", r"planes_cols_kernel<double, 1, 1, 2, 128>"),
     ("column maxima", r"colmax_kernel<double, 1>"),
