@@ -256,3 +256,37 @@ def test_zgemm_4m_2048_p8(env):
     scale = (np.abs(A.real[rows]) + np.abs(A.imag[rows])) @ (np.abs(B.real[:, cols]) + np.abs(B.imag[:, cols]))
     assert_within_ulps(got.real, want_re, scale, 2, what="4M re")
     assert_within_ulps(got.imag, want_im, scale, 2, what="4M im")
+
+
+# ---- SURVEY 8(c) reading R1 (sign-magnitude digits, emugemm_set_slice_form(h, 1)) at full size ----------------------
+# The default digit form is R24; R1, the reading SURVEY 8(c) lists, stays a complete mode: the same checks as above
+# on BASELINE configs[1] points, against the oracle's R1 mode.
+def test_sign_magnitude_form_full_size(env):
+    torch, O, _ = env
+    import paper_2606_25453_b200 as E
+    size = 8192
+    A, B = G.real_pair(size, size, size, 2.0, 1)
+    dA, dB = torch.from_numpy(A).cuda(), torch.from_numpy(B).cuda()
+    h = E.EmuGemm()
+    try:
+        h.set_slice_form(1)
+        O.set_slice_bits(O.DIGITS_SIGNMAG)
+        # all slices of the 8192 x 8192 operands, bit for bit
+        for X, dX, by_cols in ((A, dA, False), (B, dB, True)):
+            S, e = h.dbg_oz1_slices(dX, by_cols, 8)
+            oe = O.col_exponents(X) if by_cols else O.row_exponents(X)
+            want = O.oz1_slices_cols(X, oe, 8) if by_cols else O.oz1_slices_rows(X, oe, 8)
+            got = S.cpu().numpy()
+            del S
+            assert np.array_equal(e.cpu().numpy(), oe) and np.array_equal(got, want), f"R1 slices differ (by_cols={by_cols})"
+            assert got.min() >= -127 and got[1:].min() < 0          # sign-magnitude: lower slices carry signs
+        rows, cols = _samples(size, size, 7)
+        for p in (8, 3):
+            C = torch.full((size, size), float("nan"), dtype=torch.float64, device="cuda")
+            h.dgemm_oz1(dA, dB, C, p)
+            got = C[torch.from_numpy(rows).cuda()][:, torch.from_numpy(cols).cuda()].cpu().numpy()
+            assert_within_ulps(got, O.oz1_sampled(A, B, p, rows, cols), _abs_ab(A, B, rows, cols), 2, what=f"R1 8192 p={p}")
+            assert torch.isfinite(C).all()
+    finally:
+        O.set_slice_bits(7)
+        h.close()
