@@ -172,6 +172,18 @@ def test_form_switching_sign_magnitude_and_4m(env):
         C = torch.empty((130, 70), dtype=torch.float64, device="cuda")
         h2.dgemm_oz1(dev(torch, A), dev(torch, B), C, 6)
         assert_within_ulps(C.cpu().numpy(), O.dgemm_oz1(A, B, 6), np.abs(A) @ np.abs(B), 2, what="sign-magnitude form")
+        # batched and operand-handle calls in the sign-magnitude form
+        rng = np.random.default_rng(23)
+        Ab = (rng.random((3, 100, 260)) - 0.5) * np.exp(rng.standard_normal((3, 100, 260)))
+        Bb = (rng.random((3, 260, 70)) - 0.5) * np.exp(rng.standard_normal((3, 260, 70)))
+        Cb = torch.full((3, 100, 70), float("nan"), dtype=torch.float64, device="cuda")
+        h2.dgemm_oz1_strided_batched(dev(torch, Ab), dev(torch, Bb), Cb, 7)
+        for b in range(3):
+            assert_within_ulps(Cb[b].cpu().numpy(), O.dgemm_oz1(Ab[b], Bb[b], 7), np.abs(Ab[b]) @ np.abs(Bb[b]), 2, what=f"R1 batched {b}")
+        opA, opB = h2.decompose(E.OZ1, 0, dev(torch, Ab[1]), 7), h2.decompose(E.OZ1, 1, dev(torch, Bb[1]), 7)
+        Cp = torch.empty((100, 70), dtype=torch.float64, device="cuda")
+        h2.gemm_pre(opA, opB, Cp)
+        assert torch.equal(Cp, Cb[1])
         Az, Bz = G.complex_pair(40, 24, 100, 1.0, 3)
         absZ = (np.abs(Az.real) + np.abs(Az.imag)) @ (np.abs(Bz.real) + np.abs(Bz.imag))
         for form, code in ((1, O.DIGITS_SIGNMAG), (0, 7)):
